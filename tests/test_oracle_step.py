@@ -1,0 +1,232 @@
+"""Pins for the oracle's time step (not gpu): closed forms of the scheme and invariants.
+ * Stokes mode decays by the Crank-Nicolson factor (channel version of exp(-nu k^2 t));
+ * laminar Poiseuille flow is steady with G = 2/Re;
+ * the new velocity is divergence-free algebraically;
+ * the split Cahn-Hilliard solve satisfies the 4th-order operator identity (S8) and the
+   wall conditions; the tanh profile of Eq. 5 is stationary to truncation level;
+   mean(phi) is conserved for a z-odd profile;
+ * the explicit terms N_omega, N_w, S_phi, S_x-bar equal the continuous formulas of
+   Eqs. 1, 4, 7, 8, 14, 15, 17 differentiated symbolically (sympy) on a manufactured state;
+ * second-order convergence in time of the Navier-Stokes part (AB2 + CN, S7)."""
+import math
+
+import numpy as np
+import pytest
+
+import psdns_oracle as O
+import psdns_inputs as I
+
+
+def test_stokes_mode_crank_nicolson_factor():
+    g = O.Grid(8, 8, 33)
+    p = O.Params(re=50.0, dt=2e-3, phase_field=0)
+    z = O.cheb_nodes(g.N)[:, None, None]
+    y = g.ly / g.ny * np.arange(g.ny)[None, :, None]
+    ky = 2 * np.pi / g.ly * 2
+    A = 0.7
+    u = A * np.cos(np.pi * z / 2) * np.cos(ky * y) * np.ones((1, 1, g.nx))
+    zero = np.zeros_like(u)
+    orc = O.Oracle(g, p)
+    orc.set_state("physical", u, zero, zero)
+    gam = p.dt / (2 * p.re)
+    kap2 = ky ** 2 + np.pi ** 2 / 4
+    fac = (1 - gam * kap2) / (1 + gam * kap2)
+    for n in range(1, 4):
+        orc.step(1)
+        un, vn, wn = orc.get_state("physical")
+        assert np.abs(un - fac ** n * u).max() < 1e-12
+        assert np.abs(vn).max() < 1e-13 and np.abs(wn).max() < 1e-13
+    # and it approaches the viscous decay exp(-kappa^2 t / Re)
+    assert abs(fac ** 3 - math.exp(-kap2 * 3 * p.dt / p.re)) < 1e-9
+
+
+def test_poiseuille_is_steady():
+    g = O.Grid(8, 8, 17)
+    p = O.Params(re=100.0, dt=1e-3, gradp_x=2.0 / 100.0, phase_field=0)
+    z = O.cheb_nodes(g.N)[:, None, None]
+    u = (1 - z * z) * np.ones((1, g.ny, g.nx))
+    orc = O.Oracle(g, p)
+    orc.set_state("physical", u, 0 * u, 0 * u)
+    orc.step(5)
+    un, vn, wn = orc.get_state("physical")
+    assert np.abs(un - u).max() < 1e-13
+    assert np.abs(vn).max() < 1e-14 and np.abs(wn).max() < 1e-14
+
+
+def test_divergence_free_and_no_slip_after_steps():
+    c = I.small_config()
+    g = O.Grid(c.nx, c.ny, c.nz, c.lx, c.ly)
+    p = O.Params(re=c.re, dt=c.dt, pe=c.pe, ch=c.ch, we=c.we, gradp_x=c.gradp_x)
+    orc = O.Oracle(g, p)
+    orc.set_state("physical", *I.channel_state(c))
+    orc.step(2)
+    s = orc.state
+    div = O.divergence_spectrum(g, s.u, s.v, s.w)
+    assert np.abs(div).max() < 1e-13
+    for f in (s.u, s.v, s.w):
+        assert np.abs(f.sum(axis=0)).max() < 1e-12                     # value at z = +1
+        sgn = ((-1.0) ** np.arange(g.nz))[:, None, None]
+        assert np.abs((f * sgn).sum(axis=0)).max() < 1e-12             # value at z = -1
+    n2 = (np.arange(g.nz) ** 2.0)[:, None, None]
+    assert np.abs((n2 * s.w).sum(axis=0)).max() < 1e-10                # dw/dz at z = +1
+    # hidden state consistent with w: rows 0..N-2 of (D^2 - k^2) w = theta
+    lap = orc._lap(s.w)
+    assert np.abs((lap - s.theta)[: g.N - 1]).max() < 1e-8 * max(1.0, np.abs(s.theta).max())
+
+
+def test_cahn_hilliard_two_stage_identity_and_wall_conditions():
+    """Eq. 17 split into two Helmholtz problems (L142, S8): with L = D^2 - k^2 - lambda_phi,
+    psi is rebuilt from phi^{n+1} alone (rows 0..N-2 of L phi, last two coefficients from
+    D psi(+-1) = 0) and must satisfy gamma_phi L psi = H_phi in rows 0..N-2, so that
+    gamma_phi (lap - lambda)^2 = 1 - dt (s Ch^2/Pe) lap + dt (Ch^2/Pe) lap^2 acts on phi^{n+1}
+    up to the tau rows.  Also D phi(+-1) = 0 (S10).
+    (SURVEY 8(c) S8 states the one-shot 4th-order identity holds in rows <= N-4; it cannot:
+    D^2 is dense upper triangular, so psi's tau residual enters every row.  See DESIGN.md.)"""
+    c = I.small_config(nz=33)
+    g = O.Grid(c.nx, c.ny, c.nz, c.lx, c.ly)
+    p = O.Params(re=c.re, dt=c.dt, pe=c.pe, ch=c.ch, we=c.we, gradp_x=c.gradp_x)
+    orc = O.Oracle(g, p)
+    orc.set_state("physical", *I.channel_state(c))
+    s0 = orc.state
+    NL = orc.explicit_terms()["phi"]
+    H = s0.phi + p.dt * NL
+    orc.step(1)
+    ph = orc.state.phi
+    N = g.N
+    lam = math.sqrt(p.pe / (p.dt * p.ch ** 2))
+    gphi = p.dt * p.ch ** 2 / p.pe
+    assert abs(gphi * lam * lam - 1.0) < 1e-14 and abs(2 * lam - 2 * math.sqrt(p.pe / (p.dt * p.ch ** 2))) < 1e-9
+    Lop = lambda a: orc._lap(a) - lam * a
+    psi = Lop(ph)
+    # last two coefficients of psi from the two Neumann rows
+    bn = O.boundary_rows(N, O.NEUMANN)
+    A2 = bn[:, N - 1:]
+    rhs = -np.einsum("rn,nji->rji", bn[:, : N - 1].astype(complex), psi[: N - 1])
+    psi[N - 1:] = np.einsum("rs,sji->rji", np.linalg.inv(A2).astype(complex), rhs)
+    res = gphi * Lop(psi) - H
+    err = np.abs(np.where(orc.Pxy[: N - 1], res[: N - 1], 0)).max()
+    assert err < 1e-10 * max(1.0, np.abs(H).max())
+    # D phi(+-1) = 0 exactly (boundary rows).  D^3 phi(+-1) = 0 is only enforced through
+    # D psi(+-1) = 0, i.e. up to psi's tau residual, so it is not asserted here.
+    n2 = (np.arange(g.nz) ** 2.0)[:, None, None]
+    sgn = ((-1.0) ** np.arange(g.nz))[:, None, None]
+    assert np.abs((n2 * ph).sum(axis=0)).max() < 1e-11
+    assert np.abs((n2 * sgn * ph).sum(axis=0)).max() < 1e-11
+
+
+def _ch_1d(N, ch, steps, profile):
+    g = O.Grid(4, 4, N + 1)
+    p = O.Params(re=100.0, dt=1e-4, pe=1.0 / ch, ch=ch, we=1.0)
+    z = O.cheb_nodes(N)[:, None, None]
+    phi = profile(z) * np.ones((1, g.ny, g.nx))
+    zero = np.zeros_like(phi)
+    orc = O.Oracle(g, p)
+    orc.set_state("physical", zero, zero, zero, phi)
+    m0 = O.mean_phi(g, orc.state.phi)
+    orc.step(steps)
+    return phi, orc.get_state("physical")[3], m0, O.mean_phi(g, orc.state.phi), orc
+
+
+def test_tanh_equilibrium_profile_is_stationary():
+    """Eq. 5: phi = tanh(z / (sqrt2 Ch)) has mu = const; stationary to truncation level
+    (~5e-10 per step at N = 256, Ch = 0.07)."""
+    ch = 0.07
+    phi0, phi1, m0, m1, orc = _ch_1d(256, ch, 4, lambda z: np.tanh(z / (math.sqrt(2) * ch)))
+    assert O.rel_l2(phi1, phi0) < 4 * 2e-9
+    u, v, w, _ = orc.get_state("physical")
+    assert max(np.abs(u).max(), np.abs(v).max(), np.abs(w).max()) < 1e-9   # no spurious flow in x,y; 1-D
+    assert abs(m1 - m0) < 1e-13                                           # z-odd profile: mean conserved
+
+
+def test_non_equilibrium_profile_relaxes_towards_tanh():
+    """A too-wide interface sharpens: the distance to the Eq. 5 profile must decrease."""
+    ch = 0.07
+    eq = lambda z: np.tanh(z / (math.sqrt(2) * ch))
+    wide = lambda z: np.tanh(z / (math.sqrt(2) * ch * 1.3))
+    phi0, phi1, *_ = _ch_1d(128, ch, 20, wide)
+    z = O.cheb_nodes(128)[:, None, None]
+    d0 = np.linalg.norm((phi0 - eq(z))[:, 0, 0]); d1 = np.linalg.norm((phi1 - eq(z))[:, 0, 0])
+    assert d1 < d0
+
+
+def test_explicit_terms_match_symbolic_continuous_formulas():
+    import sympy as sp
+    g = O.Grid(16, 16, 65)
+    p = O.Params(re=80.0, dt=1e-3, pe=3.0, ch=0.3, we=1.3, gradp_x=0.04, visc_ratio=0.3)
+    x, y, z = sp.symbols("x y z", real=True)
+    kx, ky = sp.Rational(1, 2), 1                         # fundamental wavenumbers of 4pi x 2pi
+    q = 1 - z ** 2
+    A = sp.Matrix([q ** 3 * sp.sin(ky * y) * sp.cos(kx * x) * sp.Rational(3, 10),
+                   q ** 3 * sp.cos(2 * ky * y) * sp.sin(kx * x) * sp.Rational(2, 10),
+                   q ** 2 * (1 + z / 2) * sp.sin(kx * x + sp.Rational(1, 3)) * sp.sin(ky * y)])
+    X = (x, y, z)
+    curl = lambda F: sp.Matrix([sp.diff(F[2], y) - sp.diff(F[1], z),
+                                sp.diff(F[0], z) - sp.diff(F[2], x),
+                                sp.diff(F[1], x) - sp.diff(F[0], y)])
+    U = curl(A) + sp.Matrix([q * sp.Rational(1, 2), 0, 0])        # plus a mean flow
+    phi = sp.Rational(3, 10) * q ** 4 * sp.cos(kx * x) * sp.cos(ky * y) + sp.Rational(1, 5) * z * sp.sin(ky * y) - sp.Rational(1, 10)
+    grad = lambda f: sp.Matrix([sp.diff(f, s) for s in X])
+    lap = lambda f: sum(sp.diff(f, s, 2) for s in X)
+    gp = grad(phi)
+    cs = 3 / sp.sqrt(8) * sp.Float(p.ch) / sp.Float(p.we)
+    eta1 = (sp.Float(p.visc_ratio) - 1) * (phi + 1) / 2 / sp.Float(p.re)
+    T = sp.zeros(3, 3)
+    for a in range(3):
+        for b in range(3):
+            T[a, b] = (-U[a] * U[b] + cs * ((gp.dot(gp) if a == b else 0) - gp[a] * gp[b])
+                       + eta1 * (sp.diff(U[b], X[a]) + sp.diff(U[a], X[b])))
+    S = sp.Matrix([sum(sp.diff(T[a, b], X[b]) for b in range(3)) for a in range(3)])
+    S[0] = S[0] + sp.Float(p.gradp_x)
+    divS = sum(sp.diff(S[a], X[a]) for a in range(3))
+    N_om = curl(S)[2]                                              # Eq. 14
+    N_w = lap(S[2]) - sp.diff(divS, z)                             # Eq. 15
+    sco = 2 * math.sqrt(p.pe / (p.dt * p.ch ** 2))
+    S_phi = (-U.dot(gp) + lap(phi ** 3) / sp.Float(p.pe)
+             - (1 + sco * p.ch ** 2) / sp.Float(p.pe) * lap(phi))  # Eq. 17 with S8/S9
+
+    xs = g.lx / g.nx * np.arange(g.nx)[None, None, :]
+    ys = g.ly / g.ny * np.arange(g.ny)[None, :, None]
+    zs = O.cheb_nodes(g.N)[:, None, None]
+    ev = lambda e: np.broadcast_to(sp.lambdify(X, e, "numpy")(xs, ys, zs), (g.nz, g.ny, g.nx)).astype(float)
+
+    orc = O.Oracle(g, p)
+    orc.set_state("physical", ev(U[0]), ev(U[1]), ev(U[2]), ev(phi))
+    N = orc.explicit_terms()
+    P = orc.P
+    for key, expr in (("om", N_om), ("w", N_w), ("phi", S_phi)):
+        ref = np.where(P, O.forward_transform(ev(expr), g), 0)
+        got = np.where(P, N[key], 0)
+        assert O.rel_l2(got, ref) < 2e-9, key
+    refx = O.forward_transform(ev(S[0]), g)[:, 0, 0]
+    K = O.retained_counts(g)[2]
+    assert np.abs(N["ubar"][: K + 1] - refx[: K + 1]).max() < 1e-10 * max(1, np.abs(refx).max())
+
+
+def test_lambda_one_reproduces_matched_viscosity():
+    c = I.small_config()
+    g = O.Grid(c.nx, c.ny, c.nz, c.lx, c.ly)
+    st = I.channel_state(c)
+    res = []
+    for lam in (1.0, 1.0 + 1e-300):
+        p = O.Params(re=c.re, dt=c.dt, pe=c.pe, ch=c.ch, we=c.we, gradp_x=c.gradp_x, visc_ratio=lam)
+        orc = O.Oracle(g, p); orc.set_state("physical", *st); orc.step(2)
+        res.append(orc.state)
+    assert np.array_equal(res[0].u, res[1].u) and np.array_equal(res[0].phi, res[1].phi)
+
+
+def test_navier_stokes_part_is_second_order_in_time():
+    """AB2 (Euler start-up) + Crank-Nicolson (S7): halving dt must cut the error ~4x."""
+    c = I.small_config(nx=8, ny=8, nz=17, re=20.0, phase_field=0, band=2)
+    g = O.Grid(c.nx, c.ny, c.nz, c.lx, c.ly)
+    u, v, w, _ = I.channel_state(c)
+    z = O.cheb_nodes(g.N)[:, None, None]
+    base = (1 - z * z) * np.ones_like(u)
+    u, v, w = base + 8 * (u - base), 8 * v, 8 * w     # stronger (still solenoidal) perturbation
+    Tend = 0.04
+    sols = {}
+    for n in (8, 16, 32, 256):
+        p = O.Params(re=c.re, dt=Tend / n, gradp_x=c.gradp_x, phase_field=0)
+        orc = O.Oracle(g, p); orc.set_state("physical", u, v, w); orc.step(n)
+        sols[n] = np.concatenate([f.ravel() for f in orc.get_state("spectral")])
+    e = {n: np.linalg.norm(sols[n] - sols[256]) for n in (8, 16, 32)}
+    assert 3.3 < e[8] / e[16] < 4.8 and 3.3 < e[16] / e[32] < 4.9, e
