@@ -1,0 +1,134 @@
+/*
+ * libpsdns - B200-native (sm_100a, FP64) hot path of the pseudo-spectral multiphase channel
+ * solver of arXiv 2406.01322: per time step, batched backward transforms
+ * (Chebyshev in z, Fourier in y and x), pointwise non-linear terms in physical space,
+ * forward transforms with 2/3 dealiasing, and the batched per-(kx,ky) Chebyshev-tau
+ * Helmholtz / biharmonic solves of the IMEX scheme.
+ *
+ * Plain C ABI: opaque handle, POD structs, raw pointers, int status codes.  No exceptions,
+ * no printing, no abort.  The library never allocates or frees device memory: every d_*
+ * pointer and the workspace are DEVICE memory owned by the caller (e.g. torch tensors);
+ * h_* pointers are HOST memory (pinned for asynchronous copies) owned by the caller.
+ * All work is enqueued on the cudaStream_t given at init; calls return after enqueue and
+ * the caller synchronises.  A handle is not thread-safe; distinct handles are independent.
+ *
+ * Layouts at the boundary (internal layouts are private):
+ *   PSDNS_PHYSICAL : double  [nz][ny][nx]           x fastest; z index k <-> z_k = cos(pi k/(nz-1))
+ *                                                   (k = 0 is the wall z = +1; Gauss-Lobatto, L134/L178)
+ *   PSDNS_SPECTRAL : double  [nz][ny][nx/2+1][2]    interleaved complex; kx index i = 0..nx/2 fastest,
+ *                                                   ky in FFT order (0..ny/2, -ny/2+1..-1), n = Chebyshev mode
+ * Transform conventions (readings S1, S2 of DESIGN.md):
+ *   forward : f^(i,j,n) = 1/(nx ny) sum_xy f e^{-i(kx x + ky y)}, then a_n = 2/(N c_n) sum_k f_k cos(pi n k/N)/c_k
+ *   backward: f = sum f^ T_n(z_k) e^{+i(kx x + ky y)}, x real <-> half-complex (D2Z/Z2D, L176)
+ */
+#ifndef PSDNS_H
+#define PSDNS_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct psdns_handle psdns_handle; /* opaque; host memory owned by the library */
+
+/* Channel grid: nx, ny periodic equispaced points over lx, ly;
+ * nz Chebyshev-Gauss-Lobatto points on z in [-1, 1].
+ * Supported: nx, ny powers of two in [16, 1024]; nz - 1 a power of two in [8, 512]. */
+typedef struct {
+    int nx, ny, nz;
+    double lx, ly;
+} psdns_grid;
+
+/* Dimensionless groups: Re (Eq. 9), Pe (Eq. 2), Ch (L70), We (Eq. 10); time step dt.
+ * gradp_x   : constant mean forcing G added to S_x (reading S12; 2/Re keeps u = 1 - z^2 steady)
+ * visc_ratio: lambda, viscosity ratio; 1.0 = matched; != 1 evaluates the
+ *             explicit variable-viscosity stress pointwise (reading S14)
+ * phase_field: 0 = single-phase Navier-Stokes only (the Fig. 3 workload, L231), 1 = + Cahn-Hilliard
+ * dealias   : must be 1 for psdns_step (2/3 rule in x, y, z; reading S3).  The round-trip
+ *             call always runs with dealiasing off. */
+typedef struct {
+    double re, pe, ch, we, dt;
+    double gradp_x;
+    double visc_ratio;
+    int phase_field;
+    int dealias;
+} psdns_params;
+
+enum { PSDNS_PHYSICAL = 0, PSDNS_SPECTRAL = 1 };
+
+enum {
+    PSDNS_OK = 0,
+    PSDNS_EINVAL = -1, /* null pointer, unsupported size, non-positive dt/Re/..., bad enum */
+    PSDNS_ENOMEM = -2, /* workspace too small or misaligned (256 B) */
+    PSDNS_ESTATE = -3, /* step/get before set_state */
+    PSDNS_ECUDA = -4   /* CUDA launch/runtime failure; text via psdns_last_error */
+};
+
+/* Bytes of device workspace psdns_init needs for this grid/params (0 on invalid input).
+ * Holds twiddle tables, the retained-mode state (u^, v^, w^, phi^, theta^), the AB2 history,
+ * per-wavenumber solver tables, transform scratch and host-staging buffers. */
+size_t psdns_workspace_bytes(const psdns_grid *grid, const psdns_params *params);
+
+/* Create a handle.  d_workspace: device memory, >= psdns_workspace_bytes, 256-byte aligned,
+ * must outlive the handle.  cuda_stream: a cudaStream_t (NULL = default stream).  Builds the
+ * twiddle tables and the per-(kx,ky) solver factorisations (enqueued on the stream). */
+int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_workspace, size_t bytes,
+               void *cuda_stream, psdns_handle **out);
+
+/* Step i) of the time-step algorithm.  space = PSDNS_PHYSICAL: each field is
+ * forward transformed (x, then y, then z; L154).  space = PSDNS_SPECTRAL: fields are taken as
+ * given.  Only the retained (kx, ky) modes (i <= nx/3, |j'| <= ny/3) are kept; all nz Chebyshev
+ * modes are kept.  Derives the hidden state theta^ = (D^2 - k^2) w^ and clears the
+ * Adams-Bashforth history, so the next step is an explicit-Euler start (reading S7).
+ * d_phi may be NULL iff phase_field == 0.  Inputs are not modified. */
+int psdns_set_state(psdns_handle *h, int space, const void *d_u, const void *d_v, const void *d_w,
+                    const void *d_phi);
+
+/* Advance nsteps time steps (rows a1-a11 of DESIGN.md): non-linear terms by
+ * backward transforms -> pointwise products -> forward transforms with dealiasing; AB2 for the
+ * explicit terms; Crank-Nicolson Helmholtz solves for omega_z (Eq. 14) and the two-stage w problem
+ * (Eq. 15) with u^, v^ from Eqs. 6 and 16; implicit-Euler two-stage solve for phi (Eq. 17).
+ * Asynchronous on the stream. */
+int psdns_step(psdns_handle *h, int nsteps);
+
+/* Copy the state out in the requested space (outputs fully overwritten; non-retained modes are
+ * zero in PSDNS_SPECTRAL).  d_phi may be NULL iff phase_field == 0. */
+int psdns_get_state(psdns_handle *h, int space, void *d_u, void *d_v, void *d_w, void *d_phi);
+
+/* One forward+backward 3-D transform of a single field with dealiasing OFF (full sizes).
+ * start_space = PSDNS_PHYSICAL: d_in physical -> (d_mid spectral, nullable) -> d_out physical.
+ * start_space = PSDNS_SPECTRAL: d_in spectral -> (d_mid physical, nullable) -> d_out spectral.
+ * Does not touch the state. */
+int psdns_transform_roundtrip(psdns_handle *h, int start_space, const void *d_in, void *d_out,
+                              void *d_mid);
+
+/* Host-buffer convenience used for end-to-end timing: copies the four fields host->device
+ * (cudaMemcpyAsync on the stream), set_state, nsteps steps, get_state, device->host.
+ * h_in_* / h_out_* are HOST pointers in the boundary layout of `space` (phi pair may be NULL
+ * iff phase_field == 0).  The caller synchronises the stream before reading h_out_*. */
+int psdns_run_host(psdns_handle *h, int space, int nsteps, const void *h_in_u, const void *h_in_v,
+                   const void *h_in_w, const void *h_in_phi, void *h_out_u, void *h_out_v,
+                   void *h_out_w, void *h_out_phi);
+
+/* Number of kernel launches the library has enqueued on this handle since init. */
+long long psdns_launch_count(const psdns_handle *h);
+
+/* Enable (1) / disable (0) CUDA-event timing of the kernel class `name` inside psdns_step
+ * ("zbwd","ybwd","xbwd","pointwise","xfwd","yfwd","zfwd","rhs","solve", or "xfused").  When
+ * enabled, psdns_step records events on the stream around every launch of that class;
+ * psdns_kernel_time_ms returns the accumulated milliseconds and launch count after the caller
+ * has synchronised.  Used by bench.py for the roofline of the dominant kernel. */
+int psdns_kernel_timing(psdns_handle *h, const char *name, int enable);
+int psdns_kernel_time_ms(psdns_handle *h, double *ms_total, long long *launches);
+
+/* Release the handle (host memory only; the workspace stays the caller's). */
+int psdns_destroy(psdns_handle *h);
+
+/* Text of the last error on this handle ("" if none); valid until the next call. NULL-safe. */
+const char *psdns_last_error(const psdns_handle *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSDNS_H */

@@ -132,6 +132,13 @@ def cheb_deriv_matrix(N: int) -> np.ndarray:
     return D
 
 
+def apply_along(M: np.ndarray, a: np.ndarray, axis: int) -> np.ndarray:
+    """out[..., r, ...] = sum_c M[r, c] a[..., c, ...] along `axis`: one dense matrix product."""
+    M = M.astype(np.result_type(M.dtype, a.dtype), copy=False)
+    a = a.astype(M.dtype, copy=False)
+    return np.moveaxis(np.tensordot(M, a, axes=(1, axis)), 0, axis)
+
+
 # --------------------------------------------------------------------------------------
 # 3-D transforms (PAPER.md L154: x first, then y, then z on the way forward)
 # --------------------------------------------------------------------------------------
@@ -146,9 +153,9 @@ def forward_transform(f: np.ndarray, g: Grid) -> np.ndarray:
     Fx = dft_matrix(g.nx, -1)[: g.nkx, :] / g.nx          # [i, x]
     Fy = dft_matrix(g.ny, -1) / g.ny                      # [j, y]
     Cf = cheb_fwd_matrix(g.N)                             # [n, k]
-    a = f @ Fx.T                                          # [k, y, i]
-    a = np.einsum("jy,kyi->kji", Fy, a)                   # [k, j, i]
-    a = np.einsum("nk,kji->nji", Cf.astype(np.complex128), a)
+    a = apply_along(Fx, f, 2)                             # [k, y, i]
+    a = apply_along(Fy, a, 1)                             # [k, j, i]
+    a = apply_along(Cf, a, 0)                             # [n, j, i]
     return a
 
 
@@ -160,8 +167,8 @@ def backward_transform(a: np.ndarray, g: Grid) -> np.ndarray:
     assert a.shape == (g.nz, g.ny, g.nkx)
     Cb = cheb_bwd_matrix(g.N)
     By = dft_matrix(g.ny, +1)                             # [y, j]
-    b = np.einsum("kn,nji->kji", Cb.astype(np.complex128), a)
-    b = np.einsum("yj,kji->kyi", By, b)                   # [k, y, i]
+    b = apply_along(Cb, a, 0)                             # [k, j, i]
+    b = apply_along(By, b, 1)                             # [k, y, i]
     i = np.arange(g.nkx)
     x = np.arange(g.nx)
     w = np.full(g.nkx, 2.0)
@@ -366,10 +373,10 @@ class Oracle:
 
     # -- helpers ------------------------------------------------------------------------
     def _Dz(self, a):
-        return np.einsum("np,pji->nji", self.D.astype(np.complex128), a)
+        return apply_along(self.D, a, 0)
 
     def _D2z(self, a):
-        return np.einsum("np,pji->nji", self.D2.astype(np.complex128), a)
+        return apply_along(self.D2, a, 0)
 
     def _lap(self, a):
         return self._D2z(a) - self.K2 * a
@@ -530,7 +537,7 @@ class Oracle:
 def divergence_spectrum(g: Grid, u, v, w):
     kx, ky = wavenumbers(g)
     D = cheb_deriv_matrix(g.N).astype(np.complex128)
-    return 1j * kx[None, None, :] * u + 1j * ky[None, :, None] * v + np.einsum("np,pji->nji", D, w)
+    return 1j * kx[None, None, :] * u + 1j * ky[None, :, None] * v + apply_along(D, w, 0)
 
 
 def mean_phi(g: Grid, phi_hat):

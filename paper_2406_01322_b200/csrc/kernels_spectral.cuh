@@ -1,0 +1,452 @@
+// Spectral-space kernels: one thread per retained (kx, ky) column, sweeping the Chebyshev index
+// n sequentially; consecutive threads own consecutive columns so every access is coalesced.
+//   k_relayout   boundary <-> private spectral layouts
+//   k_lap        theta = (D^2 - k^2) w                         (hidden state, reading S13)
+//   k_prep       row a1: grad(phi) spectra [+ strain spectra]
+//   k_rhs        row a9: S = div T, N_omega (Eq. 14), N_w (Eq. 15), S_phi (Eq. 17), AB2, CN/IE
+//                right-hand sides, all derivative recurrences fused in ONE downward sweep
+//   k_helm_setup / k_helm   row a10: quasi-tridiagonal Chebyshev-tau Helmholtz solve
+//   k_infl       row a10: influence-matrix closure of the w problem (Dw(+-1) = 0)
+//   k_finish     row a11: u^, v^ from continuity (Eq. 6) and the vorticity definition (Eq. 16)
+#pragma once
+#include "fft_tile.cuh"
+
+namespace psdns {
+
+constexpr int NT_COL = 128;
+
+struct ColGeom {
+    int ncols;   // nky * kxp
+    int kxp, nkx, nky, jpos;
+    int N;       // nz - 1
+    int nkz;     // retained Chebyshev planes (K + 1)
+    double kxf, kyf;  // 2 pi / Lx, 2 pi / Ly
+};
+
+__device__ __forceinline__ void col_wavenumbers(const ColGeom &g, int col, double &kx, double &ky) {
+    const int ir = col % g.kxp, jr = col / g.kxp;
+    kx = g.kxf * (double)ir;   // pad columns (ir >= nkx) carry zeros; their k is irrelevant
+    ky = g.kyf * (double)(jr < g.jpos ? jr : jr - g.nky);
+}
+
+__device__ __forceinline__ cplx cz() { return make_double2(0.0, 0.0); }
+__device__ __forceinline__ cplx ci(cplx a) { return make_double2(-a.y, a.x); }           // i * a
+__device__ __forceinline__ cplx cfma(double s, cplx a, cplx b) {                          // s*a + b
+    return make_double2(fma(s, a.x, b.x), fma(s, a.y, b.y));
+}
+
+// ---- layout conversion ---------------------------------------------------------------------
+// Both sides are cplx [n][rows][pitch]; a side is described by (rows, pitch, jpos, nkx):
+// row r < jpos holds j' = r, row r >= jpos holds j' = r - rows; columns i < nkx are valid.
+struct SpecSide {
+    int rows, pitch, jpos, nkx;
+};
+
+__global__ void __launch_bounds__(256) k_relayout(cplx *__restrict__ dst, const cplx *__restrict__ src,
+                                                  SpecSide d, SpecSide s, int nplanes) {
+    const size_t total = (size_t)nplanes * d.rows * d.pitch;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += stride) {
+        const int i = (int)(e % d.pitch);
+        const size_t t = e / d.pitch;
+        const int r = (int)(t % d.rows);
+        const int n = (int)(t / d.rows);
+        cplx v = cz();
+        if (i < d.nkx && i < s.nkx) {
+            const int jp = r < d.jpos ? r : r - d.rows;
+            int rs = -1;
+            if (jp >= 0) { if (jp < s.jpos) rs = jp; }
+            else { if (s.rows + jp >= s.jpos) rs = s.rows + jp; }
+            if (rs >= 0) v = src[((size_t)n * s.rows + rs) * s.pitch + i];
+        }
+        dst[e] = v;
+    }
+}
+
+// ---- theta = (D^2 - k^2) w ---------------------------------------------------------------------
+// Chebyshev derivative recurrence: ct_n b_n = b_{n+2} + 2 (n+1) a_{n+1}, ct_0 = 2.
+__global__ void __launch_bounds__(NT_COL) k_lap(const __grid_constant__ ColGeom g, const cplx *__restrict__ w,
+                                                cplx *__restrict__ th) {
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const double k2 = kx * kx + ky * ky;
+    const size_t st = g.ncols;
+    cplx a1 = cz(), b1 = cz(), b2 = cz(), c1 = cz(), c2 = cz();
+    for (int n = g.N; n >= 0; --n) {
+        const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
+        const cplx an = w[n * st + col];
+        cplx bn = cscale(cfma(f, a1, b2), h);
+        cplx cn = cscale(cfma(f, b1, c2), h);
+        th[n * st + col] = cfma(-k2, an, cn);
+        a1 = an; b2 = b1; b1 = bn; c2 = c1; c1 = cn;
+    }
+}
+
+// ---- row a1: derived spectra for the backward transforms -----------------------------------------
+struct PrepArgs {
+    ColGeom g;
+    const cplx *u, *v, *w, *phi;
+    cplx *phx, *phy, *phz;
+    cplx *exx, *eyy, *exy, *exz, *eyz;
+    int phase, visc;
+};
+
+__global__ void __launch_bounds__(NT_COL) k_prep(const __grid_constant__ PrepArgs a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const size_t st = g.ncols;
+    cplx p1 = cz(), dp1 = cz(), dp2 = cz();
+    cplx u1 = cz(), du1 = cz(), du2 = cz(), v1 = cz(), dv1 = cz(), dv2 = cz();
+    for (int n = g.nkz - 1; n >= 0; --n) {
+        const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
+        const size_t o = n * st + col;
+        if (a.phase) {
+            const cplx pn = a.phi[o];
+            const cplx dpn = cscale(cfma(f, p1, dp2), h);
+            a.phx[o] = cscale(ci(pn), kx);
+            a.phy[o] = cscale(ci(pn), ky);
+            a.phz[o] = dpn;
+            p1 = pn; dp2 = dp1; dp1 = dpn;
+        }
+        if (a.visc) {
+            const cplx un = a.u[o], vn = a.v[o], wn = a.w[o];
+            const cplx dun = cscale(cfma(f, u1, du2), h);
+            const cplx dvn = cscale(cfma(f, v1, dv2), h);
+            a.exx[o] = cscale(ci(un), 2.0 * kx);
+            a.eyy[o] = cscale(ci(vn), 2.0 * ky);
+            a.exy[o] = cadd(cscale(ci(un), ky), cscale(ci(vn), kx));
+            a.exz[o] = cadd(dun, cscale(ci(wn), kx));
+            a.eyz[o] = cadd(dvn, cscale(ci(wn), ky));
+            u1 = un; du2 = du1; du1 = dun;
+            v1 = vn; dv2 = dv1; dv1 = dvn;
+        }
+    }
+}
+
+// ---- row a9: explicit terms + IMEX right-hand sides ----------------------------------------------
+struct RhsArgs {
+    ColGeom g;
+    const cplx *txx, *txy, *txz, *tyy, *tyz, *tzz, *q, *c;  // product spectra [nkz][ncols]
+    const cplx *u, *v;                                          // state [nz][ncols]
+    cplx *th, *phi;        // in: theta^n, phi^n ; out: H_w, H_phi (in place)
+    cplx *xom;             // out: H_omega
+    cplx *h_om, *h_w, *h_phi;   // AB2 history [nkz][ncols], in place
+    const double *ab;      // device: {ab0, ab1}
+    double dt, gamma, inv_pe, e_phi;   // e_phi = 1 + s Ch^2
+    double gradp;
+    int phase;
+};
+
+struct Chain1 {  // first derivative of a sequence fed top-down
+    cplx a1, b1, b2;
+    __device__ __forceinline__ void init() { a1 = b1 = b2 = cz(); }
+    __device__ __forceinline__ cplx step(cplx an, double f, double h) {
+        cplx bn = cscale(cfma(f, a1, b2), h);
+        a1 = an; b2 = b1; b1 = bn;
+        return bn;
+    }
+};
+struct Chain2 {  // second derivative
+    cplx a1, b1, b2, c1, c2;
+    __device__ __forceinline__ void init() { a1 = b1 = b2 = c1 = c2 = cz(); }
+    __device__ __forceinline__ cplx step(cplx an, double f, double h) {
+        cplx bn = cscale(cfma(f, a1, b2), h);
+        cplx cn = cscale(cfma(f, b1, c2), h);
+        a1 = an; b2 = b1; b1 = bn; c2 = c1; c1 = cn;
+        return cn;
+    }
+};
+
+__global__ void __launch_bounds__(NT_COL) k_rhs(const __grid_constant__ RhsArgs a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const double k2 = kx * kx + ky * ky;
+    const bool mean = (col == 0);
+    const size_t st = g.ncols;
+    const double ab0 = a.ab[0], ab1 = a.ab[1];
+    const double dt = a.dt, gam = a.gamma;
+    Chain1 cR, cB;
+    Chain2 cA, cE, cOm, cTh;
+    cR.init(); cB.init(); cA.init(); cE.init(); cOm.init(); cTh.init();
+    for (int n = g.N; n >= 0; --n) {
+        const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
+        const size_t o = n * st + col;
+        const bool low = n < g.nkz;
+        const cplx un = a.u[o], vn = a.v[o];
+        const cplx thn = mean ? vn : a.th[o];
+        const cplx omn = mean ? un : ci(csub(cscale(vn, kx), cscale(un, ky)));
+        cplx P = cz(), R = cz(), A = cz(), B = cz(), E = cz(), Q = cz();
+        cplx phn = cz();
+        if (a.phase) phn = a.phi[o];
+        if (low) {
+            const cplx txx = a.txx[o], txy = a.txy[o], txz = a.txz[o], tyy = a.tyy[o], tyz = a.tyz[o], tzz = a.tzz[o];
+            if (mean) {
+                R = txz;
+                B = tyz;
+            } else {
+                P = cadd(cscale(txy, ky * ky - kx * kx), cscale(csub(txx, tyy), kx * ky));
+                R = ci(csub(cscale(tyz, kx), cscale(txz, ky)));
+                A = ci(cadd(cscale(txz, kx), cscale(tyz, ky)));
+                B = cadd(cadd(cscale(txx, kx * kx), cscale(txy, 2.0 * kx * ky)), csub(cscale(tyy, ky * ky), cscale(tzz, k2)));
+            }
+            if (a.phase) {
+                Q = a.q[o];
+                E = cscale(cfma(-a.e_phi, phn, a.c[o]), a.inv_pe);
+            }
+        }
+        const cplx dR = cR.step(R, f, h);
+        const cplx dB = cB.step(B, f, h);
+        const cplx ddA = cA.step(A, f, h);
+        const cplx ddOm = cOm.step(omn, f, h);
+        const cplx ddTh = cTh.step(thn, f, h);
+        cplx n_om = cadd(P, dR);
+        if (mean && n == 0) n_om.x += a.gradp;
+        const cplx n_w = cadd(csub(dB, ddA), cscale(A, -k2));
+        cplx nl_om = cscale(n_om, ab0), nl_w = cscale(n_w, ab0);
+        if (low) {
+            nl_om = cfma(ab1, a.h_om[o], nl_om);
+            nl_w = cfma(ab1, a.h_w[o], nl_w);
+            a.h_om[o] = n_om;
+            a.h_w[o] = n_w;
+        }
+        // Crank-Nicolson right-hand sides H = x + gamma (D^2 - k^2) x + dt NL
+        a.xom[o] = cfma(dt, nl_om, cfma(gam, cfma(-k2, omn, ddOm), omn));
+        a.th[o] = cfma(dt, nl_w, cfma(gam, cfma(-k2, thn, ddTh), thn));
+        if (a.phase) {
+            const cplx ddE = cE.step(E, f, h);
+            const cplx s_phi = csub(cfma(-k2, E, ddE), Q);
+            cplx nl_phi = cscale(s_phi, ab0);
+            if (low) {
+                nl_phi = cfma(ab1, a.h_phi[o], nl_phi);
+                a.h_phi[o] = s_phi;
+            }
+            a.phi[o] = cfma(dt, nl_phi, phn);   // implicit Euler: H_phi = phi + dt NL
+        }
+    }
+}
+
+// ---- row a10: quasi-tridiagonal Chebyshev-tau Helmholtz solve ---------------------------------------
+// (D^2 - sigma) u = f in rows 0..N-2 plus two boundary rows (reading S11).  In coefficient space,
+// for k = 2..N (even and odd k decouple):
+//   a_k u_{k-2} + d_k u_k + c_k u_{k+2} = p_k f_{k-2} + q_k f_k + r_k f_{k+2} =: g_k
+//   p_k = ct_{k-2}/(4k(k-1)), q_k = -1/(2(k^2-1)), r_k = 1/(4k(k+1)), f_j := 0 for j > N-2,
+//   a_k = -sigma p_k, d_k = 1 + sigma e_{k+2}/(2(k^2-1)), c_k = -sigma e_{k+4}/(4k(k+1)), e_j = [j <= N].
+// Gauss elimination from k = N down removes c_k (pivots d'_k, stored as 1/d'_k by k_helm_setup);
+// the remaining lower-bidiagonal rows give u_k = alpha_k + beta_k u_par (par = k & 1), and the
+// boundary row of each parity fixes u_par.
+__device__ __forceinline__ double helm_p(int k) { return (k == 2 ? 2.0 : 1.0) / (4.0 * k * (double)(k - 1)); }
+__device__ __forceinline__ double helm_q(int k) { return -1.0 / (2.0 * ((double)k * k - 1.0)); }
+__device__ __forceinline__ double helm_r(int k) { return 1.0 / (4.0 * k * (double)(k + 1)); }
+
+struct HelmSetupArgs {
+    ColGeom g;
+    double *dinv;   // [N+1][ncols]
+    double shift;   // sigma = k^2 + shift
+};
+
+__global__ void __launch_bounds__(NT_COL) k_helm_setup(const __grid_constant__ HelmSetupArgs a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const double sigma = kx * kx + ky * ky + a.shift;
+    const size_t st = g.ncols;
+    const int N = g.N;
+    double di1 = 0.0, di2 = 0.0;  // 1/d'_{k+1}, 1/d'_{k+2}
+    for (int k = N; k >= 2; --k) {
+        double d = 1.0 + ((k + 2 <= N) ? sigma * (-helm_q(k)) : 0.0);
+        if (k + 4 <= N) {
+            const double ck = -sigma * helm_r(k);
+            const double ak2 = -sigma * helm_p(k + 2);
+            d -= ck * ak2 * di2;
+        }
+        const double di = 1.0 / d;
+        a.dinv[k * st + col] = di;
+        di2 = di1; di1 = di;
+    }
+    a.dinv[col] = 0.0;
+    a.dinv[st + col] = 0.0;
+}
+
+enum { BC_DIRICHLET = 0, BC_NEUMANN = 1 };
+
+struct HelmArgs {
+    ColGeom g;
+    const cplx *in;   // f (rows 0..N-2 used)
+    cplx *out;        // solution (may alias in)
+    const double *dinv;
+    double shift, scale;   // sigma = k^2 + shift ; f is multiplied by scale
+    int bc;
+    double tgt_e, tgt_o;   // boundary-row targets of the even / odd parity (0 in the time step)
+};
+
+__global__ void __launch_bounds__(NT_COL) k_helm(const __grid_constant__ HelmArgs a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const double sigma = kx * kx + ky * ky + a.shift;
+    const size_t st = g.ncols;
+    const int N = g.N;
+    const cplx *__restrict__ in = a.in + col;
+    cplx *__restrict__ out = a.out + col;
+    const double *__restrict__ dinv = a.dinv + col;
+    const double sc = a.scale;
+    // sweep 1 (down): g'_k = g_k - (c_k / d'_{k+2}) g'_{k+2}
+    {
+        cplx fp2 = cz(), fp1 = cz();
+        cplx f0 = cz(), fm1 = cz();   // f_N = f_{N-1} := 0
+        cplx gp2 = cz(), gp1 = cz();
+        double dp2 = 0.0, dp1 = 0.0;
+#pragma unroll 4
+        for (int k = N; k >= 2; --k) {
+            const cplx fm2 = cscale(in[(k - 2) * st], sc);
+            const double di = dinv[k * st];
+            cplx gk = cfma(helm_p(k), fm2, cfma(helm_q(k), f0, cscale(fp2, helm_r(k))));
+            if (k + 4 <= N) {
+                const double m = -sigma * helm_r(k) * dp2;
+                gk = cfma(-m, gp2, gk);
+            }
+            out[k * st] = gk;
+            gp2 = gp1; gp1 = gk;
+            dp2 = dp1; dp1 = di;
+            fp2 = fp1; fp1 = f0; f0 = fm1; fm1 = fm2;
+        }
+    }
+    // sweep 2 (up): alpha_k, beta_k, boundary sums
+    const bool neu = a.bc == BC_NEUMANN;
+    cplx sa_e = cz(), sa_o = cz();
+    double sb_e = neu ? 0.0 : 1.0, sb_o = 1.0;
+    {
+        cplx al2 = cz(), al1 = cz();   // alpha_{k-2}, alpha_{k-1}
+        double be2 = 1.0, be1 = 1.0;
+#pragma unroll 4
+        for (int k = 2; k <= N; ++k) {
+            const double ak = -sigma * helm_p(k);
+            const double di = dinv[k * st];
+            const cplx gk = out[k * st];
+            const cplx al = cscale(cfma(-ak, al2, gk), di);
+            const double be = -ak * be2 * di;
+            out[k * st] = al;
+            const double wk = neu ? (double)k * k : 1.0;
+            if (k & 1) { sa_o = cfma(wk, al, sa_o); sb_o += wk * be; }
+            else       { sa_e = cfma(wk, al, sa_e); sb_e += wk * be; }
+            al2 = al1; al1 = al;
+            be2 = be1; be1 = be;
+        }
+    }
+    // Dirichlet: sum_even u = tgt_e, sum_odd u = tgt_o.  Neumann: sum_even k^2 u = tgt_e, sum_odd k^2 u = tgt_o.
+    const cplx u0 = cscale(make_double2(a.tgt_e - sa_e.x, -sa_e.y), 1.0 / sb_e);
+    const cplx u1 = cscale(make_double2(a.tgt_o - sa_o.x, -sa_o.y), 1.0 / sb_o);
+    // sweep 3 (up): u_k = alpha_k + beta_k u_par
+    {
+        double be2 = 1.0, be1 = 1.0;
+        out[0] = u0;
+        out[st] = u1;
+#pragma unroll 4
+        for (int k = 2; k <= N; ++k) {
+            const double ak = -sigma * helm_p(k);
+            const double be = -ak * be2 * dinv[k * st];
+            const cplx al = out[k * st];
+            out[k * st] = cfma(be, (k & 1) ? u1 : u0, al);
+            be2 = be1; be1 = be;
+        }
+    }
+}
+
+// ---- influence-matrix closure of the w problem -----------------------------------------------------
+// theta = theta_p + A_par theta_h, w = w_p + A_par w_h with A_par chosen so that
+// sum_{k in parity} k^2 w_k = 0 for both parities  <=>  Dw(+1) = Dw(-1) = 0 (reading S10/S11).
+struct InflArgs {
+    ColGeom g;
+    cplx *th, *w;
+    const cplx *thh, *wh;   // homogeneous solutions (real, stored as cplx with zero imaginary part)
+};
+
+__global__ void __launch_bounds__(NT_COL) k_infl(const __grid_constant__ InflArgs a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols || col == 0) return;
+    const size_t st = g.ncols;
+    const int N = g.N;
+    cplx se = cz(), so = cz();
+    double he = 0.0, ho = 0.0;
+    for (int k = 1; k <= N; ++k) {
+        const double wk = (double)k * k;
+        const cplx wp = a.w[k * st + col];
+        const double wh = a.wh[k * st + col].x;
+        if (k & 1) { so = cfma(wk, wp, so); ho += wk * wh; }
+        else       { se = cfma(wk, wp, se); he += wk * wh; }
+    }
+    const cplx Ae = cscale(se, -1.0 / he), Ao = cscale(so, -1.0 / ho);
+    for (int k = 0; k <= N; ++k) {
+        const size_t o = k * st + col;
+        const cplx A = (k & 1) ? Ao : Ae;
+        const double th = a.thh[o].x, wh = a.wh[o].x;
+        a.th[o] = cfma(th, A, a.th[o]);
+        a.w[o] = cfma(wh, A, a.w[o]);
+    }
+}
+
+// ---- row a11: velocity recovery ------------------------------------------------------------------------
+struct FinishArgs {
+    ColGeom g;
+    const cplx *xom;   // omega_z^{n+1} (column 0: u-bar^{n+1})
+    cplx *u, *v, *w, *th;
+};
+
+__global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ FinishArgs a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    const size_t st = g.ncols;
+    if (col == 0) {   // mean flow: u-bar from the omega slot, v-bar from the theta slot, w = theta = 0
+        for (int n = 0; n <= g.N; ++n) {
+            const size_t o = n * st;
+            a.u[o] = a.xom[o];
+            a.v[o] = a.th[o];
+            a.w[o] = cz();
+            a.th[o] = cz();
+        }
+        return;
+    }
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const double k2 = kx * kx + ky * ky;
+    const double ik2 = (col % g.kxp < g.nkx) ? 1.0 / k2 : 0.0;
+    Chain1 cW;
+    cW.init();
+    for (int n = g.N; n >= 0; --n) {
+        const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
+        const size_t o = n * st + col;
+        const cplx dw = cW.step(a.w[o], f, h);
+        const cplx om = a.xom[o];
+        a.u[o] = cscale(ci(cadd(cscale(dw, kx), cscale(om, ky))), ik2);
+        a.v[o] = cscale(ci(csub(cscale(dw, ky), cscale(om, kx))), ik2);
+    }
+}
+
+// ---- per-step bookkeeping ---------------------------------------------------------------------------
+__global__ void k_begin_step(double *ab, int *counter) {
+    // reading S7: explicit Euler on the first step after set_state, AB2 afterwards
+    if (*counter == 0) { ab[0] = 1.0; ab[1] = 0.0; }
+    else               { ab[0] = 1.5; ab[1] = -0.5; }
+    *counter += 1;
+}
+
+__global__ void k_set_real(cplx *dst, size_t n, double re) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) dst[i] = make_double2(re, 0.0);
+}
+
+}  // namespace psdns

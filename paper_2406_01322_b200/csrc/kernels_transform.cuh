@@ -1,0 +1,260 @@
+// Batched 1-D transform passes over the private device layouts, and the pointwise kernel.
+//
+// Private layouts (x / kx fastest everywhere, never transposed):
+//   spectral  S : cplx [n ][jr][ir]   n < nk planes, jr < nky retained ky rows, ir < kxp (padded pitch)
+//   z-physical Z: cplx [k ][jr][ir]   k <= N wall-normal points
+//   zy-physical Y: cplx [k ][y ][ir]
+//   physical   P: double [k][y][x]
+// A z- or y-pass CTA owns a tile of 8 consecutive ir (one aligned 128-byte segment per row) and
+// the whole line in the transform direction; an x-pass CTA owns 16 consecutive (k,y) lines, two
+// real lines packed into one complex FFT.  This replaces the paper's transposes (L178) and MPI
+// pencil all-to-alls (L154) by strided 128-byte-row accesses of one resident array.
+#pragma once
+#include "fft_tile.cuh"
+
+namespace psdns {
+
+constexpr int MAXF = 12;      // max fields per batched launch
+constexpr int NT_FFT = 256;   // threads per transform CTA
+
+struct FieldPtrs {
+    const void *in[MAXF];
+    void *out[MAXF];
+};
+
+template <int L>
+__device__ __forceinline__ void load_twiddles(cplx *tw, const cplx *__restrict__ twg, int tid, int nt) {
+    for (int i = tid; i < L; i += nt) tw[i] = twg[i];
+}
+
+// ------------------------------------------------------------------------------------------
+// z pass: Chebyshev transform = DCT-I as the length-2N FFT of the even extension,
+// Re and Im transformed together (the DFT of a real-even sequence is real).
+//   backward (row a2): a_n, n < nk  ->  f_k = sum_n a_n cos(pi n k / N), k = 0..N
+//   forward  (row a8): f_k          ->  a_n = 1/(N c_n) DFT_n(even ext), n < nk (truncation)
+// grid = (ncols/8, nfields); L = 2N.
+// ------------------------------------------------------------------------------------------
+struct ZArgs {
+    FieldPtrs f;
+    int ncols;  // nky * kxp (multiple of 8) = plane stride in cplx
+    int nk;     // coefficient planes read (backward) or written (forward)
+};
+
+template <int L, bool FWD>
+__global__ void __launch_bounds__(NT_FFT) k_zpass(const __grid_constant__ ZArgs a, const cplx *__restrict__ twg) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx *s = reinterpret_cast<cplx *>(smem_raw);
+    cplx *tw = s + L * TILE_LINES;
+    constexpr int N = L / 2;
+    const int tid = threadIdx.x, line = tid & 7, r0 = tid >> 3;
+    constexpr int RSTEP = NT_FFT / TILE_LINES;
+    const size_t stride = (size_t)a.ncols;
+    const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[blockIdx.y]) + (size_t)blockIdx.x * 8 + line;
+    cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[blockIdx.y]) + (size_t)blockIdx.x * 8 + line;
+    load_twiddles<L>(tw, twg, tid, NT_FFT);
+    if (!FWD) {
+        const int nk = a.nk;
+        for (int n = r0; n <= N; n += RSTEP) {
+            cplx v = make_double2(0.0, 0.0);
+            if (n < nk) v = in[n * stride];
+            if (n > 0 && n < N) {
+                v = cscale(v, 0.5);
+                s[(L - n) * TILE_LINES + line] = v;
+            }
+            s[n * TILE_LINES + line] = v;
+        }
+    } else {
+        for (int k = r0; k <= N; k += RSTEP) {
+            cplx v = in[k * stride];
+            if (k > 0 && k < N) s[(L - k) * TILE_LINES + line] = v;
+            s[k * TILE_LINES + line] = v;
+        }
+    }
+    __syncthreads();
+    fft_tile<L, -1, NT_FFT>(s, tw, tid);
+    __syncthreads();
+    if (!FWD) {
+        for (int k = r0; k <= N; k += RSTEP) out[k * stride] = s[fft_pos<L>(k) * TILE_LINES + line];
+    } else {
+        const int nk = a.nk;
+        const double sc = 1.0 / N;
+        for (int n = r0; n < nk; n += RSTEP) {
+            cplx v = s[fft_pos<L>(n) * TILE_LINES + line];
+            out[n * stride] = cscale(v, (n == 0 || n == N) ? 0.5 * sc : sc);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// y pass: complex <-> complex DFT of length ny per (ir, k) line (Z2Z).
+//   backward (row a3): nky retained rows (FFT order compacted) -> ny points, e^{+i ky y}
+//   forward  (row a7): ny points -> nky retained rows, e^{-i ky y} / ny
+// grid = (kxp/8, nz, nfields); L = ny.
+// ------------------------------------------------------------------------------------------
+struct YArgs {
+    FieldPtrs f;
+    int kxp;   // row pitch in cplx (multiple of 8)
+    int nky;   // retained ky rows
+    int jpos;  // rows 0..jpos-1 are j' = jr >= 0; rows jpos.. are j' = jr - nky < 0
+};
+
+template <int L, bool FWD>
+__global__ void __launch_bounds__(NT_FFT) k_ypass(const __grid_constant__ YArgs a, const cplx *__restrict__ twg) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx *s = reinterpret_cast<cplx *>(smem_raw);
+    cplx *tw = s + L * TILE_LINES;
+    const int tid = threadIdx.x, line = tid & 7, r0 = tid >> 3;
+    constexpr int RSTEP = NT_FFT / TILE_LINES;
+    const size_t pitch = (size_t)a.kxp;
+    const int nky = a.nky, jpos = a.jpos;
+    const size_t zin = (size_t)blockIdx.y * (FWD ? L : nky) * pitch;
+    const size_t zout = (size_t)blockIdx.y * (FWD ? nky : L) * pitch;
+    const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[blockIdx.z]) + zin + (size_t)blockIdx.x * 8 + line;
+    cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[blockIdx.z]) + zout + (size_t)blockIdx.x * 8 + line;
+    load_twiddles<L>(tw, twg, tid, NT_FFT);
+    if (!FWD) {
+        for (int j = r0; j < L; j += RSTEP) {
+            // FFT-order row j holds j' = j (j < jpos) or j' = j - L (j >= L - (nky - jpos))
+            cplx v = make_double2(0.0, 0.0);
+            if (j < jpos) v = in[j * pitch];
+            else if (j >= L - (nky - jpos)) v = in[(j - (L - nky)) * pitch];
+            s[j * TILE_LINES + line] = v;
+        }
+    } else {
+        for (int y = r0; y < L; y += RSTEP) s[y * TILE_LINES + line] = in[y * pitch];
+    }
+    __syncthreads();
+    fft_tile<L, (FWD ? -1 : +1), NT_FFT>(s, tw, tid);
+    __syncthreads();
+    if (!FWD) {
+        for (int y = r0; y < L; y += RSTEP) out[y * pitch] = s[fft_pos<L>(y) * TILE_LINES + line];
+    } else {
+        const double sc = 1.0 / L;
+        for (int jr = r0; jr < nky; jr += RSTEP) {
+            const int j = jr < jpos ? jr : jr + (L - nky);
+            out[jr * pitch] = cscale(s[fft_pos<L>(j) * TILE_LINES + line], sc);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// x pass: real <-> half-complex DFT of length nx per (k, y) line (D2Z / Z2D).
+// Two real lines A, B ride one complex FFT: z = a + i b.
+//   backward (row a4): Z_i = A^_i + i B^_i, Z_{L-i} = conj(A^_i) + i conj(B^_i); the imaginary
+//                      parts of the i = 0 and i = L/2 coefficients are dropped (reading S20)
+//   forward  (row a6): A^_i = (Z_i + conj Z_{L-i})/2, B^_i = (Z_i - conj Z_{L-i})/(2i), times 1/nx,
+//                      only i < nkx kept (truncation), pad columns written as zero
+// grid = (nlines/16, nfields); L = nx; lines are the flattened (k, y) index.
+// ------------------------------------------------------------------------------------------
+struct XArgs {
+    FieldPtrs f;
+    int kxp;  // spectral row pitch
+    int nkx;  // retained kx (<= L/2 + 1)
+};
+
+template <int L, bool FWD>
+__global__ void __launch_bounds__(NT_FFT) k_xpass(const __grid_constant__ XArgs a, const cplx *__restrict__ twg) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx *s = reinterpret_cast<cplx *>(smem_raw);
+    cplx *tw = s + L * TILE_LINES;
+    const int tid = threadIdx.x, p = tid & 7, r0 = tid >> 3;
+    constexpr int RSTEP = NT_FFT / TILE_LINES;
+    const size_t lineA = (size_t)blockIdx.x * 16 + 2 * p;
+    const int kxp = a.kxp, nkx = a.nkx;
+    load_twiddles<L>(tw, twg, tid, NT_FFT);
+    if (!FWD) {
+        const cplx *__restrict__ inA = reinterpret_cast<const cplx *>(a.f.in[blockIdx.y]) + lineA * kxp;
+        const cplx *__restrict__ inB = inA + kxp;
+        for (int i = r0; i <= L / 2; i += RSTEP) {
+            cplx ca = make_double2(0.0, 0.0), cb = ca;
+            if (i < nkx) { ca = inA[i]; cb = inB[i]; }
+            if (i == 0 || i == L / 2) {
+                s[i * TILE_LINES + p] = make_double2(ca.x, cb.x);
+            } else {
+                s[i * TILE_LINES + p] = make_double2(ca.x - cb.y, ca.y + cb.x);
+                s[(L - i) * TILE_LINES + p] = make_double2(ca.x + cb.y, cb.x - ca.y);
+            }
+        }
+        __syncthreads();
+        fft_tile<L, +1, NT_FFT>(s, tw, tid);
+        __syncthreads();
+        double *__restrict__ outA = reinterpret_cast<double *>(a.f.out[blockIdx.y]) + lineA * L;
+        double *__restrict__ outB = outA + L;
+        for (int x = r0; x < L; x += RSTEP) {
+            cplx v = s[fft_pos<L>(x) * TILE_LINES + p];
+            outA[x] = v.x;
+            outB[x] = v.y;
+        }
+    } else {
+        const double *__restrict__ inA = reinterpret_cast<const double *>(a.f.in[blockIdx.y]) + lineA * L;
+        const double *__restrict__ inB = inA + L;
+        for (int x = r0; x < L; x += RSTEP) s[x * TILE_LINES + p] = make_double2(inA[x], inB[x]);
+        __syncthreads();
+        fft_tile<L, -1, NT_FFT>(s, tw, tid);
+        __syncthreads();
+        cplx *__restrict__ outA = reinterpret_cast<cplx *>(a.f.out[blockIdx.y]) + lineA * kxp;
+        cplx *__restrict__ outB = outA + kxp;
+        const double sc = 0.5 / L;
+        for (int i = r0; i < kxp; i += RSTEP) {
+            cplx ra = make_double2(0.0, 0.0), rb = ra;
+            if (i < nkx) {
+                cplx z1 = s[fft_pos<L>(i) * TILE_LINES + p];
+                cplx z2 = s[fft_pos<L>((L - i) & (L - 1)) * TILE_LINES + p];
+                // A^ = (z1 + conj z2)/2 ; B^ = (z1 - conj z2)/(2i) = (-i/2)(z1 - conj z2)
+                ra = make_double2((z1.x + z2.x) * sc, (z1.y - z2.y) * sc);
+                rb = make_double2((z1.y + z2.y) * sc, (z2.x - z1.x) * sc);
+            }
+            outA[i] = ra;
+            outB[i] = rb;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// pointwise non-linear terms (row a5; Eqs. 1, 4, 7, 8 and L182-196), in place:
+//   in : u v w [phi phx phy phz [exx eyy exy exz eyz]]     (buffers 0..11)
+//   out: Txx Txy Txz Tyy Tyz Tzz [Q C]                     (buffers 0..7)
+//   T_ij = -u_i u_j + cs (|grad phi|^2 delta_ij - phi_i phi_j) + eta1(phi) E_ij
+// ------------------------------------------------------------------------------------------
+struct PwArgs {
+    double *b[MAXF];
+    size_t n;
+    double cs;        // 3/sqrt(8) Ch/We
+    double eta_c;     // (lambda - 1) / (2 Re)
+    int phase, visc;
+};
+
+__global__ void __launch_bounds__(256) k_pointwise(const __grid_constant__ PwArgs a) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += stride) {
+        const double u = a.b[0][i], v = a.b[1][i], w = a.b[2][i];
+        double txx = -u * u, txy = -u * v, txz = -u * w, tyy = -v * v, tyz = -v * w, tzz = -w * w;
+        if (a.phase) {
+            const double ph = a.b[3][i], px = a.b[4][i], py = a.b[5][i], pz = a.b[6][i];
+            const double g2 = px * px + py * py + pz * pz;
+            const double cs = a.cs;
+            txx += cs * (g2 - px * px);
+            tyy += cs * (g2 - py * py);
+            tzz += cs * (g2 - pz * pz);
+            txy -= cs * px * py;
+            txz -= cs * px * pz;
+            tyz -= cs * py * pz;
+            if (a.visc) {
+                const double e1 = a.eta_c * (ph + 1.0);
+                const double exx = a.b[7][i], eyy = a.b[8][i], exy = a.b[9][i], exz = a.b[10][i], eyz = a.b[11][i];
+                txx += e1 * exx;
+                tyy += e1 * eyy;
+                tzz += e1 * (-exx - eyy);
+                txy += e1 * exy;
+                txz += e1 * exz;
+                tyz += e1 * eyz;
+            }
+            a.b[6][i] = u * px + v * py + w * pz;
+            a.b[7][i] = ph * ph * ph;
+        }
+        a.b[0][i] = txx; a.b[1][i] = txy; a.b[2][i] = txz;
+        a.b[3][i] = tyy; a.b[4][i] = tyz; a.b[5][i] = tzz;
+    }
+}
+
+}  // namespace psdns

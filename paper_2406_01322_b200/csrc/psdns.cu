@@ -1,0 +1,725 @@
+// libpsdns host side: C ABI of include/psdns.h, workspace carving, kernel sequencing.
+// One time step = rows a1..a11 of DESIGN.md, enqueued on the caller's stream
+// and replayed as a CUDA graph.
+#include "../../include/psdns.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "kernels_spectral.cuh"
+#include "kernels_transform.cuh"
+
+using namespace psdns;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+inline int round_up8(int x) { return (x + 7) / 8 * 8; }
+inline bool is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
+
+enum KClass { KC_ZBWD, KC_YBWD, KC_XBWD, KC_PW, KC_XFWD, KC_YFWD, KC_ZFWD, KC_RHS, KC_SOLVE, KC_MISC, KC_COUNT };
+const char *kclass_names[KC_COUNT] = {"zbwd", "ybwd", "xbwd", "pointwise", "xfwd", "yfwd", "zfwd", "rhs", "solve", "misc"};
+
+struct Dims {
+    int nx, ny, nz, N;
+    int nkx, nky, nkz, jpos, kxp;      // retained (dealiased) set
+    int nkxf, kxpf;                    // full set (round trip): nkxf = nx/2+1
+    size_t ncols;                      // nky * kxp
+    size_t s_ret;                      // cplx per retained spectrum with all nz planes
+    size_t s_low;                      // cplx per retained spectrum with nkz planes
+    size_t s_y;                        // cplx per Y array: nz * ny * kxp
+    size_t s_p;                        // doubles per physical field
+    size_t s_full;                     // cplx per full padded spectrum nz * ny * kxpf
+    size_t s_bspec;                    // cplx per boundary spectral field nz * ny * nkxf
+};
+
+struct Layout {
+    size_t tw_x, tw_y, tw_z;
+    size_t state[5];                   // u v w phi theta
+    size_t hist[3];
+    size_t dinv[3];                    // NS (beta^2), PO (k^2), CH (k^2 + lambda)
+    size_t thh, wh;
+    size_t xom;
+    size_t derived[8];                 // phx phy phz exx eyy exy exz eyz
+    size_t prod[8];                    // txx txy txz tyy tyz tzz q c
+    size_t zb[MAXF], yb[MAXF], ph[MAXF];
+    size_t small;                      // ab[2] doubles + counter
+    size_t stage[4];                   // host-staging device buffers (boundary layout)
+    size_t total;
+};
+
+}  // namespace
+
+struct psdns_handle {
+    psdns_grid g;
+    psdns_params p;
+    cudaStream_t st;
+    Dims d;
+    Layout L;
+    char *ws;
+    bool has_state;
+    cudaGraphExec_t graph;
+    bool graph_ready;
+    bool use_graph;
+    std::string err;
+    long long launches, per_step;
+    int timed_class;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tevents;
+    int nf_in, nf_out;
+
+    template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
+};
+
+namespace {
+
+bool validate(const psdns_grid *g, const psdns_params *p) {
+    if (!g || !p) return false;
+    if (!is_pow2(g->nx) || !is_pow2(g->ny) || g->nx < 16 || g->ny < 16 || g->nx > 1024 || g->ny > 1024) return false;
+    const int N = g->nz - 1;
+    if (!is_pow2(N) || N < 8 || N > 512) return false;
+    if (!(g->lx > 0) || !(g->ly > 0)) return false;
+    if (!(p->re > 0) || !(p->dt > 0)) return false;
+    if (p->phase_field != 0 && p->phase_field != 1) return false;
+    if (p->phase_field && (!(p->pe > 0) || !(p->ch > 0) || !(p->we > 0) || !(p->visc_ratio > 0))) return false;
+    return true;
+}
+
+Dims make_dims(const psdns_grid &g) {
+    Dims d;
+    d.nx = g.nx; d.ny = g.ny; d.nz = g.nz; d.N = g.nz - 1;
+    const int I = g.nx / 3, J = g.ny / 3, K = (2 * d.N) / 3;   // reading S3
+    d.nkx = I + 1; d.nky = 2 * J + 1; d.nkz = K + 1; d.jpos = J + 1;
+    d.kxp = round_up8(d.nkx);
+    d.nkxf = g.nx / 2 + 1;
+    d.kxpf = round_up8(d.nkxf);
+    d.ncols = (size_t)d.nky * d.kxp;
+    d.s_ret = (size_t)d.nz * d.ncols;
+    d.s_low = (size_t)d.nkz * d.ncols;
+    d.s_y = (size_t)d.nz * d.ny * d.kxp;
+    d.s_p = (size_t)d.nz * d.ny * d.nx;
+    d.s_full = (size_t)d.nz * d.ny * d.kxpf;
+    d.s_bspec = (size_t)d.nz * d.ny * d.nkxf;
+    return d;
+}
+
+Layout make_layout(const Dims &d, const psdns_params &p) {
+    Layout L;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
+    const size_t C = sizeof(cplx);
+    L.tw_x = take(d.nx * C);
+    L.tw_y = take(d.ny * C);
+    L.tw_z = take(2 * d.N * C);
+    for (int i = 0; i < 5; ++i) L.state[i] = take(d.s_ret * C);
+    for (int i = 0; i < 3; ++i) L.hist[i] = take(d.s_low * C);
+    for (int i = 0; i < 3; ++i) L.dinv[i] = take(d.s_ret * sizeof(double));
+    L.thh = take(d.s_ret * C);
+    L.wh = take(d.s_ret * C);
+    L.xom = take(d.s_ret * C);
+    for (int i = 0; i < 8; ++i) L.derived[i] = take(d.s_low * C);
+    for (int i = 0; i < 8; ++i) L.prod[i] = take(d.s_low * C);
+    const int nf = (p.phase_field && p.visc_ratio != 1.0) ? 12 : 8;
+    // Z / Y arrays double as the full-size round-trip scratch (3 arrays of s_full each)
+    size_t zy_bytes = 0;
+    for (int i = 0; i < MAXF; ++i) { L.zb[i] = 0; L.yb[i] = 0; L.ph[i] = 0; }
+    for (int i = 0; i < nf; ++i) { L.zb[i] = take(d.s_ret * C); zy_bytes += align_up(d.s_ret * C); }
+    for (int i = 0; i < nf; ++i) { L.yb[i] = take(d.s_y * C); zy_bytes += align_up(d.s_y * C); }
+    const size_t need_full = 3 * align_up(d.s_full * C);
+    if (zy_bytes < need_full) take(need_full - zy_bytes);
+    for (int i = 0; i < nf; ++i) L.ph[i] = take(d.s_p * sizeof(double));
+    L.small = take(64);
+    const size_t stage_bytes = std::max(d.s_p * sizeof(double), d.s_bspec * C);
+    for (int i = 0; i < 4; ++i) L.stage[i] = take(stage_bytes);
+    L.total = o;
+    return L;
+}
+
+#define CUDA_TRY(h, expr)                                                                          \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            (h)->err = std::string(#expr) + ": " + cudaGetErrorString(e__);                        \
+            return PSDNS_ECUDA;                                                                    \
+        }                                                                                          \
+    } while (0)
+
+struct LaunchScope {   // optional CUDA-event bracket around launches of the timed class
+    psdns_handle *h;
+    bool on;
+    cudaEvent_t e0, e1;
+    LaunchScope(psdns_handle *h_, int kc) : h(h_), on(h_->timed_class == kc) {
+        if (on) {
+            cudaEventCreate(&e0); cudaEventCreate(&e1);
+            cudaEventRecord(e0, h->st);
+        }
+    }
+    ~LaunchScope() {
+        if (on) {
+            cudaEventRecord(e1, h->st);
+            h->tevents.push_back({e0, e1});
+        }
+        h->launches++;
+    }
+};
+
+inline int col_grid(const Dims &d) { return (int)((d.ncols + NT_COL - 1) / NT_COL); }
+
+ColGeom geom(const psdns_handle *h) {
+    ColGeom g;
+    const Dims &d = h->d;
+    g.ncols = (int)d.ncols; g.kxp = d.kxp; g.nkx = d.nkx; g.nky = d.nky; g.jpos = d.jpos;
+    g.N = d.N; g.nkz = d.nkz;
+    g.kxf = 2.0 * M_PI / h->g.lx; g.kyf = 2.0 * M_PI / h->g.ly;
+    return g;
+}
+
+// ---- transform pass launchers ------------------------------------------------------------------
+template <int L>
+size_t fft_smem() { return (size_t)(L * TILE_LINES + L) * sizeof(cplx); }
+
+template <class K>
+cudaError_t set_smem(K kern, size_t bytes) {
+    if (bytes > 48 * 1024) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    return cudaSuccess;
+}
+
+#define DISPATCH_L(Lval, MACRO)            \
+    switch (Lval) {                        \
+        case 16: MACRO(16); break;         \
+        case 32: MACRO(32); break;         \
+        case 64: MACRO(64); break;         \
+        case 128: MACRO(128); break;       \
+        case 256: MACRO(256); break;       \
+        case 512: MACRO(512); break;       \
+        case 1024: MACRO(1024); break;     \
+        default: return cudaErrorInvalidValue; \
+    }
+
+cudaError_t launch_zpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, size_t ncols, int nk) {
+    ZArgs a; a.f = f; a.ncols = (int)ncols; a.nk = nk;
+    const cplx *tw = h->at<cplx>(h->L.tw_z);
+    dim3 grid((unsigned)(ncols / 8), nf);
+    LaunchScope ls(h, fwd ? KC_ZFWD : KC_ZBWD);
+#define ZL(LL)                                                                                          \
+    {                                                                                                   \
+        if (fwd) k_zpass<LL, true><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                     \
+        else k_zpass<LL, false><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                        \
+    }
+    DISPATCH_L(2 * h->d.N, ZL)
+#undef ZL
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ypass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, int kxp, int nky, int jpos) {
+    YArgs a; a.f = f; a.kxp = kxp; a.nky = nky; a.jpos = jpos;
+    const cplx *tw = h->at<cplx>(h->L.tw_y);
+    dim3 grid(kxp / 8, h->d.nz, nf);
+    LaunchScope ls(h, fwd ? KC_YFWD : KC_YBWD);
+#define YL(LL)                                                                                          \
+    {                                                                                                   \
+        if (fwd) k_ypass<LL, true><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                     \
+        else k_ypass<LL, false><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                        \
+    }
+    DISPATCH_L(h->d.ny, YL)
+#undef YL
+    return cudaGetLastError();
+}
+
+cudaError_t launch_xpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, int kxp, int nkx) {
+    XArgs a; a.f = f; a.kxp = kxp; a.nkx = nkx;
+    const cplx *tw = h->at<cplx>(h->L.tw_x);
+    dim3 grid((unsigned)((size_t)h->d.nz * h->d.ny / 16), nf);
+    LaunchScope ls(h, fwd ? KC_XFWD : KC_XBWD);
+#define XL(LL)                                                                                          \
+    {                                                                                                   \
+        if (fwd) k_xpass<LL, true><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                     \
+        else k_xpass<LL, false><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                        \
+    }
+    DISPATCH_L(h->d.nx, XL)
+#undef XL
+    return cudaGetLastError();
+}
+
+// opt-in to > 48 KB dynamic shared memory once, at init (not inside graph capture)
+cudaError_t setup_attrs(psdns_handle *h) {
+#define ZA(LL) { CU0(set_smem(k_zpass<LL, true>, fft_smem<LL>())); CU0(set_smem(k_zpass<LL, false>, fft_smem<LL>())); }
+#define YA(LL) { CU0(set_smem(k_ypass<LL, true>, fft_smem<LL>())); CU0(set_smem(k_ypass<LL, false>, fft_smem<LL>())); }
+#define XA(LL) { CU0(set_smem(k_xpass<LL, true>, fft_smem<LL>())); CU0(set_smem(k_xpass<LL, false>, fft_smem<LL>())); }
+#define CU0(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) return e__; } while (0)
+    DISPATCH_L(2 * h->d.N, ZA)
+    DISPATCH_L(h->d.ny, YA)
+    DISPATCH_L(h->d.nx, XA)
+#undef ZA
+#undef YA
+#undef XA
+#undef CU0
+    return cudaSuccess;
+}
+
+cudaError_t launch_relayout(psdns_handle *h, cplx *dst, const cplx *src, SpecSide ds, SpecSide ss, int nplanes) {
+    const size_t total = (size_t)nplanes * ds.rows * ds.pitch;
+    const int blocks = (int)std::min<size_t>((total + 255) / 256, 148 * 16);
+    LaunchScope ls(h, KC_MISC);
+    k_relayout<<<blocks, 256, 0, h->st>>>(dst, src, ds, ss, nplanes);
+    return cudaGetLastError();
+}
+
+SpecSide side_boundary(const Dims &d) { return SpecSide{d.ny, d.nkxf, d.ny / 2 + 1, d.nkxf}; }
+SpecSide side_ret(const Dims &d) { return SpecSide{d.nky, d.kxp, d.jpos, d.nkx}; }
+SpecSide side_full(const Dims &d) { return SpecSide{d.ny, d.kxpf, d.ny / 2 + 1, d.nkxf}; }
+
+cudaError_t launch_helm(psdns_handle *h, const cplx *in, cplx *out, int type, double shift, double scale, int bc,
+                        double te, double to) {
+    HelmArgs a;
+    a.g = geom(h); a.in = in; a.out = out; a.dinv = h->at<double>(h->L.dinv[type]);
+    a.shift = shift; a.scale = scale; a.bc = bc; a.tgt_e = te; a.tgt_o = to;
+    LaunchScope ls(h, KC_SOLVE);
+    k_helm<<<col_grid(h->d), NT_COL, 0, h->st>>>(a);
+    return cudaGetLastError();
+}
+
+struct Coefs {
+    double gamma, lam_phi, gam_phi, s_coef, cs;
+};
+Coefs coefs(const psdns_params &p) {
+    Coefs c;
+    c.gamma = p.dt / (2.0 * p.re);
+    if (p.phase_field) {
+        c.lam_phi = std::sqrt(p.pe / (p.dt * p.ch * p.ch));      // reading S8: s/2
+        c.gam_phi = p.dt * p.ch * p.ch / p.pe;
+        c.s_coef = 2.0 * c.lam_phi;
+        c.cs = 3.0 / std::sqrt(8.0) * p.ch / p.we;              // Eq. 8
+    } else {
+        c.lam_phi = 1.0; c.gam_phi = 1.0; c.s_coef = 0.0; c.cs = 0.0;
+    }
+    return c;
+}
+
+#define CU(expr)                                  \
+    do {                                          \
+        cudaError_t e__ = (expr);                 \
+        if (e__ != cudaSuccess) return e__;       \
+    } while (0)
+
+// ---- one time step (rows a1-a11) ------------------------------------------------------------------
+cudaError_t enqueue_step(psdns_handle *h) {
+    const Dims &d = h->d;
+    const Layout &L = h->L;
+    const psdns_params &p = h->p;
+    const Coefs c = coefs(p);
+    const bool phase = p.phase_field != 0;
+    const bool visc = phase && p.visc_ratio != 1.0;
+    const int nin = h->nf_in, nout = h->nf_out;
+    cplx *U = h->at<cplx>(L.state[0]), *V = h->at<cplx>(L.state[1]), *W = h->at<cplx>(L.state[2]);
+    cplx *PHI = h->at<cplx>(L.state[3]), *TH = h->at<cplx>(L.state[4]);
+    double *ab = h->at<double>(L.small);
+    int *counter = reinterpret_cast<int *>(ab + 2);
+    { LaunchScope ls(h, KC_MISC); k_begin_step<<<1, 1, 0, h->st>>>(ab, counter); CU(cudaGetLastError()); }
+
+    // a1: derived spectra
+    if (phase) {
+        PrepArgs a;
+        a.g = geom(h); a.u = U; a.v = V; a.w = W; a.phi = PHI;
+        a.phx = h->at<cplx>(L.derived[0]); a.phy = h->at<cplx>(L.derived[1]); a.phz = h->at<cplx>(L.derived[2]);
+        a.exx = h->at<cplx>(L.derived[3]); a.eyy = h->at<cplx>(L.derived[4]); a.exy = h->at<cplx>(L.derived[5]);
+        a.exz = h->at<cplx>(L.derived[6]); a.eyz = h->at<cplx>(L.derived[7]);
+        a.phase = 1; a.visc = visc;
+        LaunchScope ls(h, KC_RHS);
+        k_prep<<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        CU(cudaGetLastError());
+    }
+    // a2-a4: backward transforms of nin fields
+    FieldPtrs fz{}, fy{}, fx{};
+    const cplx *src[MAXF] = {U, V, W, PHI};
+    for (int i = 0; i < 8; ++i) src[4 + i] = h->at<cplx>(L.derived[i]);
+    for (int i = 0; i < nin; ++i) {
+        fz.in[i] = src[i]; fz.out[i] = h->at<cplx>(L.zb[i]);
+        fy.in[i] = fz.out[i]; fy.out[i] = h->at<cplx>(L.yb[i]);
+        fx.in[i] = fy.out[i]; fx.out[i] = h->at<double>(L.ph[i]);
+    }
+    CU(launch_zpass(h, false, fz, nin, d.ncols, d.nkz));
+    CU(launch_ypass(h, false, fy, nin, d.kxp, d.nky, d.jpos));
+    CU(launch_xpass(h, false, fx, nin, d.kxp, d.nkx));
+    // a5: pointwise products (in place)
+    {
+        PwArgs a;
+        for (int i = 0; i < MAXF; ++i) a.b[i] = h->at<double>(L.ph[i < std::max(nin, nout) ? i : 0]);
+        a.n = d.s_p; a.cs = c.cs; a.eta_c = (p.visc_ratio - 1.0) / (2.0 * p.re);
+        a.phase = phase; a.visc = visc;
+        LaunchScope ls(h, KC_PW);
+        k_pointwise<<<148 * 8, 256, 0, h->st>>>(a);
+        CU(cudaGetLastError());
+    }
+    // a6-a8: forward transforms of nout fields with truncation
+    FieldPtrs gx{}, gy{}, gz{};
+    for (int i = 0; i < nout; ++i) {
+        gx.in[i] = h->at<double>(L.ph[i]); gx.out[i] = h->at<cplx>(L.yb[i]);
+        gy.in[i] = gx.out[i]; gy.out[i] = h->at<cplx>(L.zb[i]);
+        gz.in[i] = gy.out[i]; gz.out[i] = h->at<cplx>(L.prod[i]);
+    }
+    CU(launch_xpass(h, true, gx, nout, d.kxp, d.nkx));
+    CU(launch_ypass(h, true, gy, nout, d.kxp, d.nky, d.jpos));
+    CU(launch_zpass(h, true, gz, nout, d.ncols, d.nkz));
+    // a9: right-hand sides
+    cplx *XOM = h->at<cplx>(L.xom);
+    {
+        RhsArgs a;
+        a.g = geom(h);
+        a.txx = h->at<cplx>(L.prod[0]); a.txy = h->at<cplx>(L.prod[1]); a.txz = h->at<cplx>(L.prod[2]);
+        a.tyy = h->at<cplx>(L.prod[3]); a.tyz = h->at<cplx>(L.prod[4]); a.tzz = h->at<cplx>(L.prod[5]);
+        a.q = h->at<cplx>(L.prod[6]); a.c = h->at<cplx>(L.prod[7]);
+        a.u = U; a.v = V; a.th = TH; a.phi = PHI; a.xom = XOM;
+        a.h_om = h->at<cplx>(L.hist[0]); a.h_w = h->at<cplx>(L.hist[1]); a.h_phi = h->at<cplx>(L.hist[2]);
+        a.ab = ab; a.dt = p.dt; a.gamma = c.gamma; a.inv_pe = phase ? 1.0 / p.pe : 0.0;
+        a.e_phi = 1.0 + c.s_coef * p.ch * p.ch;
+        a.gradp = p.gradp_x; a.phase = phase;
+        LaunchScope ls(h, KC_RHS);
+        k_rhs<<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        CU(cudaGetLastError());
+    }
+    // a10: solves.  omega_z (and u-bar in column 0): (D^2 - beta^2) x = -H/gamma, Dirichlet
+    const double inv_g = 1.0 / c.gamma;
+    CU(launch_helm(h, XOM, XOM, 0, inv_g, -inv_g, BC_DIRICHLET, 0.0, 0.0));
+    // theta_p (and v-bar in column 0), then w_p from (D^2 - k^2) w = theta, then the influence matrix
+    CU(launch_helm(h, TH, TH, 0, inv_g, -inv_g, BC_DIRICHLET, 0.0, 0.0));
+    CU(launch_helm(h, TH, W, 1, 0.0, 1.0, BC_DIRICHLET, 0.0, 0.0));
+    {
+        InflArgs a;
+        a.g = geom(h); a.th = TH; a.w = W; a.thh = h->at<cplx>(L.thh); a.wh = h->at<cplx>(L.wh);
+        LaunchScope ls(h, KC_SOLVE);
+        k_infl<<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        CU(cudaGetLastError());
+    }
+    // a11: u^, v^
+    {
+        FinishArgs a;
+        a.g = geom(h); a.xom = XOM; a.u = U; a.v = V; a.w = W; a.th = TH;
+        LaunchScope ls(h, KC_SOLVE);
+        k_finish<<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        CU(cudaGetLastError());
+    }
+    // phi: (D^2 - k^2 - lambda) psi = H/gamma_phi ; (D^2 - k^2 - lambda) phi = psi ; Neumann (L142, S8, S10)
+    if (phase) {
+        CU(launch_helm(h, PHI, PHI, 2, c.lam_phi, 1.0 / c.gam_phi, BC_NEUMANN, 0.0, 0.0));
+        CU(launch_helm(h, PHI, PHI, 2, c.lam_phi, 1.0, BC_NEUMANN, 0.0, 0.0));
+    }
+    return cudaSuccess;
+}
+
+cudaError_t build_tables(psdns_handle *h) {
+    const Dims &d = h->d;
+    const Layout &L = h->L;
+    // twiddles exp(-2 pi i k / L) in long double on the host
+    auto fill = [&](size_t off, int n) -> cudaError_t {
+        std::vector<cplx> t(n);
+        for (int k = 0; k < n; ++k) {
+            const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)n;
+            t[k] = make_double2((double)cosl(ang), (double)sinl(ang));
+        }
+        // exact values on the axes
+        t[0] = make_double2(1.0, 0.0);
+        if (n % 4 == 0) { t[n / 4] = make_double2(0.0, -1.0); t[n / 2] = make_double2(-1.0, 0.0); t[3 * n / 4] = make_double2(0.0, 1.0); }
+        cudaError_t e = cudaMemcpyAsync(h->ws + off, t.data(), n * sizeof(cplx), cudaMemcpyHostToDevice, h->st);
+        if (e != cudaSuccess) return e;
+        return cudaStreamSynchronize(h->st);   // t goes out of scope
+    };
+    CU(fill(L.tw_x, d.nx));
+    CU(fill(L.tw_y, d.ny));
+    CU(fill(L.tw_z, 2 * d.N));
+    const Coefs c = coefs(h->p);
+    const double shifts[3] = {1.0 / c.gamma, 0.0, c.lam_phi};
+    for (int t = 0; t < 3; ++t) {
+        HelmSetupArgs a;
+        a.g = geom(h); a.dinv = h->at<double>(L.dinv[t]); a.shift = shifts[t];
+        LaunchScope ls(h, KC_MISC);
+        k_helm_setup<<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        CU(cudaGetLastError());
+    }
+    // homogeneous solutions of the w problem: theta_h = Helmholtz(beta^2) with zero rhs and unit boundary
+    // targets in both parities; w_h = Poisson(k^2) of theta_h with w_h(+-1) = 0
+    cplx *thh = h->at<cplx>(L.thh), *wh = h->at<cplx>(L.wh);
+    CU(cudaMemsetAsync(thh, 0, d.s_ret * sizeof(cplx), h->st));
+    CU(launch_helm(h, thh, thh, 0, shifts[0], 1.0, BC_DIRICHLET, 1.0, 1.0));
+    CU(launch_helm(h, thh, wh, 1, 0.0, 1.0, BC_DIRICHLET, 0.0, 0.0));
+    return cudaSuccess;
+}
+
+int finish_set_state(psdns_handle *h) {
+    const Dims &d = h->d;
+    const Layout &L = h->L;
+    {
+        LaunchScope ls(h, KC_MISC);
+        k_lap<<<col_grid(d), NT_COL, 0, h->st>>>(geom(h), h->at<cplx>(L.state[2]), h->at<cplx>(L.state[4]));
+        CUDA_TRY(h, cudaGetLastError());
+    }
+    for (int i = 0; i < 3; ++i) CUDA_TRY(h, cudaMemsetAsync(h->ws + L.hist[i], 0, d.s_low * sizeof(cplx), h->st));
+    CUDA_TRY(h, cudaMemsetAsync(h->ws + L.small, 0, 64, h->st));
+    h->has_state = true;
+    return PSDNS_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+// C ABI
+// ================================================================================================
+extern "C" {
+
+size_t psdns_workspace_bytes(const psdns_grid *grid, const psdns_params *params) {
+    if (!validate(grid, params)) return 0;
+    return make_layout(make_dims(*grid), *params).total;
+}
+
+int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_workspace, size_t bytes, void *cuda_stream,
+               psdns_handle **out) {
+    if (!out) return PSDNS_EINVAL;
+    *out = nullptr;
+    if (!validate(grid, params) || !d_workspace) return PSDNS_EINVAL;
+    psdns_handle *h = new (std::nothrow) psdns_handle();
+    if (!h) return PSDNS_ENOMEM;
+    h->g = *grid; h->p = *params; h->st = (cudaStream_t)cuda_stream;
+    h->d = make_dims(*grid);
+    h->L = make_layout(h->d, *params);
+    h->ws = (char *)d_workspace;
+    h->has_state = false; h->graph = nullptr; h->graph_ready = false;
+    h->use_graph = std::getenv("PSDNS_NO_GRAPH") == nullptr;
+    h->launches = 0; h->per_step = 0; h->timed_class = -1;
+    const bool phase = params->phase_field != 0;
+    const bool visc = phase && params->visc_ratio != 1.0;
+    h->nf_in = phase ? (visc ? 12 : 7) : 3;
+    h->nf_out = phase ? 8 : 6;
+    if (bytes < h->L.total || ((uintptr_t)d_workspace % ALIGN) != 0) { delete h; return PSDNS_ENOMEM; }
+    cudaError_t e = setup_attrs(h);
+    if (e == cudaSuccess) e = build_tables(h);
+    if (e != cudaSuccess) {
+        // the handle is returned so that the caller can read the error text, then destroy it
+        h->err = std::string("psdns_init: ") + cudaGetErrorString(e);
+        *out = h;
+        return PSDNS_ECUDA;
+    }
+    *out = h;
+    return PSDNS_OK;
+}
+
+int psdns_set_state(psdns_handle *h, int space, const void *d_u, const void *d_v, const void *d_w, const void *d_phi) {
+    if (!h) return PSDNS_EINVAL;
+    const bool phase = h->p.phase_field != 0;
+    if (!d_u || !d_v || !d_w || (phase && !d_phi) || (space != PSDNS_PHYSICAL && space != PSDNS_SPECTRAL)) {
+        h->err = "psdns_set_state: null field pointer or bad space";
+        return PSDNS_EINVAL;
+    }
+    const Dims &d = h->d;
+    const Layout &L = h->L;
+    const void *src[4] = {d_u, d_v, d_w, d_phi};
+    const int nf = phase ? 4 : 3;
+    if (!phase) CUDA_TRY(h, cudaMemsetAsync(h->ws + L.state[3], 0, d.s_ret * sizeof(cplx), h->st));
+    if (space == PSDNS_SPECTRAL) {
+        for (int i = 0; i < nf; ++i)
+            CUDA_TRY(h, launch_relayout(h, h->at<cplx>(L.state[i]), (const cplx *)src[i], side_ret(d), side_boundary(d), d.nz));
+    } else {
+        // step i) (L138): forward transform x -> y -> z, keeping retained (kx, ky) and all nz Chebyshev modes
+        FieldPtrs fx{}, fy{}, fz{};
+        for (int i = 0; i < nf; ++i) {
+            fx.in[i] = src[i]; fx.out[i] = h->at<cplx>(L.yb[i]);
+            fy.in[i] = fx.out[i]; fy.out[i] = h->at<cplx>(L.zb[i]);
+            fz.in[i] = fy.out[i]; fz.out[i] = h->at<cplx>(L.state[i]);
+        }
+        CUDA_TRY(h, launch_xpass(h, true, fx, nf, d.kxp, d.nkx));
+        CUDA_TRY(h, launch_ypass(h, true, fy, nf, d.kxp, d.nky, d.jpos));
+        CUDA_TRY(h, launch_zpass(h, true, fz, nf, d.ncols, d.nz));
+    }
+    return finish_set_state(h);
+}
+
+int psdns_get_state(psdns_handle *h, int space, void *d_u, void *d_v, void *d_w, void *d_phi) {
+    if (!h) return PSDNS_EINVAL;
+    const bool phase = h->p.phase_field != 0;
+    if (!d_u || !d_v || !d_w || (phase && !d_phi) || (space != PSDNS_PHYSICAL && space != PSDNS_SPECTRAL)) {
+        h->err = "psdns_get_state: null field pointer or bad space";
+        return PSDNS_EINVAL;
+    }
+    if (!h->has_state) { h->err = "psdns_get_state: no state set"; return PSDNS_ESTATE; }
+    const Dims &d = h->d;
+    const Layout &L = h->L;
+    void *dst[4] = {d_u, d_v, d_w, d_phi};
+    const int nf = phase ? 4 : 3;
+    if (space == PSDNS_SPECTRAL) {
+        for (int i = 0; i < nf; ++i)
+            CUDA_TRY(h, launch_relayout(h, (cplx *)dst[i], h->at<cplx>(L.state[i]), side_boundary(d), side_ret(d), d.nz));
+    } else {
+        FieldPtrs fz{}, fy{}, fx{};
+        for (int i = 0; i < nf; ++i) {
+            fz.in[i] = h->at<cplx>(L.state[i]); fz.out[i] = h->at<cplx>(L.zb[i]);
+            fy.in[i] = fz.out[i]; fy.out[i] = h->at<cplx>(L.yb[i]);
+            fx.in[i] = fy.out[i]; fx.out[i] = dst[i];
+        }
+        CUDA_TRY(h, launch_zpass(h, false, fz, nf, d.ncols, d.nz));
+        CUDA_TRY(h, launch_ypass(h, false, fy, nf, d.kxp, d.nky, d.jpos));
+        CUDA_TRY(h, launch_xpass(h, false, fx, nf, d.kxp, d.nkx));
+    }
+    return PSDNS_OK;
+}
+
+int psdns_step(psdns_handle *h, int nsteps) {
+    if (!h) return PSDNS_EINVAL;
+    if (nsteps < 0) { h->err = "psdns_step: nsteps < 0"; return PSDNS_EINVAL; }
+    if (!h->p.dealias) { h->err = "psdns_step: dealias must be 1 (2/3 rule, reading S3)"; return PSDNS_EINVAL; }
+    if (!h->has_state) { h->err = "psdns_step: no state set"; return PSDNS_ESTATE; }
+    const bool direct = !h->use_graph || h->timed_class >= 0;
+    if (direct) {
+        for (int i = 0; i < nsteps; ++i) CUDA_TRY(h, enqueue_step(h));
+        return PSDNS_OK;
+    }
+    if (!h->graph_ready) {
+        // run one un-captured step's worth of attribute setup first (cudaFuncSetAttribute is not capturable
+        // on every driver): do the capture on a private stream so a failure leaves the user's stream clean
+        cudaStream_t user = h->st, cap;
+        CUDA_TRY(h, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+        cudaGraph_t graph = nullptr;
+        h->st = cap;
+        const long long before = h->launches;
+        cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+        if (e == cudaSuccess) e = enqueue_step(h);
+        cudaError_t e2 = cudaStreamEndCapture(cap, &graph);
+        h->st = user;
+        h->per_step = h->launches - before;
+        h->launches = before;
+        if (e == cudaSuccess) e = e2;
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&h->graph, graph, 0);
+        if (graph) cudaGraphDestroy(graph);
+        cudaStreamDestroy(cap);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            h->use_graph = false;   // fall back to direct launches (same kernels)
+            for (int i = 0; i < nsteps; ++i) CUDA_TRY(h, enqueue_step(h));
+            return PSDNS_OK;
+        }
+        h->graph_ready = true;
+    }
+    for (int i = 0; i < nsteps; ++i) {
+        CUDA_TRY(h, cudaGraphLaunch(h->graph, h->st));
+        h->launches += h->per_step;
+    }
+    return PSDNS_OK;
+}
+
+int psdns_transform_roundtrip(psdns_handle *h, int start_space, const void *d_in, void *d_out, void *d_mid) {
+    if (!h) return PSDNS_EINVAL;
+    if (!d_in || !d_out || (start_space != PSDNS_PHYSICAL && start_space != PSDNS_SPECTRAL)) {
+        h->err = "psdns_transform_roundtrip: null pointer or bad space";
+        return PSDNS_EINVAL;
+    }
+    const Dims &d = h->d;
+    const Layout &L = h->L;
+    // full-size scratch aliases the Z/Y transform buffers
+    cplx *A = h->at<cplx>(L.zb[0]);
+    cplx *B = reinterpret_cast<cplx *>(reinterpret_cast<char *>(A) + align_up(d.s_full * sizeof(cplx)));
+    cplx *C = reinterpret_cast<cplx *>(reinterpret_cast<char *>(B) + align_up(d.s_full * sizeof(cplx)));
+    const size_t ncols_f = (size_t)d.ny * d.kxpf;
+    auto forward = [&](const double *phys, cplx *spec_boundary) -> int {
+        FieldPtrs f{};
+        f.in[0] = phys; f.out[0] = A;
+        CUDA_TRY(h, launch_xpass(h, true, f, 1, d.kxpf, d.nkxf));
+        f.in[0] = A; f.out[0] = B;
+        CUDA_TRY(h, launch_ypass(h, true, f, 1, d.kxpf, d.ny, d.ny));
+        f.in[0] = B; f.out[0] = C;
+        CUDA_TRY(h, launch_zpass(h, true, f, 1, ncols_f, d.nz));
+        CUDA_TRY(h, launch_relayout(h, spec_boundary, C, side_boundary(d), side_full(d), d.nz));
+        return PSDNS_OK;
+    };
+    auto backward = [&](const cplx *spec_boundary, double *phys) -> int {
+        CUDA_TRY(h, launch_relayout(h, C, spec_boundary, side_full(d), side_boundary(d), d.nz));
+        FieldPtrs f{};
+        f.in[0] = C; f.out[0] = B;
+        CUDA_TRY(h, launch_zpass(h, false, f, 1, ncols_f, d.nz));
+        f.in[0] = B; f.out[0] = A;
+        CUDA_TRY(h, launch_ypass(h, false, f, 1, d.kxpf, d.ny, d.ny));
+        f.in[0] = A; f.out[0] = phys;
+        CUDA_TRY(h, launch_xpass(h, false, f, 1, d.kxpf, d.nkxf));
+        return PSDNS_OK;
+    };
+    int rc;
+    if (start_space == PSDNS_PHYSICAL) {
+        cplx *mid = d_mid ? (cplx *)d_mid : h->at<cplx>(L.stage[0]);
+        if ((rc = forward((const double *)d_in, mid)) != PSDNS_OK) return rc;
+        if ((rc = backward(mid, (double *)d_out)) != PSDNS_OK) return rc;
+    } else {
+        double *mid = d_mid ? (double *)d_mid : h->at<double>(L.stage[0]);
+        if ((rc = backward((const cplx *)d_in, mid)) != PSDNS_OK) return rc;
+        if ((rc = forward(mid, (cplx *)d_out)) != PSDNS_OK) return rc;
+    }
+    return PSDNS_OK;
+}
+
+int psdns_run_host(psdns_handle *h, int space, int nsteps, const void *h_in_u, const void *h_in_v, const void *h_in_w,
+                   const void *h_in_phi, void *h_out_u, void *h_out_v, void *h_out_w, void *h_out_phi) {
+    if (!h) return PSDNS_EINVAL;
+    const bool phase = h->p.phase_field != 0;
+    if (!h_in_u || !h_in_v || !h_in_w || !h_out_u || !h_out_v || !h_out_w || (phase && (!h_in_phi || !h_out_phi)) ||
+        (space != PSDNS_PHYSICAL && space != PSDNS_SPECTRAL)) {
+        h->err = "psdns_run_host: null pointer or bad space";
+        return PSDNS_EINVAL;
+    }
+    const Dims &d = h->d;
+    const size_t bytes = space == PSDNS_PHYSICAL ? d.s_p * sizeof(double) : d.s_bspec * sizeof(cplx);
+    const void *hin[4] = {h_in_u, h_in_v, h_in_w, h_in_phi};
+    void *hout[4] = {h_out_u, h_out_v, h_out_w, h_out_phi};
+    void *dev[4];
+    const int nf = phase ? 4 : 3;
+    for (int i = 0; i < 4; ++i) dev[i] = h->ws + h->L.stage[i];
+    for (int i = 0; i < nf; ++i) CUDA_TRY(h, cudaMemcpyAsync(dev[i], hin[i], bytes, cudaMemcpyHostToDevice, h->st));
+    int rc = psdns_set_state(h, space, dev[0], dev[1], dev[2], phase ? dev[3] : nullptr);
+    if (rc != PSDNS_OK) return rc;
+    if ((rc = psdns_step(h, nsteps)) != PSDNS_OK) return rc;
+    if ((rc = psdns_get_state(h, space, dev[0], dev[1], dev[2], phase ? dev[3] : nullptr)) != PSDNS_OK) return rc;
+    for (int i = 0; i < nf; ++i) CUDA_TRY(h, cudaMemcpyAsync(hout[i], dev[i], bytes, cudaMemcpyDeviceToHost, h->st));
+    return PSDNS_OK;
+}
+
+long long psdns_launch_count(const psdns_handle *h) { return h ? h->launches : 0; }
+
+int psdns_kernel_timing(psdns_handle *h, const char *name, int enable) {
+    if (!h || !name) return PSDNS_EINVAL;
+    for (auto &pr : h->tevents) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+    h->tevents.clear();
+    if (!enable) { h->timed_class = -1; return PSDNS_OK; }
+    for (int i = 0; i < KC_COUNT; ++i)
+        if (std::strcmp(name, kclass_names[i]) == 0) { h->timed_class = i; return PSDNS_OK; }
+    h->err = std::string("psdns_kernel_timing: unknown kernel class ") + name;
+    return PSDNS_EINVAL;
+}
+
+int psdns_kernel_time_ms(psdns_handle *h, double *ms_total, long long *launches) {
+    if (!h || !ms_total || !launches) return PSDNS_EINVAL;
+    double tot = 0.0;
+    for (auto &pr : h->tevents) {
+        CUDA_TRY(h, cudaEventSynchronize(pr.second));
+        float ms = 0.f;
+        CUDA_TRY(h, cudaEventElapsedTime(&ms, pr.first, pr.second));
+        tot += ms;
+    }
+    *ms_total = tot;
+    *launches = (long long)h->tevents.size();
+    return PSDNS_OK;
+}
+
+int psdns_destroy(psdns_handle *h) {
+    if (!h) return PSDNS_EINVAL;
+    if (h->graph) cudaGraphExecDestroy(h->graph);
+    for (auto &pr : h->tevents) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+    delete h;
+    return PSDNS_OK;
+}
+
+const char *psdns_last_error(const psdns_handle *h) { return h ? h->err.c_str() : "null handle"; }
+
+}  // extern "C"
