@@ -150,42 +150,90 @@ __device__ __forceinline__ int fft_pos(int k) {
     return pos;
 }
 
+// shared-memory index of (row, line).  SWZ = false: s[row*8 + line].  SWZ = true: the line index is
+// rotated by the row, s[row*8 + ((line + row) & 7)], which keeps the butterfly accesses conflict free
+// (a quarter-warp still covers one whole row) AND makes "one thread reads all 8 lines of its own row"
+// conflict free when consecutive threads own consecutive rows (used by the fused x kernel's pointwise stage).
+template <bool SWZ>
+__device__ __forceinline__ int tile_idx(int row, int line) {
+    return SWZ ? row * TILE_LINES + ((line + row) & (TILE_LINES - 1)) : row * TILE_LINES + line;
+}
+
 // one DIF pass: sub-length LS, radix R, over all L/R butterflies of each of the 8 lines
-template <int L, int LS, int R, int SIGN, int NT>
+template <int L, int LS, int R, int SIGN, int NT, bool SWZ = false>
 __device__ __forceinline__ void fft_pass(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid) {
     constexpr int STRIDE = LS / R;
     constexpr int NBF = L / R;
     const int line = tid & (TILE_LINES - 1);
     for (int b = tid >> 3; b < NBF; b += NT / TILE_LINES) {
         const int blk = b / STRIDE, j = b % STRIDE;
-        cplx *p = s + (size_t)(blk * LS + j) * TILE_LINES + line;
+        const int row0 = blk * LS + j;
         cplx v[R];
 #pragma unroll
-        for (int m = 0; m < R; ++m) v[m] = p[m * STRIDE * TILE_LINES];
+        for (int m = 0; m < R; ++m) v[m] = s[tile_idx<SWZ>(row0 + m * STRIDE, line)];
         RegFFT<R, SIGN>::run(v);
 #pragma unroll
         for (int q = 0; q < R; ++q) {
             cplx o = v[q];
             if (LS > R && q > 0) o = cmultw<SIGN>(o, tw[(L / LS) * j * q]);
-            p[q * STRIDE * TILE_LINES] = o;
+            s[tile_idx<SWZ>(row0 + q * STRIDE, line)] = o;
         }
     }
 }
 
-// Full in-place FFT of the 8-line tile.  Caller must __syncthreads() before (data + twiddles
-// visible) and after (before reading results).
-template <int L, int SIGN, int NT>
+// one DIT pass (inverse data flow of fft_pass): twiddle the inputs, then butterfly
+template <int L, int LS, int R, int SIGN, int NT, bool SWZ = false>
+__device__ __forceinline__ void fft_pass_dit(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid) {
+    constexpr int STRIDE = LS / R;
+    constexpr int NBF = L / R;
+    const int line = tid & (TILE_LINES - 1);
+    for (int b = tid >> 3; b < NBF; b += NT / TILE_LINES) {
+        const int blk = b / STRIDE, j = b % STRIDE;
+        const int row0 = blk * LS + j;
+        cplx v[R];
+#pragma unroll
+        for (int m = 0; m < R; ++m) {
+            cplx x = s[tile_idx<SWZ>(row0 + m * STRIDE, line)];
+            if (LS > R && m > 0) x = cmultw<SIGN>(x, tw[(L / LS) * j * m]);
+            v[m] = x;
+        }
+        RegFFT<R, SIGN>::run(v);
+#pragma unroll
+        for (int q = 0; q < R; ++q) s[tile_idx<SWZ>(row0 + q * STRIDE, line)] = v[q];
+    }
+}
+
+// Full in-place DIF FFT of the 8-line tile: natural-order rows in, element k at row fft_pos<L>(k) out.
+// Caller must __syncthreads() before (data + twiddles visible) and after (before reading results).
+template <int L, int SIGN, int NT, bool SWZ = false>
 __device__ __forceinline__ void fft_tile(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid) {
     constexpr int R1 = Plan<L>::R1, R2 = Plan<L>::R2, R3 = Plan<L>::R3;
-    fft_pass<L, L, R1, SIGN, NT>(s, tw, tid);
+    fft_pass<L, L, R1, SIGN, NT, SWZ>(s, tw, tid);
     if constexpr (R2 > 1) {
         __syncthreads();
-        fft_pass<L, L / R1, R2, SIGN, NT>(s, tw, tid);
+        fft_pass<L, L / R1, R2, SIGN, NT, SWZ>(s, tw, tid);
     }
     if constexpr (R3 > 1) {
         __syncthreads();
-        fft_pass<L, L / (R1 * R2), R3, SIGN, NT>(s, tw, tid);
+        fft_pass<L, L / (R1 * R2), R3, SIGN, NT, SWZ>(s, tw, tid);
     }
+}
+
+// Full in-place DIT FFT: element n at row fft_pos<L>(n) in (exactly the order fft_tile leaves),
+// natural-order rows out.  Lets backward-FFT -> pointwise -> forward-FFT run without any reordering.
+template <int L, int SIGN, int NT, bool SWZ = false>
+__device__ __forceinline__ void fft_tile_dit(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid) {
+    constexpr int R1 = Plan<L>::R1, R2 = Plan<L>::R2, R3 = Plan<L>::R3;
+    if constexpr (R3 > 1) {
+        fft_pass_dit<L, R3, R3, SIGN, NT, SWZ>(s, tw, tid);
+        __syncthreads();
+        fft_pass_dit<L, R3 * R2, R2, SIGN, NT, SWZ>(s, tw, tid);
+        __syncthreads();
+    } else if constexpr (R2 > 1) {
+        fft_pass_dit<L, R2, R2, SIGN, NT, SWZ>(s, tw, tid);
+        __syncthreads();
+    }
+    fft_pass_dit<L, L, R1, SIGN, NT, SWZ>(s, tw, tid);
 }
 
 }  // namespace psdns

@@ -16,6 +16,7 @@
 
 #include "kernels_spectral.cuh"
 #include "kernels_transform.cuh"
+#include "kernels_xfused.cuh"
 
 using namespace psdns;
 
@@ -26,8 +27,8 @@ inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 inline int round_up8(int x) { return (x + 7) / 8 * 8; }
 inline bool is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
 
-enum KClass { KC_ZBWD, KC_YBWD, KC_XBWD, KC_PW, KC_XFWD, KC_YFWD, KC_ZFWD, KC_RHS, KC_SOLVE, KC_MISC, KC_COUNT };
-const char *kclass_names[KC_COUNT] = {"zbwd", "ybwd", "xbwd", "pointwise", "xfwd", "yfwd", "zfwd", "rhs", "solve", "misc"};
+enum KClass { KC_ZBWD, KC_YBWD, KC_XBWD, KC_PW, KC_XFWD, KC_YFWD, KC_ZFWD, KC_RHS, KC_SOLVE, KC_MISC, KC_XFUSED, KC_COUNT };
+const char *kclass_names[KC_COUNT] = {"zbwd", "ybwd", "xbwd", "pointwise", "xfwd", "yfwd", "zfwd", "rhs", "solve", "misc", "xfused"};
 
 struct Dims {
     int nx, ny, nz, N;
@@ -75,6 +76,7 @@ struct psdns_handle {
     int timed_class;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tevents;
     int nf_in, nf_out;
+    bool use_xfused;
 
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
 };
@@ -186,6 +188,9 @@ ColGeom geom(const psdns_handle *h) {
 template <int L>
 size_t fft_smem() { return (size_t)(L * TILE_LINES + L) * sizeof(cplx); }
 
+template <int L>
+size_t xfused_smem() { return (size_t)((L / 2) * TILE_LINES + L / 2) * sizeof(cplx); }
+
 template <class K>
 cudaError_t set_smem(K kern, size_t bytes) {
     if (bytes > 48 * 1024) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
@@ -258,11 +263,24 @@ cudaError_t setup_attrs(psdns_handle *h) {
     DISPATCH_L(2 * h->d.N, ZA)
     DISPATCH_L(h->d.ny, YA)
     DISPATCH_L(h->d.nx, XA)
+#define XFA(LL) { CU0(set_smem(k_xfused<LL>, xfused_smem<LL>())); }
+    DISPATCH_L(h->d.nx, XFA)
+#undef XFA
 #undef ZA
 #undef YA
 #undef XA
 #undef CU0
     return cudaSuccess;
+}
+
+cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
+    const cplx *tw = h->at<cplx>(h->L.tw_x);
+    const int grid = std::min(a.nlines, 148 * 12);
+    LaunchScope ls(h, KC_XFUSED);
+#define XF(LL) k_xfused<LL><<<grid, NT_FFT, xfused_smem<LL>(), h->st>>>(a, tw);
+    DISPATCH_L(h->d.nx, XF)
+#undef XF
+    return cudaGetLastError();
 }
 
 cudaError_t launch_relayout(psdns_handle *h, cplx *dst, const cplx *src, SpecSide ds, SpecSide ss, int nplanes) {
@@ -348,25 +366,35 @@ cudaError_t enqueue_step(psdns_handle *h) {
     }
     CU(launch_zpass(h, false, fz, nin, d.ncols, d.nkz));
     CU(launch_ypass(h, false, fy, nin, d.kxp, d.nky, d.jpos));
-    CU(launch_xpass(h, false, fx, nin, d.kxp, d.nkx));
-    // a5: pointwise products (in place)
-    {
-        PwArgs a;
-        for (int i = 0; i < MAXF; ++i) a.b[i] = h->at<double>(L.ph[i < std::max(nin, nout) ? i : 0]);
-        a.n = d.s_p; a.cs = c.cs; a.eta_c = (p.visc_ratio - 1.0) / (2.0 * p.re);
-        a.phase = phase; a.visc = visc;
-        LaunchScope ls(h, KC_PW);
-        k_pointwise<<<148 * 8, 256, 0, h->st>>>(a);
-        CU(cudaGetLastError());
-    }
-    // a6-a8: forward transforms of nout fields with truncation
     FieldPtrs gx{}, gy{}, gz{};
     for (int i = 0; i < nout; ++i) {
         gx.in[i] = h->at<double>(L.ph[i]); gx.out[i] = h->at<cplx>(L.yb[i]);
         gy.in[i] = gx.out[i]; gy.out[i] = h->at<cplx>(L.zb[i]);
         gz.in[i] = gy.out[i]; gz.out[i] = h->at<cplx>(L.prod[i]);
     }
-    CU(launch_xpass(h, true, gx, nout, d.kxp, d.nkx));
+    if (h->use_xfused && !visc) {
+        // a4 + a5 + a6 fused: physical space never leaves the SM; in place on the Y arrays
+        XFArgs a;
+        for (int i = 0; i < 8; ++i) { a.in[i] = h->at<cplx>(L.yb[i < nin ? i : 0]); a.out[i] = h->at<cplx>(L.yb[i < nout ? i : 0]); }
+        a.kxp = d.kxp; a.nkx = d.nkx; a.nlines = d.nz * d.ny; a.nin = nin; a.nout = nout;
+        a.cs = c.cs; a.phase = phase;
+        CU(launch_xfused(h, a));
+    } else {
+        CU(launch_xpass(h, false, fx, nin, d.kxp, d.nkx));
+        // a5: pointwise products (in place)
+        {
+            PwArgs a;
+            for (int i = 0; i < MAXF; ++i) a.b[i] = h->at<double>(L.ph[i < std::max(nin, nout) ? i : 0]);
+            a.n = d.s_p; a.cs = c.cs; a.eta_c = (p.visc_ratio - 1.0) / (2.0 * p.re);
+            a.phase = phase; a.visc = visc;
+            LaunchScope ls(h, KC_PW);
+            k_pointwise<<<148 * 8, 256, 0, h->st>>>(a);
+            CU(cudaGetLastError());
+        }
+        // a6: forward x with truncation
+        CU(launch_xpass(h, true, gx, nout, d.kxp, d.nkx));
+    }
+    // a7-a8: forward y, z with truncation
     CU(launch_ypass(h, true, gy, nout, d.kxp, d.nky, d.jpos));
     CU(launch_zpass(h, true, gz, nout, d.ncols, d.nkz));
     // a9: right-hand sides
@@ -492,6 +520,7 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->ws = (char *)d_workspace;
     h->has_state = false; h->graph = nullptr; h->graph_ready = false;
     h->use_graph = std::getenv("PSDNS_NO_GRAPH") == nullptr;
+    h->use_xfused = std::getenv("PSDNS_NO_XFUSE") == nullptr;
     h->launches = 0; h->per_step = 0; h->timed_class = -1;
     const bool phase = params->phase_field != 0;
     const bool visc = phase && params->visc_ratio != 1.0;
