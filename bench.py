@@ -79,6 +79,7 @@ def algorithmic_bytes(c):
         "xfwd": nout * (R + S_pyz),
         "yfwd": nout * (S_pyz + S_ppz),
         "zfwd": nout * (S_ppz + S_ppp),
+        "xfused": (nin + nout) * S_pyz,
     }
     # fused-pipeline figure of SURVEY 8(d): physical-space arrays never leave the SM
     step_fused = (4 * S_ppp + nin * S_ppz) + nin * (S_ppz + S_pyz) + (nin + nout) * S_pyz \
@@ -332,12 +333,14 @@ def run_ours(args):
     kernels = {}
     if rank == 0:
         ksteps = max(1, min(args.steps, 3))
-        for name in ["zbwd", "ybwd", "xbwd", "pointwise", "xfwd", "yfwd", "zfwd", "rhs", "solve"]:
+        for name in ["zbwd", "ybwd", "xbwd", "pointwise", "xfused", "xfwd", "yfwd", "zfwd", "rhs", "solve"]:
             solver.kernel_timing(name, True)
             solver.step(ksteps)
             torch.cuda.synchronize()
             tot, n = solver.kernel_time_ms()
             solver.kernel_timing(name, False)
+            if n == 0:
+                continue
             ent = {"ms_per_step": tot / ksteps, "launches_per_step": n / ksteps}
             if name in per_kernel:
                 ent["alg_bytes_per_step"] = per_kernel[name]

@@ -364,6 +364,325 @@ __global__ void __launch_bounds__(NT_COL) k_helm(const __grid_constant__ HelmArg
     }
 }
 
+// ================================================================================================
+// Two-sweep form of the same tau solve, used by the time step (k_helm above builds the init tables).
+//
+// Down sweep (rows k = N..2): Gauss elimination of c_k as in k_helm, PLUS the adjoint weights
+//   z_k = (w_k - a_{k+2} z_{k+2}) / d'_k     (L^T z = w, L = reduced lower-bidiagonal system)
+// so that the boundary functional of the particular solution is known without a substitution pass:
+//   sum_{k>=2} w_k alpha_k = sum_k z_k g'_k =: J_par,   sum_{k>=2} w_k beta_k = -a_{par+2} z_{par+2}
+//   u_par = (target - J_par) / (w_par - a_{par+2} z_{par+2}).
+// The down sweep therefore ends knowing u_0, u_1 (stored in the two unused slots of the g' array) and ONE
+// up sweep u_k = (g'_k - a_k u_{k-2}) / d'_k finishes the solve.  A second weight set (k^2) gives
+// sum k^2 w_k of the Dirichlet solution for the influence-matrix coefficient of the w problem.
+// ================================================================================================
+struct ElimDown {
+    cplx fp2, fp1, f0, fm1;   // F(k+2), F(k+1), F(k), F(k-1) of the next row k
+    cplx gp2, gp1;            // g'_{k+2}, g'_{k+1}
+    double dp2, dp1;          // 1/d'_{k+2}, 1/d'_{k+1}
+    double zp2, zp1;          // boundary-row adjoint weights z_{k+2}, z_{k+1}
+    double yp2, yp1;          // second functional (weights k^2)
+    cplx Je, Jo, Ke, Ko;
+    __device__ __forceinline__ void init() {
+        fp2 = fp1 = f0 = fm1 = gp2 = gp1 = Je = Jo = Ke = Ko = cz();
+        dp2 = dp1 = zp2 = zp1 = yp2 = yp1 = 0.0;
+    }
+    // row k (N >= k >= 2): fm2 = F(k-2) (scaled RHS, zero-extended above N-2), di = 1/d'_k.  Returns g'_k.
+    template <bool NEU, bool SECOND>
+    __device__ __forceinline__ cplx row(int k, int N, double sigma, cplx fm2, double di) {
+        cplx g = cfma(helm_p(k), fm2, cfma(helm_q(k), f0, cscale(fp2, helm_r(k))));
+        if (k + 4 <= N) g = cfma(sigma * helm_r(k) * dp2, gp2, g);   // g - (c_k/d'_{k+2}) g'_{k+2}, c_k = -sigma r_k
+        const double sp = (k + 2 <= N) ? sigma * helm_p(k + 2) : 0.0;   // -a_{k+2}
+        const double wk = NEU ? (double)k * k : 1.0;
+        const double z = (wk + sp * zp2) * di;
+        if (k & 1) Jo = cfma(z, g, Jo); else Je = cfma(z, g, Je);
+        if (SECOND) {
+            const double y = ((double)k * k + sp * yp2) * di;
+            if (k & 1) Ko = cfma(y, g, Ko); else Ke = cfma(y, g, Ke);
+            yp2 = yp1; yp1 = y;
+        }
+        zp2 = zp1; zp1 = z;
+        gp2 = gp1; gp1 = g;
+        dp2 = dp1; dp1 = di;
+        fp2 = fp1; fp1 = f0; f0 = fm1; fm1 = fm2;
+        return g;
+    }
+    // after row 2: zp1 = z_2, zp2 = z_3.  Boundary rows: Dirichlet sum u = tgt; Neumann sum k^2 u = tgt.
+    template <bool NEU>
+    __device__ __forceinline__ void finish(double sigma, double tgt_e, double tgt_o, cplx &u0, cplx &u1) const {
+        const double se = (NEU ? 0.0 : 1.0) + sigma * helm_p(2) * zp1;
+        const double so = 1.0 + sigma * helm_p(3) * zp2;
+        u0 = cscale(make_double2(tgt_e - Je.x, -Je.y), 1.0 / se);
+        u1 = cscale(make_double2(tgt_o - Jo.x, -Jo.y), 1.0 / so);
+    }
+    // sum_{k in parity} k^2 u_k of the finished solution (needs SECOND)
+    __device__ __forceinline__ void second(double sigma, cplx u0, cplx u1, cplx &de, cplx &dodd) const {
+        de = cfma(sigma * helm_p(2) * yp1, u0, Ke);                    // 0^2 u_0 + K_e + u_0 sum k^2 beta_k
+        dodd = cadd(u1, cfma(sigma * helm_p(3) * yp2, u1, Ko));          // 1^2 u_1 + K_o + u_1 sum k^2 beta_k
+    }
+};
+
+// ---- K_A: row a9 + first elimination, one thread per (column, chain) ---------------------------------
+// chain 0: omega_z (column 0: u-bar)   f = -H_omega / gamma,  sigma = k^2 + 1/gamma, Dirichlet
+// chain 1: theta   (column 0: v-bar)   f = -H_w / gamma,      same sigma, Dirichlet (homogeneous part added later)
+// chain 2: psi                         f = H_phi / gamma_phi, sigma = k^2 + lambda_phi, Neumann
+struct RhsElimArgs {
+    ColGeom g;
+    const cplx *txx, *txy, *txz, *tyy, *tyz, *tzz, *q, *c;
+    const cplx *u, *v;
+    cplx *th, *phi, *xom;             // in: theta^n, phi^n; out: g' arrays (slots 0,1 = u_0, u_1)
+    cplx *h_om, *h_w, *h_phi;
+    const double *dinv_ns, *dinv_ch;
+    const double *ab;
+    double dt, gamma, inv_pe, e_phi, gradp, lam_phi, gam_phi;
+    int phase;
+};
+
+__global__ void __launch_bounds__(NT_COL) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    const int chain = blockIdx.y;
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const double k2 = kx * kx + ky * ky;
+    const bool mean = (col == 0);
+    const size_t st = g.ncols;
+    const int N = g.N;
+    const double ab0 = a.ab[0], ab1 = a.ab[1];
+    const double dt = a.dt, gam = a.gamma;
+    ElimDown el;
+    el.init();
+    if (chain == 0) {
+        const double sigma = k2 + 1.0 / gam, fs = -1.0 / gam;
+        const double *__restrict__ dinv = a.dinv_ns + col;
+        Chain1 cR; Chain2 cOm;
+        cR.init(); cOm.init();
+        for (int n = N; n >= 0; --n) {
+            const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
+            const size_t o = n * st + col;
+            const bool low = n < g.nkz;
+            const cplx un = a.u[o], vn = a.v[o];
+            const cplx omn = mean ? un : ci(csub(cscale(vn, kx), cscale(un, ky)));
+            cplx P = cz(), R = cz();
+            if (low) {
+                const cplx txz = a.txz[o];
+                if (mean) {
+                    R = txz;
+                } else {
+                    const cplx txx = a.txx[o], txy = a.txy[o], tyy = a.tyy[o], tyz = a.tyz[o];
+                    P = cadd(cscale(txy, ky * ky - kx * kx), cscale(csub(txx, tyy), kx * ky));
+                    R = ci(csub(cscale(tyz, kx), cscale(txz, ky)));
+                }
+            }
+            const cplx dR = cR.step(R, f, h);
+            const cplx ddOm = cOm.step(omn, f, h);
+            cplx n_om = cadd(P, dR);
+            if (mean && n == 0) n_om.x += a.gradp;
+            cplx nl = cscale(n_om, ab0);
+            if (low) { nl = cfma(ab1, a.h_om[o], nl); a.h_om[o] = n_om; }
+            const cplx H = cfma(dt, nl, cfma(gam, cfma(-k2, omn, ddOm), omn));
+            if (n <= N - 2) {
+                const int k = n + 2;
+                a.xom[k * st + col] = el.row<false, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
+            }
+        }
+        cplx u0, u1;
+        el.finish<false>(sigma, 0.0, 0.0, u0, u1);
+        a.xom[col] = u0; a.xom[st + col] = u1;
+    } else if (chain == 1) {
+        const double sigma = k2 + 1.0 / gam, fs = -1.0 / gam;
+        const double *__restrict__ dinv = a.dinv_ns + col;
+        Chain1 cB; Chain2 cA, cTh;
+        cB.init(); cA.init(); cTh.init();
+        for (int n = N; n >= 0; --n) {
+            const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
+            const size_t o = n * st + col;
+            const bool low = n < g.nkz;
+            const cplx thn = mean ? a.v[o] : a.th[o];
+            cplx A = cz(), B = cz();
+            if (low) {
+                const cplx tyz = a.tyz[o];
+                if (mean) {
+                    B = tyz;
+                } else {
+                    const cplx txx = a.txx[o], txy = a.txy[o], txz = a.txz[o], tyy = a.tyy[o], tzz = a.tzz[o];
+                    A = ci(cadd(cscale(txz, kx), cscale(tyz, ky)));
+                    B = cadd(cadd(cscale(txx, kx * kx), cscale(txy, 2.0 * kx * ky)), csub(cscale(tyy, ky * ky), cscale(tzz, k2)));
+                }
+            }
+            const cplx dB = cB.step(B, f, h);
+            const cplx ddA = cA.step(A, f, h);
+            const cplx ddTh = cTh.step(thn, f, h);
+            const cplx n_w = cadd(csub(dB, ddA), cscale(A, -k2));
+            cplx nl = cscale(n_w, ab0);
+            if (low) { nl = cfma(ab1, a.h_w[o], nl); a.h_w[o] = n_w; }
+            const cplx H = cfma(dt, nl, cfma(gam, cfma(-k2, thn, ddTh), thn));
+            if (n <= N - 2) {
+                const int k = n + 2;
+                a.th[k * st + col] = el.row<false, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
+            }
+        }
+        cplx u0, u1;
+        el.finish<false>(sigma, 0.0, 0.0, u0, u1);
+        a.th[col] = u0; a.th[st + col] = u1;
+    } else {
+        if (!a.phase) return;
+        const double sigma = k2 + a.lam_phi, fs = 1.0 / a.gam_phi;
+        const double *__restrict__ dinv = a.dinv_ch + col;
+        Chain2 cE;
+        cE.init();
+        for (int n = N; n >= 0; --n) {
+            const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
+            const size_t o = n * st + col;
+            const bool low = n < g.nkz;
+            const cplx phn = a.phi[o];
+            cplx E = cz(), Q = cz();
+            if (low) {
+                Q = a.q[o];
+                E = cscale(cfma(-a.e_phi, phn, a.c[o]), a.inv_pe);
+            }
+            const cplx ddE = cE.step(E, f, h);
+            const cplx s_phi = csub(cfma(-k2, E, ddE), Q);
+            cplx nl = cscale(s_phi, ab0);
+            if (low) { nl = cfma(ab1, a.h_phi[o], nl); a.h_phi[o] = s_phi; }
+            const cplx H = cfma(dt, nl, phn);
+            if (n <= N - 2) {
+                const int k = n + 2;
+                a.phi[k * st + col] = el.row<true, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
+            }
+        }
+        cplx u0, u1;
+        el.finish<true>(sigma, 0.0, 0.0, u0, u1);
+        a.phi[col] = u0; a.phi[st + col] = u1;
+    }
+}
+
+// ---- K_B / K_D: up sweep u_k = (g'_k - a_k u_{k-2}) / d'_k, optional homogeneous correction ------------
+struct SubstArgs {
+    ColGeom g;
+    cplx *x[3];                 // per chain: g' array in (slots 0,1 = u_0,u_1), solution out (in place)
+    const double *dinv[3];
+    double shift[3];
+    int nchains;
+    // influence-matrix correction (chain 0 only, when coef != nullptr): x += A_par * wh ; th += A_par * thh
+    const cplx *coef;           // [2][ncols]: A_e, A_o
+    const double *wh, *thh;     // real homogeneous solutions [nz][ncols]
+    cplx *th;
+};
+
+__global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstArgs a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    const int chain = blockIdx.y;
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const double sigma = kx * kx + ky * ky + a.shift[chain];
+    const size_t st = g.ncols;
+    const int N = g.N;
+    cplx *x = a.x[chain] + col;
+    const double *__restrict__ dinv = a.dinv[chain] + col;
+    const bool corr = (chain == 0 && a.coef != nullptr);
+    cplx Ae = cz(), Ao = cz();
+    if (corr) { Ae = a.coef[col]; Ao = a.coef[st + col]; }
+    cplx um2 = x[0], um1 = x[st];
+    if (corr) {
+        x[0] = cfma(a.wh[col], Ae, um2);
+        x[st] = cfma(a.wh[st + col], Ao, um1);
+        a.th[col] = cfma(a.thh[col], Ae, a.th[col]);
+        a.th[st + col] = cfma(a.thh[st + col], Ao, a.th[st + col]);
+    }
+#pragma unroll 4
+    for (int k = 2; k <= N; ++k) {
+        const double ak = -sigma * helm_p(k);
+        const cplx u = cscale(cfma(-ak, um2, x[k * st]), dinv[k * st]);
+        um2 = um1; um1 = u;
+        if (corr) {
+            const size_t o = k * st + col;
+            const cplx A = (k & 1) ? Ao : Ae;
+            x[k * st] = cfma(a.wh[o], A, u);
+            a.th[o] = cfma(a.thh[o], A, a.th[o]);
+        } else {
+            x[k * st] = u;
+        }
+    }
+}
+
+// ---- K_C: second elimination of the two-stage problems (RHS = the first stage's solution) ----------------
+// chain 0: (D^2 - k^2) w = theta_p, Dirichlet, plus the influence coefficient A_par = -sum k^2 w_p / sum k^2 w_h
+// chain 1: (D^2 - k^2 - lambda) phi = psi, Neumann (in place)
+struct Elim2Args {
+    ColGeom g;
+    const cplx *th;   cplx *w;      // chain 0
+    cplx *phi;                      // chain 1 (in place)
+    const double *dinv_po, *dinv_ch;
+    const double *hw;               // [2][ncols]: sum_{even} k^2 w_h, sum_{odd} k^2 w_h
+    cplx *coef;                     // [2][ncols] out
+    double lam_phi;
+    int phase;
+};
+
+__global__ void __launch_bounds__(NT_COL) k_elim2(const __grid_constant__ Elim2Args a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    const int chain = blockIdx.y;
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const double k2 = kx * kx + ky * ky;
+    const size_t st = g.ncols;
+    const int N = g.N;
+    ElimDown el;
+    el.init();
+    if (chain == 0) {
+        const cplx *__restrict__ in = a.th + col;
+        cplx *__restrict__ out = a.w + col;
+        const double *__restrict__ dinv = a.dinv_po + col;
+#pragma unroll 4
+        for (int k = N; k >= 2; --k) out[k * st] = el.row<false, true>(k, N, k2, in[(k - 2) * st], dinv[k * st]);
+        cplx u0, u1, de, dodd;
+        el.finish<false>(k2, 0.0, 0.0, u0, u1);
+        el.second(k2, u0, u1, de, dodd);
+        out[0] = u0; out[st] = u1;
+        const bool off = (col == 0);
+        a.coef[col] = off ? cz() : cscale(de, -1.0 / a.hw[col]);
+        a.coef[st + col] = off ? cz() : cscale(dodd, -1.0 / a.hw[st + col]);
+    } else {
+        if (!a.phase) return;
+        const double sigma = k2 + a.lam_phi;
+        cplx *x = a.phi + col;
+        const double *__restrict__ dinv = a.dinv_ch + col;
+#pragma unroll 4
+        for (int k = N; k >= 2; --k) {
+            const cplx fm2 = x[(k - 2) * st];
+            x[k * st] = el.row<true, false>(k, N, sigma, fm2, dinv[k * st]);
+        }
+        cplx u0, u1;
+        el.finish<true>(sigma, 0.0, 0.0, u0, u1);
+        x[0] = u0; x[st] = u1;
+    }
+}
+
+// ---- init helper: real copies of the homogeneous solutions and their k^2 sums --------------------------
+__global__ void __launch_bounds__(NT_COL) k_hom_tables(const __grid_constant__ ColGeom g, const cplx *__restrict__ thh_c,
+                                                       const cplx *__restrict__ wh_c, double *__restrict__ thh,
+                                                       double *__restrict__ wh, double *__restrict__ hw) {
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    const size_t st = g.ncols;
+    double he = 0.0, ho = 0.0;
+    for (int k = 0; k <= g.N; ++k) {
+        const size_t o = k * st + col;
+        const double w = wh_c[o].x;
+        thh[o] = thh_c[o].x;
+        wh[o] = w;
+        if (k & 1) ho += (double)k * k * w; else he += (double)k * k * w;
+    }
+    hw[col] = he;
+    hw[st + col] = ho;
+}
+
 // ---- influence-matrix closure of the w problem -----------------------------------------------------
 // theta = theta_p + A_par theta_h, w = w_p + A_par w_h with A_par chosen so that
 // sum_{k in parity} k^2 w_k = 0 for both parities  <=>  Dw(+1) = Dw(-1) = 0 (reading S10/S11).

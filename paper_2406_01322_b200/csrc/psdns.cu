@@ -48,7 +48,8 @@ struct Layout {
     size_t state[5];                   // u v w phi theta
     size_t hist[3];
     size_t dinv[3];                    // NS (beta^2), PO (k^2), CH (k^2 + lambda)
-    size_t thh, wh;
+    size_t thh, wh;                    // real homogeneous solutions [nz][ncols]
+    size_t hw, coef;                   // [2][ncols] doubles / cplx
     size_t xom;
     size_t derived[8];                 // phx phy phz exx eyy exy exz eyz
     size_t prod[8];                    // txx txy txz tyy tyz tzz q c
@@ -124,8 +125,10 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     for (int i = 0; i < 5; ++i) L.state[i] = take(d.s_ret * C);
     for (int i = 0; i < 3; ++i) L.hist[i] = take(d.s_low * C);
     for (int i = 0; i < 3; ++i) L.dinv[i] = take(d.s_ret * sizeof(double));
-    L.thh = take(d.s_ret * C);
-    L.wh = take(d.s_ret * C);
+    L.thh = take(d.s_ret * sizeof(double));
+    L.wh = take(d.s_ret * sizeof(double));
+    L.hw = take(2 * d.ncols * sizeof(double));
+    L.coef = take(2 * d.ncols * C);
     L.xom = take(d.s_ret * C);
     for (int i = 0; i < 8; ++i) L.derived[i] = take(d.s_low * C);
     for (int i = 0; i < 8; ++i) L.prod[i] = take(d.s_low * C);
@@ -397,34 +400,57 @@ cudaError_t enqueue_step(psdns_handle *h) {
     // a7-a8: forward y, z with truncation
     CU(launch_ypass(h, true, gy, nout, d.kxp, d.nky, d.jpos));
     CU(launch_zpass(h, true, gz, nout, d.ncols, d.nkz));
-    // a9: right-hand sides
+    // a9 + first elimination (K_A), substitution (K_B), second elimination (K_C), substitution +
+    // influence-matrix correction (K_D), velocity recovery (a11)
     cplx *XOM = h->at<cplx>(L.xom);
+    const double inv_g = 1.0 / c.gamma;
+    const double *dNS = h->at<double>(L.dinv[0]), *dPO = h->at<double>(L.dinv[1]), *dCH = h->at<double>(L.dinv[2]);
     {
-        RhsArgs a;
+        RhsElimArgs a;
         a.g = geom(h);
         a.txx = h->at<cplx>(L.prod[0]); a.txy = h->at<cplx>(L.prod[1]); a.txz = h->at<cplx>(L.prod[2]);
         a.tyy = h->at<cplx>(L.prod[3]); a.tyz = h->at<cplx>(L.prod[4]); a.tzz = h->at<cplx>(L.prod[5]);
         a.q = h->at<cplx>(L.prod[6]); a.c = h->at<cplx>(L.prod[7]);
         a.u = U; a.v = V; a.th = TH; a.phi = PHI; a.xom = XOM;
         a.h_om = h->at<cplx>(L.hist[0]); a.h_w = h->at<cplx>(L.hist[1]); a.h_phi = h->at<cplx>(L.hist[2]);
+        a.dinv_ns = dNS; a.dinv_ch = dCH;
         a.ab = ab; a.dt = p.dt; a.gamma = c.gamma; a.inv_pe = phase ? 1.0 / p.pe : 0.0;
         a.e_phi = 1.0 + c.s_coef * p.ch * p.ch;
-        a.gradp = p.gradp_x; a.phase = phase;
+        a.gradp = p.gradp_x; a.lam_phi = c.lam_phi; a.gam_phi = c.gam_phi; a.phase = phase;
         LaunchScope ls(h, KC_RHS);
-        k_rhs<<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        k_rhs_elim<<<dim3(col_grid(d), phase ? 3 : 2), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
-    // a10: solves.  omega_z (and u-bar in column 0): (D^2 - beta^2) x = -H/gamma, Dirichlet
-    const double inv_g = 1.0 / c.gamma;
-    CU(launch_helm(h, XOM, XOM, 0, inv_g, -inv_g, BC_DIRICHLET, 0.0, 0.0));
-    // theta_p (and v-bar in column 0), then w_p from (D^2 - k^2) w = theta, then the influence matrix
-    CU(launch_helm(h, TH, TH, 0, inv_g, -inv_g, BC_DIRICHLET, 0.0, 0.0));
-    CU(launch_helm(h, TH, W, 1, 0.0, 1.0, BC_DIRICHLET, 0.0, 0.0));
     {
-        InflArgs a;
-        a.g = geom(h); a.th = TH; a.w = W; a.thh = h->at<cplx>(L.thh); a.wh = h->at<cplx>(L.wh);
+        SubstArgs a;
+        a.g = geom(h);
+        a.x[0] = XOM; a.x[1] = TH; a.x[2] = PHI;
+        a.dinv[0] = dNS; a.dinv[1] = dNS; a.dinv[2] = dCH;
+        a.shift[0] = inv_g; a.shift[1] = inv_g; a.shift[2] = c.lam_phi;
+        a.nchains = phase ? 3 : 2;
+        a.coef = nullptr; a.wh = nullptr; a.thh = nullptr; a.th = nullptr;
         LaunchScope ls(h, KC_SOLVE);
-        k_infl<<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        k_subst<<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
+        CU(cudaGetLastError());
+    }
+    {
+        Elim2Args a;
+        a.g = geom(h); a.th = TH; a.w = W; a.phi = PHI; a.dinv_po = dPO; a.dinv_ch = dCH;
+        a.hw = h->at<double>(L.hw); a.coef = h->at<cplx>(L.coef); a.lam_phi = c.lam_phi; a.phase = phase;
+        LaunchScope ls(h, KC_SOLVE);
+        k_elim2<<<dim3(col_grid(d), phase ? 2 : 1), NT_COL, 0, h->st>>>(a);
+        CU(cudaGetLastError());
+    }
+    {
+        SubstArgs a;
+        a.g = geom(h);
+        a.x[0] = W; a.x[1] = PHI; a.x[2] = nullptr;
+        a.dinv[0] = dPO; a.dinv[1] = dCH; a.dinv[2] = nullptr;
+        a.shift[0] = 0.0; a.shift[1] = c.lam_phi; a.shift[2] = 0.0;
+        a.nchains = phase ? 2 : 1;
+        a.coef = h->at<cplx>(L.coef); a.wh = h->at<double>(L.wh); a.thh = h->at<double>(L.thh); a.th = TH;
+        LaunchScope ls(h, KC_SOLVE);
+        k_subst<<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     // a11: u^, v^
@@ -434,11 +460,6 @@ cudaError_t enqueue_step(psdns_handle *h) {
         LaunchScope ls(h, KC_SOLVE);
         k_finish<<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
-    }
-    // phi: (D^2 - k^2 - lambda) psi = H/gamma_phi ; (D^2 - k^2 - lambda) phi = psi ; Neumann (L142, S8, S10)
-    if (phase) {
-        CU(launch_helm(h, PHI, PHI, 2, c.lam_phi, 1.0 / c.gam_phi, BC_NEUMANN, 0.0, 0.0));
-        CU(launch_helm(h, PHI, PHI, 2, c.lam_phi, 1.0, BC_NEUMANN, 0.0, 0.0));
     }
     return cudaSuccess;
 }
@@ -473,11 +494,18 @@ cudaError_t build_tables(psdns_handle *h) {
         CU(cudaGetLastError());
     }
     // homogeneous solutions of the w problem: theta_h = Helmholtz(beta^2) with zero rhs and unit boundary
-    // targets in both parities; w_h = Poisson(k^2) of theta_h with w_h(+-1) = 0
-    cplx *thh = h->at<cplx>(L.thh), *wh = h->at<cplx>(L.wh);
-    CU(cudaMemsetAsync(thh, 0, d.s_ret * sizeof(cplx), h->st));
-    CU(launch_helm(h, thh, thh, 0, shifts[0], 1.0, BC_DIRICHLET, 1.0, 1.0));
-    CU(launch_helm(h, thh, wh, 1, 0.0, 1.0, BC_DIRICHLET, 0.0, 0.0));
+    // targets in both parities; w_h = Poisson(k^2) of theta_h with w_h(+-1) = 0.  Solved as complex in
+    // scratch, then kept as real tables together with sum k^2 w_h per parity.
+    cplx *thh_c = h->at<cplx>(L.zb[0]), *wh_c = h->at<cplx>(L.zb[1]);
+    CU(cudaMemsetAsync(thh_c, 0, d.s_ret * sizeof(cplx), h->st));
+    CU(launch_helm(h, thh_c, thh_c, 0, shifts[0], 1.0, BC_DIRICHLET, 1.0, 1.0));
+    CU(launch_helm(h, thh_c, wh_c, 1, 0.0, 1.0, BC_DIRICHLET, 0.0, 0.0));
+    {
+        LaunchScope ls(h, KC_MISC);
+        k_hom_tables<<<col_grid(d), NT_COL, 0, h->st>>>(geom(h), thh_c, wh_c, h->at<double>(L.thh), h->at<double>(L.wh),
+                                                        h->at<double>(L.hw));
+        CU(cudaGetLastError());
+    }
     return cudaSuccess;
 }
 
