@@ -438,7 +438,7 @@ struct RhsElimArgs {
     int phase;
 };
 
-__global__ void __launch_bounds__(NT_COL) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
+__global__ void __launch_bounds__(NT_COL, 4) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= g.ncols) return;
@@ -623,7 +623,7 @@ struct Elim2Args {
     int phase;
 };
 
-__global__ void __launch_bounds__(NT_COL) k_elim2(const __grid_constant__ Elim2Args a) {
+__global__ void __launch_bounds__(NT_COL, 5) k_elim2(const __grid_constant__ Elim2Args a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= g.ncols) return;

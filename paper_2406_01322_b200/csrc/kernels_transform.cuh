@@ -15,7 +15,9 @@
 namespace psdns {
 
 constexpr int MAXF = 12;      // max fields per batched launch
-constexpr int NT_FFT = 256;   // threads per transform CTA
+constexpr int NT_FFT = 256;   // threads per transform CTA (tiles up to 74 KB, >= 3 CTAs per SM)
+// the 147 KB tile (L = 1024) allows one CTA per SM: give it 16 warps instead of 8 to hide latency
+template <int L> __host__ __device__ constexpr int tile_threads() { return L >= 1024 ? 512 : 256; }
 
 struct FieldPtrs {
     const void *in[MAXF];
@@ -41,17 +43,18 @@ struct ZArgs {
 };
 
 template <int L, bool FWD>
-__global__ void __launch_bounds__(NT_FFT) k_zpass(const __grid_constant__ ZArgs a, const cplx *__restrict__ twg) {
+__global__ void __launch_bounds__(tile_threads<L>()) k_zpass(const __grid_constant__ ZArgs a, const cplx *__restrict__ twg) {
+    constexpr int NT = tile_threads<L>();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
     cplx *tw = s + L * TILE_LINES;
     constexpr int N = L / 2;
     const int tid = threadIdx.x, line = tid & 7, r0 = tid >> 3;
-    constexpr int RSTEP = NT_FFT / TILE_LINES;
+    constexpr int RSTEP = NT / TILE_LINES;
     const size_t stride = (size_t)a.ncols;
     const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[blockIdx.y]) + (size_t)blockIdx.x * 8 + line;
     cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[blockIdx.y]) + (size_t)blockIdx.x * 8 + line;
-    load_twiddles<L>(tw, twg, tid, NT_FFT);
+    load_twiddles<L>(tw, twg, tid, NT);
     if (!FWD) {
         const int nk = a.nk;
         for (int n = r0; n <= N; n += RSTEP) {
@@ -71,7 +74,7 @@ __global__ void __launch_bounds__(NT_FFT) k_zpass(const __grid_constant__ ZArgs 
         }
     }
     __syncthreads();
-    fft_tile<L, -1, NT_FFT>(s, tw, tid);
+    fft_tile<L, -1, NT>(s, tw, tid);
     __syncthreads();
     if (!FWD) {
         for (int k = r0; k <= N; k += RSTEP) out[k * stride] = s[fft_pos<L>(k) * TILE_LINES + line];
@@ -99,19 +102,20 @@ struct YArgs {
 };
 
 template <int L, bool FWD>
-__global__ void __launch_bounds__(NT_FFT) k_ypass(const __grid_constant__ YArgs a, const cplx *__restrict__ twg) {
+__global__ void __launch_bounds__(tile_threads<L>()) k_ypass(const __grid_constant__ YArgs a, const cplx *__restrict__ twg) {
+    constexpr int NT = tile_threads<L>();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
     cplx *tw = s + L * TILE_LINES;
     const int tid = threadIdx.x, line = tid & 7, r0 = tid >> 3;
-    constexpr int RSTEP = NT_FFT / TILE_LINES;
+    constexpr int RSTEP = NT / TILE_LINES;
     const size_t pitch = (size_t)a.kxp;
     const int nky = a.nky, jpos = a.jpos;
     const size_t zin = (size_t)blockIdx.y * (FWD ? L : nky) * pitch;
     const size_t zout = (size_t)blockIdx.y * (FWD ? nky : L) * pitch;
     const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[blockIdx.z]) + zin + (size_t)blockIdx.x * 8 + line;
     cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[blockIdx.z]) + zout + (size_t)blockIdx.x * 8 + line;
-    load_twiddles<L>(tw, twg, tid, NT_FFT);
+    load_twiddles<L>(tw, twg, tid, NT);
     if (!FWD) {
         for (int j = r0; j < L; j += RSTEP) {
             // FFT-order row j holds j' = j (j < jpos) or j' = j - L (j >= L - (nky - jpos))
@@ -124,7 +128,7 @@ __global__ void __launch_bounds__(NT_FFT) k_ypass(const __grid_constant__ YArgs 
         for (int y = r0; y < L; y += RSTEP) s[y * TILE_LINES + line] = in[y * pitch];
     }
     __syncthreads();
-    fft_tile<L, (FWD ? -1 : +1), NT_FFT>(s, tw, tid);
+    fft_tile<L, (FWD ? -1 : +1), NT>(s, tw, tid);
     __syncthreads();
     if (!FWD) {
         for (int y = r0; y < L; y += RSTEP) out[y * pitch] = s[fft_pos<L>(y) * TILE_LINES + line];
@@ -153,15 +157,16 @@ struct XArgs {
 };
 
 template <int L, bool FWD>
-__global__ void __launch_bounds__(NT_FFT) k_xpass(const __grid_constant__ XArgs a, const cplx *__restrict__ twg) {
+__global__ void __launch_bounds__(tile_threads<L>()) k_xpass(const __grid_constant__ XArgs a, const cplx *__restrict__ twg) {
+    constexpr int NT = tile_threads<L>();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
     cplx *tw = s + L * TILE_LINES;
     const int tid = threadIdx.x, p = tid & 7, r0 = tid >> 3;
-    constexpr int RSTEP = NT_FFT / TILE_LINES;
+    constexpr int RSTEP = NT / TILE_LINES;
     const size_t lineA = (size_t)blockIdx.x * 16 + 2 * p;
     const int kxp = a.kxp, nkx = a.nkx;
-    load_twiddles<L>(tw, twg, tid, NT_FFT);
+    load_twiddles<L>(tw, twg, tid, NT);
     if (!FWD) {
         const cplx *__restrict__ inA = reinterpret_cast<const cplx *>(a.f.in[blockIdx.y]) + lineA * kxp;
         const cplx *__restrict__ inB = inA + kxp;
@@ -176,7 +181,7 @@ __global__ void __launch_bounds__(NT_FFT) k_xpass(const __grid_constant__ XArgs 
             }
         }
         __syncthreads();
-        fft_tile<L, +1, NT_FFT>(s, tw, tid);
+        fft_tile<L, +1, NT>(s, tw, tid);
         __syncthreads();
         double *__restrict__ outA = reinterpret_cast<double *>(a.f.out[blockIdx.y]) + lineA * L;
         double *__restrict__ outB = outA + L;
@@ -190,7 +195,7 @@ __global__ void __launch_bounds__(NT_FFT) k_xpass(const __grid_constant__ XArgs 
         const double *__restrict__ inB = inA + L;
         for (int x = r0; x < L; x += RSTEP) s[x * TILE_LINES + p] = make_double2(inA[x], inB[x]);
         __syncthreads();
-        fft_tile<L, -1, NT_FFT>(s, tw, tid);
+        fft_tile<L, -1, NT>(s, tw, tid);
         __syncthreads();
         cplx *__restrict__ outA = reinterpret_cast<cplx *>(a.f.out[blockIdx.y]) + lineA * kxp;
         cplx *__restrict__ outB = outA + kxp;

@@ -27,7 +27,7 @@ struct XFArgs {
 };
 
 template <int L>
-__global__ void __launch_bounds__(NT_FFT) k_xfused(const __grid_constant__ XFArgs a, const cplx *__restrict__ twx) {
+__global__ void __launch_bounds__(NT_FFT, (L >= 1024 ? 3 : 2)) k_xfused(const __grid_constant__ XFArgs a, const cplx *__restrict__ twx) {
     constexpr int H = L / 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);

@@ -219,8 +219,8 @@ cudaError_t launch_zpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, 
     LaunchScope ls(h, fwd ? KC_ZFWD : KC_ZBWD);
 #define ZL(LL)                                                                                          \
     {                                                                                                   \
-        if (fwd) k_zpass<LL, true><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                     \
-        else k_zpass<LL, false><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                        \
+        if (fwd) k_zpass<LL, true><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                     \
+        else k_zpass<LL, false><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                        \
     }
     DISPATCH_L(2 * h->d.N, ZL)
 #undef ZL
@@ -234,8 +234,8 @@ cudaError_t launch_ypass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, 
     LaunchScope ls(h, fwd ? KC_YFWD : KC_YBWD);
 #define YL(LL)                                                                                          \
     {                                                                                                   \
-        if (fwd) k_ypass<LL, true><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                     \
-        else k_ypass<LL, false><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                        \
+        if (fwd) k_ypass<LL, true><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                     \
+        else k_ypass<LL, false><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                        \
     }
     DISPATCH_L(h->d.ny, YL)
 #undef YL
@@ -249,8 +249,8 @@ cudaError_t launch_xpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, 
     LaunchScope ls(h, fwd ? KC_XFWD : KC_XBWD);
 #define XL(LL)                                                                                          \
     {                                                                                                   \
-        if (fwd) k_xpass<LL, true><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                     \
-        else k_xpass<LL, false><<<grid, NT_FFT, fft_smem<LL>(), h->st>>>(a, tw);                        \
+        if (fwd) k_xpass<LL, true><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                     \
+        else k_xpass<LL, false><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                        \
     }
     DISPATCH_L(h->d.nx, XL)
 #undef XL
