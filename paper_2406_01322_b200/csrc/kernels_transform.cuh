@@ -89,6 +89,86 @@ __global__ void __launch_bounds__(tile_threads<L>()) k_zpass(const __grid_consta
 }
 
 // ------------------------------------------------------------------------------------------
+// z pass, half-length form (the optimisation PAPER.md L178 attributes to Makhoul [32]: "does not require
+// performing a transform of size 2N but only of size N by re-ordering the input signal").
+// With e = even extension (length 2N) of the complex column, g_m = e_{2m}, h_m = e_{2m+1} (m < N):
+//   E_k = DFT_2N(e)_k = G_k + w_2N^k H_k.  Pack z_m = g_m + i h_m (complex arithmetic), Z = FFT_N(z).
+//   g is even (G_{N-k} = G_k) and h is half-sample symmetric (H_{N-k} = w_N^k H_k), so
+//   Z_k - Z_{N-k} = i (1 - w_N^k) H_k and
+//   E_k = Z_k + c_k (Z_k - Z_{N-k}),  c_k = -(1 + sin t)/(2 sin t) + i cos t/(2 sin t),  t = pi k / N,
+//   c_{N-k} = conj(c_k); k = 0 and k = N need H_0 = sum_m h_m (reduced while loading):
+//   G_0 = Z_0 - i H_0, E_0 = G_0 + H_0, E_N = G_0 - H_0.
+// One N-point complex FFT per complex column: half the flops and half the shared memory of the 2N form
+// (64 KB tile at N = 512, three CTAs per SM).  Rounding error is amplified by |c_k| <= ~N/(2 pi k) in the
+// lowest/highest modes (<= 1e-14 relative at N = 512; tolerance 1e-11).
+//   grid = (ncols/8, nfields); template N = nz - 1.
+// ------------------------------------------------------------------------------------------
+template <int N, bool FWD>
+__global__ void __launch_bounds__(NT_FFT) k_zpass_h(const __grid_constant__ ZArgs a, const cplx *__restrict__ tw2n,
+                                                    const cplx *__restrict__ ctab) {
+    constexpr int NT = NT_FFT;
+    constexpr int NW = NT / 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx *s = reinterpret_cast<cplx *>(smem_raw);
+    cplx *tw = s + N * TILE_LINES;
+    cplx *red = tw + N;                       // [NW][8] partial sums of H_0
+    const int tid = threadIdx.x, line = tid & 7, r0 = tid >> 3;
+    constexpr int RSTEP = NT / TILE_LINES;
+    const size_t stride = (size_t)a.ncols;
+    const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[blockIdx.y]) + (size_t)blockIdx.x * 8 + line;
+    cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[blockIdx.y]) + (size_t)blockIdx.x * 8 + line;
+    for (int i = tid; i < N; i += NT) tw[i] = tw2n[2 * i];
+    const int nin = FWD ? N + 1 : a.nk;       // input rows that are not structurally zero
+    cplx h0 = make_double2(0.0, 0.0);
+    for (int m = r0; m <= N / 2; m += RSTEP) {
+        const int ne = 2 * m;
+        cplx ev = make_double2(0.0, 0.0), op = ev, om = ev;
+        if (ne < nin) ev = in[ne * stride];
+        if (m < N / 2 && ne + 1 < nin) op = in[(ne + 1) * stride];
+        if (m >= 1 && ne - 1 < nin) om = in[(ne - 1) * stride];
+        if (!FWD) {                           // backward: interior coefficients enter with weight 1/2
+            if (ne > 0 && ne < N) ev = cscale(ev, 0.5);
+            op = cscale(op, 0.5);             // odd rows are always interior
+            om = cscale(om, 0.5);
+        }
+        // z_m = e_{2m} + i e_{2m+1} ; z_{N-m} = e_{2m} + i e_{2m-1}
+        if (m < N / 2) s[m * TILE_LINES + line] = make_double2(ev.x - op.y, ev.y + op.x);
+        if (m >= 1) s[(N - m) * TILE_LINES + line] = make_double2(ev.x - om.y, ev.y + om.x);
+        h0 = cadd(h0, cadd(op, om));
+    }
+    // reduce H_0 over the threads that share this line: lanes differ in bits 3, 4 within a warp
+    h0.x += __shfl_xor_sync(0xffffffffu, h0.x, 8);  h0.y += __shfl_xor_sync(0xffffffffu, h0.y, 8);
+    h0.x += __shfl_xor_sync(0xffffffffu, h0.x, 16); h0.y += __shfl_xor_sync(0xffffffffu, h0.y, 16);
+    if ((tid & 31) < 8) red[(tid >> 5) * 8 + line] = h0;
+    __syncthreads();
+    fft_tile<N, -1, NT>(s, tw, tid);
+    __syncthreads();
+    const int nout = FWD ? a.nk : N + 1;      // output rows kept
+    const double sc = FWD ? 1.0 / N : 1.0;
+    for (int k = r0; k <= N / 2; k += RSTEP) {
+        const int kb = N - k;
+        if (k == 0) {
+            cplx H0 = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int w = 0; w < NW; ++w) H0 = cadd(H0, red[w * 8 + line]);
+            const cplx z0 = s[line];          // fft_pos(0) = 0
+            const cplx G0 = make_double2(z0.x + H0.y, z0.y - H0.x);   // Z_0 - i H_0
+            out[0] = cscale(cadd(G0, H0), FWD ? 0.5 * sc : sc);
+            if (N < nout) out[(size_t)N * stride] = cscale(csub(G0, H0), FWD ? 0.5 * sc : sc);
+        } else {
+            const cplx za = s[fft_pos<N>(k) * TILE_LINES + line];
+            const cplx zb = s[fft_pos<N>(kb) * TILE_LINES + line];
+            const cplx c = ctab[k];
+            const cplx d = csub(za, zb);
+            const cplx cd = make_double2(c.x * d.x - c.y * d.y, c.x * d.y + c.y * d.x);     // c_k d
+            const cplx ccd = make_double2(c.x * d.x + c.y * d.y, c.x * d.y - c.y * d.x);    // conj(c_k) d
+            if (k < nout) out[(size_t)k * stride] = cscale(cadd(za, cd), sc);
+            if (kb != k && kb < nout) out[(size_t)kb * stride] = cscale(csub(zb, ccd), sc);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // y pass: complex <-> complex DFT of length ny per (ir, k) line (Z2Z).
 //   backward (row a3): nky retained rows (FFT order compacted) -> ny points, e^{+i ky y}
 //   forward  (row a7): ny points -> nky retained rows, e^{-i ky y} / ny

@@ -17,6 +17,33 @@
 
 namespace psdns {
 
+// ---- TMA (bulk async copy) + mbarrier helpers, sm_90+/sm_100a PTX ------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    unsigned done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    }
+}
+// global -> shared bulk copy (1-D TMA, SASS UBLKCP); bytes multiple of 16, both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 struct XFArgs {
     const cplx *in[8];
     cplx *out[8];
@@ -26,12 +53,18 @@ struct XFArgs {
     int phase;
 };
 
+// shared memory: tile [H][8] | twiddles [H] | stage [nin][kxp + 1] | mbarrier.  The stage receives the NEXT
+// line's nin spectra rows by TMA bulk copies while the current line is transformed (pitch kxp + 1 keeps the
+// 8 fields of one k in 8 different 16-byte bank groups).
 template <int L>
-__global__ void __launch_bounds__(NT_FFT, (L >= 1024 ? 3 : 2)) k_xfused(const __grid_constant__ XFArgs a, const cplx *__restrict__ twx) {
+__global__ void __launch_bounds__(NT_FFT, 2) k_xfused(const __grid_constant__ XFArgs a, const cplx *__restrict__ twx) {
     constexpr int H = L / 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
     cplx *tw = s + H * TILE_LINES;
+    cplx *stage = tw + H;
+    const int spitch = a.kxp + 1;
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)8 * spitch);
     const int tid = threadIdx.x, f = tid & 7, r0 = tid >> 3;
     constexpr int RSTEP = NT_FFT / TILE_LINES;
     const int kxp = a.kxp, nkx = a.nkx;
@@ -39,15 +72,29 @@ __global__ void __launch_bounds__(NT_FFT, (L >= 1024 ? 3 : 2)) k_xfused(const __
     const cplx *inf = a.in[f < a.nin ? f : 0];   // may alias outf (in-place per line)
     cplx *outf = a.out[f < a.nout ? f : 0];
     const double sc = 1.0 / L;
+    const unsigned row_bytes = (unsigned)(nkx * sizeof(cplx));
+    auto issue = [&](int line) {   // one thread: arm the barrier and launch nin bulk copies
+        mbar_expect_tx(bar, row_bytes * a.nin);
+        for (int q = 0; q < a.nin; ++q) bulk_g2s(stage + (size_t)q * spitch, a.in[q] + (size_t)line * kxp, row_bytes, bar);
+    };
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        if ((int)blockIdx.x < a.nlines) issue(blockIdx.x);
+    }
+    __syncthreads();
+    unsigned parity = 0;
+    const cplx *sf = stage + (size_t)(f < a.nin ? f : 0) * spitch;
     for (int line = blockIdx.x; line < a.nlines; line += gridDim.x) {
         const size_t base = (size_t)line * kxp;
-        // ---- load + pre-twiddle (pairs k, H-k) ----
+        mbar_wait(bar, parity);
+        parity ^= 1;
+        // ---- pre-twiddle from the staged rows (pairs k, H-k) ----
         for (int k = r0; k <= H / 2; k += RSTEP) {
             const int kb = H - k;
             cplx xa = make_double2(0.0, 0.0), xb = xa;
             if (f < a.nin) {
-                if (k < nkx) xa = inf[base + k];
-                if (kb < nkx) xb = inf[base + kb];
+                if (k < nkx) xa = sf[k];
+                if (kb < nkx) xb = sf[kb];
             }
             if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
             const cplx w = twx[k];
@@ -59,6 +106,10 @@ __global__ void __launch_bounds__(NT_FFT, (L >= 1024 ? 3 : 2)) k_xfused(const __
             if (k != 0 && kb != k) s[tile_idx<true>(kb, f)] = cconj(csub(S, T));
         }
         __syncthreads();
+        if (tid == 0 && line + (int)gridDim.x < a.nlines) {   // stage is free: prefetch the next line
+            fence_proxy_async();
+            issue(line + gridDim.x);
+        }
         fft_tile<H, +1, NT_FFT, true>(s, tw, tid);
         __syncthreads();
         // ---- pointwise: each thread owns whole rows (both packed points x_{2n}, x_{2n+1}) ----

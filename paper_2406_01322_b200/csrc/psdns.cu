@@ -45,6 +45,7 @@ struct Dims {
 
 struct Layout {
     size_t tw_x, tw_y, tw_z;
+    size_t ctab_z;                     // c_k of the half-length Chebyshev transform, k <= N/2
     size_t state[5];                   // u v w phi theta
     size_t hist[3];
     size_t dinv[3];                    // NS (beta^2), PO (k^2), CH (k^2 + lambda)
@@ -77,7 +78,7 @@ struct psdns_handle {
     int timed_class;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tevents;
     int nf_in, nf_out;
-    bool use_xfused;
+    bool use_xfused, use_zhalf;
 
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
 };
@@ -122,6 +123,7 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.tw_x = take(d.nx * C);
     L.tw_y = take(d.ny * C);
     L.tw_z = take(2 * d.N * C);
+    L.ctab_z = take((d.N / 2 + 1) * C);
     for (int i = 0; i < 5; ++i) L.state[i] = take(d.s_ret * C);
     for (int i = 0; i < 3; ++i) L.hist[i] = take(d.s_low * C);
     for (int i = 0; i < 3; ++i) L.dinv[i] = take(d.s_ret * sizeof(double));
@@ -191,8 +193,9 @@ ColGeom geom(const psdns_handle *h) {
 template <int L>
 size_t fft_smem() { return (size_t)(L * TILE_LINES + L) * sizeof(cplx); }
 
+// tile + twiddles + stage [8][kxp + 1] + mbarrier
 template <int L>
-size_t xfused_smem() { return (size_t)((L / 2) * TILE_LINES + L / 2) * sizeof(cplx); }
+size_t xfused_smem(int kxp) { return (size_t)((L / 2) * TILE_LINES + L / 2 + 8 * (kxp + 1)) * sizeof(cplx) + 16; }
 
 template <class K>
 cudaError_t set_smem(K kern, size_t bytes) {
@@ -212,11 +215,37 @@ cudaError_t set_smem(K kern, size_t bytes) {
         default: return cudaErrorInvalidValue; \
     }
 
+template <int N>
+size_t zhalf_smem() { return (size_t)(N * TILE_LINES + N + (NT_FFT / 32) * 8) * sizeof(cplx); }
+
+#define DISPATCH_N(Nval, MACRO)            \
+    switch (Nval) {                        \
+        case 8: MACRO(8); break;           \
+        case 16: MACRO(16); break;         \
+        case 32: MACRO(32); break;         \
+        case 64: MACRO(64); break;         \
+        case 128: MACRO(128); break;       \
+        case 256: MACRO(256); break;       \
+        case 512: MACRO(512); break;       \
+        default: return cudaErrorInvalidValue; \
+    }
+
 cudaError_t launch_zpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, size_t ncols, int nk) {
     ZArgs a; a.f = f; a.ncols = (int)ncols; a.nk = nk;
     const cplx *tw = h->at<cplx>(h->L.tw_z);
     dim3 grid((unsigned)(ncols / 8), nf);
     LaunchScope ls(h, fwd ? KC_ZFWD : KC_ZBWD);
+    if (h->use_zhalf) {
+        const cplx *ct = h->at<cplx>(h->L.ctab_z);
+#define ZH(NN)                                                                                           \
+    {                                                                                                    \
+        if (fwd) k_zpass_h<NN, true><<<grid, NT_FFT, zhalf_smem<NN>(), h->st>>>(a, tw, ct);              \
+        else k_zpass_h<NN, false><<<grid, NT_FFT, zhalf_smem<NN>(), h->st>>>(a, tw, ct);                 \
+    }
+        DISPATCH_N(h->d.N, ZH)
+#undef ZH
+        return cudaGetLastError();
+    }
 #define ZL(LL)                                                                                          \
     {                                                                                                   \
         if (fwd) k_zpass<LL, true><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                     \
@@ -264,9 +293,12 @@ cudaError_t setup_attrs(psdns_handle *h) {
 #define XA(LL) { CU0(set_smem(k_xpass<LL, true>, fft_smem<LL>())); CU0(set_smem(k_xpass<LL, false>, fft_smem<LL>())); }
 #define CU0(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) return e__; } while (0)
     DISPATCH_L(2 * h->d.N, ZA)
+#define ZHA(NN) { CU0(set_smem(k_zpass_h<NN, true>, zhalf_smem<NN>())); CU0(set_smem(k_zpass_h<NN, false>, zhalf_smem<NN>())); }
+    DISPATCH_N(h->d.N, ZHA)
+#undef ZHA
     DISPATCH_L(h->d.ny, YA)
     DISPATCH_L(h->d.nx, XA)
-#define XFA(LL) { CU0(set_smem(k_xfused<LL>, xfused_smem<LL>())); }
+#define XFA(LL) { CU0(set_smem(k_xfused<LL>, xfused_smem<LL>(h->d.kxp))); }
     DISPATCH_L(h->d.nx, XFA)
 #undef XFA
 #undef ZA
@@ -278,9 +310,9 @@ cudaError_t setup_attrs(psdns_handle *h) {
 
 cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
     const cplx *tw = h->at<cplx>(h->L.tw_x);
-    const int grid = std::min(a.nlines, 148 * 12);
+    const int grid = std::min(a.nlines, 148 * 2 * 4);
     LaunchScope ls(h, KC_XFUSED);
-#define XF(LL) k_xfused<LL><<<grid, NT_FFT, xfused_smem<LL>(), h->st>>>(a, tw);
+#define XF(LL) k_xfused<LL><<<grid, NT_FFT, xfused_smem<LL>(h->d.kxp), h->st>>>(a, tw);
     DISPATCH_L(h->d.nx, XF)
 #undef XF
     return cudaGetLastError();
@@ -484,6 +516,17 @@ cudaError_t build_tables(psdns_handle *h) {
     CU(fill(L.tw_x, d.nx));
     CU(fill(L.tw_y, d.ny));
     CU(fill(L.tw_z, 2 * d.N));
+    {   // c_k = -(1 + sin t)/(2 sin t) + i cos t/(2 sin t), t = pi k / N  (kernels_transform.cuh, k_zpass_h)
+        std::vector<cplx> t(d.N / 2 + 1);
+        t[0] = make_double2(0.0, 0.0);
+        for (int k = 1; k <= d.N / 2; ++k) {
+            const long double th = 3.14159265358979323846264338327950288L * (long double)k / (long double)d.N;
+            const long double sn = sinl(th), cs = cosl(th);
+            t[k] = make_double2((double)(-(1.0L + sn) / (2.0L * sn)), (double)(cs / (2.0L * sn)));
+        }
+        CU(cudaMemcpyAsync(h->ws + L.ctab_z, t.data(), t.size() * sizeof(cplx), cudaMemcpyHostToDevice, h->st));
+        CU(cudaStreamSynchronize(h->st));
+    }
     const Coefs c = coefs(h->p);
     const double shifts[3] = {1.0 / c.gamma, 0.0, c.lam_phi};
     for (int t = 0; t < 3; ++t) {
@@ -549,6 +592,7 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->has_state = false; h->graph = nullptr; h->graph_ready = false;
     h->use_graph = std::getenv("PSDNS_NO_GRAPH") == nullptr;
     h->use_xfused = std::getenv("PSDNS_NO_XFUSE") == nullptr;
+    h->use_zhalf = std::getenv("PSDNS_Z2N") == nullptr;
     h->launches = 0; h->per_step = 0; h->timed_class = -1;
     const bool phase = params->phase_field != 0;
     const bool visc = phase && params->visc_ratio != 1.0;
