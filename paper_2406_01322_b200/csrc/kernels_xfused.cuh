@@ -1,16 +1,22 @@
-// Fused x pass (rows a4 + a5 + a6): for one (k, y) line at a time, C2R of the 7 input fields,
-// pointwise non-linear terms, R2C of the 8 product fields - physical-space arrays never reach HBM
+// Fused x pass (rows a4 + a5 + a6): for one (k, y) line at a time, C2R of the input fields,
+// pointwise non-linear terms, R2C of the product fields - physical-space arrays never reach HBM
 // ("physical-space arrays never leave the SM"; PAPER.md L166-176 for the transforms,
 // L182-196 and Eqs. 1, 4, 7, 8 for the products).
 //
-// Tile: the 8 tile lines of fft_tile are the FIELDS; the FFT is the half-length real transform:
-//   backward: Z_k = (X_k + conj X_{H-k}) + i conj(w_k) (X_k - conj X_{H-k}),  w_k = exp(-2 pi i k / L), H = L/2,
+// Tile: 8 FIELDS side by side, s[row][field]; the FFT is the half-length real transform (H = L/2):
+//   backward: Z_k = (X_k + conj X_{H-k}) + i conj(w_k) (X_k - conj X_{H-k}),  w_k = exp(-2 pi i k / L),
 //             z = IFFT_H(Z) gives z_n = x_{2n} + i x_{2n+1}
 //   forward : A_k = (Z_k + conj Z_{H-k})/2, B_k = (Z_k - conj Z_{H-k})/(2i), X_k = (A_k + w_k B_k)/L
-// so one line of 8 fields at nx = 1024 is 64 KB of shared memory (3 CTAs per SM).  The backward FFT is
-// decimation in frequency (digit-reversed output), the products are elementwise so order does not matter,
-// and the forward FFT is decimation in time (digit-reversed input, natural output): no reordering at all.
-// The swizzled tile layout makes both the butterflies and the per-row pointwise stage bank-conflict free.
+// with H = R1 * R2 * 2.  Shared-memory traffic is what bounds this kernel (128 B/clk/SM), so every stage
+// that can stay in registers does:
+//   A  pre-twiddle straight from the TMA-staged spectra + DIF pass R1            -> tile
+//   B  DIF pass R2                                                   tile -> tile
+//   C  DIF radix 2 + pointwise products + DIT radix 2 (a thread owns two rows x all 8 fields)
+//   D  DIT pass R2                                                   tile -> tile
+//   E  DIT pass R1, results kept in registers and published to the tile
+//   F  post-twiddle with the partner row H-k read from the tile, truncated store to HBM
+// i.e. 5 tile round trips per line instead of 9.  The backward FFT is decimation in frequency, the
+// products are elementwise, the forward FFT is decimation in time: no reordering anywhere.
 #pragma once
 #include "fft_tile.cuh"
 #include "kernels_transform.cuh"
@@ -44,38 +50,144 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// ---- plan of the half-length FFT: H = R1 * R2 * 2 ---------------------------------------------------
+template <int H> struct XPlan;
+template <> struct XPlan<8>   { static constexpr int R1 = 4,  R2 = 1; };
+template <> struct XPlan<16>  { static constexpr int R1 = 8,  R2 = 1; };
+template <> struct XPlan<32>  { static constexpr int R1 = 16, R2 = 1; };
+template <> struct XPlan<64>  { static constexpr int R1 = 8,  R2 = 4; };
+template <> struct XPlan<128> { static constexpr int R1 = 8,  R2 = 8; };
+template <> struct XPlan<256> { static constexpr int R1 = 16, R2 = 8; };
+template <> struct XPlan<512> { static constexpr int R1 = 16, R2 = 16; };
+
+// threads per CTA: one thread per (butterfly of pass R1, field)
+template <int L> __host__ __device__ constexpr int xf_threads() {
+    return (8 * (L / 2) / XPlan<L / 2>::R1) > 64 ? (8 * (L / 2) / XPlan<L / 2>::R1) : 64;
+}
+
+// tile index: the field slot is rotated by row/2, so that (i) a quarter-warp that touches one row with its
+// 8 fields and (ii) 8 consecutive threads that each touch their own row PAIR (2t, 2t+1) at the same field
+// both cover all eight 16-byte bank groups: conflict free in every stage.
+__device__ __forceinline__ int xidx(int row, int f) { return row * TILE_LINES + ((f + (row >> 1)) & (TILE_LINES - 1)); }
+
+// w_H^i = w_L^{2i} from the table tw[k] = w_L^k, k < H (w_L^{k+H} = -w_L^k), 0 <= i < H
+template <int H>
+__device__ __forceinline__ cplx tw_half(const cplx *__restrict__ tw, int i) {
+    const int idx = 2 * i;
+    cplx w = tw[idx & (H - 1)];
+    const int sgn = (idx & H) ? (int)0x80000000 : 0;
+    w.x = __hiloint2double(__double2hiint(w.x) ^ sgn, __double2loint(w.x));
+    w.y = __hiloint2double(__double2hiint(w.y) ^ sgn, __double2loint(w.y));
+    return w;
+}
+
+// in-place DIF pass on the x tile (sub-length LS, radix R): butterfly, then twiddle
+template <int H, int LS, int R, int SIGN, int NT>
+__device__ __forceinline__ void xpass_dif(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid) {
+    constexpr int STRIDE = LS / R;
+    constexpr int NBF = H / R;
+    const int f = tid & (TILE_LINES - 1);
+    for (int b = tid >> 3; b < NBF; b += NT / TILE_LINES) {
+        const int blk = b / STRIDE, j = b % STRIDE;
+        const int row0 = blk * LS + j;
+        cplx v[R];
+#pragma unroll
+        for (int m = 0; m < R; ++m) v[m] = s[xidx(row0 + m * STRIDE, f)];
+        RegFFT<R, SIGN>::run(v);
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            cplx o = v[q];
+            if (LS > R && q > 0) o = cmultw<SIGN>(o, tw_half<H>(tw, (H / LS) * j * q));
+            s[xidx(row0 + q * STRIDE, f)] = o;
+        }
+    }
+}
+
+// in-place DIT pass: twiddle the inputs, then butterfly
+template <int H, int LS, int R, int SIGN, int NT>
+__device__ __forceinline__ void xpass_dit(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid) {
+    constexpr int STRIDE = LS / R;
+    constexpr int NBF = H / R;
+    const int f = tid & (TILE_LINES - 1);
+    for (int b = tid >> 3; b < NBF; b += NT / TILE_LINES) {
+        const int blk = b / STRIDE, j = b % STRIDE;
+        const int row0 = blk * LS + j;
+        cplx v[R];
+#pragma unroll
+        for (int m = 0; m < R; ++m) {
+            cplx x = s[xidx(row0 + m * STRIDE, f)];
+            if (LS > R && m > 0) x = cmultw<SIGN>(x, tw_half<H>(tw, (H / LS) * j * m));
+            v[m] = x;
+        }
+        RegFFT<R, SIGN>::run(v);
+#pragma unroll
+        for (int q = 0; q < R; ++q) s[xidx(row0 + q * STRIDE, f)] = v[q];
+    }
+}
+
+// ---- pointwise products at one grid point (row a5; Eqs. 1, 4, 7, 8) --------------------------
+//   in : u v w [phi phx phy phz]      out: Txx Txy Txz Tyy Tyz Tzz [Q C]
+//   T_ij = -u_i u_j + cs (|grad phi|^2 delta_ij - phi_i phi_j),  Q = u . grad phi,  C = phi^3
+template <bool PHASE>
+__device__ __forceinline__ void nl_point(const double (&in)[8], double (&o)[8], double cs) {
+    const double u = in[0], v = in[1], w = in[2];
+    double txx = -u * u, txy = -u * v, txz = -u * w, tyy = -v * v, tyz = -v * w, tzz = -w * w;
+    if (PHASE) {
+        const double ph = in[3], px = in[4], py = in[5], pz = in[6];
+        const double g2 = px * px + py * py + pz * pz;
+        txx += cs * (g2 - px * px);
+        tyy += cs * (g2 - py * py);
+        tzz += cs * (g2 - pz * pz);
+        txy -= cs * px * py;
+        txz -= cs * px * pz;
+        tyz -= cs * py * pz;
+        o[6] = u * px + v * py + w * pz;
+        o[7] = ph * ph * ph;
+    } else {
+        o[6] = 0.0; o[7] = 0.0;
+    }
+    o[0] = txx; o[1] = txy; o[2] = txz; o[3] = tyy; o[4] = tyz; o[5] = tzz;
+}
+
 struct XFArgs {
     const cplx *in[8];
     cplx *out[8];
     int kxp, nkx, nlines;
-    int nin, nout;
     double cs;
-    int phase;
 };
 
-// shared memory: tile [H][8] | twiddles [H] | stage [nin][kxp + 1] | mbarrier.  The stage receives the NEXT
-// line's nin spectra rows by TMA bulk copies while the current line is transformed (pitch kxp + 1 keeps the
-// 8 fields of one k in 8 different 16-byte bank groups).
-template <int L>
-__global__ void __launch_bounds__(NT_FFT, 2) k_xfused(const __grid_constant__ XFArgs a, const cplx *__restrict__ twx) {
+// stage pitch (cplx): odd, so that the 8 fields of one k sit in 8 different 16-byte bank groups
+__host__ __device__ inline int xf_spitch(int nkx) { return nkx | 1; }
+
+// shared memory: tile [H][8] | twiddles w_L^k [H] | stage [NIN][spitch] | mbarrier.  The stage receives the
+// NEXT line's NIN spectra rows by TMA bulk copies while the current line is transformed.
+template <int L, bool PHASE>
+__global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused(const __grid_constant__ XFArgs a,
+                                                                               const cplx *__restrict__ twx) {
     constexpr int H = L / 2;
+    constexpr int R1 = XPlan<H>::R1, R2 = XPlan<H>::R2;
+    constexpr int NT = xf_threads<L>();
+    constexpr int S1 = H / R1;              // stride of pass R1 = number of its butterflies per field
+    constexpr int NIN = PHASE ? 7 : 3, NOUT = PHASE ? 8 : 6;
+    static_assert(R1 * R2 * 2 == H, "plan");
+    static_assert(S1 * TILE_LINES <= NT, "one (butterfly, field) item per thread in stages A and E");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
     cplx *tw = s + H * TILE_LINES;
     cplx *stage = tw + H;
-    const int spitch = a.kxp + 1;
-    unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)8 * spitch);
-    const int tid = threadIdx.x, f = tid & 7, r0 = tid >> 3;
-    constexpr int RSTEP = NT_FFT / TILE_LINES;
     const int kxp = a.kxp, nkx = a.nkx;
-    for (int i = tid; i < H; i += NT_FFT) tw[i] = twx[2 * i];
-    const cplx *inf = a.in[f < a.nin ? f : 0];   // may alias outf (in-place per line)
-    cplx *outf = a.out[f < a.nout ? f : 0];
-    const double sc = 1.0 / L;
+    const int spitch = xf_spitch(nkx);
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)NIN * spitch);
+    const int tid = threadIdx.x, f = tid & 7, j = tid >> 3;
+    const bool item = j < S1;               // this thread owns butterfly j of field f in stages A, E, F
+    for (int i = tid; i < H; i += NT) tw[i] = twx[i];
+    cplx *outf = a.out[f < NOUT ? f : 0];
+    const double sc = 0.5 / L;
     const unsigned row_bytes = (unsigned)(nkx * sizeof(cplx));
-    auto issue = [&](int line) {   // one thread: arm the barrier and launch nin bulk copies
-        mbar_expect_tx(bar, row_bytes * a.nin);
-        for (int q = 0; q < a.nin; ++q) bulk_g2s(stage + (size_t)q * spitch, a.in[q] + (size_t)line * kxp, row_bytes, bar);
+    auto issue = [&](int line) {   // one thread: arm the barrier and launch NIN bulk copies
+        mbar_expect_tx(bar, row_bytes * NIN);
+#pragma unroll
+        for (int q = 0; q < NIN; ++q) bulk_g2s(stage + (size_t)q * spitch, a.in[q] + (size_t)line * kxp, row_bytes, bar);
     };
     if (tid == 0) {
         mbar_init(bar, 1);
@@ -83,86 +195,110 @@ __global__ void __launch_bounds__(NT_FFT, 2) k_xfused(const __grid_constant__ XF
     }
     __syncthreads();
     unsigned parity = 0;
-    const cplx *sf = stage + (size_t)(f < a.nin ? f : 0) * spitch;
+    const cplx *sf = stage + (size_t)(f < NIN ? f : 0) * spitch;
     for (int line = blockIdx.x; line < a.nlines; line += gridDim.x) {
         const size_t base = (size_t)line * kxp;
         mbar_wait(bar, parity);
         parity ^= 1;
-        // ---- pre-twiddle from the staged rows (pairs k, H-k) ----
-        for (int k = r0; k <= H / 2; k += RSTEP) {
-            const int kb = H - k;
-            cplx xa = make_double2(0.0, 0.0), xb = xa;
-            if (f < a.nin) {
-                if (k < nkx) xa = sf[k];
-                if (kb < nkx) xb = sf[kb];
+        // ---- A: pre-twiddle from the staged rows + DIF pass R1 (inverse transform, sign +) ----
+        if (item) {
+            cplx v[R1];
+#pragma unroll
+            for (int m = 0; m < R1; ++m) {
+                const int k = j + S1 * m, kb = H - k;
+                cplx xa = make_double2(0.0, 0.0), xb = xa;
+                if (f < NIN) {
+                    if (k < nkx) xa = sf[k];
+                    if (kb < nkx) xb = sf[kb];
+                }
+                if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
+                const cplx w = tw[k];
+                const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
+                // Z = S + i conj(w) D
+                v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
             }
-            if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
-            const cplx w = twx[k];
-            const cplx S = make_double2(xa.x + xb.x, xa.y - xb.y);
-            const cplx D = make_double2(xa.x - xb.x, xa.y + xb.y);
-            // T = i * conj(w) * D
-            const cplx T = make_double2(-(w.x * D.y - w.y * D.x), w.x * D.x + w.y * D.y);
-            s[tile_idx<true>(k, f)] = cadd(S, T);
-            if (k != 0 && kb != k) s[tile_idx<true>(kb, f)] = cconj(csub(S, T));
+            RegFFT<R1, +1>::run(v);
+#pragma unroll
+            for (int q = 0; q < R1; ++q) {
+                cplx o = v[q];
+                if (q > 0) o = cmultw<+1>(o, tw_half<H>(tw, j * q));
+                s[xidx(j + S1 * q, f)] = o;
+            }
         }
         __syncthreads();
         if (tid == 0 && line + (int)gridDim.x < a.nlines) {   // stage is free: prefetch the next line
             fence_proxy_async();
             issue(line + gridDim.x);
         }
-        fft_tile<H, +1, NT_FFT, true>(s, tw, tid);
-        __syncthreads();
-        // ---- pointwise: each thread owns whole rows (both packed points x_{2n}, x_{2n+1}) ----
-        for (int r = tid; r < H; r += NT_FFT) {
-            cplx v[8];
+        // ---- B: DIF pass R2 ----
+        if constexpr (R2 > 1) {
+            xpass_dif<H, H / R1, R2, +1, NT>(s, tw, tid);
+            __syncthreads();
+        }
+        // ---- C: last DIF radix 2, pointwise products, first DIT radix 2: rows (2t, 2t+1) x all fields ----
+        for (int t = tid; t < H / 2; t += NT) {
+            cplx z0[8], z1[8];
 #pragma unroll
-            for (int q = 0; q < 8; ++q) v[q] = s[tile_idx<true>(r, q)];
-            cplx o[8];
-#pragma unroll
-            for (int c = 0; c < 2; ++c) {
-                const double u = c ? v[0].y : v[0].x, vv = c ? v[1].y : v[1].x, w = c ? v[2].y : v[2].x;
-                double txx = -u * u, txy = -u * vv, txz = -u * w, tyy = -vv * vv, tyz = -vv * w, tzz = -w * w;
-                double qq = 0.0, cc = 0.0;
-                if (a.phase) {
-                    const double ph = c ? v[3].y : v[3].x, px = c ? v[4].y : v[4].x, py = c ? v[5].y : v[5].x,
-                                 pz = c ? v[6].y : v[6].x;
-                    const double g2 = px * px + py * py + pz * pz;
-                    const double cs = a.cs;
-                    txx += cs * (g2 - px * px);
-                    tyy += cs * (g2 - py * py);
-                    tzz += cs * (g2 - pz * pz);
-                    txy -= cs * px * py;
-                    txz -= cs * px * pz;
-                    tyz -= cs * py * pz;
-                    qq = u * px + vv * py + w * pz;
-                    cc = ph * ph * ph;
-                }
-                if (c == 0) {
-                    o[0].x = txx; o[1].x = txy; o[2].x = txz; o[3].x = tyy; o[4].x = tyz; o[5].x = tzz; o[6].x = qq; o[7].x = cc;
-                } else {
-                    o[0].y = txx; o[1].y = txy; o[2].y = txz; o[3].y = tyy; o[4].y = tyz; o[5].y = tzz; o[6].y = qq; o[7].y = cc;
-                }
+            for (int q = 0; q < NIN; ++q) {
+                const cplx p = s[xidx(2 * t, q)], m = s[xidx(2 * t + 1, q)];
+                z0[q] = cadd(p, m);
+                z1[q] = csub(p, m);
             }
+            double in[8], o00[8], o01[8], o10[8], o11[8];
 #pragma unroll
-            for (int q = 0; q < 8; ++q) s[tile_idx<true>(r, q)] = o[q];
+            for (int q = 0; q < NIN; ++q) in[q] = z0[q].x;
+            nl_point<PHASE>(in, o00, a.cs);
+#pragma unroll
+            for (int q = 0; q < NIN; ++q) in[q] = z0[q].y;
+            nl_point<PHASE>(in, o01, a.cs);
+#pragma unroll
+            for (int q = 0; q < NIN; ++q) in[q] = z1[q].x;
+            nl_point<PHASE>(in, o10, a.cs);
+#pragma unroll
+            for (int q = 0; q < NIN; ++q) in[q] = z1[q].y;
+            nl_point<PHASE>(in, o11, a.cs);
+#pragma unroll
+            for (int q = 0; q < NOUT; ++q) {
+                s[xidx(2 * t, q)] = make_double2(o00[q] + o10[q], o01[q] + o11[q]);
+                s[xidx(2 * t + 1, q)] = make_double2(o00[q] - o10[q], o01[q] - o11[q]);
+            }
         }
         __syncthreads();
-        fft_tile_dit<H, -1, NT_FFT, true>(s, tw, tid);
-        __syncthreads();
-        // ---- post-twiddle + truncated store ----
-        if (f < a.nout) {
-            for (int k = r0; k <= H / 2; k += RSTEP) {
-                const int kb = H - k;
-                const cplx za = s[tile_idx<true>(k, f)];
-                const cplx zb = s[tile_idx<true>(kb & (H - 1), f)];
-                const cplx A = make_double2(0.5 * (za.x + zb.x), 0.5 * (za.y - zb.y));
-                const cplx B = make_double2(0.5 * (za.y + zb.y), -0.5 * (za.x - zb.x));
-                const cplx w = twx[k];
-                const cplx wB = make_double2(w.x * B.x - w.y * B.y, w.x * B.y + w.y * B.x);
-                if (k < nkx) outf[base + k] = cscale(cadd(A, wB), sc);
-                if (k != kb && kb < nkx) outf[base + kb] = cscale(cconj(csub(A, wB)), sc);   // k = 0: X_H = A_0 - B_0
+        // ---- D: DIT pass R2 (forward transform, sign -) ----
+        if constexpr (R2 > 1) {
+            xpass_dit<H, 2 * R2, R2, -1, NT>(s, tw, tid);
+            __syncthreads();
+        }
+        // ---- E: DIT pass R1, results stay in registers and are published to the tile ----
+        cplx v[R1];
+        if (item) {
+#pragma unroll
+            for (int m = 0; m < R1; ++m) {
+                cplx x = s[xidx(j + S1 * m, f)];
+                if (m > 0) x = cmultw<-1>(x, tw_half<H>(tw, j * m));
+                v[m] = x;
             }
-            for (int i = nkx + r0; i < kxp; i += RSTEP) outf[base + i] = make_double2(0.0, 0.0);
+            RegFFT<R1, -1>::run(v);
+#pragma unroll
+            for (int q = 0; q < R1; ++q) s[xidx(j + S1 * q, f)] = v[q];
+        }
+        __syncthreads();
+        // ---- F: post-twiddle against the partner row H - k, truncated store ----
+        if (item && f < NOUT) {
+#pragma unroll
+            for (int q = 0; q < R1; ++q) {
+                const int k = j + S1 * q;
+                if (k < nkx) {
+                    const cplx za = v[q];
+                    const cplx zb = s[xidx((H - k) & (H - 1), f)];
+                    const cplx w = tw[k];
+                    const double Sx = za.x + zb.x, Sy = za.y - zb.y, Dx = za.x - zb.x, Dy = za.y + zb.y;
+                    // X_k = (S - i w D) / (2 L)
+                    outf[base + k] = make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy)));
+                } else if (k < kxp) {
+                    outf[base + k] = make_double2(0.0, 0.0);
+                }
+            }
         }
         __syncthreads();
     }

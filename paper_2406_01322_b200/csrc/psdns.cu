@@ -79,6 +79,7 @@ struct psdns_handle {
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tevents;
     int nf_in, nf_out;
     bool use_xfused, use_zhalf;
+    int xf_occ, n_sm;
 
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
 };
@@ -193,9 +194,9 @@ ColGeom geom(const psdns_handle *h) {
 template <int L>
 size_t fft_smem() { return (size_t)(L * TILE_LINES + L) * sizeof(cplx); }
 
-// tile + twiddles + stage [8][kxp + 1] + mbarrier
+// tile + twiddles + stage [nin][spitch] + mbarrier
 template <int L>
-size_t xfused_smem(int kxp) { return (size_t)((L / 2) * TILE_LINES + L / 2 + 8 * (kxp + 1)) * sizeof(cplx) + 16; }
+size_t xfused_smem(int nkx, int nin) { return (size_t)((L / 2) * TILE_LINES + L / 2 + nin * xf_spitch(nkx)) * sizeof(cplx) + 16; }
 
 template <class K>
 cudaError_t set_smem(K kern, size_t bytes) {
@@ -298,8 +299,20 @@ cudaError_t setup_attrs(psdns_handle *h) {
 #undef ZHA
     DISPATCH_L(h->d.ny, YA)
     DISPATCH_L(h->d.nx, XA)
-#define XFA(LL) { CU0(set_smem(k_xfused<LL>, xfused_smem<LL>(h->d.kxp))); }
-    DISPATCH_L(h->d.nx, XFA)
+#define XFA(LL)                                                                                              \
+    {                                                                                                        \
+        const size_t sm = xfused_smem<LL>(h->d.nkx, h->nf_in);                                               \
+        int occ = 0;                                                                                         \
+        if (h->p.phase_field) {                                                                              \
+            CU0(set_smem(k_xfused<LL, true>, sm));                                                           \
+            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfused<LL, true>, xf_threads<LL>(), sm)); \
+        } else {                                                                                             \
+            CU0(set_smem(k_xfused<LL, false>, sm));                                                          \
+            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfused<LL, false>, xf_threads<LL>(), sm)); \
+        }                                                                                                    \
+        h->xf_occ = occ;                                                                                     \
+    }
+    if (h->nf_in <= 7) { DISPATCH_L(h->d.nx, XFA) }
 #undef XFA
 #undef ZA
 #undef YA
@@ -310,9 +323,14 @@ cudaError_t setup_attrs(psdns_handle *h) {
 
 cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
     const cplx *tw = h->at<cplx>(h->L.tw_x);
-    const int grid = std::min(a.nlines, 148 * 2 * 4);
+    const int grid = std::min(a.nlines, h->n_sm * std::max(h->xf_occ, 1));   // persistent: one wave
     LaunchScope ls(h, KC_XFUSED);
-#define XF(LL) k_xfused<LL><<<grid, NT_FFT, xfused_smem<LL>(h->d.kxp), h->st>>>(a, tw);
+#define XF(LL)                                                                                               \
+    {                                                                                                        \
+        const size_t sm = xfused_smem<LL>(h->d.nkx, h->nf_in);                                               \
+        if (h->p.phase_field) k_xfused<LL, true><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);              \
+        else k_xfused<LL, false><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);                              \
+    }
     DISPATCH_L(h->d.nx, XF)
 #undef XF
     return cudaGetLastError();
@@ -411,8 +429,8 @@ cudaError_t enqueue_step(psdns_handle *h) {
         // a4 + a5 + a6 fused: physical space never leaves the SM; in place on the Y arrays
         XFArgs a;
         for (int i = 0; i < 8; ++i) { a.in[i] = h->at<cplx>(L.yb[i < nin ? i : 0]); a.out[i] = h->at<cplx>(L.yb[i < nout ? i : 0]); }
-        a.kxp = d.kxp; a.nkx = d.nkx; a.nlines = d.nz * d.ny; a.nin = nin; a.nout = nout;
-        a.cs = c.cs; a.phase = phase;
+        a.kxp = d.kxp; a.nkx = d.nkx; a.nlines = d.nz * d.ny;
+        a.cs = c.cs;
         CU(launch_xfused(h, a));
     } else {
         CU(launch_xpass(h, false, fx, nin, d.kxp, d.nkx));
@@ -598,6 +616,12 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     const bool visc = phase && params->visc_ratio != 1.0;
     h->nf_in = phase ? (visc ? 12 : 7) : 3;
     h->nf_out = phase ? 8 : 6;
+    h->xf_occ = 1; h->n_sm = 148;
+    {
+        int dev = 0, nsm = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0)
+            h->n_sm = nsm;
+    }
     if (bytes < h->L.total || ((uintptr_t)d_workspace % ALIGN) != 0) { delete h; return PSDNS_ENOMEM; }
     cudaError_t e = setup_attrs(h);
     if (e == cudaSuccess) e = build_tables(h);
