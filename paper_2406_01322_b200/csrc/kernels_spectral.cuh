@@ -35,6 +35,11 @@ __device__ __forceinline__ cplx cfma(double s, cplx a, cplx b) {                
     return make_double2(fma(s, a.x, b.x), fma(s, a.y, b.y));
 }
 
+// L2 prefetch of the cache line that holds p: the column sweeps below touch one 16-byte element per array
+// per row, so the rows PF_ROWS ahead are requested early and the demand loads become L2 hits.
+__device__ __forceinline__ void pf_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+constexpr int PF_ROWS = 6;
+
 // ---- layout conversion ---------------------------------------------------------------------
 // Both sides are cplx [n][rows][pitch]; a side is described by (rows, pitch, jpos, nkx):
 // row r < jpos holds j' = r, row r >= jpos holds j' = r - rows; columns i < nkx are valid.
@@ -63,10 +68,12 @@ __global__ void __launch_bounds__(256) k_relayout(cplx *__restrict__ dst, const 
     }
 }
 
-// ---- theta = (D^2 - k^2) w ---------------------------------------------------------------------
+// ---- hidden state: theta = (D^2 - k^2) w (reading S13), omega_z = i kx v - i ky u (Eq. 16) ------------
 // Chebyshev derivative recurrence: ct_n b_n = b_{n+2} + 2 (n+1) a_{n+1}, ct_0 = 2.
-__global__ void __launch_bounds__(NT_COL) k_lap(const __grid_constant__ ColGeom g, const cplx *__restrict__ w,
-                                                cplx *__restrict__ th) {
+// Column (0,0) carries the mean flow instead: the omega slot holds u-bar, the theta slot v-bar (reading S12).
+__global__ void __launch_bounds__(NT_COL) k_hidden_state(const __grid_constant__ ColGeom g, const cplx *__restrict__ u,
+                                                         const cplx *__restrict__ v, const cplx *__restrict__ w,
+                                                         cplx *__restrict__ th, cplx *__restrict__ om) {
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= g.ncols) return;
     double kx, ky;
@@ -76,21 +83,30 @@ __global__ void __launch_bounds__(NT_COL) k_lap(const __grid_constant__ ColGeom 
     cplx a1 = cz(), b1 = cz(), b2 = cz(), c1 = cz(), c2 = cz();
     for (int n = g.N; n >= 0; --n) {
         const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
-        const cplx an = w[n * st + col];
+        const size_t o = n * st + col;
+        const cplx an = w[o], un = u[o], vn = v[o];
         cplx bn = cscale(cfma(f, a1, b2), h);
         cplx cn = cscale(cfma(f, b1, c2), h);
-        th[n * st + col] = cfma(-k2, an, cn);
+        if (col == 0) {
+            th[o] = vn;
+            om[o] = un;
+        } else {
+            th[o] = cfma(-k2, an, cn);
+            om[o] = ci(csub(cscale(vn, kx), cscale(un, ky)));
+        }
         a1 = an; b2 = b1; b1 = bn; c2 = c1; c1 = cn;
     }
 }
 
-// ---- row a1: derived spectra for the backward transforms -----------------------------------------
+// ---- row a1: derived spectra that need a z derivative ----------------------------------------------------
+// phz = D phi^ (only at set_state: k_finish maintains it afterwards); the five strain spectra of the
+// variable-viscosity term (config 4, reading S14).  i kx phi^ and i ky phi^ are formed inside the z pass.
 struct PrepArgs {
     ColGeom g;
     const cplx *u, *v, *w, *phi;
-    cplx *phx, *phy, *phz;
+    cplx *phz;
     cplx *exx, *eyy, *exy, *exz, *eyz;
-    int phase, visc;
+    int do_phz, visc;
 };
 
 __global__ void __launch_bounds__(NT_COL) k_prep(const __grid_constant__ PrepArgs a) {
@@ -102,14 +118,13 @@ __global__ void __launch_bounds__(NT_COL) k_prep(const __grid_constant__ PrepArg
     const size_t st = g.ncols;
     cplx p1 = cz(), dp1 = cz(), dp2 = cz();
     cplx u1 = cz(), du1 = cz(), du2 = cz(), v1 = cz(), dv1 = cz(), dv2 = cz();
+    // every derivative is taken of the TRUNCATED field (P first, then D)
     for (int n = g.nkz - 1; n >= 0; --n) {
         const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
         const size_t o = n * st + col;
-        if (a.phase) {
+        if (a.do_phz) {
             const cplx pn = a.phi[o];
             const cplx dpn = cscale(cfma(f, p1, dp2), h);
-            a.phx[o] = cscale(ci(pn), kx);
-            a.phy[o] = cscale(ci(pn), ky);
             a.phz[o] = dpn;
             p1 = pn; dp2 = dp1; dp1 = dpn;
         }
@@ -128,20 +143,7 @@ __global__ void __launch_bounds__(NT_COL) k_prep(const __grid_constant__ PrepArg
     }
 }
 
-// ---- row a9: explicit terms + IMEX right-hand sides ----------------------------------------------
-struct RhsArgs {
-    ColGeom g;
-    const cplx *txx, *txy, *txz, *tyy, *tyz, *tzz, *q, *c;  // product spectra [nkz][ncols]
-    const cplx *u, *v;                                          // state [nz][ncols]
-    cplx *th, *phi;        // in: theta^n, phi^n ; out: H_w, H_phi (in place)
-    cplx *xom;             // out: H_omega
-    cplx *h_om, *h_w, *h_phi;   // AB2 history [nkz][ncols], in place
-    const double *ab;      // device: {ab0, ab1}
-    double dt, gamma, inv_pe, e_phi;   // e_phi = 1 + s Ch^2
-    double gradp;
-    int phase;
-};
-
+// ---- derivative recurrences fed top-down (used by rows a1, a9, a11) ------------------------------------
 struct Chain1 {  // first derivative of a sequence fed top-down
     cplx a1, b1, b2;
     __device__ __forceinline__ void init() { a1 = b1 = b2 = cz(); }
@@ -161,77 +163,6 @@ struct Chain2 {  // second derivative
         return cn;
     }
 };
-
-__global__ void __launch_bounds__(NT_COL) k_rhs(const __grid_constant__ RhsArgs a) {
-    const ColGeom &g = a.g;
-    const int col = blockIdx.x * blockDim.x + threadIdx.x;
-    if (col >= g.ncols) return;
-    double kx, ky;
-    col_wavenumbers(g, col, kx, ky);
-    const double k2 = kx * kx + ky * ky;
-    const bool mean = (col == 0);
-    const size_t st = g.ncols;
-    const double ab0 = a.ab[0], ab1 = a.ab[1];
-    const double dt = a.dt, gam = a.gamma;
-    Chain1 cR, cB;
-    Chain2 cA, cE, cOm, cTh;
-    cR.init(); cB.init(); cA.init(); cE.init(); cOm.init(); cTh.init();
-    for (int n = g.N; n >= 0; --n) {
-        const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
-        const size_t o = n * st + col;
-        const bool low = n < g.nkz;
-        const cplx un = a.u[o], vn = a.v[o];
-        const cplx thn = mean ? vn : a.th[o];
-        const cplx omn = mean ? un : ci(csub(cscale(vn, kx), cscale(un, ky)));
-        cplx P = cz(), R = cz(), A = cz(), B = cz(), E = cz(), Q = cz();
-        cplx phn = cz();
-        if (a.phase) phn = a.phi[o];
-        if (low) {
-            const cplx txx = a.txx[o], txy = a.txy[o], txz = a.txz[o], tyy = a.tyy[o], tyz = a.tyz[o], tzz = a.tzz[o];
-            if (mean) {
-                R = txz;
-                B = tyz;
-            } else {
-                P = cadd(cscale(txy, ky * ky - kx * kx), cscale(csub(txx, tyy), kx * ky));
-                R = ci(csub(cscale(tyz, kx), cscale(txz, ky)));
-                A = ci(cadd(cscale(txz, kx), cscale(tyz, ky)));
-                B = cadd(cadd(cscale(txx, kx * kx), cscale(txy, 2.0 * kx * ky)), csub(cscale(tyy, ky * ky), cscale(tzz, k2)));
-            }
-            if (a.phase) {
-                Q = a.q[o];
-                E = cscale(cfma(-a.e_phi, phn, a.c[o]), a.inv_pe);
-            }
-        }
-        const cplx dR = cR.step(R, f, h);
-        const cplx dB = cB.step(B, f, h);
-        const cplx ddA = cA.step(A, f, h);
-        const cplx ddOm = cOm.step(omn, f, h);
-        const cplx ddTh = cTh.step(thn, f, h);
-        cplx n_om = cadd(P, dR);
-        if (mean && n == 0) n_om.x += a.gradp;
-        const cplx n_w = cadd(csub(dB, ddA), cscale(A, -k2));
-        cplx nl_om = cscale(n_om, ab0), nl_w = cscale(n_w, ab0);
-        if (low) {
-            nl_om = cfma(ab1, a.h_om[o], nl_om);
-            nl_w = cfma(ab1, a.h_w[o], nl_w);
-            a.h_om[o] = n_om;
-            a.h_w[o] = n_w;
-        }
-        // Crank-Nicolson right-hand sides H = x + gamma (D^2 - k^2) x + dt NL
-        a.xom[o] = cfma(dt, nl_om, cfma(gam, cfma(-k2, omn, ddOm), omn));
-        a.th[o] = cfma(dt, nl_w, cfma(gam, cfma(-k2, thn, ddTh), thn));
-        if (a.phase) {
-            const cplx ddE = cE.step(E, f, h);
-            const cplx s_phi = csub(cfma(-k2, E, ddE), Q);
-            cplx nl_phi = cscale(s_phi, ab0);
-            if (low) {
-                nl_phi = cfma(ab1, a.h_phi[o], nl_phi);
-                a.h_phi[o] = s_phi;
-            }
-            a.phi[o] = cfma(dt, nl_phi, phn);   // implicit Euler: H_phi = phi + dt NL
-        }
-    }
-}
 
 // ---- row a10: quasi-tridiagonal Chebyshev-tau Helmholtz solve ---------------------------------------
 // (D^2 - sigma) u = f in rows 0..N-2 plus two boundary rows (reading S11).  In coefficient space,
@@ -422,15 +353,17 @@ struct ElimDown {
     }
 };
 
-// ---- K_A: row a9 + first elimination, one thread per (column, chain) ---------------------------------
+// ---- K_A: row a9 + first elimination ------------------------------------------------------------------
+// One WARP per (32 consecutive columns, chain); the chains of the same columns sit in one CTA so that the
+// product rows two chains share are fetched from HBM once (the second warp hits L1/L2).
 // chain 0: omega_z (column 0: u-bar)   f = -H_omega / gamma,  sigma = k^2 + 1/gamma, Dirichlet
 // chain 1: theta   (column 0: v-bar)   f = -H_w / gamma,      same sigma, Dirichlet (homogeneous part added later)
 // chain 2: psi                         f = H_phi / gamma_phi, sigma = k^2 + lambda_phi, Neumann
+// Every chain works in place: it reads x^n at row n going down and writes g' at row n + 2.
 struct RhsElimArgs {
     ColGeom g;
-    const cplx *txx, *txy, *txz, *tyy, *tyz, *tzz, *q, *c;
-    const cplx *u, *v;
-    cplx *th, *phi, *xom;             // in: theta^n, phi^n; out: g' arrays (slots 0,1 = u_0, u_1)
+    const cplx *txx, *txy, *txz, *tyy, *tyz, *q, *c;   // txx, tyy hold the deviatoric T_xx - T_zz, T_yy - T_zz
+    cplx *om, *th, *phi;              // in: omega^n, theta^n, phi^n; out: g' arrays (slots 0,1 = u_0, u_1)
     cplx *h_om, *h_w, *h_phi;
     const double *dinv_ns, *dinv_ch;
     const double *ab;
@@ -438,41 +371,50 @@ struct RhsElimArgs {
     int phase;
 };
 
-__global__ void __launch_bounds__(NT_COL, 4) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
+constexpr int RHS_COLS = 32;   // columns per CTA of k_rhs_elim (blockDim = 32 * number of chains)
+
+__global__ void __launch_bounds__(96, 5) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
     const ColGeom &g = a.g;
-    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    const int col = blockIdx.x * RHS_COLS + (threadIdx.x & 31);
     if (col >= g.ncols) return;
-    const int chain = blockIdx.y;
+    const int chain = threadIdx.x >> 5;
     double kx, ky;
     col_wavenumbers(g, col, kx, ky);
     const double k2 = kx * kx + ky * ky;
     const bool mean = (col == 0);
     const size_t st = g.ncols;
-    const int N = g.N;
+    const int N = g.N, nkz = g.nkz;
     const double ab0 = a.ab[0], ab1 = a.ab[1];
     const double dt = a.dt, gam = a.gamma;
+    const cplx *__restrict__ txx = a.txx + col, *__restrict__ txy = a.txy + col, *__restrict__ txz = a.txz + col;
+    const cplx *__restrict__ tyy = a.tyy + col, *__restrict__ tyz = a.tyz + col;
     ElimDown el;
     el.init();
     if (chain == 0) {
         const double sigma = k2 + 1.0 / gam, fs = -1.0 / gam;
         const double *__restrict__ dinv = a.dinv_ns + col;
+        cplx *x = a.om + col, *hist = a.h_om + col;
         Chain1 cR; Chain2 cOm;
         cR.init(); cOm.init();
         for (int n = N; n >= 0; --n) {
+            const int np = n - PF_ROWS;
+            if (np >= 0) {
+                pf_l2(x + np * st); pf_l2(dinv + (np + 2) * st);
+                if (np < nkz) { pf_l2(txz + np * st); pf_l2(txx + np * st); pf_l2(txy + np * st); pf_l2(tyy + np * st); pf_l2(tyz + np * st); pf_l2(hist + np * st); }
+            }
             const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
-            const size_t o = n * st + col;
-            const bool low = n < g.nkz;
-            const cplx un = a.u[o], vn = a.v[o];
-            const cplx omn = mean ? un : ci(csub(cscale(vn, kx), cscale(un, ky)));
+            const size_t o = n * st;
+            const bool low = n < nkz;
+            const cplx omn = x[o];
             cplx P = cz(), R = cz();
             if (low) {
-                const cplx txz = a.txz[o];
+                const cplx vxz = txz[o];
                 if (mean) {
-                    R = txz;
+                    R = vxz;
                 } else {
-                    const cplx txx = a.txx[o], txy = a.txy[o], tyy = a.tyy[o], tyz = a.tyz[o];
-                    P = cadd(cscale(txy, ky * ky - kx * kx), cscale(csub(txx, tyy), kx * ky));
-                    R = ci(csub(cscale(tyz, kx), cscale(txz, ky)));
+                    const cplx vxx = txx[o], vxy = txy[o], vyy = tyy[o], vyz = tyz[o];
+                    P = cadd(cscale(vxy, ky * ky - kx * kx), cscale(csub(vxx, vyy), kx * ky));
+                    R = ci(csub(cscale(vyz, kx), cscale(vxz, ky)));
                 }
             }
             const cplx dR = cR.step(R, f, h);
@@ -480,35 +422,42 @@ __global__ void __launch_bounds__(NT_COL, 4) k_rhs_elim(const __grid_constant__ 
             cplx n_om = cadd(P, dR);
             if (mean && n == 0) n_om.x += a.gradp;
             cplx nl = cscale(n_om, ab0);
-            if (low) { nl = cfma(ab1, a.h_om[o], nl); a.h_om[o] = n_om; }
+            if (low) { nl = cfma(ab1, hist[o], nl); hist[o] = n_om; }
             const cplx H = cfma(dt, nl, cfma(gam, cfma(-k2, omn, ddOm), omn));
             if (n <= N - 2) {
                 const int k = n + 2;
-                a.xom[k * st + col] = el.row<false, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
+                x[k * st] = el.row<false, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
             }
         }
         cplx u0, u1;
         el.finish<false>(sigma, 0.0, 0.0, u0, u1);
-        a.xom[col] = u0; a.xom[st + col] = u1;
+        x[0] = u0; x[st] = u1;
     } else if (chain == 1) {
         const double sigma = k2 + 1.0 / gam, fs = -1.0 / gam;
         const double *__restrict__ dinv = a.dinv_ns + col;
+        cplx *x = a.th + col, *hist = a.h_w + col;
         Chain1 cB; Chain2 cA, cTh;
         cB.init(); cA.init(); cTh.init();
         for (int n = N; n >= 0; --n) {
+            const int np = n - PF_ROWS;
+            if (np >= 0) {
+                pf_l2(x + np * st); pf_l2(dinv + (np + 2) * st);
+                if (np < nkz) { pf_l2(tyz + np * st); pf_l2(txx + np * st); pf_l2(txy + np * st); pf_l2(txz + np * st); pf_l2(tyy + np * st); pf_l2(hist + np * st); }
+            }
             const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
-            const size_t o = n * st + col;
-            const bool low = n < g.nkz;
-            const cplx thn = mean ? a.v[o] : a.th[o];
+            const size_t o = n * st;
+            const bool low = n < nkz;
+            const cplx thn = x[o];
             cplx A = cz(), B = cz();
             if (low) {
-                const cplx tyz = a.tyz[o];
+                const cplx vyz = tyz[o];
                 if (mean) {
-                    B = tyz;
+                    B = vyz;
                 } else {
-                    const cplx txx = a.txx[o], txy = a.txy[o], txz = a.txz[o], tyy = a.tyy[o], tzz = a.tzz[o];
-                    A = ci(cadd(cscale(txz, kx), cscale(tyz, ky)));
-                    B = cadd(cadd(cscale(txx, kx * kx), cscale(txy, 2.0 * kx * ky)), csub(cscale(tyy, ky * ky), cscale(tzz, k2)));
+                    const cplx vxx = txx[o], vxy = txy[o], vxz = txz[o], vyy = tyy[o];
+                    A = ci(cadd(cscale(vxz, kx), cscale(vyz, ky)));
+                    // kx^2 Txx + 2 kx ky Txy + ky^2 Tyy - k^2 Tzz with the deviatoric inputs
+                    B = cadd(cadd(cscale(vxx, kx * kx), cscale(vxy, 2.0 * kx * ky)), cscale(vyy, ky * ky));
                 }
             }
             const cplx dB = cB.step(B, f, h);
@@ -516,45 +465,51 @@ __global__ void __launch_bounds__(NT_COL, 4) k_rhs_elim(const __grid_constant__ 
             const cplx ddTh = cTh.step(thn, f, h);
             const cplx n_w = cadd(csub(dB, ddA), cscale(A, -k2));
             cplx nl = cscale(n_w, ab0);
-            if (low) { nl = cfma(ab1, a.h_w[o], nl); a.h_w[o] = n_w; }
+            if (low) { nl = cfma(ab1, hist[o], nl); hist[o] = n_w; }
             const cplx H = cfma(dt, nl, cfma(gam, cfma(-k2, thn, ddTh), thn));
             if (n <= N - 2) {
                 const int k = n + 2;
-                a.th[k * st + col] = el.row<false, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
+                x[k * st] = el.row<false, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
             }
         }
         cplx u0, u1;
         el.finish<false>(sigma, 0.0, 0.0, u0, u1);
-        a.th[col] = u0; a.th[st + col] = u1;
+        x[0] = u0; x[st] = u1;
     } else {
-        if (!a.phase) return;
         const double sigma = k2 + a.lam_phi, fs = 1.0 / a.gam_phi;
         const double *__restrict__ dinv = a.dinv_ch + col;
+        const cplx *__restrict__ qq = a.q + col, *__restrict__ cc = a.c + col;
+        cplx *x = a.phi + col, *hist = a.h_phi + col;
         Chain2 cE;
         cE.init();
         for (int n = N; n >= 0; --n) {
+            const int np = n - PF_ROWS;
+            if (np >= 0) {
+                pf_l2(x + np * st); pf_l2(dinv + (np + 2) * st);
+                if (np < nkz) { pf_l2(qq + np * st); pf_l2(cc + np * st); pf_l2(hist + np * st); }
+            }
             const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
-            const size_t o = n * st + col;
-            const bool low = n < g.nkz;
-            const cplx phn = a.phi[o];
+            const size_t o = n * st;
+            const bool low = n < nkz;
+            const cplx phn = x[o];
             cplx E = cz(), Q = cz();
             if (low) {
-                Q = a.q[o];
-                E = cscale(cfma(-a.e_phi, phn, a.c[o]), a.inv_pe);
+                Q = qq[o];
+                E = cscale(cfma(-a.e_phi, phn, cc[o]), a.inv_pe);
             }
             const cplx ddE = cE.step(E, f, h);
             const cplx s_phi = csub(cfma(-k2, E, ddE), Q);
             cplx nl = cscale(s_phi, ab0);
-            if (low) { nl = cfma(ab1, a.h_phi[o], nl); a.h_phi[o] = s_phi; }
+            if (low) { nl = cfma(ab1, hist[o], nl); hist[o] = s_phi; }
             const cplx H = cfma(dt, nl, phn);
             if (n <= N - 2) {
                 const int k = n + 2;
-                a.phi[k * st + col] = el.row<true, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
+                x[k * st] = el.row<true, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
             }
         }
         cplx u0, u1;
         el.finish<true>(sigma, 0.0, 0.0, u0, u1);
-        a.phi[col] = u0; a.phi[st + col] = u1;
+        x[0] = u0; x[st] = u1;
     }
 }
 
@@ -595,6 +550,11 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
     }
 #pragma unroll 4
     for (int k = 2; k <= N; ++k) {
+        const int kp = k + PF_ROWS;
+        if (kp <= N) {
+            pf_l2(x + kp * st); pf_l2(dinv + kp * st);
+            if (corr) { pf_l2(a.wh + kp * st + col); pf_l2(a.thh + kp * st + col); pf_l2(a.th + kp * st + col); }
+        }
         const double ak = -sigma * helm_p(k);
         const cplx u = cscale(cfma(-ak, um2, x[k * st]), dinv[k * st]);
         um2 = um1; um1 = u;
@@ -640,7 +600,11 @@ __global__ void __launch_bounds__(NT_COL, 5) k_elim2(const __grid_constant__ Eli
         cplx *__restrict__ out = a.w + col;
         const double *__restrict__ dinv = a.dinv_po + col;
 #pragma unroll 4
-        for (int k = N; k >= 2; --k) out[k * st] = el.row<false, true>(k, N, k2, in[(k - 2) * st], dinv[k * st]);
+        for (int k = N; k >= 2; --k) {
+            const int kp = k - PF_ROWS;
+            if (kp >= 2) { pf_l2(in + (kp - 2) * st); pf_l2(dinv + kp * st); }
+            out[k * st] = el.row<false, true>(k, N, k2, in[(k - 2) * st], dinv[k * st]);
+        }
         cplx u0, u1, de, dodd;
         el.finish<false>(k2, 0.0, 0.0, u0, u1);
         el.second(k2, u0, u1, de, dodd);
@@ -655,6 +619,8 @@ __global__ void __launch_bounds__(NT_COL, 5) k_elim2(const __grid_constant__ Eli
         const double *__restrict__ dinv = a.dinv_ch + col;
 #pragma unroll 4
         for (int k = N; k >= 2; --k) {
+            const int kp = k - PF_ROWS;
+            if (kp >= 2) { pf_l2(x + (kp - 2) * st); pf_l2(dinv + kp * st); }
             const cplx fm2 = x[(k - 2) * st];
             x[k * st] = el.row<true, false>(k, N, sigma, fm2, dinv[k * st]);
         }
@@ -683,45 +649,14 @@ __global__ void __launch_bounds__(NT_COL) k_hom_tables(const __grid_constant__ C
     hw[st + col] = ho;
 }
 
-// ---- influence-matrix closure of the w problem -----------------------------------------------------
-// theta = theta_p + A_par theta_h, w = w_p + A_par w_h with A_par chosen so that
-// sum_{k in parity} k^2 w_k = 0 for both parities  <=>  Dw(+1) = Dw(-1) = 0 (reading S10/S11).
-struct InflArgs {
-    ColGeom g;
-    cplx *th, *w;
-    const cplx *thh, *wh;   // homogeneous solutions (real, stored as cplx with zero imaginary part)
-};
-
-__global__ void __launch_bounds__(NT_COL) k_infl(const __grid_constant__ InflArgs a) {
-    const ColGeom &g = a.g;
-    const int col = blockIdx.x * blockDim.x + threadIdx.x;
-    if (col >= g.ncols || col == 0) return;
-    const size_t st = g.ncols;
-    const int N = g.N;
-    cplx se = cz(), so = cz();
-    double he = 0.0, ho = 0.0;
-    for (int k = 1; k <= N; ++k) {
-        const double wk = (double)k * k;
-        const cplx wp = a.w[k * st + col];
-        const double wh = a.wh[k * st + col].x;
-        if (k & 1) { so = cfma(wk, wp, so); ho += wk * wh; }
-        else       { se = cfma(wk, wp, se); he += wk * wh; }
-    }
-    const cplx Ae = cscale(se, -1.0 / he), Ao = cscale(so, -1.0 / ho);
-    for (int k = 0; k <= N; ++k) {
-        const size_t o = k * st + col;
-        const cplx A = (k & 1) ? Ao : Ae;
-        const double th = a.thh[o].x, wh = a.wh[o].x;
-        a.th[o] = cfma(th, A, a.th[o]);
-        a.w[o] = cfma(wh, A, a.w[o]);
-    }
-}
-
-// ---- row a11: velocity recovery ------------------------------------------------------------------------
+// ---- row a11: velocity recovery, plus D phi^ for the next step's grad(phi) (row a1) -----------------------
 struct FinishArgs {
     ColGeom g;
-    const cplx *xom;   // omega_z^{n+1} (column 0: u-bar^{n+1})
-    cplx *u, *v, *w, *th;
+    const cplx *om;    // omega_z^{n+1} (column 0: u-bar^{n+1})
+    const cplx *th;    // column 0 only: v-bar^{n+1}
+    cplx *u, *v, *w;
+    const cplx *phi;   // nullable (single-phase)
+    cplx *phz;         // [nkz][ncols]: D phi^, truncated (operator P)
 };
 
 __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ FinishArgs a) {
@@ -729,29 +664,34 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= g.ncols) return;
     const size_t st = g.ncols;
-    if (col == 0) {   // mean flow: u-bar from the omega slot, v-bar from the theta slot, w = theta = 0
-        for (int n = 0; n <= g.N; ++n) {
-            const size_t o = n * st;
-            a.u[o] = a.xom[o];
-            a.v[o] = a.th[o];
-            a.w[o] = cz();
-            a.th[o] = cz();
-        }
-        return;
-    }
     double kx, ky;
     col_wavenumbers(g, col, kx, ky);
     const double k2 = kx * kx + ky * ky;
-    const double ik2 = (col % g.kxp < g.nkx) ? 1.0 / k2 : 0.0;
-    Chain1 cW;
-    cW.init();
+    const bool mean = (col == 0);
+    const double ik2 = (!mean && col % g.kxp < g.nkx) ? 1.0 / k2 : 0.0;
+    const bool phase = a.phi != nullptr;
+    Chain1 cW, cP;
+    cW.init(); cP.init();
     for (int n = g.N; n >= 0; --n) {
-        const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
         const size_t o = n * st + col;
-        const cplx dw = cW.step(a.w[o], f, h);
-        const cplx om = a.xom[o];
-        a.u[o] = cscale(ci(cadd(cscale(dw, kx), cscale(om, ky))), ik2);
-        a.v[o] = cscale(ci(csub(cscale(dw, ky), cscale(om, kx))), ik2);
+        const int np = n - PF_ROWS;
+        if (np >= 0) {
+            const size_t op = np * st + col;
+            pf_l2(a.w + op); pf_l2(a.om + op);
+            if (phase && np < g.nkz) pf_l2(a.phi + op);
+        }
+        const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
+        if (phase && n < g.nkz) a.phz[o] = cP.step(a.phi[o], f, h);   // D of the truncated phi^ (P first, then D)
+        if (mean) {   // mean flow: u-bar from the omega slot, v-bar from the theta slot, w = 0 (reading S12)
+            a.u[o] = a.om[o];
+            a.v[o] = a.th[o];
+            a.w[o] = cz();
+        } else {
+            const cplx dw = cW.step(a.w[o], f, h);
+            const cplx om = a.om[o];
+            a.u[o] = cscale(ci(cadd(cscale(dw, kx), cscale(om, ky))), ik2);
+            a.v[o] = cscale(ci(csub(cscale(dw, ky), cscale(om, kx))), ik2);
+        }
     }
 }
 

@@ -11,11 +11,11 @@
 // pencil all-to-alls (L154) by strided 128-byte-row accesses of one resident array.
 #pragma once
 #include "fft_tile.cuh"
+#include "fft_fused.cuh"
 
 namespace psdns {
 
 constexpr int MAXF = 12;      // max fields per batched launch
-constexpr int NT_FFT = 256;   // threads per transform CTA (tiles up to 74 KB, >= 3 CTAs per SM)
 // the 147 KB tile (L = 1024) allows one CTA per SM: give it 16 warps instead of 8 to hide latency
 template <int L> __host__ __device__ constexpr int tile_threads() { return L >= 1024 ? 512 : 256; }
 
@@ -30,83 +30,45 @@ __device__ __forceinline__ void load_twiddles(cplx *tw, const cplx *__restrict__
 }
 
 // ------------------------------------------------------------------------------------------
-// z pass: Chebyshev transform = DCT-I as the length-2N FFT of the even extension,
-// Re and Im transformed together (the DFT of a real-even sequence is real).
+// z pass: Chebyshev transform = DCT-I ("FFT of a 2N even extension ... transposes"), in the
+// half-length form that L178 attributes to Makhoul [32] ("does not require performing a transform of size 2N
+// but only of size N by re-ordering the input signal"), Re and Im transformed together, no transposes.
 //   backward (row a2): a_n, n < nk  ->  f_k = sum_n a_n cos(pi n k / N), k = 0..N
-//   forward  (row a8): f_k          ->  a_n = 1/(N c_n) DFT_n(even ext), n < nk (truncation)
-// grid = (ncols/8, nfields); L = 2N.
-// ------------------------------------------------------------------------------------------
-struct ZArgs {
-    FieldPtrs f;
-    int ncols;  // nky * kxp (multiple of 8) = plane stride in cplx
-    int nk;     // coefficient planes read (backward) or written (forward)
-};
-
-template <int L, bool FWD>
-__global__ void __launch_bounds__(tile_threads<L>()) k_zpass(const __grid_constant__ ZArgs a, const cplx *__restrict__ twg) {
-    constexpr int NT = tile_threads<L>();
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx *s = reinterpret_cast<cplx *>(smem_raw);
-    cplx *tw = s + L * TILE_LINES;
-    constexpr int N = L / 2;
-    const int tid = threadIdx.x, line = tid & 7, r0 = tid >> 3;
-    constexpr int RSTEP = NT / TILE_LINES;
-    const size_t stride = (size_t)a.ncols;
-    const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[blockIdx.y]) + (size_t)blockIdx.x * 8 + line;
-    cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[blockIdx.y]) + (size_t)blockIdx.x * 8 + line;
-    load_twiddles<L>(tw, twg, tid, NT);
-    if (!FWD) {
-        const int nk = a.nk;
-        for (int n = r0; n <= N; n += RSTEP) {
-            cplx v = make_double2(0.0, 0.0);
-            if (n < nk) v = in[n * stride];
-            if (n > 0 && n < N) {
-                v = cscale(v, 0.5);
-                s[(L - n) * TILE_LINES + line] = v;
-            }
-            s[n * TILE_LINES + line] = v;
-        }
-    } else {
-        for (int k = r0; k <= N; k += RSTEP) {
-            cplx v = in[k * stride];
-            if (k > 0 && k < N) s[(L - k) * TILE_LINES + line] = v;
-            s[k * TILE_LINES + line] = v;
-        }
-    }
-    __syncthreads();
-    fft_tile<L, -1, NT>(s, tw, tid);
-    __syncthreads();
-    if (!FWD) {
-        for (int k = r0; k <= N; k += RSTEP) out[k * stride] = s[fft_pos<L>(k) * TILE_LINES + line];
-    } else {
-        const int nk = a.nk;
-        const double sc = 1.0 / N;
-        for (int n = r0; n < nk; n += RSTEP) {
-            cplx v = s[fft_pos<L>(n) * TILE_LINES + line];
-            out[n * stride] = cscale(v, (n == 0 || n == N) ? 0.5 * sc : sc);
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------------
-// z pass, half-length form (the optimisation PAPER.md L178 attributes to Makhoul [32]: "does not require
-// performing a transform of size 2N but only of size N by re-ordering the input signal").
-// With e = even extension (length 2N) of the complex column, g_m = e_{2m}, h_m = e_{2m+1} (m < N):
+//   forward  (row a8): f_k          ->  a_n = 2/(N c_n) sum_k f_k cos(pi n k / N) / c_k, n < nk (truncation)
+// With e = even extension (length 2N) of the (weighted) column, g_m = e_{2m}, h_m = e_{2m+1} (m < N):
 //   E_k = DFT_2N(e)_k = G_k + w_2N^k H_k.  Pack z_m = g_m + i h_m (complex arithmetic), Z = FFT_N(z).
 //   g is even (G_{N-k} = G_k) and h is half-sample symmetric (H_{N-k} = w_N^k H_k), so
 //   Z_k - Z_{N-k} = i (1 - w_N^k) H_k and
 //   E_k = Z_k + c_k (Z_k - Z_{N-k}),  c_k = -(1 + sin t)/(2 sin t) + i cos t/(2 sin t),  t = pi k / N,
 //   c_{N-k} = conj(c_k); k = 0 and k = N need H_0 = sum_m h_m (reduced while loading):
 //   G_0 = Z_0 - i H_0, E_0 = G_0 + H_0, E_N = G_0 - H_0.
-// One N-point complex FFT per complex column: half the flops and half the shared memory of the 2N form
-// (64 KB tile at N = 512, three CTAs per SM).  Rounding error is amplified by |c_k| <= ~N/(2 pi k) in the
-// lowest/highest modes (<= 1e-14 relative at N = 512; tolerance 1e-11).
-//   grid = (ncols/8, nfields); template N = nz - 1.
+// Rounding error is amplified by |c_k| <= ~N/(2 pi k) in the lowest/highest modes (<= 1e-14 relative at
+// N = 512; tolerance 1e-11).
+// Persistent CTAs loop over tiles of 8 consecutive columns; the first FFT pass is fed from global memory
+// through registers (fft_fused.cuh).  Optional derived outputs i kx X and i ky X of one field (row a1:
+// the x / y derivatives of phi commute with the z transform, so they cost no transform of their own).
 // ------------------------------------------------------------------------------------------
+struct ZArgs {
+    FieldPtrs f;
+    int nf;     // fields
+    int ncols;  // nky * kxp (multiple of 8) = plane stride in cplx
+    int nk;     // coefficient planes read (backward) or written (forward)
+    // derived outputs of field dfield (backward only; either pointer may be null; dfield < 0: none)
+    int dfield;
+    cplx *out_dx, *out_dy;
+    int kxp, nky, jpos;
+    double kxf, kyf;
+};
+
+template <int N> __host__ __device__ constexpr int zpass_smem_cplx() {
+    return N * TILE_LINES + N + (fused_threads<N>() / 32) * 8;
+}
+
 template <int N, bool FWD>
-__global__ void __launch_bounds__(NT_FFT) k_zpass_h(const __grid_constant__ ZArgs a, const cplx *__restrict__ tw2n,
-                                                    const cplx *__restrict__ ctab) {
-    constexpr int NT = NT_FFT;
+__global__ void __launch_bounds__(fused_threads<N>(), (N >= 512 ? 2 : 3)) k_zpass(const __grid_constant__ ZArgs a,
+                                                                               const cplx *__restrict__ tw2n,
+                                                                               const cplx *__restrict__ ctab) {
+    constexpr int NT = fused_threads<N>();
     constexpr int NW = NT / 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
@@ -115,56 +77,79 @@ __global__ void __launch_bounds__(NT_FFT) k_zpass_h(const __grid_constant__ ZArg
     const int tid = threadIdx.x, line = tid & 7, r0 = tid >> 3;
     constexpr int RSTEP = NT / TILE_LINES;
     const size_t stride = (size_t)a.ncols;
-    const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[blockIdx.y]) + (size_t)blockIdx.x * 8 + line;
-    cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[blockIdx.y]) + (size_t)blockIdx.x * 8 + line;
     for (int i = tid; i < N; i += NT) tw[i] = tw2n[2 * i];
+    __syncthreads();
     const int nin = FWD ? N + 1 : a.nk;       // input rows that are not structurally zero
-    cplx h0 = make_double2(0.0, 0.0);
-    for (int m = r0; m <= N / 2; m += RSTEP) {
-        const int ne = 2 * m;
-        cplx ev = make_double2(0.0, 0.0), op = ev, om = ev;
-        if (ne < nin) ev = in[ne * stride];
-        if (m < N / 2 && ne + 1 < nin) op = in[(ne + 1) * stride];
-        if (m >= 1 && ne - 1 < nin) om = in[(ne - 1) * stride];
-        if (!FWD) {                           // backward: interior coefficients enter with weight 1/2
-            if (ne > 0 && ne < N) ev = cscale(ev, 0.5);
-            op = cscale(op, 0.5);             // odd rows are always interior
-            om = cscale(om, 0.5);
-        }
-        // z_m = e_{2m} + i e_{2m+1} ; z_{N-m} = e_{2m} + i e_{2m-1}
-        if (m < N / 2) s[m * TILE_LINES + line] = make_double2(ev.x - op.y, ev.y + op.x);
-        if (m >= 1) s[(N - m) * TILE_LINES + line] = make_double2(ev.x - om.y, ev.y + om.x);
-        h0 = cadd(h0, cadd(op, om));
-    }
-    // reduce H_0 over the threads that share this line: lanes differ in bits 3, 4 within a warp
-    h0.x += __shfl_xor_sync(0xffffffffu, h0.x, 8);  h0.y += __shfl_xor_sync(0xffffffffu, h0.y, 8);
-    h0.x += __shfl_xor_sync(0xffffffffu, h0.x, 16); h0.y += __shfl_xor_sync(0xffffffffu, h0.y, 16);
-    if ((tid & 31) < 8) red[(tid >> 5) * 8 + line] = h0;
-    __syncthreads();
-    fft_tile<N, -1, NT>(s, tw, tid);
-    __syncthreads();
     const int nout = FWD ? a.nk : N + 1;      // output rows kept
     const double sc = FWD ? 1.0 / N : 1.0;
-    for (int k = r0; k <= N / 2; k += RSTEP) {
-        const int kb = N - k;
-        if (k == 0) {
-            cplx H0 = make_double2(0.0, 0.0);
-#pragma unroll
-            for (int w = 0; w < NW; ++w) H0 = cadd(H0, red[w * 8 + line]);
-            const cplx z0 = s[line];          // fft_pos(0) = 0
-            const cplx G0 = make_double2(z0.x + H0.y, z0.y - H0.x);   // Z_0 - i H_0
-            out[0] = cscale(cadd(G0, H0), FWD ? 0.5 * sc : sc);
-            if (N < nout) out[(size_t)N * stride] = cscale(csub(G0, H0), FWD ? 0.5 * sc : sc);
-        } else {
-            const cplx za = s[fft_pos<N>(k) * TILE_LINES + line];
-            const cplx zb = s[fft_pos<N>(kb) * TILE_LINES + line];
-            const cplx c = ctab[k];
-            const cplx d = csub(za, zb);
-            const cplx cd = make_double2(c.x * d.x - c.y * d.y, c.x * d.y + c.y * d.x);     // c_k d
-            const cplx ccd = make_double2(c.x * d.x + c.y * d.y, c.x * d.y - c.y * d.x);    // conj(c_k) d
-            if (k < nout) out[(size_t)k * stride] = cscale(cadd(za, cd), sc);
-            if (kb != k && kb < nout) out[(size_t)kb * stride] = cscale(csub(zb, ccd), sc);
+    const int tiles_per_field = a.ncols / 8;
+    const int ntiles = tiles_per_field * a.nf;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int fld = tile / tiles_per_field, ct = tile - fld * tiles_per_field;
+        const size_t col = (size_t)ct * 8 + line;
+        const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[fld]) + col;
+        cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[fld]) + col;
+        cplx h0 = make_double2(0.0, 0.0);
+        // z_m = e_{2m} + i e_{2m+1}; for m >= N/2 the even extension folds back: e_j = a_{2N-j}
+        fft_head<N, -1, NT>(s, tw, tid, [&](int m) {
+            const int ne = (m < N / 2) ? 2 * m : 2 * N - 2 * m;
+            const int no = (m < N / 2) ? 2 * m + 1 : 2 * N - 2 * m - 1;
+            cplx e0 = make_double2(0.0, 0.0), e1 = e0;
+            if (ne < nin) e0 = in[ne * stride];
+            if (no < nin) e1 = in[no * stride];
+            if (!FWD) {                       // backward: interior coefficients enter with weight 1/2
+                if (ne > 0 && ne < N) e0 = cscale(e0, 0.5);
+                e1 = cscale(e1, 0.5);         // odd rows are always interior
+            }
+            h0 = cadd(h0, e1);
+            return make_double2(e0.x - e1.y, e0.y + e1.x);
+        });
+        // reduce H_0 over the threads that share this line: lanes differ in bits 3, 4 within a warp
+        h0.x += __shfl_xor_sync(0xffffffffu, h0.x, 8);  h0.y += __shfl_xor_sync(0xffffffffu, h0.y, 8);
+        h0.x += __shfl_xor_sync(0xffffffffu, h0.x, 16); h0.y += __shfl_xor_sync(0xffffffffu, h0.y, 16);
+        if ((tid & 31) < 8) red[(tid >> 5) * 8 + line] = h0;
+        fft_rest_inplace<N, -1, NT>(s, tw, tid);
+        __syncthreads();
+        // derived outputs: i kx E, i ky E of this column
+        const bool der = !FWD && fld == a.dfield;
+        double kx = 0.0, ky = 0.0;
+        cplx *odx = nullptr, *ody = nullptr;
+        if (der) {
+            const int ir = (int)(col % a.kxp), jr = (int)(col / a.kxp);
+            kx = a.kxf * (double)ir;
+            ky = a.kyf * (double)(jr < a.jpos ? jr : jr - a.nky);
+            if (a.out_dx) odx = a.out_dx + col;
+            if (a.out_dy) ody = a.out_dy + col;
         }
+        auto emit = [&](int k, cplx v) {
+            out[(size_t)k * stride] = v;
+            if (der) {
+                if (odx) odx[(size_t)k * stride] = make_double2(-kx * v.y, kx * v.x);
+                if (ody) ody[(size_t)k * stride] = make_double2(-ky * v.y, ky * v.x);
+            }
+        };
+        for (int k = r0; k <= N / 2; k += RSTEP) {
+            const int kb = N - k;
+            if (k == 0) {
+                cplx H0 = make_double2(0.0, 0.0);
+#pragma unroll
+                for (int w = 0; w < NW; ++w) H0 = cadd(H0, red[w * 8 + line]);
+                const cplx z0 = s[line];          // fft_pos_f(0) = 0
+                const cplx G0 = make_double2(z0.x + H0.y, z0.y - H0.x);   // Z_0 - i H_0
+                emit(0, cscale(cadd(G0, H0), FWD ? 0.5 * sc : sc));
+                if (N < nout) emit(N, cscale(csub(G0, H0), FWD ? 0.5 * sc : sc));
+            } else {
+                const cplx za = s[fft_pos_f<N>(k) * TILE_LINES + line];
+                const cplx zb = s[fft_pos_f<N>(kb) * TILE_LINES + line];
+                const cplx c = ctab[k];
+                const cplx d = csub(za, zb);
+                const cplx cd = make_double2(c.x * d.x - c.y * d.y, c.x * d.y + c.y * d.x);     // c_k d
+                const cplx ccd = make_double2(c.x * d.x + c.y * d.y, c.x * d.y - c.y * d.x);    // conj(c_k) d
+                if (k < nout) emit(k, cscale(cadd(za, cd), sc));
+                if (kb != k && kb < nout) emit(kb, cscale(csub(zb, ccd), sc));
+            }
+        }
+        __syncthreads();
     }
 }
 
@@ -172,52 +157,58 @@ __global__ void __launch_bounds__(NT_FFT) k_zpass_h(const __grid_constant__ ZArg
 // y pass: complex <-> complex DFT of length ny per (ir, k) line (Z2Z).
 //   backward (row a3): nky retained rows (FFT order compacted) -> ny points, e^{+i ky y}
 //   forward  (row a7): ny points -> nky retained rows, e^{-i ky y} / ny
-// grid = (kxp/8, nz, nfields); L = ny.
+// Persistent CTAs loop over tiles (8 consecutive ir) x (one z plane) x (one field); first pass fed from
+// global memory through registers, last pass drained to global memory (fft_fused.cuh).
 // ------------------------------------------------------------------------------------------
 struct YArgs {
     FieldPtrs f;
+    int nf, nz;
     int kxp;   // row pitch in cplx (multiple of 8)
     int nky;   // retained ky rows
     int jpos;  // rows 0..jpos-1 are j' = jr >= 0; rows jpos.. are j' = jr - nky < 0
 };
 
 template <int L, bool FWD>
-__global__ void __launch_bounds__(tile_threads<L>()) k_ypass(const __grid_constant__ YArgs a, const cplx *__restrict__ twg) {
-    constexpr int NT = tile_threads<L>();
+__global__ void __launch_bounds__(fused_threads<L>(), (L >= 512 ? 2 : 3)) k_ypass(const __grid_constant__ YArgs a,
+                                                                               const cplx *__restrict__ twg) {
+    constexpr int NT = fused_threads<L>();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
     cplx *tw = s + L * TILE_LINES;
-    const int tid = threadIdx.x, line = tid & 7, r0 = tid >> 3;
-    constexpr int RSTEP = NT / TILE_LINES;
+    const int tid = threadIdx.x, line = tid & 7;
     const size_t pitch = (size_t)a.kxp;
     const int nky = a.nky, jpos = a.jpos;
-    const size_t zin = (size_t)blockIdx.y * (FWD ? L : nky) * pitch;
-    const size_t zout = (size_t)blockIdx.y * (FWD ? nky : L) * pitch;
-    const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[blockIdx.z]) + zin + (size_t)blockIdx.x * 8 + line;
-    cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[blockIdx.z]) + zout + (size_t)blockIdx.x * 8 + line;
+    const int nneg = nky - jpos;              // retained rows with j' < 0
     load_twiddles<L>(tw, twg, tid, NT);
-    if (!FWD) {
-        for (int j = r0; j < L; j += RSTEP) {
-            // FFT-order row j holds j' = j (j < jpos) or j' = j - L (j >= L - (nky - jpos))
-            cplx v = make_double2(0.0, 0.0);
-            if (j < jpos) v = in[j * pitch];
-            else if (j >= L - (nky - jpos)) v = in[(j - (L - nky)) * pitch];
-            s[j * TILE_LINES + line] = v;
-        }
-    } else {
-        for (int y = r0; y < L; y += RSTEP) s[y * TILE_LINES + line] = in[y * pitch];
-    }
     __syncthreads();
-    fft_tile<L, (FWD ? -1 : +1), NT>(s, tw, tid);
-    __syncthreads();
-    if (!FWD) {
-        for (int y = r0; y < L; y += RSTEP) out[y * pitch] = s[fft_pos<L>(y) * TILE_LINES + line];
-    } else {
-        const double sc = 1.0 / L;
-        for (int jr = r0; jr < nky; jr += RSTEP) {
-            const int j = jr < jpos ? jr : jr + (L - nky);
-            out[jr * pitch] = cscale(s[fft_pos<L>(j) * TILE_LINES + line], sc);
+    const int tiles_x = a.kxp / 8;
+    const int ntiles = tiles_x * a.nz * a.nf;
+    const double sc = 1.0 / L;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int cx = tile % tiles_x;
+        const int t2 = tile / tiles_x;
+        const int z = t2 % a.nz, fld = t2 / a.nz;
+        const size_t zin = (size_t)z * (FWD ? L : nky) * pitch;
+        const size_t zout = (size_t)z * (FWD ? nky : L) * pitch;
+        const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[fld]) + zin + (size_t)cx * 8 + line;
+        cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[fld]) + zout + (size_t)cx * 8 + line;
+        if (!FWD) {
+            // FFT-order row j holds j' = j (j < jpos) or j' = j - L (j >= L - nneg); the rest is zero
+            fft_head<L, +1, NT>(s, tw, tid, [&](int j) {
+                cplx v = make_double2(0.0, 0.0);
+                if (j < jpos) v = in[j * pitch];
+                else if (j >= L - nneg) v = in[(j - (L - nky)) * pitch];
+                return v;
+            });
+            fft_rest_store<L, +1, NT>(s, tw, tid, [&](int y, cplx v) { out[y * pitch] = v; });
+        } else {
+            fft_head<L, -1, NT>(s, tw, tid, [&](int y) { return in[y * pitch]; });
+            fft_rest_store<L, -1, NT>(s, tw, tid, [&](int j, cplx v) {
+                if (j < jpos) out[j * pitch] = cscale(v, sc);
+                else if (j >= L - nneg) out[(j - (L - nky)) * pitch] = cscale(v, sc);
+            });
         }
+        __syncthreads();
     }
 }
 
@@ -296,13 +287,16 @@ __global__ void __launch_bounds__(tile_threads<L>()) k_xpass(const __grid_consta
 }
 
 // ------------------------------------------------------------------------------------------
-// pointwise non-linear terms (row a5; Eqs. 1, 4, 7, 8 and L182-196), in place:
-//   in : u v w [phi phx phy phz [exx eyy exy exz eyz]]     (buffers 0..11)
-//   out: Txx Txy Txz Tyy Tyz Tzz [Q C]                     (buffers 0..7)
-//   T_ij = -u_i u_j + cs (|grad phi|^2 delta_ij - phi_i phi_j) + eta1(phi) E_ij
+// pointwise non-linear terms (row a5; Eqs. 1, 4, 7, 8 and L182-196), unfused form (variable
+// viscosity, reading S14; the matched-viscosity step uses the fused x kernel):
+//   in : u v w [phi phx phy phz [exx eyy exy exz eyz]]     (b[0..11])
+//   out: Txx-Tzz Txy Txz Tyy-Tzz Tyz [Q C]                 (o[0..6]; may alias the inputs)
+//   T_ij = -u_i u_j + cs (|grad phi|^2 delta_ij - phi_i phi_j) + eta1(phi) E_ij; only the deviatoric
+//   combinations enter Eqs. 14-15, so T_zz is subtracted here instead of being transformed.
 // ------------------------------------------------------------------------------------------
 struct PwArgs {
-    double *b[MAXF];
+    const double *b[MAXF];
+    double *o[8];
     size_t n;
     double cs;        // 3/sqrt(8) Ch/We
     double eta_c;     // (lambda - 1) / (2 Re)
@@ -313,32 +307,30 @@ __global__ void __launch_bounds__(256) k_pointwise(const __grid_constant__ PwArg
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += stride) {
         const double u = a.b[0][i], v = a.b[1][i], w = a.b[2][i];
-        double txx = -u * u, txy = -u * v, txz = -u * w, tyy = -v * v, tyz = -v * w, tzz = -w * w;
+        double dxx = w * w - u * u, dyy = w * w - v * v, txy = -u * v, txz = -u * w, tyz = -v * w;
+        double q = 0.0, c3 = 0.0;
         if (a.phase) {
             const double ph = a.b[3][i], px = a.b[4][i], py = a.b[5][i], pz = a.b[6][i];
-            const double g2 = px * px + py * py + pz * pz;
             const double cs = a.cs;
-            txx += cs * (g2 - px * px);
-            tyy += cs * (g2 - py * py);
-            tzz += cs * (g2 - pz * pz);
+            dxx += cs * (pz * pz - px * px);
+            dyy += cs * (pz * pz - py * py);
             txy -= cs * px * py;
             txz -= cs * px * pz;
             tyz -= cs * py * pz;
             if (a.visc) {
                 const double e1 = a.eta_c * (ph + 1.0);
                 const double exx = a.b[7][i], eyy = a.b[8][i], exy = a.b[9][i], exz = a.b[10][i], eyz = a.b[11][i];
-                txx += e1 * exx;
-                tyy += e1 * eyy;
-                tzz += e1 * (-exx - eyy);
+                dxx += e1 * (2.0 * exx + eyy);     // E_xx - E_zz, E_zz = -E_xx - E_yy
+                dyy += e1 * (exx + 2.0 * eyy);
                 txy += e1 * exy;
                 txz += e1 * exz;
                 tyz += e1 * eyz;
             }
-            a.b[6][i] = u * px + v * py + w * pz;
-            a.b[7][i] = ph * ph * ph;
+            q = u * px + v * py + w * pz;
+            c3 = ph * ph * ph;
         }
-        a.b[0][i] = txx; a.b[1][i] = txy; a.b[2][i] = txz;
-        a.b[3][i] = tyy; a.b[4][i] = tyz; a.b[5][i] = tzz;
+        a.o[0][i] = dxx; a.o[1][i] = txy; a.o[2][i] = txz; a.o[3][i] = dyy; a.o[4][i] = tyz;
+        if (a.phase) { a.o[5][i] = q; a.o[6][i] = c3; }
     }
 }
 

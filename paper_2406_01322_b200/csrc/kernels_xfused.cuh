@@ -81,86 +81,108 @@ __device__ __forceinline__ cplx tw_half(const cplx *__restrict__ tw, int i) {
     return w;
 }
 
-// in-place DIF pass on the x tile (sub-length LS, radix R): butterfly, then twiddle
-template <int H, int LS, int R, int SIGN, int NT>
-__device__ __forceinline__ void xpass_dif(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid) {
-    constexpr int STRIDE = LS / R;
-    constexpr int NBF = H / R;
+// compile-time twiddle w_LS^q = exp(-2 pi i q / LS) for LS in {4, 8, 16, 32}, 0 <= q < LS/2
+__device__ __forceinline__ constexpr double cos32(int i) {   // cos(2 pi i / 32), 0 <= i <= 16
+    constexpr double C[9] = {1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708,
+                             0.70710678118654752440, 0.55557023301960222474, 0.38268343236508977173,
+                             0.19509032201612826785, 0.0};
+    return i <= 8 ? C[i] : -C[16 - i];
+}
+template <int LS>
+__device__ __forceinline__ constexpr double wc_re(int q) { return cos32(q * (32 / LS)); }
+template <int LS>
+__device__ __forceinline__ constexpr double wc_im(int q) {   // -sin(2 pi q / LS)
+    return q * (32 / LS) <= 8 ? -cos32(8 - q * (32 / LS)) : -cos32(q * (32 / LS) - 8);
+}
+
+// In-place pass of sub-length LS = 2 R (stride 2) on the x tile.  The two twiddle classes j = 0 (no twiddle)
+// and j = 1 (w_LS^q, compile-time constants) are assigned to different WARPS, so that no twiddle is ever
+// loaded from shared memory (a broadcast LDS.128 costs as many wavefronts as a data access).
+template <int H, int R, int SIGN, int NT, bool DIT>
+__device__ __forceinline__ void xpass_mid(cplx *__restrict__ s, int tid) {
+    constexpr int LS = 2 * R;
+    constexpr int NBLK = H / LS;           // blocks per field; items per field = 2 * NBLK
+    static_assert(NBLK % 4 == 0, "j must be uniform over a warp (4 butterflies x 8 fields)");
     const int f = tid & (TILE_LINES - 1);
-    for (int b = tid >> 3; b < NBF; b += NT / TILE_LINES) {
-        const int blk = b / STRIDE, j = b % STRIDE;
+    for (int b = tid >> 3; b < 2 * NBLK; b += NT / TILE_LINES) {
+        const int j = b / NBLK, blk = b % NBLK;
         const int row0 = blk * LS + j;
         cplx v[R];
 #pragma unroll
-        for (int m = 0; m < R; ++m) v[m] = s[xidx(row0 + m * STRIDE, f)];
-        RegFFT<R, SIGN>::run(v);
+        for (int m = 0; m < R; ++m) v[m] = s[xidx(row0 + 2 * m, f)];
+        if (DIT && j) {
 #pragma unroll
-        for (int q = 0; q < R; ++q) {
-            cplx o = v[q];
-            if (LS > R && q > 0) o = cmultw<SIGN>(o, tw_half<H>(tw, (H / LS) * j * q));
-            s[xidx(row0 + q * STRIDE, f)] = o;
+            for (int m = 1; m < R; ++m) v[m] = cmultw<SIGN>(v[m], make_double2(wc_re<LS>(m), wc_im<LS>(m)));
         }
+        RegFFT<R, SIGN>::run(v);
+        if (!DIT && j) {
+#pragma unroll
+            for (int q = 1; q < R; ++q) v[q] = cmultw<SIGN>(v[q], make_double2(wc_re<LS>(q), wc_im<LS>(q)));
+        }
+#pragma unroll
+        for (int q = 0; q < R; ++q) s[xidx(row0 + 2 * q, f)] = v[q];
     }
 }
 
-// in-place DIT pass: twiddle the inputs, then butterfly
-template <int H, int LS, int R, int SIGN, int NT>
-__device__ __forceinline__ void xpass_dit(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid) {
-    constexpr int STRIDE = LS / R;
-    constexpr int NBF = H / R;
-    const int f = tid & (TILE_LINES - 1);
-    for (int b = tid >> 3; b < NBF; b += NT / TILE_LINES) {
-        const int blk = b / STRIDE, j = b % STRIDE;
-        const int row0 = blk * LS + j;
-        cplx v[R];
-#pragma unroll
-        for (int m = 0; m < R; ++m) {
-            cplx x = s[xidx(row0 + m * STRIDE, f)];
-            if (LS > R && m > 0) x = cmultw<SIGN>(x, tw_half<H>(tw, (H / LS) * j * m));
-            v[m] = x;
-        }
-        RegFFT<R, SIGN>::run(v);
-#pragma unroll
-        for (int q = 0; q < R; ++q) s[xidx(row0 + q * STRIDE, f)] = v[q];
+// Powers w^1 .. w^{R-1} of a per-thread base twiddle from the loop-invariant set {w, w^2, w^4, w^8}:
+// the R1-pass twiddles w_H^{j q} depend on the thread (j) only, so they live in registers instead of
+// being re-read from shared memory for every line.
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+template <int R>
+struct TwPow {
+    cplx w1, w2, w4, w8;
+    __device__ __forceinline__ void init(cplx w) {
+        w1 = w; w2 = cmul(w, w); w4 = cmul(w2, w2); w8 = cmul(w4, w4);
     }
-}
+    // out[q] = w^q, q = 1 .. R-1
+    __device__ __forceinline__ void powers(cplx (&o)[R]) const {
+        o[1] = w1;
+        if (R > 2) { o[2] = w2; o[3] = cmul(w2, w1); }
+        if (R > 4) { o[4] = w4; o[5] = cmul(w4, w1); o[6] = cmul(w4, w2); o[7] = cmul(w4, o[3]); }
+        if (R > 8) {
+            o[8] = w8;
+#pragma unroll
+            for (int q = 1; q < 8; ++q) o[8 + q] = cmul(w8, o[q]);
+        }
+    }
+};
 
 // ---- pointwise products at one grid point (row a5; Eqs. 1, 4, 7, 8) --------------------------
-//   in : u v w [phi phx phy phz]      out: Txx Txy Txz Tyy Tyz Tzz [Q C]
-//   T_ij = -u_i u_j + cs (|grad phi|^2 delta_ij - phi_i phi_j),  Q = u . grad phi,  C = phi^3
+//   in : u v w [phi phx phy phz]      out: Txx-Tzz Txy Txz Tyy-Tzz Tyz [Q C]
+//   T_ij = -u_i u_j + cs (|grad phi|^2 delta_ij - phi_i phi_j),  Q = u . grad phi,  C = phi^3.
+//   Only the deviatoric combinations enter Eqs. 14-15 (see enqueue_step), so T_zz is subtracted here.
 template <bool PHASE>
 __device__ __forceinline__ void nl_point(const double (&in)[8], double (&o)[8], double cs) {
     const double u = in[0], v = in[1], w = in[2];
-    double txx = -u * u, txy = -u * v, txz = -u * w, tyy = -v * v, tyz = -v * w, tzz = -w * w;
+    double dxx = w * w - u * u, dyy = w * w - v * v, txy = -u * v, txz = -u * w, tyz = -v * w;
     if (PHASE) {
         const double ph = in[3], px = in[4], py = in[5], pz = in[6];
-        const double g2 = px * px + py * py + pz * pz;
-        txx += cs * (g2 - px * px);
-        tyy += cs * (g2 - py * py);
-        tzz += cs * (g2 - pz * pz);
+        dxx += cs * (pz * pz - px * px);
+        dyy += cs * (pz * pz - py * py);
         txy -= cs * px * py;
         txz -= cs * px * pz;
         tyz -= cs * py * pz;
-        o[6] = u * px + v * py + w * pz;
-        o[7] = ph * ph * ph;
+        o[5] = u * px + v * py + w * pz;
+        o[6] = ph * ph * ph;
     } else {
-        o[6] = 0.0; o[7] = 0.0;
+        o[5] = 0.0; o[6] = 0.0;
     }
-    o[0] = txx; o[1] = txy; o[2] = txz; o[3] = tyy; o[4] = tyz; o[5] = tzz;
+    o[0] = dxx; o[1] = txy; o[2] = txz; o[3] = dyy; o[4] = tyz; o[7] = 0.0;
 }
 
 struct XFArgs {
-    const cplx *in[8];
-    cplx *out[8];
+    const cplx *in[6];      // Y arrays: u v w [phi phy phz]
+    cplx *out[8];           // Y arrays: Txx-Tzz Txy Txz Tyy-Tzz Tyz [Q C]
     int kxp, nkx, nlines;
     double cs;
+    double kxf;             // 2 pi / Lx: the phx row is i kx times the staged phi row (row a1)
 };
 
 // stage pitch (cplx): odd, so that the 8 fields of one k sit in 8 different 16-byte bank groups
 __host__ __device__ inline int xf_spitch(int nkx) { return nkx | 1; }
 
-// shared memory: tile [H][8] | twiddles w_L^k [H] | stage [NIN][spitch] | mbarrier.  The stage receives the
-// NEXT line's NIN spectra rows by TMA bulk copies while the current line is transformed.
+// shared memory: tile [H][8] | twiddles w_L^k [H] | stage [NST][spitch] | mbarrier.  The stage receives the
+// NEXT line's NST spectra rows by TMA bulk copies while the current line is transformed.
 template <int L, bool PHASE>
 __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused(const __grid_constant__ XFArgs a,
                                                                                const cplx *__restrict__ twx) {
@@ -168,7 +190,8 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
     constexpr int R1 = XPlan<H>::R1, R2 = XPlan<H>::R2;
     constexpr int NT = xf_threads<L>();
     constexpr int S1 = H / R1;              // stride of pass R1 = number of its butterflies per field
-    constexpr int NIN = PHASE ? 7 : 3, NOUT = PHASE ? 8 : 6;
+    constexpr int NIN = PHASE ? 7 : 3, NOUT = PHASE ? 7 : 5;   // fields through the backward / forward FFT
+    constexpr int NST = PHASE ? 6 : 3;                         // staged spectra rows: u v w [phi phy phz]
     static_assert(R1 * R2 * 2 == H, "plan");
     static_assert(S1 * TILE_LINES <= NT, "one (butterfly, field) item per thread in stages A and E");
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -177,7 +200,7 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
     cplx *stage = tw + H;
     const int kxp = a.kxp, nkx = a.nkx;
     const int spitch = xf_spitch(nkx);
-    unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)NIN * spitch);
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)NST * spitch);
     const int tid = threadIdx.x, f = tid & 7, j = tid >> 3;
     const bool item = j < S1;               // this thread owns butterfly j of field f in stages A, E, F
     for (int i = tid; i < H; i += NT) tw[i] = twx[i];
@@ -185,17 +208,21 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
     const double sc = 0.5 / L;
     const unsigned row_bytes = (unsigned)(nkx * sizeof(cplx));
     auto issue = [&](int line) {   // one thread: arm the barrier and launch NIN bulk copies
-        mbar_expect_tx(bar, row_bytes * NIN);
+        mbar_expect_tx(bar, row_bytes * NST);
 #pragma unroll
-        for (int q = 0; q < NIN; ++q) bulk_g2s(stage + (size_t)q * spitch, a.in[q] + (size_t)line * kxp, row_bytes, bar);
+        for (int q = 0; q < NST; ++q) bulk_g2s(stage + (size_t)q * spitch, a.in[q] + (size_t)line * kxp, row_bytes, bar);
     };
     if (tid == 0) {
         mbar_init(bar, 1);
         if ((int)blockIdx.x < a.nlines) issue(blockIdx.x);
     }
     __syncthreads();
+    TwPow<R1> tp;                           // w_H^j: twiddle base of this thread's R1-pass butterfly
+    tp.init(tw_half<H>(tw, item ? j : 0));
     unsigned parity = 0;
-    const cplx *sf = stage + (size_t)(f < NIN ? f : 0) * spitch;
+    // field -> staged row: u v w phi phx phy phz  <-  0 1 2 3 3 4 5 (phx = i kx phi)
+    const cplx *sf = stage + (size_t)(f < 4 ? (f < NST ? f : 0) : (f < NIN ? f - 1 : 0)) * spitch;
+    const double dkx = (PHASE && f == 4) ? a.kxf : 0.0;
     for (int line = blockIdx.x; line < a.nlines; line += gridDim.x) {
         const size_t base = (size_t)line * kxp;
         mbar_wait(bar, parity);
@@ -211,6 +238,11 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
                     if (k < nkx) xa = sf[k];
                     if (kb < nkx) xb = sf[kb];
                 }
+                if (PHASE && f == 4) {                    // i kx X
+                    const double ka = dkx * (double)k, kc = dkx * (double)kb;
+                    xa = make_double2(-ka * xa.y, ka * xa.x);
+                    xb = make_double2(-kc * xb.y, kc * xb.x);
+                }
                 if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
                 const cplx w = tw[k];
                 const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
@@ -218,12 +250,11 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
                 v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
             }
             RegFFT<R1, +1>::run(v);
+            cplx wq[R1];
+            tp.powers(wq);
+            s[xidx(j, f)] = v[0];
 #pragma unroll
-            for (int q = 0; q < R1; ++q) {
-                cplx o = v[q];
-                if (q > 0) o = cmultw<+1>(o, tw_half<H>(tw, j * q));
-                s[xidx(j + S1 * q, f)] = o;
-            }
+            for (int q = 1; q < R1; ++q) s[xidx(j + S1 * q, f)] = cmultw<+1>(v[q], wq[q]);
         }
         __syncthreads();
         if (tid == 0 && line + (int)gridDim.x < a.nlines) {   // stage is free: prefetch the next line
@@ -232,7 +263,7 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
         }
         // ---- B: DIF pass R2 ----
         if constexpr (R2 > 1) {
-            xpass_dif<H, H / R1, R2, +1, NT>(s, tw, tid);
+            xpass_mid<H, R2, +1, NT, false>(s, tid);
             __syncthreads();
         }
         // ---- C: last DIF radix 2, pointwise products, first DIT radix 2: rows (2t, 2t+1) x all fields ----
@@ -266,18 +297,17 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
         __syncthreads();
         // ---- D: DIT pass R2 (forward transform, sign -) ----
         if constexpr (R2 > 1) {
-            xpass_dit<H, 2 * R2, R2, -1, NT>(s, tw, tid);
+            xpass_mid<H, R2, -1, NT, true>(s, tid);
             __syncthreads();
         }
         // ---- E: DIT pass R1, results stay in registers and are published to the tile ----
         cplx v[R1];
         if (item) {
+            cplx wq[R1];
+            tp.powers(wq);
+            v[0] = s[xidx(j, f)];
 #pragma unroll
-            for (int m = 0; m < R1; ++m) {
-                cplx x = s[xidx(j + S1 * m, f)];
-                if (m > 0) x = cmultw<-1>(x, tw_half<H>(tw, j * m));
-                v[m] = x;
-            }
+            for (int m = 1; m < R1; ++m) v[m] = cmultw<-1>(s[xidx(j + S1 * m, f)], wq[m]);
             RegFFT<R1, -1>::run(v);
 #pragma unroll
             for (int q = 0; q < R1; ++q) s[xidx(j + S1 * q, f)] = v[q];

@@ -52,8 +52,8 @@ struct Layout {
     size_t thh, wh;                    // real homogeneous solutions [nz][ncols]
     size_t hw, coef;                   // [2][ncols] doubles / cplx
     size_t xom;
-    size_t derived[8];                 // phx phy phz exx eyy exy exz eyz
-    size_t prod[8];                    // txx txy txz tyy tyz tzz q c
+    size_t derived[8];                 // phz [exx eyy exy exz eyz]
+    size_t prod[8];                    // txx-tzz txy txz tyy-tzz tyz q c
     size_t zb[MAXF], yb[MAXF], ph[MAXF];
     size_t small;                      // ab[2] doubles + counter
     size_t stage[4];                   // host-staging device buffers (boundary layout)
@@ -78,8 +78,9 @@ struct psdns_handle {
     int timed_class;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tevents;
     int nf_in, nf_out;
-    bool use_xfused, use_zhalf;
+    bool use_xfused;
     int xf_occ, n_sm;
+    int occ_z[2], occ_y[2];     // resident CTAs per SM of the persistent z / y passes, [fwd]
 
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
 };
@@ -133,9 +134,12 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.hw = take(2 * d.ncols * sizeof(double));
     L.coef = take(2 * d.ncols * C);
     L.xom = take(d.s_ret * C);
-    for (int i = 0; i < 8; ++i) L.derived[i] = take(d.s_low * C);
-    for (int i = 0; i < 8; ++i) L.prod[i] = take(d.s_low * C);
-    const int nf = (p.phase_field && p.visc_ratio != 1.0) ? 12 : 8;
+    const bool visc_l = p.phase_field && p.visc_ratio != 1.0;
+    for (int i = 0; i < 8; ++i) L.derived[i] = 0;
+    for (int i = 0; i < (visc_l ? 6 : 1); ++i) L.derived[i] = take(d.s_low * C);   // phz [+ 5 strains]
+    for (int i = 0; i < 8; ++i) L.prod[i] = 0;
+    for (int i = 0; i < 7; ++i) L.prod[i] = take(d.s_low * C);
+    const int nf = visc_l ? 12 : 7;
     // Z / Y arrays double as the full-size round-trip scratch (3 arrays of s_full each)
     size_t zy_bytes = 0;
     for (int i = 0; i < MAXF; ++i) { L.zb[i] = 0; L.yb[i] = 0; L.ph[i] = 0; }
@@ -217,7 +221,7 @@ cudaError_t set_smem(K kern, size_t bytes) {
     }
 
 template <int N>
-size_t zhalf_smem() { return (size_t)(N * TILE_LINES + N + (NT_FFT / 32) * 8) * sizeof(cplx); }
+size_t zpass_smem() { return (size_t)zpass_smem_cplx<N>() * sizeof(cplx); }
 
 #define DISPATCH_N(Nval, MACRO)            \
     switch (Nval) {                        \
@@ -231,41 +235,43 @@ size_t zhalf_smem() { return (size_t)(N * TILE_LINES + N + (NT_FFT / 32) * 8) * 
         default: return cudaErrorInvalidValue; \
     }
 
-cudaError_t launch_zpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, size_t ncols, int nk) {
-    ZArgs a; a.f = f; a.ncols = (int)ncols; a.nk = nk;
+// derived outputs of the backward z pass (row a1): i kx X and / or i ky X of field dfield
+struct ZDerived {
+    int dfield = -1;
+    cplx *out_dx = nullptr, *out_dy = nullptr;
+};
+
+cudaError_t launch_zpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, size_t ncols, int nk, int kxp, int nky,
+                         int jpos, const ZDerived &zd = ZDerived()) {
+    ZArgs a; a.f = f; a.nf = nf; a.ncols = (int)ncols; a.nk = nk;
+    a.dfield = fwd ? -1 : zd.dfield; a.out_dx = zd.out_dx; a.out_dy = zd.out_dy;
+    a.kxp = kxp; a.nky = nky; a.jpos = jpos;
+    a.kxf = 2.0 * M_PI / h->g.lx; a.kyf = 2.0 * M_PI / h->g.ly;
     const cplx *tw = h->at<cplx>(h->L.tw_z);
-    dim3 grid((unsigned)(ncols / 8), nf);
+    const cplx *ct = h->at<cplx>(h->L.ctab_z);
+    const long long ntiles = (long long)(ncols / 8) * nf;
+    const int grid = (int)std::min<long long>(ntiles, (long long)h->n_sm * std::max(h->occ_z[fwd], 1));
     LaunchScope ls(h, fwd ? KC_ZFWD : KC_ZBWD);
-    if (h->use_zhalf) {
-        const cplx *ct = h->at<cplx>(h->L.ctab_z);
 #define ZH(NN)                                                                                           \
     {                                                                                                    \
-        if (fwd) k_zpass_h<NN, true><<<grid, NT_FFT, zhalf_smem<NN>(), h->st>>>(a, tw, ct);              \
-        else k_zpass_h<NN, false><<<grid, NT_FFT, zhalf_smem<NN>(), h->st>>>(a, tw, ct);                 \
+        if (fwd) k_zpass<NN, true><<<grid, fused_threads<NN>(), zpass_smem<NN>(), h->st>>>(a, tw, ct);   \
+        else k_zpass<NN, false><<<grid, fused_threads<NN>(), zpass_smem<NN>(), h->st>>>(a, tw, ct);      \
     }
-        DISPATCH_N(h->d.N, ZH)
+    DISPATCH_N(h->d.N, ZH)
 #undef ZH
-        return cudaGetLastError();
-    }
-#define ZL(LL)                                                                                          \
-    {                                                                                                   \
-        if (fwd) k_zpass<LL, true><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                     \
-        else k_zpass<LL, false><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                        \
-    }
-    DISPATCH_L(2 * h->d.N, ZL)
-#undef ZL
     return cudaGetLastError();
 }
 
 cudaError_t launch_ypass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, int kxp, int nky, int jpos) {
-    YArgs a; a.f = f; a.kxp = kxp; a.nky = nky; a.jpos = jpos;
+    YArgs a; a.f = f; a.nf = nf; a.nz = h->d.nz; a.kxp = kxp; a.nky = nky; a.jpos = jpos;
     const cplx *tw = h->at<cplx>(h->L.tw_y);
-    dim3 grid(kxp / 8, h->d.nz, nf);
+    const long long ntiles = (long long)(kxp / 8) * h->d.nz * nf;
+    const int grid = (int)std::min<long long>(ntiles, (long long)h->n_sm * std::max(h->occ_y[fwd], 1));
     LaunchScope ls(h, fwd ? KC_YFWD : KC_YBWD);
 #define YL(LL)                                                                                          \
     {                                                                                                   \
-        if (fwd) k_ypass<LL, true><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                     \
-        else k_ypass<LL, false><<<grid, tile_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);                        \
+        if (fwd) k_ypass<LL, true><<<grid, fused_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);        \
+        else k_ypass<LL, false><<<grid, fused_threads<LL>(), fft_smem<LL>(), h->st>>>(a, tw);           \
     }
     DISPATCH_L(h->d.ny, YL)
 #undef YL
@@ -287,21 +293,28 @@ cudaError_t launch_xpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, 
     return cudaGetLastError();
 }
 
-// opt-in to > 48 KB dynamic shared memory once, at init (not inside graph capture)
+// opt-in to > 48 KB dynamic shared memory once, at init (not inside graph capture), and size the persistent grids
 cudaError_t setup_attrs(psdns_handle *h) {
-#define ZA(LL) { CU0(set_smem(k_zpass<LL, true>, fft_smem<LL>())); CU0(set_smem(k_zpass<LL, false>, fft_smem<LL>())); }
-#define YA(LL) { CU0(set_smem(k_ypass<LL, true>, fft_smem<LL>())); CU0(set_smem(k_ypass<LL, false>, fft_smem<LL>())); }
-#define XA(LL) { CU0(set_smem(k_xpass<LL, true>, fft_smem<LL>())); CU0(set_smem(k_xpass<LL, false>, fft_smem<LL>())); }
 #define CU0(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) return e__; } while (0)
-    DISPATCH_L(2 * h->d.N, ZA)
-#define ZHA(NN) { CU0(set_smem(k_zpass_h<NN, true>, zhalf_smem<NN>())); CU0(set_smem(k_zpass_h<NN, false>, zhalf_smem<NN>())); }
-    DISPATCH_N(h->d.N, ZHA)
-#undef ZHA
+#define ZA(NN)                                                                                                         \
+    {                                                                                                                  \
+        CU0(set_smem(k_zpass<NN, true>, zpass_smem<NN>())); CU0(set_smem(k_zpass<NN, false>, zpass_smem<NN>()));        \
+        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_z[1], k_zpass<NN, true>, fused_threads<NN>(), zpass_smem<NN>()));  \
+        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_z[0], k_zpass<NN, false>, fused_threads<NN>(), zpass_smem<NN>())); \
+    }
+#define YA(LL)                                                                                                         \
+    {                                                                                                                  \
+        CU0(set_smem(k_ypass<LL, true>, fft_smem<LL>())); CU0(set_smem(k_ypass<LL, false>, fft_smem<LL>()));            \
+        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_y[1], k_ypass<LL, true>, fused_threads<LL>(), fft_smem<LL>()));    \
+        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_y[0], k_ypass<LL, false>, fused_threads<LL>(), fft_smem<LL>()));   \
+    }
+#define XA(LL) { CU0(set_smem(k_xpass<LL, true>, fft_smem<LL>())); CU0(set_smem(k_xpass<LL, false>, fft_smem<LL>())); }
+    DISPATCH_N(h->d.N, ZA)
     DISPATCH_L(h->d.ny, YA)
     DISPATCH_L(h->d.nx, XA)
 #define XFA(LL)                                                                                              \
     {                                                                                                        \
-        const size_t sm = xfused_smem<LL>(h->d.nkx, h->nf_in);                                               \
+        const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 6 : 3);                               \
         int occ = 0;                                                                                         \
         if (h->p.phase_field) {                                                                              \
             CU0(set_smem(k_xfused<LL, true>, sm));                                                           \
@@ -327,7 +340,7 @@ cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
     LaunchScope ls(h, KC_XFUSED);
 #define XF(LL)                                                                                               \
     {                                                                                                        \
-        const size_t sm = xfused_smem<LL>(h->d.nkx, h->nf_in);                                               \
+        const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 6 : 3);                               \
         if (h->p.phase_field) k_xfused<LL, true><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);              \
         else k_xfused<LL, false><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);                              \
     }
@@ -382,6 +395,13 @@ Coefs coefs(const psdns_params &p) {
     } while (0)
 
 // ---- one time step (rows a1-a11) ------------------------------------------------------------------
+// Field bookkeeping (matched viscosity, phase field on):
+//   backward: 5 z transforms (u, v, w, phi, D phi) whose epilogue also emits i ky phi (row a1), 6 y
+//             transforms, and the fused x kernel forms i kx phi from the staged phi row: 7 physical fields.
+//   forward : 7 product fields Txx - Tzz, Txy, Txz, Tyy - Tzz, Tyz, Q, C.  Only the deviatoric part of T
+//             enters Eqs. 14-15 (the isotropic part g delta_ij gives S = grad g, which the curl and the
+//             k^2 S_z + D(ikx S_x + iky S_y) combination annihilate identically in the discrete operators), so
+//             T_zz is subtracted pointwise instead of being transformed on its own.
 cudaError_t enqueue_step(psdns_handle *h) {
     const Dims &d = h->d;
     const Layout &L = h->L;
@@ -389,92 +409,113 @@ cudaError_t enqueue_step(psdns_handle *h) {
     const Coefs c = coefs(p);
     const bool phase = p.phase_field != 0;
     const bool visc = phase && p.visc_ratio != 1.0;
-    const int nin = h->nf_in, nout = h->nf_out;
+    const int nout = h->nf_out;
     cplx *U = h->at<cplx>(L.state[0]), *V = h->at<cplx>(L.state[1]), *W = h->at<cplx>(L.state[2]);
-    cplx *PHI = h->at<cplx>(L.state[3]), *TH = h->at<cplx>(L.state[4]);
+    cplx *PHI = h->at<cplx>(L.state[3]), *TH = h->at<cplx>(L.state[4]), *OM = h->at<cplx>(L.xom);
+    cplx *PHZ = h->at<cplx>(L.derived[0]);
     double *ab = h->at<double>(L.small);
     int *counter = reinterpret_cast<int *>(ab + 2);
     { LaunchScope ls(h, KC_MISC); k_begin_step<<<1, 1, 0, h->st>>>(ab, counter); CU(cudaGetLastError()); }
 
-    // a1: derived spectra
-    if (phase) {
+    // a1 (variable viscosity only): strain spectra
+    if (visc) {
         PrepArgs a;
-        a.g = geom(h); a.u = U; a.v = V; a.w = W; a.phi = PHI;
-        a.phx = h->at<cplx>(L.derived[0]); a.phy = h->at<cplx>(L.derived[1]); a.phz = h->at<cplx>(L.derived[2]);
-        a.exx = h->at<cplx>(L.derived[3]); a.eyy = h->at<cplx>(L.derived[4]); a.exy = h->at<cplx>(L.derived[5]);
-        a.exz = h->at<cplx>(L.derived[6]); a.eyz = h->at<cplx>(L.derived[7]);
-        a.phase = 1; a.visc = visc;
+        a.g = geom(h); a.u = U; a.v = V; a.w = W; a.phi = PHI; a.phz = PHZ;
+        a.exx = h->at<cplx>(L.derived[1]); a.eyy = h->at<cplx>(L.derived[2]); a.exy = h->at<cplx>(L.derived[3]);
+        a.exz = h->at<cplx>(L.derived[4]); a.eyz = h->at<cplx>(L.derived[5]);
+        a.do_phz = 0; a.visc = 1;
         LaunchScope ls(h, KC_RHS);
         k_prep<<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
-    // a2-a4: backward transforms of nin fields
-    FieldPtrs fz{}, fy{}, fx{};
-    const cplx *src[MAXF] = {U, V, W, PHI};
-    for (int i = 0; i < 8; ++i) src[4 + i] = h->at<cplx>(L.derived[i]);
-    for (int i = 0; i < nin; ++i) {
-        fz.in[i] = src[i]; fz.out[i] = h->at<cplx>(L.zb[i]);
-        fy.in[i] = fz.out[i]; fy.out[i] = h->at<cplx>(L.yb[i]);
-        fx.in[i] = fy.out[i]; fx.out[i] = h->at<double>(L.ph[i]);
+    // a2-a3: backward z and y transforms
+    FieldPtrs fz{}, fy{};
+    ZDerived zd;
+    int nz_f = 3, ny_f = 3;   // fields through the z pass / the y pass
+    const cplx *src[MAXF] = {U, V, W, PHI, PHZ};
+    if (phase) {
+        nz_f = 5;
+        if (visc) {
+            for (int i = 0; i < 5; ++i) src[5 + i] = h->at<cplx>(L.derived[1 + i]);
+            nz_f = 10;
+            zd.dfield = 3; zd.out_dx = h->at<cplx>(L.zb[10]); zd.out_dy = h->at<cplx>(L.zb[11]);
+            ny_f = 12;
+        } else {
+            const bool fused = h->use_xfused;
+            zd.dfield = 3; zd.out_dx = fused ? nullptr : h->at<cplx>(L.zb[6]); zd.out_dy = h->at<cplx>(L.zb[5]);
+            ny_f = fused ? 6 : 7;
+        }
     }
-    CU(launch_zpass(h, false, fz, nin, d.ncols, d.nkz));
-    CU(launch_ypass(h, false, fy, nin, d.kxp, d.nky, d.jpos));
-    FieldPtrs gx{}, gy{}, gz{};
+    for (int i = 0; i < nz_f; ++i) { fz.in[i] = src[i]; fz.out[i] = h->at<cplx>(L.zb[i]); }
+    for (int i = 0; i < ny_f; ++i) { fy.in[i] = h->at<cplx>(L.zb[i]); fy.out[i] = h->at<cplx>(L.yb[i]); }
+    CU(launch_zpass(h, false, fz, nz_f, d.ncols, d.nkz, d.kxp, d.nky, d.jpos, zd));
+    CU(launch_ypass(h, false, fy, ny_f, d.kxp, d.nky, d.jpos));
+    FieldPtrs gy{}, gz{};
     for (int i = 0; i < nout; ++i) {
-        gx.in[i] = h->at<double>(L.ph[i]); gx.out[i] = h->at<cplx>(L.yb[i]);
-        gy.in[i] = gx.out[i]; gy.out[i] = h->at<cplx>(L.zb[i]);
+        gy.in[i] = h->at<cplx>(L.yb[i]); gy.out[i] = h->at<cplx>(L.zb[i]);
         gz.in[i] = gy.out[i]; gz.out[i] = h->at<cplx>(L.prod[i]);
     }
     if (h->use_xfused && !visc) {
         // a4 + a5 + a6 fused: physical space never leaves the SM; in place on the Y arrays
         XFArgs a;
-        for (int i = 0; i < 8; ++i) { a.in[i] = h->at<cplx>(L.yb[i < nin ? i : 0]); a.out[i] = h->at<cplx>(L.yb[i < nout ? i : 0]); }
+        const int stage_src[6] = {0, 1, 2, 3, 5, 4};   // u v w phi phy phz  <-  Y arrays u v w phi phz phy
+        for (int i = 0; i < 6; ++i) a.in[i] = h->at<cplx>(L.yb[phase ? stage_src[i] : (i < 3 ? i : 0)]);
+        for (int i = 0; i < 8; ++i) a.out[i] = h->at<cplx>(L.yb[i < nout ? i : 0]);
         a.kxp = d.kxp; a.nkx = d.nkx; a.nlines = d.nz * d.ny;
-        a.cs = c.cs;
+        a.cs = c.cs; a.kxf = 2.0 * M_PI / h->g.lx;
         CU(launch_xfused(h, a));
     } else {
-        CU(launch_xpass(h, false, fx, nin, d.kxp, d.nkx));
-        // a5: pointwise products (in place)
+        // unfused path (variable viscosity, or PSDNS_NO_XFUSE): a4, a5, a6 as separate kernels
+        FieldPtrs fx{}, gx{};
+        const int nx_f = ny_f;
+        for (int i = 0; i < nx_f; ++i) { fx.in[i] = h->at<cplx>(L.yb[i]); fx.out[i] = h->at<double>(L.ph[i]); }
+        CU(launch_xpass(h, false, fx, nx_f, d.kxp, d.nkx));
         {
             PwArgs a;
-            for (int i = 0; i < MAXF; ++i) a.b[i] = h->at<double>(L.ph[i < std::max(nin, nout) ? i : 0]);
+            // pointwise order: u v w phi phx phy phz exx eyy exy exz eyz  <-  buffers 0 1 2 3 10 11 4 5 6 7 8 9
+            //                                                            (matched viscosity: 0 1 2 3 6 5 4)
+            const int order_v[MAXF] = {0, 1, 2, 3, 10, 11, 4, 5, 6, 7, 8, 9};
+            const int order_m[MAXF] = {0, 1, 2, 3, 6, 5, 4, 0, 0, 0, 0, 0};
+            for (int i = 0; i < MAXF; ++i)
+                a.b[i] = h->at<double>(L.ph[phase ? (visc ? order_v[i] : order_m[i]) : (i < 3 ? i : 0)]);
+            for (int i = 0; i < 8; ++i) a.o[i] = h->at<double>(L.ph[i < nout ? i : 0]);
             a.n = d.s_p; a.cs = c.cs; a.eta_c = (p.visc_ratio - 1.0) / (2.0 * p.re);
             a.phase = phase; a.visc = visc;
             LaunchScope ls(h, KC_PW);
             k_pointwise<<<148 * 8, 256, 0, h->st>>>(a);
             CU(cudaGetLastError());
         }
-        // a6: forward x with truncation
+        for (int i = 0; i < nout; ++i) { gx.in[i] = h->at<double>(L.ph[i]); gx.out[i] = h->at<cplx>(L.yb[i]); }
         CU(launch_xpass(h, true, gx, nout, d.kxp, d.nkx));
     }
     // a7-a8: forward y, z with truncation
     CU(launch_ypass(h, true, gy, nout, d.kxp, d.nky, d.jpos));
-    CU(launch_zpass(h, true, gz, nout, d.ncols, d.nkz));
+    CU(launch_zpass(h, true, gz, nout, d.ncols, d.nkz, d.kxp, d.nky, d.jpos));
     // a9 + first elimination (K_A), substitution (K_B), second elimination (K_C), substitution +
     // influence-matrix correction (K_D), velocity recovery (a11)
-    cplx *XOM = h->at<cplx>(L.xom);
     const double inv_g = 1.0 / c.gamma;
     const double *dNS = h->at<double>(L.dinv[0]), *dPO = h->at<double>(L.dinv[1]), *dCH = h->at<double>(L.dinv[2]);
     {
         RhsElimArgs a;
         a.g = geom(h);
         a.txx = h->at<cplx>(L.prod[0]); a.txy = h->at<cplx>(L.prod[1]); a.txz = h->at<cplx>(L.prod[2]);
-        a.tyy = h->at<cplx>(L.prod[3]); a.tyz = h->at<cplx>(L.prod[4]); a.tzz = h->at<cplx>(L.prod[5]);
-        a.q = h->at<cplx>(L.prod[6]); a.c = h->at<cplx>(L.prod[7]);
-        a.u = U; a.v = V; a.th = TH; a.phi = PHI; a.xom = XOM;
+        a.tyy = h->at<cplx>(L.prod[3]); a.tyz = h->at<cplx>(L.prod[4]);
+        a.q = h->at<cplx>(L.prod[5]); a.c = h->at<cplx>(L.prod[6]);
+        a.om = OM; a.th = TH; a.phi = PHI;
         a.h_om = h->at<cplx>(L.hist[0]); a.h_w = h->at<cplx>(L.hist[1]); a.h_phi = h->at<cplx>(L.hist[2]);
         a.dinv_ns = dNS; a.dinv_ch = dCH;
         a.ab = ab; a.dt = p.dt; a.gamma = c.gamma; a.inv_pe = phase ? 1.0 / p.pe : 0.0;
         a.e_phi = 1.0 + c.s_coef * p.ch * p.ch;
         a.gradp = p.gradp_x; a.lam_phi = c.lam_phi; a.gam_phi = c.gam_phi; a.phase = phase;
+        const int grid = (int)((d.ncols + RHS_COLS - 1) / RHS_COLS);
         LaunchScope ls(h, KC_RHS);
-        k_rhs_elim<<<dim3(col_grid(d), phase ? 3 : 2), NT_COL, 0, h->st>>>(a);
+        k_rhs_elim<<<grid, 32 * (phase ? 3 : 2), 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     {
         SubstArgs a;
         a.g = geom(h);
-        a.x[0] = XOM; a.x[1] = TH; a.x[2] = PHI;
+        a.x[0] = OM; a.x[1] = TH; a.x[2] = PHI;
         a.dinv[0] = dNS; a.dinv[1] = dNS; a.dinv[2] = dCH;
         a.shift[0] = inv_g; a.shift[1] = inv_g; a.shift[2] = c.lam_phi;
         a.nchains = phase ? 3 : 2;
@@ -503,10 +544,11 @@ cudaError_t enqueue_step(psdns_handle *h) {
         k_subst<<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
-    // a11: u^, v^
+    // a11: u^, v^ (and D phi^ for the next step)
     {
         FinishArgs a;
-        a.g = geom(h); a.xom = XOM; a.u = U; a.v = V; a.w = W; a.th = TH;
+        a.g = geom(h); a.om = OM; a.th = TH; a.u = U; a.v = V; a.w = W;
+        a.phi = phase ? PHI : nullptr; a.phz = PHZ;
         LaunchScope ls(h, KC_SOLVE);
         k_finish<<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
@@ -575,7 +617,17 @@ int finish_set_state(psdns_handle *h) {
     const Layout &L = h->L;
     {
         LaunchScope ls(h, KC_MISC);
-        k_lap<<<col_grid(d), NT_COL, 0, h->st>>>(geom(h), h->at<cplx>(L.state[2]), h->at<cplx>(L.state[4]));
+        k_hidden_state<<<col_grid(d), NT_COL, 0, h->st>>>(geom(h), h->at<cplx>(L.state[0]), h->at<cplx>(L.state[1]),
+                                                          h->at<cplx>(L.state[2]), h->at<cplx>(L.state[4]),
+                                                          h->at<cplx>(L.xom));
+        CUDA_TRY(h, cudaGetLastError());
+    }
+    if (h->p.phase_field) {   // D phi^ for the first step (k_finish maintains it afterwards)
+        PrepArgs a{};
+        a.g = geom(h); a.phi = h->at<cplx>(L.state[3]); a.phz = h->at<cplx>(L.derived[0]);
+        a.do_phz = 1; a.visc = 0;
+        LaunchScope ls(h, KC_MISC);
+        k_prep<<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CUDA_TRY(h, cudaGetLastError());
     }
     for (int i = 0; i < 3; ++i) CUDA_TRY(h, cudaMemsetAsync(h->ws + L.hist[i], 0, d.s_low * sizeof(cplx), h->st));
@@ -610,13 +662,13 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->has_state = false; h->graph = nullptr; h->graph_ready = false;
     h->use_graph = std::getenv("PSDNS_NO_GRAPH") == nullptr;
     h->use_xfused = std::getenv("PSDNS_NO_XFUSE") == nullptr;
-    h->use_zhalf = std::getenv("PSDNS_Z2N") == nullptr;
     h->launches = 0; h->per_step = 0; h->timed_class = -1;
     const bool phase = params->phase_field != 0;
     const bool visc = phase && params->visc_ratio != 1.0;
     h->nf_in = phase ? (visc ? 12 : 7) : 3;
-    h->nf_out = phase ? 8 : 6;
+    h->nf_out = phase ? 7 : 5;
     h->xf_occ = 1; h->n_sm = 148;
+    h->occ_z[0] = h->occ_z[1] = h->occ_y[0] = h->occ_y[1] = 1;
     {
         int dev = 0, nsm = 0;
         if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0)
@@ -660,7 +712,7 @@ int psdns_set_state(psdns_handle *h, int space, const void *d_u, const void *d_v
         }
         CUDA_TRY(h, launch_xpass(h, true, fx, nf, d.kxp, d.nkx));
         CUDA_TRY(h, launch_ypass(h, true, fy, nf, d.kxp, d.nky, d.jpos));
-        CUDA_TRY(h, launch_zpass(h, true, fz, nf, d.ncols, d.nz));
+        CUDA_TRY(h, launch_zpass(h, true, fz, nf, d.ncols, d.nz, d.kxp, d.nky, d.jpos));
     }
     return finish_set_state(h);
 }
@@ -687,7 +739,7 @@ int psdns_get_state(psdns_handle *h, int space, void *d_u, void *d_v, void *d_w,
             fy.in[i] = fz.out[i]; fy.out[i] = h->at<cplx>(L.yb[i]);
             fx.in[i] = fy.out[i]; fx.out[i] = dst[i];
         }
-        CUDA_TRY(h, launch_zpass(h, false, fz, nf, d.ncols, d.nz));
+        CUDA_TRY(h, launch_zpass(h, false, fz, nf, d.ncols, d.nz, d.kxp, d.nky, d.jpos));
         CUDA_TRY(h, launch_ypass(h, false, fy, nf, d.kxp, d.nky, d.jpos));
         CUDA_TRY(h, launch_xpass(h, false, fx, nf, d.kxp, d.nkx));
     }
@@ -757,7 +809,7 @@ int psdns_transform_roundtrip(psdns_handle *h, int start_space, const void *d_in
         f.in[0] = A; f.out[0] = B;
         CUDA_TRY(h, launch_ypass(h, true, f, 1, d.kxpf, d.ny, d.ny));
         f.in[0] = B; f.out[0] = C;
-        CUDA_TRY(h, launch_zpass(h, true, f, 1, ncols_f, d.nz));
+        CUDA_TRY(h, launch_zpass(h, true, f, 1, ncols_f, d.nz, d.kxpf, d.ny, d.ny));
         CUDA_TRY(h, launch_relayout(h, spec_boundary, C, side_boundary(d), side_full(d), d.nz));
         return PSDNS_OK;
     };
@@ -765,7 +817,7 @@ int psdns_transform_roundtrip(psdns_handle *h, int start_space, const void *d_in
         CUDA_TRY(h, launch_relayout(h, C, spec_boundary, side_full(d), side_boundary(d), d.nz));
         FieldPtrs f{};
         f.in[0] = C; f.out[0] = B;
-        CUDA_TRY(h, launch_zpass(h, false, f, 1, ncols_f, d.nz));
+        CUDA_TRY(h, launch_zpass(h, false, f, 1, ncols_f, d.nz, d.kxpf, d.ny, d.ny));
         f.in[0] = B; f.out[0] = A;
         CUDA_TRY(h, launch_ypass(h, false, f, 1, d.kxpf, d.ny, d.ny));
         f.in[0] = A; f.out[0] = phys;
