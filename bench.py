@@ -69,19 +69,26 @@ def algorithmic_bytes(c):
     visc = phase and c.visc_ratio != 1.0
     nin = (12 if visc else 7) if phase else 3
     nout = 8 if phase else 6
-    nstate = 5 if phase else 4        # u v w theta (+phi), all nz planes
-    nhist = 3 if phase else 2
+    # field counts of the pipeline AS BUILT: matched viscosity sends 5 spectra through the
+    # backward z pass (u v w phi Dphi; i ky phi is a second output of the phi columns), 6 through the backward y
+    # pass (i kx phi is formed inside the fused x kernel) and 7 deviatoric products through the forward passes
+    # (T_zz is subtracted pointwise).  Variable viscosity: 10 / 12 / 12 backward, unfused x passes.
+    if phase:
+        nzr, nzw, nyb, nfw = (10, 12, 12, 7) if visc else (5, 6, 6, 7)
+    else:
+        nzr, nzw, nyb, nfw = 3, 3, 3, 5
     per_kernel = {
-        "zbwd": nin * (S_ppp + S_ppz),
-        "ybwd": nin * (S_ppz + S_pyz),
-        "xbwd": nin * (S_pyz + R),
-        "pointwise": (nin + nout) * R,
-        "xfwd": nout * (R + S_pyz),
-        "yfwd": nout * (S_pyz + S_ppz),
-        "zfwd": nout * (S_ppz + S_ppp),
-        "xfused": (nin + nout) * S_pyz,
+        "zbwd": nzr * S_ppp + nzw * S_ppz,
+        "ybwd": nyb * (S_ppz + S_pyz),
+        "xbwd": nyb * (S_pyz + R),
+        "pointwise": (nyb + nfw) * R,
+        "xfwd": nfw * (R + S_pyz),
+        "yfwd": nfw * (S_pyz + S_ppz),
+        "zfwd": nfw * (S_ppz + S_ppp),
+        "xfused": (nyb + nfw) * S_pyz,
     }
-    # fused-pipeline figure of SURVEY 8(d): physical-space arrays never leave the SM
+    # fused-pipeline figure of SURVEY 8(d) (7 in / 8 out fields; the contract figure, about 310 B per grid point):
+    # physical-space arrays never leave the SM
     step_fused = (4 * S_ppp + nin * S_ppz) + nin * (S_ppz + S_pyz) + (nin + nout) * S_pyz \
         + nout * (S_pyz + S_ppz) + (nout * S_ppz + 7 * S_ppp + 7 * S_ppp)
     return per_kernel, step_fused, dict(nkx=nkx, nky=nky, nkz=nkz, nin=nin, nout=nout)
