@@ -134,15 +134,25 @@ struct TwPow {
     __device__ __forceinline__ void init(cplx w) {
         w1 = w; w2 = cmul(w, w); w4 = cmul(w2, w2); w8 = cmul(w4, w4);
     }
-    // out[q] = w^q, q = 1 .. R-1
-    __device__ __forceinline__ void powers(cplx (&o)[R]) const {
-        o[1] = w1;
-        if (R > 2) { o[2] = w2; o[3] = cmul(w2, w1); }
-        if (R > 4) { o[4] = w4; o[5] = cmul(w4, w1); o[6] = cmul(w4, w2); o[7] = cmul(w4, o[3]); }
+    // visits fn(q, w^q) for q = 1 .. R-1 in an order that needs at most two temporaries besides {w, w^2, w^4, w^8}
+    // (an array of all R-1 powers next to the R butterfly values does not fit in 128 registers)
+    template <class Fn>
+    __device__ __forceinline__ void each(Fn fn) const {
+        fn(1, w1);
+        if (R > 2) { fn(2, w2); fn(3, cmul(w2, w1)); }
+        if (R > 4) {
+            fn(4, w4); fn(5, cmul(w4, w1));
+            const cplx w6 = cmul(w4, w2);
+            fn(6, w6); fn(7, cmul(w6, w1));
+        }
         if (R > 8) {
-            o[8] = w8;
-#pragma unroll
-            for (int q = 1; q < 8; ++q) o[8 + q] = cmul(w8, o[q]);
+            fn(8, w8); fn(9, cmul(w8, w1));
+            const cplx w10 = cmul(w8, w2);
+            fn(10, w10); fn(11, cmul(w10, w1));
+            const cplx w12 = cmul(w8, w4);
+            fn(12, w12); fn(13, cmul(w12, w1));
+            const cplx w14 = cmul(w12, w2);
+            fn(14, w14); fn(15, cmul(w14, w1));
         }
     }
 };
@@ -151,23 +161,28 @@ struct TwPow {
 //   in : u v w [phi phx phy phz]      out: Txx-Tzz Txy Txz Tyy-Tzz Tyz [Q C]
 //   T_ij = -u_i u_j + cs (|grad phi|^2 delta_ij - phi_i phi_j),  Q = u . grad phi,  C = phi^3.
 //   Only the deviatoric combinations enter Eqs. 14-15 (see enqueue_step), so T_zz is subtracted here.
-template <bool PHASE>
-__device__ __forceinline__ void nl_point(const double (&in)[8], double (&o)[8], double cs) {
+template <int Q, bool PHASE>
+__device__ __forceinline__ double nl_out(const double (&in)[8], double cs) {
     const double u = in[0], v = in[1], w = in[2];
-    double dxx = w * w - u * u, dyy = w * w - v * v, txy = -u * v, txz = -u * w, tyz = -v * w;
-    if (PHASE) {
-        const double ph = in[3], px = in[4], py = in[5], pz = in[6];
-        dxx += cs * (pz * pz - px * px);
-        dyy += cs * (pz * pz - py * py);
-        txy -= cs * px * py;
-        txz -= cs * px * pz;
-        tyz -= cs * py * pz;
-        o[5] = u * px + v * py + w * pz;
-        o[6] = ph * ph * ph;
-    } else {
-        o[5] = 0.0; o[6] = 0.0;
-    }
-    o[0] = dxx; o[1] = txy; o[2] = txz; o[3] = dyy; o[4] = tyz; o[7] = 0.0;
+    const double px = in[4], py = in[5], pz = in[6];
+    if (Q == 0) { double r = w * w - u * u; if (PHASE) r += cs * (pz * pz - px * px); return r; }
+    if (Q == 1) { double r = -u * v; if (PHASE) r -= cs * px * py; return r; }
+    if (Q == 2) { double r = -u * w; if (PHASE) r -= cs * px * pz; return r; }
+    if (Q == 3) { double r = w * w - v * v; if (PHASE) r += cs * (pz * pz - py * py); return r; }
+    if (Q == 4) { double r = -v * w; if (PHASE) r -= cs * py * pz; return r; }
+    if (Q == 5) return u * px + v * py + w * pz;
+    return in[3] * in[3] * in[3];
+}
+
+// one output field of the row pair (2t, 2t+1): the products at the four points held by this thread, recombined
+// by the first DIT radix-2 butterfly and stored; inputs stay in registers, outputs never accumulate
+template <int Q, bool PHASE>
+__device__ __forceinline__ void nl_store(cplx *__restrict__ s, int t, const double (&p00)[8], const double (&p01)[8],
+                                         const double (&p10)[8], const double (&p11)[8], double cs) {
+    const double o00 = nl_out<Q, PHASE>(p00, cs), o01 = nl_out<Q, PHASE>(p01, cs);
+    const double o10 = nl_out<Q, PHASE>(p10, cs), o11 = nl_out<Q, PHASE>(p11, cs);
+    s[xidx(2 * t, Q)] = make_double2(o00 + o10, o01 + o11);
+    s[xidx(2 * t + 1, Q)] = make_double2(o00 - o10, o01 - o11);
 }
 
 struct XFArgs {
@@ -183,8 +198,11 @@ __host__ __device__ inline int xf_spitch(int nkx) { return nkx | 1; }
 
 // shared memory: tile [H][8] | twiddles w_L^k [H] | stage [NST][spitch] | mbarrier.  The stage receives the
 // NEXT line's NST spectra rows by TMA bulk copies while the current line is transformed.
+#ifndef XF_MINB
+#define XF_MINB 2
+#endif
 template <int L, bool PHASE>
-__global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused(const __grid_constant__ XFArgs a,
+__global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_xfused(const __grid_constant__ XFArgs a,
                                                                                const cplx *__restrict__ twx) {
     constexpr int H = L / 2;
     constexpr int R1 = XPlan<H>::R1, R2 = XPlan<H>::R2;
@@ -219,42 +237,48 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
     __syncthreads();
     TwPow<R1> tp;                           // w_H^j: twiddle base of this thread's R1-pass butterfly
     tp.init(tw_half<H>(tw, item ? j : 0));
+    // w_L^k for k = j + S1 m is w_L^j times the compile-time constant w_{2 R1}^m: no table look-up per element
+    cplx wj = tw[item ? j : 0];
     unsigned parity = 0;
     // field -> staged row: u v w phi phx phy phz  <-  0 1 2 3 3 4 5 (phx = i kx phi)
     const cplx *sf = stage + (size_t)(f < 4 ? (f < NST ? f : 0) : (f < NIN ? f - 1 : 0)) * spitch;
-    const double dkx = (PHASE && f == 4) ? a.kxf : 0.0;
+    // i kx of the phx slot: kx(k) = kxf (j + S1 m) = dk0 + m dks, kx(H - k) = dkh - kx(k)
+    const bool isdx = PHASE && f == 4;
+    double dk0 = isdx ? a.kxf * (double)j : 0.0, dks = isdx ? a.kxf * (double)S1 : 0.0, dkh = isdx ? a.kxf * (double)H : 0.0;
     for (int line = blockIdx.x; line < a.nlines; line += gridDim.x) {
         const size_t base = (size_t)line * kxp;
         mbar_wait(bar, parity);
         parity ^= 1;
+        // the twiddle bases are loop invariant; keep the compiler from hoisting the 2 x (R1 - 1) derived powers
+        // out of the line loop (they would be spilled to local memory and re-read for every line)
+        asm volatile("" : "+d"(tp.w1.x), "+d"(tp.w1.y), "+d"(tp.w2.x), "+d"(tp.w2.y), "+d"(tp.w4.x), "+d"(tp.w4.y),
+                     "+d"(tp.w8.x), "+d"(tp.w8.y), "+d"(wj.x), "+d"(wj.y), "+d"(dk0), "+d"(dks), "+d"(dkh));
         // ---- A: pre-twiddle from the staged rows + DIF pass R1 (inverse transform, sign +) ----
         if (item) {
             cplx v[R1];
 #pragma unroll
             for (int m = 0; m < R1; ++m) {
+                if (m && (m & 3) == 0) asm volatile("" ::: "memory");   // at most 4 elements' staged loads in flight
                 const int k = j + S1 * m, kb = H - k;
                 cplx xa = make_double2(0.0, 0.0), xb = xa;
                 if (f < NIN) {
                     if (k < nkx) xa = sf[k];
                     if (kb < nkx) xb = sf[kb];
                 }
-                if (PHASE && f == 4) {                    // i kx X
-                    const double ka = dkx * (double)k, kc = dkx * (double)kb;
+                if (isdx) {                               // i kx X
+                    const double ka = fma((double)m, dks, dk0), kc = dkh - ka;
                     xa = make_double2(-ka * xa.y, ka * xa.x);
                     xb = make_double2(-kc * xb.y, kc * xb.x);
                 }
                 if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
-                const cplx w = tw[k];
+                const cplx w = m ? cmul(wj, make_double2(wc_re<2 * R1>(m), wc_im<2 * R1>(m))) : wj;
                 const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
                 // Z = S + i conj(w) D
                 v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
             }
             RegFFT<R1, +1>::run(v);
-            cplx wq[R1];
-            tp.powers(wq);
             s[xidx(j, f)] = v[0];
-#pragma unroll
-            for (int q = 1; q < R1; ++q) s[xidx(j + S1 * q, f)] = cmultw<+1>(v[q], wq[q]);
+            tp.each([&](int q, cplx wq) { s[xidx(j + S1 * q, f)] = cmultw<+1>(v[q], wq); });
         }
         __syncthreads();
         if (tid == 0 && line + (int)gridDim.x < a.nlines) {   // stage is free: prefetch the next line
@@ -268,30 +292,21 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
         }
         // ---- C: last DIF radix 2, pointwise products, first DIT radix 2: rows (2t, 2t+1) x all fields ----
         for (int t = tid; t < H / 2; t += NT) {
-            cplx z0[8], z1[8];
+            double p00[8], p01[8], p10[8], p11[8];   // the four grid points of this row pair, all input fields
 #pragma unroll
             for (int q = 0; q < NIN; ++q) {
                 const cplx p = s[xidx(2 * t, q)], m = s[xidx(2 * t + 1, q)];
-                z0[q] = cadd(p, m);
-                z1[q] = csub(p, m);
+                p00[q] = p.x + m.x; p01[q] = p.y + m.y;
+                p10[q] = p.x - m.x; p11[q] = p.y - m.y;
             }
-            double in[8], o00[8], o01[8], o10[8], o11[8];
-#pragma unroll
-            for (int q = 0; q < NIN; ++q) in[q] = z0[q].x;
-            nl_point<PHASE>(in, o00, a.cs);
-#pragma unroll
-            for (int q = 0; q < NIN; ++q) in[q] = z0[q].y;
-            nl_point<PHASE>(in, o01, a.cs);
-#pragma unroll
-            for (int q = 0; q < NIN; ++q) in[q] = z1[q].x;
-            nl_point<PHASE>(in, o10, a.cs);
-#pragma unroll
-            for (int q = 0; q < NIN; ++q) in[q] = z1[q].y;
-            nl_point<PHASE>(in, o11, a.cs);
-#pragma unroll
-            for (int q = 0; q < NOUT; ++q) {
-                s[xidx(2 * t, q)] = make_double2(o00[q] + o10[q], o01[q] + o11[q]);
-                s[xidx(2 * t + 1, q)] = make_double2(o00[q] - o10[q], o01[q] - o11[q]);
+            nl_store<0, PHASE>(s, t, p00, p01, p10, p11, a.cs);
+            nl_store<1, PHASE>(s, t, p00, p01, p10, p11, a.cs);
+            nl_store<2, PHASE>(s, t, p00, p01, p10, p11, a.cs);
+            nl_store<3, PHASE>(s, t, p00, p01, p10, p11, a.cs);
+            nl_store<4, PHASE>(s, t, p00, p01, p10, p11, a.cs);
+            if (PHASE) {
+                nl_store<5, PHASE>(s, t, p00, p01, p10, p11, a.cs);
+                nl_store<6, PHASE>(s, t, p00, p01, p10, p11, a.cs);
             }
         }
         __syncthreads();
@@ -302,12 +317,12 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
         }
         // ---- E: DIT pass R1, results stay in registers and are published to the tile ----
         cplx v[R1];
+        // (same powers as stage A: recompute instead of carrying 15 complex values across stages B-D)
+        asm volatile("" : "+d"(tp.w1.x), "+d"(tp.w1.y), "+d"(tp.w2.x), "+d"(tp.w2.y), "+d"(tp.w4.x), "+d"(tp.w4.y),
+                     "+d"(tp.w8.x), "+d"(tp.w8.y), "+d"(wj.x), "+d"(wj.y));
         if (item) {
-            cplx wq[R1];
-            tp.powers(wq);
             v[0] = s[xidx(j, f)];
-#pragma unroll
-            for (int m = 1; m < R1; ++m) v[m] = cmultw<-1>(s[xidx(j + S1 * m, f)], wq[m]);
+            tp.each([&](int m, cplx wq) { v[m] = cmultw<-1>(s[xidx(j + S1 * m, f)], wq); });
             RegFFT<R1, -1>::run(v);
 #pragma unroll
             for (int q = 0; q < R1; ++q) s[xidx(j + S1 * q, f)] = v[q];
@@ -321,7 +336,7 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? 2 : 3)) k_xfused
                 if (k < nkx) {
                     const cplx za = v[q];
                     const cplx zb = s[xidx((H - k) & (H - 1), f)];
-                    const cplx w = tw[k];
+                    const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
                     const double Sx = za.x + zb.x, Sy = za.y - zb.y, Dx = za.x - zb.x, Dy = za.y + zb.y;
                     // X_k = (S - i w D) / (2 L)
                     outf[base + k] = make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy)));
