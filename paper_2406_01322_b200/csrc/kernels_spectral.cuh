@@ -373,7 +373,10 @@ struct RhsElimArgs {
 
 constexpr int RHS_COLS = 32;   // columns per CTA of k_rhs_elim (blockDim = 32 * number of chains)
 
-__global__ void __launch_bounds__(96, 5) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
+#ifndef RHS_MINB
+#define RHS_MINB 3
+#endif
+__global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * RHS_COLS + (threadIdx.x & 31);
     if (col >= g.ncols) return;
@@ -390,13 +393,29 @@ __global__ void __launch_bounds__(96, 5) k_rhs_elim(const __grid_constant__ RhsE
     const cplx *__restrict__ tyy = a.tyy + col, *__restrict__ tyz = a.tyz + col;
     ElimDown el;
     el.init();
-    if (chain == 0) {
+    // Software pipelining: the operands of row n - 1 are loaded into registers before row n is computed, so
+    // each row costs one (prefetched, L2-hit) load latency instead of one per dependent load group
+    // (profiles/r1c: 77 % of the stall samples were long-scoreboard waits).
+    struct RowIn { cplx x, h, t0, t1, t2, t3, t4; double di; };
+    if (chain == 0 || chain == 1) {
         const double sigma = k2 + 1.0 / gam, fs = -1.0 / gam;
         const double *__restrict__ dinv = a.dinv_ns + col;
-        cplx *x = a.om + col, *hist = a.h_om + col;
-        Chain1 cR; Chain2 cOm;
-        cR.init(); cOm.init();
+        cplx *x = (chain == 0 ? a.om : a.th) + col, *hist = (chain == 0 ? a.h_om : a.h_w) + col;
+        auto load = [&](int n) {
+            RowIn r;
+            const size_t o = n * st;
+            r.x = x[o];
+            r.di = (n <= N - 2) ? dinv[(n + 2) * st] : 0.0;
+            r.h = r.t0 = r.t1 = r.t2 = r.t3 = r.t4 = cz();
+            if (n < nkz) { r.h = hist[o]; r.t0 = txx[o]; r.t1 = txy[o]; r.t2 = txz[o]; r.t3 = tyy[o]; r.t4 = tyz[o]; }
+            return r;
+        };
+        Chain1 c1; Chain2 c2a, c2x;
+        c1.init(); c2a.init(); c2x.init();
+        RowIn nx = load(N);
         for (int n = N; n >= 0; --n) {
+            const RowIn r = nx;
+            if (n > 0) nx = load(n - 1);
             const int np = n - PF_ROWS;
             if (np >= 0) {
                 pf_l2(x + np * st); pf_l2(dinv + (np + 2) * st);
@@ -405,71 +424,44 @@ __global__ void __launch_bounds__(96, 5) k_rhs_elim(const __grid_constant__ RhsE
             const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
             const size_t o = n * st;
             const bool low = n < nkz;
-            const cplx omn = x[o];
-            cplx P = cz(), R = cz();
-            if (low) {
-                const cplx vxz = txz[o];
-                if (mean) {
-                    R = vxz;
-                } else {
-                    const cplx vxx = txx[o], vxy = txy[o], vyy = tyy[o], vyz = tyz[o];
-                    P = cadd(cscale(vxy, ky * ky - kx * kx), cscale(csub(vxx, vyy), kx * ky));
-                    R = ci(csub(cscale(vyz, kx), cscale(vxz, ky)));
+            cplx nlin;
+            cplx ddX;
+            if (chain == 0) {
+                // N_omega = P + D R (Eq. 14 expanded); column 0: S-bar_x = D T_xz (+ G)
+                cplx P = cz(), R = cz();
+                if (low) {
+                    if (mean) R = r.t2;
+                    else {
+                        P = cadd(cscale(r.t1, ky * ky - kx * kx), cscale(csub(r.t0, r.t3), kx * ky));
+                        R = ci(csub(cscale(r.t4, kx), cscale(r.t2, ky)));
+                    }
                 }
+                const cplx dR = c1.step(R, f, h);
+                ddX = c2x.step(r.x, f, h);
+                nlin = cadd(P, dR);
+                if (mean && n == 0) nlin.x += a.gradp;
+            } else {
+                // N_w = D B - D^2 A - k^2 A (Eq. 15 expanded); column 0: S-bar_y = D T_yz
+                cplx A = cz(), B = cz();
+                if (low) {
+                    if (mean) B = r.t4;
+                    else {
+                        A = ci(cadd(cscale(r.t2, kx), cscale(r.t4, ky)));
+                        // kx^2 Txx + 2 kx ky Txy + ky^2 Tyy - k^2 Tzz with the deviatoric inputs
+                        B = cadd(cadd(cscale(r.t0, kx * kx), cscale(r.t1, 2.0 * kx * ky)), cscale(r.t3, ky * ky));
+                    }
+                }
+                const cplx dB = c1.step(B, f, h);
+                const cplx ddA = c2a.step(A, f, h);
+                ddX = c2x.step(r.x, f, h);
+                nlin = cadd(csub(dB, ddA), cscale(A, -k2));
             }
-            const cplx dR = cR.step(R, f, h);
-            const cplx ddOm = cOm.step(omn, f, h);
-            cplx n_om = cadd(P, dR);
-            if (mean && n == 0) n_om.x += a.gradp;
-            cplx nl = cscale(n_om, ab0);
-            if (low) { nl = cfma(ab1, hist[o], nl); hist[o] = n_om; }
-            const cplx H = cfma(dt, nl, cfma(gam, cfma(-k2, omn, ddOm), omn));
+            cplx nl = cscale(nlin, ab0);
+            if (low) { nl = cfma(ab1, r.h, nl); hist[o] = nlin; }
+            const cplx H = cfma(dt, nl, cfma(gam, cfma(-k2, r.x, ddX), r.x));
             if (n <= N - 2) {
                 const int k = n + 2;
-                x[k * st] = el.row<false, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
-            }
-        }
-        cplx u0, u1;
-        el.finish<false>(sigma, 0.0, 0.0, u0, u1);
-        x[0] = u0; x[st] = u1;
-    } else if (chain == 1) {
-        const double sigma = k2 + 1.0 / gam, fs = -1.0 / gam;
-        const double *__restrict__ dinv = a.dinv_ns + col;
-        cplx *x = a.th + col, *hist = a.h_w + col;
-        Chain1 cB; Chain2 cA, cTh;
-        cB.init(); cA.init(); cTh.init();
-        for (int n = N; n >= 0; --n) {
-            const int np = n - PF_ROWS;
-            if (np >= 0) {
-                pf_l2(x + np * st); pf_l2(dinv + (np + 2) * st);
-                if (np < nkz) { pf_l2(tyz + np * st); pf_l2(txx + np * st); pf_l2(txy + np * st); pf_l2(txz + np * st); pf_l2(tyy + np * st); pf_l2(hist + np * st); }
-            }
-            const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
-            const size_t o = n * st;
-            const bool low = n < nkz;
-            const cplx thn = x[o];
-            cplx A = cz(), B = cz();
-            if (low) {
-                const cplx vyz = tyz[o];
-                if (mean) {
-                    B = vyz;
-                } else {
-                    const cplx vxx = txx[o], vxy = txy[o], vxz = txz[o], vyy = tyy[o];
-                    A = ci(cadd(cscale(vxz, kx), cscale(vyz, ky)));
-                    // kx^2 Txx + 2 kx ky Txy + ky^2 Tyy - k^2 Tzz with the deviatoric inputs
-                    B = cadd(cadd(cscale(vxx, kx * kx), cscale(vxy, 2.0 * kx * ky)), cscale(vyy, ky * ky));
-                }
-            }
-            const cplx dB = cB.step(B, f, h);
-            const cplx ddA = cA.step(A, f, h);
-            const cplx ddTh = cTh.step(thn, f, h);
-            const cplx n_w = cadd(csub(dB, ddA), cscale(A, -k2));
-            cplx nl = cscale(n_w, ab0);
-            if (low) { nl = cfma(ab1, hist[o], nl); hist[o] = n_w; }
-            const cplx H = cfma(dt, nl, cfma(gam, cfma(-k2, thn, ddTh), thn));
-            if (n <= N - 2) {
-                const int k = n + 2;
-                x[k * st] = el.row<false, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
+                x[k * st] = el.row<false, false>(k, N, sigma, cscale(H, fs), r.di);
             }
         }
         cplx u0, u1;
@@ -480,9 +472,21 @@ __global__ void __launch_bounds__(96, 5) k_rhs_elim(const __grid_constant__ RhsE
         const double *__restrict__ dinv = a.dinv_ch + col;
         const cplx *__restrict__ qq = a.q + col, *__restrict__ cc = a.c + col;
         cplx *x = a.phi + col, *hist = a.h_phi + col;
+        auto load = [&](int n) {
+            RowIn r;
+            const size_t o = n * st;
+            r.x = x[o];
+            r.di = (n <= N - 2) ? dinv[(n + 2) * st] : 0.0;
+            r.h = r.t0 = r.t1 = cz();
+            if (n < nkz) { r.h = hist[o]; r.t0 = qq[o]; r.t1 = cc[o]; }
+            return r;
+        };
         Chain2 cE;
         cE.init();
+        RowIn nx = load(N);
         for (int n = N; n >= 0; --n) {
+            const RowIn r = nx;
+            if (n > 0) nx = load(n - 1);
             const int np = n - PF_ROWS;
             if (np >= 0) {
                 pf_l2(x + np * st); pf_l2(dinv + (np + 2) * st);
@@ -491,20 +495,19 @@ __global__ void __launch_bounds__(96, 5) k_rhs_elim(const __grid_constant__ RhsE
             const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
             const size_t o = n * st;
             const bool low = n < nkz;
-            const cplx phn = x[o];
             cplx E = cz(), Q = cz();
             if (low) {
-                Q = qq[o];
-                E = cscale(cfma(-a.e_phi, phn, cc[o]), a.inv_pe);
+                Q = r.t0;
+                E = cscale(cfma(-a.e_phi, r.x, r.t1), a.inv_pe);
             }
             const cplx ddE = cE.step(E, f, h);
             const cplx s_phi = csub(cfma(-k2, E, ddE), Q);
             cplx nl = cscale(s_phi, ab0);
-            if (low) { nl = cfma(ab1, hist[o], nl); hist[o] = s_phi; }
-            const cplx H = cfma(dt, nl, phn);
+            if (low) { nl = cfma(ab1, r.h, nl); hist[o] = s_phi; }
+            const cplx H = cfma(dt, nl, r.x);
             if (n <= N - 2) {
                 const int k = n + 2;
-                x[k * st] = el.row<true, false>(k, N, sigma, cscale(H, fs), dinv[k * st]);
+                x[k * st] = el.row<true, false>(k, N, sigma, cscale(H, fs), r.di);
             }
         }
         cplx u0, u1;
