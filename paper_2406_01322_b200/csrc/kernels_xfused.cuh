@@ -196,11 +196,17 @@ struct XFArgs {
 // stage pitch (cplx): odd, so that the 8 fields of one k sit in 8 different 16-byte bank groups
 __host__ __device__ inline int xf_spitch(int nkx) { return nkx | 1; }
 
-// shared memory: tile [H][8] | twiddles w_L^k [H] | stage [NST][spitch] | mbarrier.  The stage receives the
-// NEXT line's NST spectra rows by TMA bulk copies while the current line is transformed.
+// shared memory: tile [H][8] | stage [NST][spitch] | mbarrier.  The stage receives the NEXT line's spectra rows
+// by TMA bulk copies while the current line is transformed; with the phase field its last row is derived in
+// place: i kx phi^ (row a1), so that the x derivative of phi costs no FP64 work in the butterfly warps.
+// Register budget (128 at 2 CTAs/SM): only the thread's base twiddle w_L^j is carried across the line loop;
+// its powers are re-derived per stage and nothing is held in registers across a barrier (profiles/r1d: the
+// previous form spilled 456 B/thread, 8 GB of extra DRAM writes per step and 15 % of the time in LDL waits).
 #ifndef XF_MINB
 #define XF_MINB 2
 #endif
+template <bool PHASE> __host__ __device__ constexpr int xf_nstage() { return PHASE ? 7 : 3; }
+
 template <int L, bool PHASE>
 __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_xfused(const __grid_constant__ XFArgs a,
                                                                                const cplx *__restrict__ twx) {
@@ -209,50 +215,52 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
     constexpr int NT = xf_threads<L>();
     constexpr int S1 = H / R1;              // stride of pass R1 = number of its butterflies per field
     constexpr int NIN = PHASE ? 7 : 3, NOUT = PHASE ? 7 : 5;   // fields through the backward / forward FFT
-    constexpr int NST = PHASE ? 6 : 3;                         // staged spectra rows: u v w [phi phy phz]
+    constexpr int NTMA = PHASE ? 6 : 3;                        // rows staged by TMA: u v w [phi phy phz]
+    constexpr int NST = xf_nstage<PHASE>();                    // + derived row i kx phi
     static_assert(R1 * R2 * 2 == H, "plan");
     static_assert(S1 * TILE_LINES <= NT, "one (butterfly, field) item per thread in stages A and E");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
-    cplx *tw = s + H * TILE_LINES;
-    cplx *stage = tw + H;
+    cplx *stage = s + H * TILE_LINES;
     const int kxp = a.kxp, nkx = a.nkx;
     const int spitch = xf_spitch(nkx);
     unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)NST * spitch);
     const int tid = threadIdx.x, f = tid & 7, j = tid >> 3;
     const bool item = j < S1;               // this thread owns butterfly j of field f in stages A, E, F
-    for (int i = tid; i < H; i += NT) tw[i] = twx[i];
     cplx *outf = a.out[f < NOUT ? f : 0];
     const double sc = 0.5 / L;
     const unsigned row_bytes = (unsigned)(nkx * sizeof(cplx));
-    auto issue = [&](int line) {   // one thread: arm the barrier and launch NIN bulk copies
-        mbar_expect_tx(bar, row_bytes * NST);
+    auto issue = [&](int line) {   // one thread: arm the barrier and launch the bulk copies
+        mbar_expect_tx(bar, row_bytes * NTMA);
 #pragma unroll
-        for (int q = 0; q < NST; ++q) bulk_g2s(stage + (size_t)q * spitch, a.in[q] + (size_t)line * kxp, row_bytes, bar);
+        for (int q = 0; q < NTMA; ++q) bulk_g2s(stage + (size_t)q * spitch, a.in[q] + (size_t)line * kxp, row_bytes, bar);
     };
     if (tid == 0) {
         mbar_init(bar, 1);
         if ((int)blockIdx.x < a.nlines) issue(blockIdx.x);
     }
     __syncthreads();
-    TwPow<R1> tp;                           // w_H^j: twiddle base of this thread's R1-pass butterfly
-    tp.init(tw_half<H>(tw, item ? j : 0));
-    // w_L^k for k = j + S1 m is w_L^j times the compile-time constant w_{2 R1}^m: no table look-up per element
-    cplx wj = tw[item ? j : 0];
+    // w_L^k for k = j + S1 m is w_L^j times the compile-time constant w_{2 R1}^m; the pass twiddles are powers
+    // of w_H^j = (w_L^j)^2: no table look-up per element
+    cplx wj = twx[item ? j : 0];
     unsigned parity = 0;
-    // field -> staged row: u v w phi phx phy phz  <-  0 1 2 3 3 4 5 (phx = i kx phi)
-    const cplx *sf = stage + (size_t)(f < 4 ? (f < NST ? f : 0) : (f < NIN ? f - 1 : 0)) * spitch;
-    // i kx of the phx slot: kx(k) = kxf (j + S1 m) = dk0 + m dks, kx(H - k) = dkh - kx(k)
-    const bool isdx = PHASE && f == 4;
-    double dk0 = isdx ? a.kxf * (double)j : 0.0, dks = isdx ? a.kxf * (double)S1 : 0.0, dkh = isdx ? a.kxf * (double)H : 0.0;
+    // field -> staged row: u v w phi phx phy phz  <-  0 1 2 3 6 4 5
+    const int srow = !PHASE ? (f < NST ? f : 0) : (f < 4 ? f : (f == 4 ? 6 : (f < NIN ? f - 1 : 0)));
+    const cplx *sf = stage + (size_t)srow * spitch;
     for (int line = blockIdx.x; line < a.nlines; line += gridDim.x) {
         const size_t base = (size_t)line * kxp;
         mbar_wait(bar, parity);
         parity ^= 1;
-        // the twiddle bases are loop invariant; keep the compiler from hoisting the 2 x (R1 - 1) derived powers
-        // out of the line loop (they would be spilled to local memory and re-read for every line)
-        asm volatile("" : "+d"(tp.w1.x), "+d"(tp.w1.y), "+d"(tp.w2.x), "+d"(tp.w2.y), "+d"(tp.w4.x), "+d"(tp.w4.y),
-                     "+d"(tp.w8.x), "+d"(tp.w8.y), "+d"(wj.x), "+d"(wj.y), "+d"(dk0), "+d"(dks), "+d"(dkh));
+        if constexpr (PHASE) {              // row a1: phx^ = i kx phi^
+            for (int k = tid; k < nkx; k += NT) {
+                const cplx p = stage[3 * spitch + k];
+                const double kk = a.kxf * (double)k;
+                stage[6 * spitch + k] = make_double2(-kk * p.y, kk * p.x);
+            }
+            __syncthreads();
+        }
+        // keep the compiler from hoisting per-line derived twiddles out of the line loop (they would be spilled)
+        asm volatile("" : "+d"(wj.x), "+d"(wj.y));
         // ---- A: pre-twiddle from the staged rows + DIF pass R1 (inverse transform, sign +) ----
         if (item) {
             cplx v[R1];
@@ -265,11 +273,6 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
                     if (k < nkx) xa = sf[k];
                     if (kb < nkx) xb = sf[kb];
                 }
-                if (isdx) {                               // i kx X
-                    const double ka = fma((double)m, dks, dk0), kc = dkh - ka;
-                    xa = make_double2(-ka * xa.y, ka * xa.x);
-                    xb = make_double2(-kc * xb.y, kc * xb.x);
-                }
                 if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
                 const cplx w = m ? cmul(wj, make_double2(wc_re<2 * R1>(m), wc_im<2 * R1>(m))) : wj;
                 const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
@@ -277,6 +280,8 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
                 v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
             }
             RegFFT<R1, +1>::run(v);
+            TwPow<R1> tp;
+            tp.init(cmul(wj, wj));
             s[xidx(j, f)] = v[0];
             tp.each([&](int q, cplx wq) { s[xidx(j + S1 * q, f)] = cmultw<+1>(v[q], wq); });
         }
@@ -315,12 +320,12 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
             xpass_mid<H, R2, -1, NT, true>(s, tid);
             __syncthreads();
         }
-        // ---- E: DIT pass R1, results stay in registers and are published to the tile ----
-        cplx v[R1];
-        // (same powers as stage A: recompute instead of carrying 15 complex values across stages B-D)
-        asm volatile("" : "+d"(tp.w1.x), "+d"(tp.w1.y), "+d"(tp.w2.x), "+d"(tp.w2.y), "+d"(tp.w4.x), "+d"(tp.w4.y),
-                     "+d"(tp.w8.x), "+d"(tp.w8.y), "+d"(wj.x), "+d"(wj.y));
+        // ---- E: DIT pass R1, in place on the tile ----
+        asm volatile("" : "+d"(wj.x), "+d"(wj.y));
         if (item) {
+            cplx v[R1];
+            TwPow<R1> tp;
+            tp.init(cmul(wj, wj));
             v[0] = s[xidx(j, f)];
             tp.each([&](int m, cplx wq) { v[m] = cmultw<-1>(s[xidx(j + S1 * m, f)], wq); });
             RegFFT<R1, -1>::run(v);
@@ -328,13 +333,13 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
             for (int q = 0; q < R1; ++q) s[xidx(j + S1 * q, f)] = v[q];
         }
         __syncthreads();
-        // ---- F: post-twiddle against the partner row H - k, truncated store ----
+        // ---- F: post-twiddle of row k against the partner row H - k, truncated store ----
         if (item && f < NOUT) {
 #pragma unroll
             for (int q = 0; q < R1; ++q) {
                 const int k = j + S1 * q;
                 if (k < nkx) {
-                    const cplx za = v[q];
+                    const cplx za = s[xidx(k, f)];
                     const cplx zb = s[xidx((H - k) & (H - 1), f)];
                     const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
                     const double Sx = za.x + zb.x, Sy = za.y - zb.y, Dx = za.x - zb.x, Dy = za.y + zb.y;

@@ -198,9 +198,9 @@ ColGeom geom(const psdns_handle *h) {
 template <int L>
 size_t fft_smem() { return (size_t)(L * TILE_LINES + L) * sizeof(cplx); }
 
-// tile + twiddles + stage [nin][spitch] + mbarrier
+// tile + stage [nst][spitch] + mbarrier
 template <int L>
-size_t xfused_smem(int nkx, int nin) { return (size_t)((L / 2) * TILE_LINES + L / 2 + nin * xf_spitch(nkx)) * sizeof(cplx) + 16; }
+size_t xfused_smem(int nkx, int nst) { return (size_t)((L / 2) * TILE_LINES + nst * xf_spitch(nkx)) * sizeof(cplx) + 16; }
 
 template <class K>
 cudaError_t set_smem(K kern, size_t bytes) {
@@ -314,7 +314,7 @@ cudaError_t setup_attrs(psdns_handle *h) {
     DISPATCH_L(h->d.nx, XA)
 #define XFA(LL)                                                                                              \
     {                                                                                                        \
-        const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 6 : 3);                               \
+        const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                               \
         int occ = 0;                                                                                         \
         if (h->p.phase_field) {                                                                              \
             CU0(set_smem(k_xfused<LL, true>, sm));                                                           \
@@ -340,7 +340,7 @@ cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
     LaunchScope ls(h, KC_XFUSED);
 #define XF(LL)                                                                                               \
     {                                                                                                        \
-        const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 6 : 3);                               \
+        const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                               \
         if (h->p.phase_field) k_xfused<LL, true><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);              \
         else k_xfused<LL, false><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);                              \
     }
