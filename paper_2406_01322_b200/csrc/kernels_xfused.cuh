@@ -50,6 +50,15 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// An opaque copy of a loop-invariant index: address arithmetic derived from it is redone where it is used
+// instead of being hoisted out of the line loop and spilled (profiles/r1d: 30 hoisted shared-memory addresses
+// were spilled and re-read from local memory for every line).
+__device__ __forceinline__ int opaque(int v) { asm volatile("" : "+r"(v)); return v; }
+// global store that the compiler may move shared-memory loads across (a store through a generic pointer may not)
+__device__ __forceinline__ void stg(cplx *p, cplx v) {
+    asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(__cvta_generic_to_global(p)), "d"(v.x), "d"(v.y));
+}
+
 // ---- plan of the half-length FFT: H = R1 * R2 * 2 ---------------------------------------------------
 template <int H> struct XPlan;
 template <> struct XPlan<8>   { static constexpr int R1 = 4,  R2 = 1; };
@@ -100,6 +109,7 @@ __device__ __forceinline__ constexpr double wc_im(int q) {   // -sin(2 pi q / LS
 // loaded from shared memory (a broadcast LDS.128 costs as many wavefronts as a data access).
 template <int H, int R, int SIGN, int NT, bool DIT>
 __device__ __forceinline__ void xpass_mid(cplx *__restrict__ s, int tid) {
+    tid = opaque(tid);
     constexpr int LS = 2 * R;
     constexpr int NBLK = H / LS;           // blocks per field; items per field = 2 * NBLK
     static_assert(NBLK % 4 == 0, "j must be uniform over a warp (4 butterflies x 8 fields)");
@@ -263,6 +273,7 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
         asm volatile("" : "+d"(wj.x), "+d"(wj.y));
         // ---- A: pre-twiddle from the staged rows + DIF pass R1 (inverse transform, sign +) ----
         if (item) {
+            const int j = opaque(tid) >> 3;
             cplx v[R1];
 #pragma unroll
             for (int m = 0; m < R1; ++m) {
@@ -296,7 +307,7 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
             __syncthreads();
         }
         // ---- C: last DIF radix 2, pointwise products, first DIT radix 2: rows (2t, 2t+1) x all fields ----
-        for (int t = tid; t < H / 2; t += NT) {
+        for (int t = opaque(tid); t < H / 2; t += NT) {
             double p00[8], p01[8], p10[8], p11[8];   // the four grid points of this row pair, all input fields
 #pragma unroll
             for (int q = 0; q < NIN; ++q) {
@@ -323,6 +334,7 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
         // ---- E: DIT pass R1, in place on the tile ----
         asm volatile("" : "+d"(wj.x), "+d"(wj.y));
         if (item) {
+            const int j = opaque(tid) >> 3;
             cplx v[R1];
             TwPow<R1> tp;
             tp.init(cmul(wj, wj));
@@ -335,18 +347,28 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
         __syncthreads();
         // ---- F: post-twiddle of row k against the partner row H - k, truncated store ----
         if (item && f < NOUT) {
+            const int j = opaque(tid) >> 3;
+            cplx *o = outf + base;
 #pragma unroll
-            for (int q = 0; q < R1; ++q) {
-                const int k = j + S1 * q;
-                if (k < nkx) {
-                    const cplx za = s[xidx(k, f)];
-                    const cplx zb = s[xidx((H - k) & (H - 1), f)];
-                    const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
-                    const double Sx = za.x + zb.x, Sy = za.y - zb.y, Dx = za.x - zb.x, Dy = za.y + zb.y;
-                    // X_k = (S - i w D) / (2 L)
-                    outf[base + k] = make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy)));
-                } else if (k < kxp) {
-                    outf[base + k] = make_double2(0.0, 0.0);
+            for (int q0 = 0; q0 < R1; q0 += 4) {          // four rows' loads in flight, then their stores
+                cplx za[4], zb[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int k = j + S1 * (q0 + i);
+                    za[i] = s[xidx(k, f)];                 // every row k < H exists: no predicate on the loads
+                    zb[i] = s[xidx((H - k) & (H - 1), f)];
+                }
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int q = q0 + i, k = j + S1 * q;
+                    if (k < nkx) {
+                        const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
+                        const double Sx = za[i].x + zb[i].x, Sy = za[i].y - zb[i].y, Dx = za[i].x - zb[i].x, Dy = za[i].y + zb[i].y;
+                        // X_k = (S - i w D) / (2 L)
+                        stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
+                    } else if (k < kxp) {
+                        stg(o + k, make_double2(0.0, 0.0));
+                    }
                 }
             }
         }
