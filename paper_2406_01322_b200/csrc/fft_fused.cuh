@@ -87,6 +87,17 @@ __device__ __forceinline__ void fft_rest_inplace(cplx *__restrict__ s, const cpl
     }
 }
 
+// Same without the leading barrier (the caller has already synchronised after the head pass).
+template <int L, int SIGN, int NT>
+__device__ __forceinline__ void fft_rest_inplace_nb(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid) {
+    constexpr int R1 = PlanF<L>::R1, R2 = PlanF<L>::R2, R3 = PlanF<L>::R3;
+    if constexpr (R2 > 1) fft_pass<L, L / R1, R2, SIGN, NT>(s, tw, tid);
+    if constexpr (R3 > 1) {
+        __syncthreads();
+        fft_pass<L, L / (R1 * R2), R3, SIGN, NT>(s, tw, tid);
+    }
+}
+
 // Remaining passes with the last one drained into Store = void operator()(int k, cplx v), k natural.
 template <int L, int SIGN, int NT, class Store>
 __device__ __forceinline__ void fft_rest_store(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid, Store store) {

@@ -24,6 +24,13 @@ struct FieldPtrs {
     void *out[MAXF];
 };
 
+// Ampere-style asynchronous copy (LDGSTS): 16 bytes global -> shared without passing through registers
+__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 template <int L>
 __device__ __forceinline__ void load_twiddles(cplx *tw, const cplx *__restrict__ twg, int tid, int nt) {
     for (int i = tid; i < L; i += nt) tw[i] = twg[i];
@@ -44,8 +51,10 @@ __device__ __forceinline__ void load_twiddles(cplx *tw, const cplx *__restrict__
 //   G_0 = Z_0 - i H_0, E_0 = G_0 + H_0, E_N = G_0 - H_0.
 // Rounding error is amplified by |c_k| <= ~N/(2 pi k) in the lowest/highest modes (<= 1e-14 relative at
 // N = 512; tolerance 1e-11).
-// Persistent CTAs loop over tiles of 8 consecutive columns; the first FFT pass is fed from global memory
-// through registers (fft_fused.cuh).  Optional derived outputs i kx X and i ky X of one field (row a1:
+// Persistent CTAs loop over tiles of 8 consecutive columns; the first FFT pass is fed through registers
+// (fft_fused.cuh): the even rows straight from global memory, the odd rows from a shared-memory stage that
+// cp.async fills one tile ahead (a thread cannot keep all 32 of its 16-byte loads in flight in 128 registers;
+// profiles/r1d: 35 % of the samples were long-scoreboard waits in the head pass).  Optional derived outputs i kx X and i ky X of one field (row a1:
 // the x / y derivatives of phi commute with the z transform, so they cost no transform of their own).
 // ------------------------------------------------------------------------------------------
 struct ZArgs {
@@ -60,43 +69,59 @@ struct ZArgs {
     double kxf, kyf;
 };
 
-template <int N> __host__ __device__ constexpr int zpass_smem_cplx() {
-    return N * TILE_LINES + N + (fused_threads<N>() / 32) * 8;
+template <int N, bool FWD> __host__ __device__ constexpr int zpass_smem_cplx() {
+    return N * TILE_LINES + N + (fused_threads<N>() / 32) * 8 + (N / 2 + 1) + (FWD ? 0 : (N / 2) * TILE_LINES);
 }
 
 template <int N, bool FWD>
 __global__ void __launch_bounds__(fused_threads<N>(), (N >= 512 ? 2 : 3)) k_zpass(const __grid_constant__ ZArgs a,
                                                                                const cplx *__restrict__ tw2n,
-                                                                               const cplx *__restrict__ ctab) {
+                                                                               const cplx *__restrict__ ctab_g) {
     constexpr int NT = fused_threads<N>();
     constexpr int NW = NT / 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
     cplx *tw = s + N * TILE_LINES;
     cplx *red = tw + N;                       // [NW][8] partial sums of H_0
+    cplx *ctab = red + NW * 8;                // c_k, k <= N/2
+    cplx *stg = ctab + (N / 2 + 1);           // [N/2][8]: odd input rows 1, 3, .., N-1 of the next tile
     const int tid = threadIdx.x, line = tid & 7, r0 = tid >> 3;
     constexpr int RSTEP = NT / TILE_LINES;
     const size_t stride = (size_t)a.ncols;
     for (int i = tid; i < N; i += NT) tw[i] = tw2n[2 * i];
-    __syncthreads();
+    for (int i = tid; i <= N / 2; i += NT) ctab[i] = ctab_g[i];
     const int nin = FWD ? N + 1 : a.nk;       // input rows that are not structurally zero
     const int nout = FWD ? a.nk : N + 1;      // output rows kept
     const double sc = FWD ? 1.0 / N : 1.0;
     const int tiles_per_field = a.ncols / 8;
     const int ntiles = tiles_per_field * a.nf;
+    // measured (B200, N = 512): staging helps the backward pass (2/3 of the rows are structurally zero, so the
+    // remaining direct loads all fit in flight: 3.03 -> 2.74 ms) and hurts the forward pass (3.0 -> 3.5 ms)
+    constexpr bool STAGE = !FWD;
+    auto prefetch = [&](int t) {              // odd rows of tile t -> stage (each thread: its line of rows r0, r0 + RSTEP, ..)
+        if (STAGE && t < ntiles) {
+            const int fl = t / tiles_per_field;
+            const cplx *src = reinterpret_cast<const cplx *>(a.f.in[fl]) + (size_t)(t - fl * tiles_per_field) * 8 + line;
+            for (int r = r0; 2 * r + 1 < nin && r < N / 2; r += RSTEP) cp_async16(stg + r * TILE_LINES + line, src + (size_t)(2 * r + 1) * stride);
+        }
+        cp_async_commit();
+    };
+    prefetch(blockIdx.x);
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int fld = tile / tiles_per_field, ct = tile - fld * tiles_per_field;
         const size_t col = (size_t)ct * 8 + line;
         const cplx *__restrict__ in = reinterpret_cast<const cplx *>(a.f.in[fld]) + col;
         cplx *__restrict__ out = reinterpret_cast<cplx *>(a.f.out[fld]) + col;
+        cp_async_wait_all();
+        __syncthreads();                      // stage (and, first time, the tables) visible to all threads
         cplx h0 = make_double2(0.0, 0.0);
         // z_m = e_{2m} + i e_{2m+1}; for m >= N/2 the even extension folds back: e_j = a_{2N-j}
         fft_head<N, -1, NT>(s, tw, tid, [&](int m) {
             const int ne = (m < N / 2) ? 2 * m : 2 * N - 2 * m;
             const int no = (m < N / 2) ? 2 * m + 1 : 2 * N - 2 * m - 1;
             cplx e0 = make_double2(0.0, 0.0), e1 = e0;
-            if (ne < nin) e0 = in[ne * stride];
-            if (no < nin) e1 = in[no * stride];
+            if (ne < nin) e0 = __ldcg(in + ne * stride);
+            if (no < nin) e1 = STAGE ? stg[(no >> 1) * TILE_LINES + line] : __ldcg(in + no * stride);
             if (!FWD) {                       // backward: interior coefficients enter with weight 1/2
                 if (ne > 0 && ne < N) e0 = cscale(e0, 0.5);
                 e1 = cscale(e1, 0.5);         // odd rows are always interior
@@ -108,7 +133,9 @@ __global__ void __launch_bounds__(fused_threads<N>(), (N >= 512 ? 2 : 3)) k_zpas
         h0.x += __shfl_xor_sync(0xffffffffu, h0.x, 8);  h0.y += __shfl_xor_sync(0xffffffffu, h0.y, 8);
         h0.x += __shfl_xor_sync(0xffffffffu, h0.x, 16); h0.y += __shfl_xor_sync(0xffffffffu, h0.y, 16);
         if ((tid & 31) < 8) red[(tid >> 5) * 8 + line] = h0;
-        fft_rest_inplace<N, -1, NT>(s, tw, tid);
+        __syncthreads();                      // head pass done: the stage is free
+        prefetch(tile + gridDim.x);
+        fft_rest_inplace_nb<N, -1, NT>(s, tw, tid);
         __syncthreads();
         // derived outputs: i kx E, i ky E of this column
         const bool der = !FWD && fld == a.dfield;
@@ -196,13 +223,13 @@ __global__ void __launch_bounds__(fused_threads<L>(), (L >= 512 ? 2 : 3)) k_ypas
             // FFT-order row j holds j' = j (j < jpos) or j' = j - L (j >= L - nneg); the rest is zero
             fft_head<L, +1, NT>(s, tw, tid, [&](int j) {
                 cplx v = make_double2(0.0, 0.0);
-                if (j < jpos) v = in[j * pitch];
-                else if (j >= L - nneg) v = in[(j - (L - nky)) * pitch];
+                if (j < jpos) v = __ldcg(in + j * pitch);
+                else if (j >= L - nneg) v = __ldcg(in + (j - (L - nky)) * pitch);
                 return v;
             });
             fft_rest_store<L, +1, NT>(s, tw, tid, [&](int y, cplx v) { out[y * pitch] = v; });
         } else {
-            fft_head<L, -1, NT>(s, tw, tid, [&](int y) { return in[y * pitch]; });
+            fft_head<L, -1, NT>(s, tw, tid, [&](int y) { return __ldcg(in + y * pitch); });
             fft_rest_store<L, -1, NT>(s, tw, tid, [&](int j, cplx v) {
                 if (j < jpos) out[j * pitch] = cscale(v, sc);
                 else if (j >= L - nneg) out[(j - (L - nky)) * pitch] = cscale(v, sc);

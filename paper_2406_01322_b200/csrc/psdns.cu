@@ -220,8 +220,8 @@ cudaError_t set_smem(K kern, size_t bytes) {
         default: return cudaErrorInvalidValue; \
     }
 
-template <int N>
-size_t zpass_smem() { return (size_t)zpass_smem_cplx<N>() * sizeof(cplx); }
+template <int N, bool FWD>
+size_t zpass_smem() { return (size_t)zpass_smem_cplx<N, FWD>() * sizeof(cplx); }
 
 #define DISPATCH_N(Nval, MACRO)            \
     switch (Nval) {                        \
@@ -254,8 +254,8 @@ cudaError_t launch_zpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, 
     LaunchScope ls(h, fwd ? KC_ZFWD : KC_ZBWD);
 #define ZH(NN)                                                                                           \
     {                                                                                                    \
-        if (fwd) k_zpass<NN, true><<<grid, fused_threads<NN>(), zpass_smem<NN>(), h->st>>>(a, tw, ct);   \
-        else k_zpass<NN, false><<<grid, fused_threads<NN>(), zpass_smem<NN>(), h->st>>>(a, tw, ct);      \
+        if (fwd) k_zpass<NN, true><<<grid, fused_threads<NN>(), zpass_smem<NN, true>(), h->st>>>(a, tw, ct);   \
+        else k_zpass<NN, false><<<grid, fused_threads<NN>(), zpass_smem<NN, false>(), h->st>>>(a, tw, ct);      \
     }
     DISPATCH_N(h->d.N, ZH)
 #undef ZH
@@ -298,9 +298,9 @@ cudaError_t setup_attrs(psdns_handle *h) {
 #define CU0(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) return e__; } while (0)
 #define ZA(NN)                                                                                                         \
     {                                                                                                                  \
-        CU0(set_smem(k_zpass<NN, true>, zpass_smem<NN>())); CU0(set_smem(k_zpass<NN, false>, zpass_smem<NN>()));        \
-        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_z[1], k_zpass<NN, true>, fused_threads<NN>(), zpass_smem<NN>()));  \
-        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_z[0], k_zpass<NN, false>, fused_threads<NN>(), zpass_smem<NN>())); \
+        CU0(set_smem(k_zpass<NN, true>, zpass_smem<NN, true>())); CU0(set_smem(k_zpass<NN, false>, zpass_smem<NN, false>()));        \
+        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_z[1], k_zpass<NN, true>, fused_threads<NN>(), zpass_smem<NN, true>()));  \
+        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_z[0], k_zpass<NN, false>, fused_threads<NN>(), zpass_smem<NN, false>())); \
     }
 #define YA(LL)                                                                                                         \
     {                                                                                                                  \
