@@ -355,6 +355,15 @@ def run_ours(args):
                 ent["frac"] = ent["gbs"] / peak if tot > 0 else None
             kernels[name] = ent
     dominant = max((k for k in kernels if k in per_kernel), key=lambda k: kernels[k]["ms_per_step"], default=None)
+    # measured DRAM traffic per launch from the committed ncu --set full capture of this workload (text summary
+    # under profiles/; null for workloads that were not captured)
+    traffic = {}
+    try:
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r1d_traffic_5c.json")))
+        if tj.get("workload") == args.workload:
+            traffic = tj["bytes_per_launch"]
+    except Exception:
+        pass
 
     # ---- end to end through the C ABI with host buffers -----------------------------------------------
     pinned_out = [torch.empty_like(t).pin_memory() for t in pinned_in]
@@ -379,7 +388,8 @@ def run_ours(args):
         if dominant is not None:
             k = kernels[dominant]
             roof = {"bound": "hbm", "kernel": dominant, "achieved": k["gbs"], "peak": peak, "unit": "GB/s",
-                    "frac": k["frac"], "traffic": None, "peak_source": peak_src,
+                    "frac": k["frac"], "traffic": traffic.get(dominant), "traffic_unit": "bytes per launch (ncu dram read + write)",
+                    "alg_bytes_per_launch": k["alg_bytes_per_step"] / max(k["launches_per_step"], 1), "peak_source": peak_src,
                     "launch_ms": k["ms_per_step"] / max(k["launches_per_step"], 1)}
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
