@@ -331,18 +331,22 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
             xpass_mid<H, R2, -1, NT, true>(s, tid);
             __syncthreads();
         }
-        // ---- E: DIT pass R1, in place on the tile ----
+        // ---- E: DIT pass R1; the results stay in registers, only the rows some partner needs go to the tile ----
         asm volatile("" : "+d"(wj.x), "+d"(wj.y));
+        cplx v[R1];
         if (item) {
             const int j = opaque(tid) >> 3;
-            cplx v[R1];
             TwPow<R1> tp;
             tp.init(cmul(wj, wj));
             v[0] = s[xidx(j, f)];
             tp.each([&](int m, cplx wq) { v[m] = cmultw<-1>(s[xidx(j + S1 * m, f)], wq); });
             RegFFT<R1, -1>::run(v);
+            // in place: a thread reads and writes the same rows j + S1 m of its own field
 #pragma unroll
-            for (int q = 0; q < R1; ++q) s[xidx(j + S1 * q, f)] = v[q];
+            for (int q = 0; q < R1; ++q) {     // row r is read as the partner H - k of some kept k < nkx iff r > H - nkx
+                const int r = j + S1 * q;
+                if (r > H - nkx) s[xidx(r, f)] = v[q];
+            }
         }
         __syncthreads();
         // ---- F: post-twiddle of row k against the partner row H - k, truncated store ----
@@ -350,24 +354,27 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
             const int j = opaque(tid) >> 3;
             cplx *o = outf + base;
 #pragma unroll
-            for (int q0 = 0; q0 < R1; q0 += 4) {          // four rows' loads in flight, then their stores
-                cplx za[4], zb[4];
+            for (int q0 = 0; q0 < R1; q0 += 4) {          // four rows' partner loads in flight, then their stores
+                if (S1 * q0 < kxp) {                       // CTA-uniform: no row of this group is kept otherwise
+                    cplx zb[4];
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const int k = j + S1 * (q0 + i);
-                    za[i] = s[xidx(k, f)];                 // every row k < H exists: no predicate on the loads
-                    zb[i] = s[xidx((H - k) & (H - 1), f)];
-                }
+                    for (int i = 0; i < 4; ++i) {
+                        const int k = j + S1 * (q0 + i);
+                        zb[i] = s[xidx((H - k) & (H - 1), f)];   // every row exists: no predicate on the loads
+                    }
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const int q = q0 + i, k = j + S1 * q;
-                    if (k < nkx) {
-                        const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
-                        const double Sx = za[i].x + zb[i].x, Sy = za[i].y - zb[i].y, Dx = za[i].x - zb[i].x, Dy = za[i].y + zb[i].y;
-                        // X_k = (S - i w D) / (2 L)
-                        stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
-                    } else if (k < kxp) {
-                        stg(o + k, make_double2(0.0, 0.0));
+                    for (int i = 0; i < 4; ++i) {
+                        const int q = q0 + i, k = j + S1 * q;
+                        if (k < nkx) {
+                            const cplx za = v[q];
+                            const cplx zp = k ? zb[i] : za;      // k = 0 is its own partner (row 0 was not republished)
+                            const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
+                            const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
+                            // X_k = (S - i w D) / (2 L)
+                            stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
+                        } else if (k < kxp) {
+                            stg(o + k, make_double2(0.0, 0.0));
+                        }
                     }
                 }
             }
