@@ -38,7 +38,17 @@ __device__ __forceinline__ cplx cfma(double s, cplx a, cplx b) {                
 // L2 prefetch of the cache line that holds p: the column sweeps below touch one 16-byte element per array
 // per row, so the rows PF_ROWS ahead are requested early and the demand loads become L2 hits.
 __device__ __forceinline__ void pf_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-constexpr int PF_ROWS = 6;
+// Distances measured on B200 at 1024x512x513: the substitution / second-elimination / finish kernels keep every column
+// resident at once, so rows x arrays x 1.9 MB of prefetched data must stay well inside the 126 MB L2 (6 rows ahead thrashed
+// it: +2 GB of re-reads per kernel); k_rhs_elim has 12 % of the columns resident and likes a longer distance.
+#ifndef PF_ROWS_N
+#define PF_ROWS_N 2
+#endif
+#ifndef PF_ROWS_RHS_N
+#define PF_ROWS_RHS_N 4
+#endif
+constexpr int PF_ROWS = PF_ROWS_N;
+constexpr int PF_ROWS_RHS = PF_ROWS_RHS_N;
 
 // ---- layout conversion ---------------------------------------------------------------------
 // Both sides are cplx [n][rows][pitch]; a side is described by (rows, pitch, jpos, nkx):
@@ -416,7 +426,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
         for (int n = N; n >= 0; --n) {
             const RowIn r = nx;
             if (n > 0) nx = load(n - 1);
-            const int np = n - PF_ROWS;
+            const int np = n - PF_ROWS_RHS;
             if (np >= 0) {
                 pf_l2(x + np * st); pf_l2(dinv + (np + 2) * st);
                 if (np < nkz) { pf_l2(txz + np * st); pf_l2(txx + np * st); pf_l2(txy + np * st); pf_l2(tyy + np * st); pf_l2(tyz + np * st); pf_l2(hist + np * st); }
@@ -487,7 +497,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
         for (int n = N; n >= 0; --n) {
             const RowIn r = nx;
             if (n > 0) nx = load(n - 1);
-            const int np = n - PF_ROWS;
+            const int np = n - PF_ROWS_RHS;
             if (np >= 0) {
                 pf_l2(x + np * st); pf_l2(dinv + (np + 2) * st);
                 if (np < nkz) { pf_l2(qq + np * st); pf_l2(cc + np * st); pf_l2(hist + np * st); }
