@@ -23,7 +23,11 @@ template <> struct PlanF<32>   { static constexpr int R1 = 8,  R2 = 4,  R3 = 1; 
 template <> struct PlanF<64>   { static constexpr int R1 = 8,  R2 = 8,  R3 = 1; };
 template <> struct PlanF<128>  { static constexpr int R1 = 16, R2 = 8,  R3 = 1; };
 template <> struct PlanF<256>  { static constexpr int R1 = 16, R2 = 16, R3 = 1; };
+#ifdef PLANF512_888
+template <> struct PlanF<512>  { static constexpr int R1 = 8,  R2 = 8,  R3 = 8; };
+#else
 template <> struct PlanF<512>  { static constexpr int R1 = 16, R2 = 8,  R3 = 4; };
+#endif
 template <> struct PlanF<1024> { static constexpr int R1 = 16, R2 = 8,  R3 = 8; };
 
 template <int L> __host__ __device__ constexpr int planf_npass() {
