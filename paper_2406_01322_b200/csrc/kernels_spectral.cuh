@@ -363,11 +363,54 @@ struct ElimDown {
     }
 };
 
+// Real-component form of ElimDown for TWO right-hand sides that share sigma, the pivots and the Dirichlet adjoint
+// weights (the omega_z and theta problems of one column: both sigma = k^2 + 1/gamma).  The tau system has real
+// coefficients, so the real and imaginary parts of a column are two independent real problems.
+struct ElimDown2R {
+    double fp2[2], fp1[2], f0[2], fm1[2];   // F(k+2), F(k+1), F(k), F(k-1) of the next row k, per right-hand side
+    double gp2[2], gp1[2];                  // g'_{k+2}, g'_{k+1}
+    double Je[2], Jo[2];
+    double dp2, dp1, zp2, zp1;
+    __device__ __forceinline__ void init() {
+#pragma unroll
+        for (int i = 0; i < 2; ++i) fp2[i] = fp1[i] = f0[i] = fm1[i] = gp2[i] = gp1[i] = Je[i] = Jo[i] = 0.0;
+        dp2 = dp1 = zp2 = zp1 = 0.0;
+    }
+    __device__ __forceinline__ void row(int k, int N, double sigma, double fa, double fb, double di, double &ga, double &gb) {
+        const double pk = helm_p(k), qk = helm_q(k), rk = helm_r(k);
+        const double fm2[2] = {fa, fb};
+        double g[2];
+        const double m = (k + 4 <= N) ? sigma * rk * dp2 : 0.0;
+        const double sp = (k + 2 <= N) ? sigma * helm_p(k + 2) : 0.0;
+        const double z = (1.0 + sp * zp2) * di;
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            g[i] = fma(pk, fm2[i], fma(qk, f0[i], fp2[i] * rk));
+            g[i] = fma(m, gp2[i], g[i]);
+            if (k & 1) Jo[i] = fma(z, g[i], Jo[i]); else Je[i] = fma(z, g[i], Je[i]);
+            gp2[i] = gp1[i]; gp1[i] = g[i];
+            fp2[i] = fp1[i]; fp1[i] = f0[i]; f0[i] = fm1[i]; fm1[i] = fm2[i];
+        }
+        zp2 = zp1; zp1 = z;
+        dp2 = dp1; dp1 = di;
+        ga = g[0]; gb = g[1];
+    }
+    // homogeneous Dirichlet rows: u_0 = -J_e / s_e, u_1 = -J_o / s_o
+    __device__ __forceinline__ void finish(double sigma, int i, double &u0, double &u1) const {
+        const double se = 1.0 + sigma * helm_p(2) * zp1;
+        const double so = 1.0 + sigma * helm_p(3) * zp2;
+        u0 = -Je[i] / se;
+        u1 = -Jo[i] / so;
+    }
+};
+
 // ---- K_A: row a9 + first elimination ------------------------------------------------------------------
-// One WARP per (32 consecutive columns, chain); the chains of the same columns sit in one CTA so that the
-// product rows two chains share are fetched from HBM once (the second warp hits L1/L2).
-// chain 0: omega_z (column 0: u-bar)   f = -H_omega / gamma,  sigma = k^2 + 1/gamma, Dirichlet
-// chain 1: theta   (column 0: v-bar)   f = -H_w / gamma,      same sigma, Dirichlet (homogeneous part added later)
+// CTA = 32 consecutive columns, three warps.  Warps 0 and 1: the omega_z AND theta chains of 16 columns each, one
+// thread per (column, real / imaginary part) - both chains need the same five product rows and the same pivots,
+// so these are fetched once (profiles/r1d: as separate warps the two chains read them twice, 3.7 GB per step).
+// Warp 2: the psi chain of all 32 columns (complex).
+// omega_z (column 0: u-bar)   f = -H_omega / gamma,  sigma = k^2 + 1/gamma, Dirichlet
+// theta   (column 0: v-bar)   f = -H_w / gamma,      same sigma, Dirichlet (homogeneous part added later)
 // chain 2: psi                         f = H_phi / gamma_phi, sigma = k^2 + lambda_phi, Neumann
 // Every chain works in place: it reads x^n at row n going down and writes g' at row n + 2.
 struct RhsElimArgs {
@@ -388,9 +431,10 @@ constexpr int RHS_COLS = 32;   // columns per CTA of k_rhs_elim (blockDim = 32 *
 #endif
 __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
     const ColGeom &g = a.g;
-    const int col = blockIdx.x * RHS_COLS + (threadIdx.x & 31);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool nschain = warp < 2;
+    const int col = blockIdx.x * RHS_COLS + (nschain ? warp * 16 + (lane >> 1) : lane);
     if (col >= g.ncols) return;
-    const int chain = threadIdx.x >> 5;
     double kx, ky;
     col_wavenumbers(g, col, kx, ky);
     const double k2 = kx * kx + ky * ky;
@@ -399,89 +443,111 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
     const int N = g.N, nkz = g.nkz;
     const double ab0 = a.ab[0], ab1 = a.ab[1];
     const double dt = a.dt, gam = a.gamma;
-    const cplx *__restrict__ txx = a.txx + col, *__restrict__ txy = a.txy + col, *__restrict__ txz = a.txz + col;
-    const cplx *__restrict__ tyy = a.tyy + col, *__restrict__ tyz = a.tyz + col;
-    ElimDown el;
-    el.init();
     // Software pipelining: the operands of row n - 1 are loaded into registers before row n is computed, so
     // each row costs one (prefetched, L2-hit) load latency instead of one per dependent load group
     // (profiles/r1c: 77 % of the stall samples were long-scoreboard waits).
-    struct RowIn { cplx x, h, t0, t1, t2, t3, t4; double di; };
-    if (chain == 0 || chain == 1) {
+    if (nschain) {
+        const int c = lane & 1;                       // 0: real part, 1: imaginary part
+        const double sg = c ? 1.0 : -1.0;             // (i z)_c = sg * z_{1-c}
         const double sigma = k2 + 1.0 / gam, fs = -1.0 / gam;
         const double *__restrict__ dinv = a.dinv_ns + col;
-        cplx *x = (chain == 0 ? a.om : a.th) + col, *hist = (chain == 0 ? a.h_om : a.h_w) + col;
+        const cplx *__restrict__ txx = a.txx + col, *__restrict__ txy = a.txy + col, *__restrict__ txz = a.txz + col;
+        const cplx *__restrict__ tyy = a.tyy + col, *__restrict__ tyz = a.tyz + col;
+        // component views: element (n, col) of a cplx array = doubles 2 (n st + col) + {0, 1}
+        double *xo = reinterpret_cast<double *>(a.om + col) + c, *xt = reinterpret_cast<double *>(a.th + col) + c;
+        double *ho = reinterpret_cast<double *>(a.h_om + col) + c, *hw = reinterpret_cast<double *>(a.h_w + col) + c;
+        const size_t st2 = 2 * st;
+        struct RowIn { double xo, xt, ho, hw, t0, t1, t3, di; cplx t2, t4; };
         auto load = [&](int n) {
             RowIn r;
-            const size_t o = n * st;
-            r.x = x[o];
+            r.xo = xo[n * st2]; r.xt = xt[n * st2];
             r.di = (n <= N - 2) ? dinv[(n + 2) * st] : 0.0;
-            r.h = r.t0 = r.t1 = r.t2 = r.t3 = r.t4 = cz();
-            if (n < nkz) { r.h = hist[o]; r.t0 = txx[o]; r.t1 = txy[o]; r.t2 = txz[o]; r.t3 = tyy[o]; r.t4 = tyz[o]; }
+            r.ho = r.hw = r.t0 = r.t1 = r.t3 = 0.0; r.t2 = r.t4 = cz();
+            if (n < nkz) {
+                const size_t o = n * st;
+                r.ho = ho[n * st2]; r.hw = hw[n * st2];
+                r.t0 = reinterpret_cast<const double *>(txx + o)[c];
+                r.t1 = reinterpret_cast<const double *>(txy + o)[c];
+                r.t3 = reinterpret_cast<const double *>(tyy + o)[c];
+                r.t2 = txz[o]; r.t4 = tyz[o];
+            }
             return r;
         };
-        Chain1 c1; Chain2 c2a, c2x;
-        c1.init(); c2a.init(); c2x.init();
+        // derivative chains of real sequences (same recurrences as Chain1 / Chain2)
+        double Ra1 = 0, Rb1 = 0, Rb2 = 0;                               // D R
+        double Ba1 = 0, Bb1 = 0, Bb2 = 0;                               // D B
+        double Aa1 = 0, Ab1 = 0, Ab2 = 0, Ac1 = 0, Ac2 = 0;             // D^2 A
+        double Oa1 = 0, Ob1 = 0, Ob2 = 0, Oc1 = 0, Oc2 = 0;             // D^2 omega
+        double Ta1 = 0, Tb1 = 0, Tb2 = 0, Tc1 = 0, Tc2 = 0;             // D^2 theta
+        ElimDown2R el;
+        el.init();
         RowIn nx = load(N);
         for (int n = N; n >= 0; --n) {
             const RowIn r = nx;
             if (n > 0) nx = load(n - 1);
             const int np = n - PF_ROWS_RHS;
-            if (np >= 0) {
-                pf_l2(x + np * st); pf_l2(dinv + (np + 2) * st);
-                if (np < nkz) { pf_l2(txz + np * st); pf_l2(txx + np * st); pf_l2(txy + np * st); pf_l2(tyy + np * st); pf_l2(tyz + np * st); pf_l2(hist + np * st); }
+            if (np >= 0 && c == 0) {
+                pf_l2(a.om + col + np * st); pf_l2(a.th + col + np * st); pf_l2(dinv + (np + 2) * st);
+                if (np < nkz) {
+                    pf_l2(txz + np * st); pf_l2(txx + np * st); pf_l2(txy + np * st); pf_l2(tyy + np * st); pf_l2(tyz + np * st);
+                    pf_l2(a.h_om + col + np * st); pf_l2(a.h_w + col + np * st);
+                }
             }
             const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
-            const size_t o = n * st;
             const bool low = n < nkz;
-            cplx nlin;
-            cplx ddX;
-            if (chain == 0) {
-                // N_omega = P + D R (Eq. 14 expanded); column 0: S-bar_x = D T_xz (+ G)
-                cplx P = cz(), R = cz();
-                if (low) {
-                    if (mean) R = r.t2;
-                    else {
-                        P = cadd(cscale(r.t1, ky * ky - kx * kx), cscale(csub(r.t0, r.t3), kx * ky));
-                        R = ci(csub(cscale(r.t4, kx), cscale(r.t2, ky)));
-                    }
+            const double t2c = c ? r.t2.y : r.t2.x, t2o = c ? r.t2.x : r.t2.y;
+            const double t4c = c ? r.t4.y : r.t4.x, t4o = c ? r.t4.x : r.t4.y;
+            // N_omega = P + D R (Eq. 14 expanded); column 0: S-bar_x = D T_xz (+ G)
+            // N_w = D B - D^2 A - k^2 A (Eq. 15 expanded); column 0: S-bar_y = D T_yz
+            double P = 0.0, R = 0.0, A = 0.0, B = 0.0;
+            if (low) {
+                if (mean) { R = t2c; B = t4c; }
+                else {
+                    P = r.t1 * (ky * ky - kx * kx) + (r.t0 - r.t3) * (kx * ky);
+                    R = sg * (kx * t4o - ky * t2o);
+                    A = sg * (kx * t2o + ky * t4o);
+                    // kx^2 Txx + 2 kx ky Txy + ky^2 Tyy - k^2 Tzz with the deviatoric inputs
+                    B = r.t0 * (kx * kx) + r.t1 * (2.0 * kx * ky) + r.t3 * (ky * ky);
                 }
-                const cplx dR = c1.step(R, f, h);
-                ddX = c2x.step(r.x, f, h);
-                nlin = cadd(P, dR);
-                if (mean && n == 0) nlin.x += a.gradp;
-            } else {
-                // N_w = D B - D^2 A - k^2 A (Eq. 15 expanded); column 0: S-bar_y = D T_yz
-                cplx A = cz(), B = cz();
-                if (low) {
-                    if (mean) B = r.t4;
-                    else {
-                        A = ci(cadd(cscale(r.t2, kx), cscale(r.t4, ky)));
-                        // kx^2 Txx + 2 kx ky Txy + ky^2 Tyy - k^2 Tzz with the deviatoric inputs
-                        B = cadd(cadd(cscale(r.t0, kx * kx), cscale(r.t1, 2.0 * kx * ky)), cscale(r.t3, ky * ky));
-                    }
-                }
-                const cplx dB = c1.step(B, f, h);
-                const cplx ddA = c2a.step(A, f, h);
-                ddX = c2x.step(r.x, f, h);
-                nlin = cadd(csub(dB, ddA), cscale(A, -k2));
             }
-            cplx nl = cscale(nlin, ab0);
-            if (low) { nl = cfma(ab1, r.h, nl); hist[o] = nlin; }
-            const cplx H = cfma(dt, nl, cfma(gam, cfma(-k2, r.x, ddX), r.x));
+            const double dR = fma(f, Ra1, Rb2) * h; Ra1 = R; Rb2 = Rb1; Rb1 = dR;
+            const double dB = fma(f, Ba1, Bb2) * h; Ba1 = B; Bb2 = Bb1; Bb1 = dB;
+            const double dA = fma(f, Aa1, Ab2) * h, ddA = fma(f, Ab1, Ac2) * h;
+            Aa1 = A; Ab2 = Ab1; Ab1 = dA; Ac2 = Ac1; Ac1 = ddA;
+            const double dO = fma(f, Oa1, Ob2) * h, ddO = fma(f, Ob1, Oc2) * h;
+            Oa1 = r.xo; Ob2 = Ob1; Ob1 = dO; Oc2 = Oc1; Oc1 = ddO;
+            const double dT = fma(f, Ta1, Tb2) * h, ddT = fma(f, Tb1, Tc2) * h;
+            Ta1 = r.xt; Tb2 = Tb1; Tb1 = dT; Tc2 = Tc1; Tc1 = ddT;
+            double nl_o = P + dR;
+            if (mean && n == 0 && c == 0) nl_o += a.gradp;
+            const double nl_w = (dB - ddA) + A * (-k2);
+            double so = nl_o * ab0, sw = nl_w * ab0;
+            if (low) {
+                so = fma(ab1, r.ho, so); sw = fma(ab1, r.hw, sw);
+                ho[n * st2] = nl_o; hw[n * st2] = nl_w;
+            }
+            const double Ho = fma(dt, so, fma(gam, fma(-k2, r.xo, ddO), r.xo));
+            const double Hw = fma(dt, sw, fma(gam, fma(-k2, r.xt, ddT), r.xt));
             if (n <= N - 2) {
                 const int k = n + 2;
-                x[k * st] = el.row<false, false>(k, N, sigma, cscale(H, fs), r.di);
+                double go, gw;
+                el.row(k, N, sigma, Ho * fs, Hw * fs, r.di, go, gw);
+                xo[k * st2] = go; xt[k * st2] = gw;
             }
         }
-        cplx u0, u1;
-        el.finish<false>(sigma, 0.0, 0.0, u0, u1);
-        x[0] = u0; x[st] = u1;
+        double u0, u1;
+        el.finish(sigma, 0, u0, u1);
+        xo[0] = u0; xo[st2] = u1;
+        el.finish(sigma, 1, u0, u1);
+        xt[0] = u0; xt[st2] = u1;
     } else {
         const double sigma = k2 + a.lam_phi, fs = 1.0 / a.gam_phi;
         const double *__restrict__ dinv = a.dinv_ch + col;
         const cplx *__restrict__ qq = a.q + col, *__restrict__ cc = a.c + col;
         cplx *x = a.phi + col, *hist = a.h_phi + col;
+        struct RowIn { cplx x, h, t0, t1; double di; };
+        ElimDown el;
+        el.init();
         auto load = [&](int n) {
             RowIn r;
             const size_t o = n * st;
