@@ -183,9 +183,36 @@ struct Chain2 {  // second derivative
 // Gauss elimination from k = N down removes c_k (pivots d'_k, stored as 1/d'_k by k_helm_setup);
 // the remaining lower-bidiagonal rows give u_k = alpha_k + beta_k u_par (par = k & 1), and the
 // boundary row of each parity fixes u_par.
-__device__ __forceinline__ double helm_p(int k) { return (k == 2 ? 2.0 : 1.0) / (4.0 * k * (double)(k - 1)); }
-__device__ __forceinline__ double helm_q(int k) { return -1.0 / (2.0 * ((double)k * k - 1.0)); }
-__device__ __forceinline__ double helm_r(int k) { return 1.0 / (4.0 * k * (double)(k + 1)); }
+// p_k, q_k, r_k depend on k only and every thread of a warp is at the same k: constant-memory tables (one broadcast
+// read instead of an FP64 division each; filled once by psdns_init with the host versions of the same formulas,
+// k <= HELM_KMAX = N_max + 2).
+constexpr int HELM_KMAX = 516;
+__constant__ double c_helm_p[HELM_KMAX + 1], c_helm_q[HELM_KMAX + 1], c_helm_r[HELM_KMAX + 1];
+inline double helm_p_host(int k) { return k < 2 ? 0.0 : (k == 2 ? 2.0 : 1.0) / (4.0 * k * (double)(k - 1)); }
+inline double helm_q_host(int k) { return k < 2 ? 0.0 : -1.0 / (2.0 * ((double)k * k - 1.0)); }
+inline double helm_r_host(int k) { return k < 1 ? 0.0 : 1.0 / (4.0 * k * (double)(k + 1)); }
+__device__ __forceinline__ double helm_p(int k) { return c_helm_p[k]; }
+__device__ __forceinline__ double helm_q(int k) { return c_helm_q[k]; }
+__device__ __forceinline__ double helm_r(int k) { return c_helm_r[k]; }
+
+// Pivots of the downward elimination, d'_k = d_k - c_k a_{k+2} / d'_{k+2} (the recurrence of k_helm_setup), recomputed
+// on the fly by the down sweeps instead of being read from the [N+1][ncols] table (the up sweeps, which need them in
+// ascending order, still read the table): saves 0.48 GB of reads per down sweep at 1024x512x513.
+struct PivotDown {
+    double di1, di2;   // 1/d'_{k+1}, 1/d'_{k+2}
+    __device__ __forceinline__ void init() { di1 = di2 = 0.0; }
+    __device__ __forceinline__ double step(int k, int N, double sigma) {
+        double d = 1.0 + ((k + 2 <= N) ? sigma * (-helm_q(k)) : 0.0);
+        if (k + 4 <= N) {
+            const double ck = -sigma * helm_r(k);
+            const double ak2 = -sigma * helm_p(k + 2);
+            d -= ck * ak2 * di2;
+        }
+        const double di = 1.0 / d;
+        di2 = di1; di1 = di;
+        return di;
+    }
+};
 
 struct HelmSetupArgs {
     ColGeom g;
@@ -202,18 +229,9 @@ __global__ void __launch_bounds__(NT_COL) k_helm_setup(const __grid_constant__ H
     const double sigma = kx * kx + ky * ky + a.shift;
     const size_t st = g.ncols;
     const int N = g.N;
-    double di1 = 0.0, di2 = 0.0;  // 1/d'_{k+1}, 1/d'_{k+2}
-    for (int k = N; k >= 2; --k) {
-        double d = 1.0 + ((k + 2 <= N) ? sigma * (-helm_q(k)) : 0.0);
-        if (k + 4 <= N) {
-            const double ck = -sigma * helm_r(k);
-            const double ak2 = -sigma * helm_p(k + 2);
-            d -= ck * ak2 * di2;
-        }
-        const double di = 1.0 / d;
-        a.dinv[k * st + col] = di;
-        di2 = di1; di1 = di;
-    }
+    PivotDown pv;
+    pv.init();
+    for (int k = N; k >= 2; --k) a.dinv[k * st + col] = pv.step(k, N, sigma);
     a.dinv[col] = 0.0;
     a.dinv[st + col] = 0.0;
 }
@@ -450,18 +468,18 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
         const int c = lane & 1;                       // 0: real part, 1: imaginary part
         const double sg = c ? 1.0 : -1.0;             // (i z)_c = sg * z_{1-c}
         const double sigma = k2 + 1.0 / gam, fs = -1.0 / gam;
-        const double *__restrict__ dinv = a.dinv_ns + col;
         const cplx *__restrict__ txx = a.txx + col, *__restrict__ txy = a.txy + col, *__restrict__ txz = a.txz + col;
         const cplx *__restrict__ tyy = a.tyy + col, *__restrict__ tyz = a.tyz + col;
         // component views: element (n, col) of a cplx array = doubles 2 (n st + col) + {0, 1}
         double *xo = reinterpret_cast<double *>(a.om + col) + c, *xt = reinterpret_cast<double *>(a.th + col) + c;
         double *ho = reinterpret_cast<double *>(a.h_om + col) + c, *hw = reinterpret_cast<double *>(a.h_w + col) + c;
         const size_t st2 = 2 * st;
-        struct RowIn { double xo, xt, ho, hw, t0, t1, t3, di; cplx t2, t4; };
+        struct RowIn { double xo, xt, ho, hw, t0, t1, t3; cplx t2, t4; };
+        PivotDown pv;
+        pv.init();
         auto load = [&](int n) {
             RowIn r;
             r.xo = xo[n * st2]; r.xt = xt[n * st2];
-            r.di = (n <= N - 2) ? dinv[(n + 2) * st] : 0.0;
             r.ho = r.hw = r.t0 = r.t1 = r.t3 = 0.0; r.t2 = r.t4 = cz();
             if (n < nkz) {
                 const size_t o = n * st;
@@ -487,7 +505,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
             if (n > 0) nx = load(n - 1);
             const int np = n - PF_ROWS_RHS;
             if (np >= 0 && c == 0) {
-                pf_l2(a.om + col + np * st); pf_l2(a.th + col + np * st); pf_l2(dinv + (np + 2) * st);
+                pf_l2(a.om + col + np * st); pf_l2(a.th + col + np * st);
                 if (np < nkz) {
                     pf_l2(txz + np * st); pf_l2(txx + np * st); pf_l2(txy + np * st); pf_l2(tyy + np * st); pf_l2(tyz + np * st);
                     pf_l2(a.h_om + col + np * st); pf_l2(a.h_w + col + np * st);
@@ -531,7 +549,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
             if (n <= N - 2) {
                 const int k = n + 2;
                 double go, gw;
-                el.row(k, N, sigma, Ho * fs, Hw * fs, r.di, go, gw);
+                el.row(k, N, sigma, Ho * fs, Hw * fs, pv.step(k, N, sigma), go, gw);
                 xo[k * st2] = go; xt[k * st2] = gw;
             }
         }
@@ -542,17 +560,17 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
         xt[0] = u0; xt[st2] = u1;
     } else {
         const double sigma = k2 + a.lam_phi, fs = 1.0 / a.gam_phi;
-        const double *__restrict__ dinv = a.dinv_ch + col;
         const cplx *__restrict__ qq = a.q + col, *__restrict__ cc = a.c + col;
         cplx *x = a.phi + col, *hist = a.h_phi + col;
-        struct RowIn { cplx x, h, t0, t1; double di; };
+        struct RowIn { cplx x, h, t0, t1; };
         ElimDown el;
         el.init();
+        PivotDown pv;
+        pv.init();
         auto load = [&](int n) {
             RowIn r;
             const size_t o = n * st;
             r.x = x[o];
-            r.di = (n <= N - 2) ? dinv[(n + 2) * st] : 0.0;
             r.h = r.t0 = r.t1 = cz();
             if (n < nkz) { r.h = hist[o]; r.t0 = qq[o]; r.t1 = cc[o]; }
             return r;
@@ -565,7 +583,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
             if (n > 0) nx = load(n - 1);
             const int np = n - PF_ROWS_RHS;
             if (np >= 0) {
-                pf_l2(x + np * st); pf_l2(dinv + (np + 2) * st);
+                pf_l2(x + np * st);
                 if (np < nkz) { pf_l2(qq + np * st); pf_l2(cc + np * st); pf_l2(hist + np * st); }
             }
             const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
@@ -583,7 +601,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
             const cplx H = cfma(dt, nl, r.x);
             if (n <= N - 2) {
                 const int k = n + 2;
-                x[k * st] = el.row<true, false>(k, N, sigma, cscale(H, fs), r.di);
+                x[k * st] = el.row<true, false>(k, N, sigma, cscale(H, fs), pv.step(k, N, sigma));
             }
         }
         cplx u0, u1;
@@ -677,12 +695,13 @@ __global__ void __launch_bounds__(NT_COL, 5) k_elim2(const __grid_constant__ Eli
     if (chain == 0) {
         const cplx *__restrict__ in = a.th + col;
         cplx *__restrict__ out = a.w + col;
-        const double *__restrict__ dinv = a.dinv_po + col;
+        PivotDown pv;
+        pv.init();
 #pragma unroll 4
         for (int k = N; k >= 2; --k) {
             const int kp = k - PF_ROWS;
-            if (kp >= 2) { pf_l2(in + (kp - 2) * st); pf_l2(dinv + kp * st); }
-            out[k * st] = el.row<false, true>(k, N, k2, in[(k - 2) * st], dinv[k * st]);
+            if (kp >= 2) pf_l2(in + (kp - 2) * st);
+            out[k * st] = el.row<false, true>(k, N, k2, in[(k - 2) * st], pv.step(k, N, k2));
         }
         cplx u0, u1, de, dodd;
         el.finish<false>(k2, 0.0, 0.0, u0, u1);
@@ -695,13 +714,14 @@ __global__ void __launch_bounds__(NT_COL, 5) k_elim2(const __grid_constant__ Eli
         if (!a.phase) return;
         const double sigma = k2 + a.lam_phi;
         cplx *x = a.phi + col;
-        const double *__restrict__ dinv = a.dinv_ch + col;
+        PivotDown pv;
+        pv.init();
 #pragma unroll 4
         for (int k = N; k >= 2; --k) {
             const int kp = k - PF_ROWS;
-            if (kp >= 2) { pf_l2(x + (kp - 2) * st); pf_l2(dinv + kp * st); }
+            if (kp >= 2) pf_l2(x + (kp - 2) * st);
             const cplx fm2 = x[(k - 2) * st];
-            x[k * st] = el.row<true, false>(k, N, sigma, fm2, dinv[k * st]);
+            x[k * st] = el.row<true, false>(k, N, sigma, fm2, pv.step(k, N, sigma));
         }
         cplx u0, u1;
         el.finish<true>(sigma, 0.0, 0.0, u0, u1);

@@ -587,6 +587,14 @@ cudaError_t build_tables(psdns_handle *h) {
         CU(cudaMemcpyAsync(h->ws + L.ctab_z, t.data(), t.size() * sizeof(cplx), cudaMemcpyHostToDevice, h->st));
         CU(cudaStreamSynchronize(h->st));
     }
+    {   // p_k, q_k, r_k of the quasi-tridiagonal recurrence (kernels_spectral.cuh), k-only: constant memory
+        static double hp[HELM_KMAX + 1], hq[HELM_KMAX + 1], hr[HELM_KMAX + 1];
+        for (int k = 0; k <= HELM_KMAX; ++k) { hp[k] = helm_p_host(k); hq[k] = helm_q_host(k); hr[k] = helm_r_host(k); }
+        CU(cudaMemcpyToSymbolAsync(c_helm_p, hp, sizeof(hp), 0, cudaMemcpyHostToDevice, h->st));
+        CU(cudaMemcpyToSymbolAsync(c_helm_q, hq, sizeof(hq), 0, cudaMemcpyHostToDevice, h->st));
+        CU(cudaMemcpyToSymbolAsync(c_helm_r, hr, sizeof(hr), 0, cudaMemcpyHostToDevice, h->st));
+        CU(cudaStreamSynchronize(h->st));
+    }
     const Coefs c = coefs(h->p);
     const double shifts[3] = {1.0 / c.gamma, 0.0, c.lam_phi};
     for (int t = 0; t < 3; ++t) {
