@@ -617,6 +617,7 @@ struct SubstArgs {
     const double *dinv[3];
     double shift[3];
     int nchains;
+    int pair01;                 // chains 0 and 1 share sigma and the pivot table: one thread does both (grid.y = nchains - 1)
     // influence-matrix correction (chain 0 only, when coef != nullptr): x += A_par * wh ; th += A_par * thh
     const cplx *coef;           // [2][ncols]: A_e, A_o
     const double *wh, *thh;     // real homogeneous solutions [nz][ncols]
@@ -627,12 +628,29 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= g.ncols) return;
-    const int chain = blockIdx.y;
+    const int chain = a.pair01 ? blockIdx.y + 1 : blockIdx.y;
     double kx, ky;
     col_wavenumbers(g, col, kx, ky);
-    const double sigma = kx * kx + ky * ky + a.shift[chain];
     const size_t st = g.ncols;
     const int N = g.N;
+    if (a.pair01 && blockIdx.y == 0) {      // omega_z and theta: same recurrence coefficients, two right-hand sides
+        const double sigma = kx * kx + ky * ky + a.shift[0];
+        cplx *x0 = a.x[0] + col, *x1 = a.x[1] + col;
+        const double *__restrict__ dinv = a.dinv[0] + col;
+        cplx um2 = x0[0], um1 = x0[st], vm2 = x1[0], vm1 = x1[st];
+#pragma unroll 4
+        for (int k = 2; k <= N; ++k) {
+            const int kp = k + PF_ROWS;
+            if (kp <= N) { pf_l2(x0 + kp * st); pf_l2(x1 + kp * st); pf_l2(dinv + kp * st); }
+            const double ak = -sigma * helm_p(k), di = dinv[k * st];
+            const cplx u = cscale(cfma(-ak, um2, x0[k * st]), di);
+            const cplx v = cscale(cfma(-ak, vm2, x1[k * st]), di);
+            um2 = um1; um1 = u; vm2 = vm1; vm1 = v;
+            x0[k * st] = u; x1[k * st] = v;
+        }
+        return;
+    }
+    const double sigma = kx * kx + ky * ky + a.shift[chain];
     cplx *x = a.x[chain] + col;
     const double *__restrict__ dinv = a.dinv[chain] + col;
     const bool corr = (chain == 0 && a.coef != nullptr);

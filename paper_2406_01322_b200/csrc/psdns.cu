@@ -519,9 +519,10 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.dinv[0] = dNS; a.dinv[1] = dNS; a.dinv[2] = dCH;
         a.shift[0] = inv_g; a.shift[1] = inv_g; a.shift[2] = c.lam_phi;
         a.nchains = phase ? 3 : 2;
+        a.pair01 = 1;
         a.coef = nullptr; a.wh = nullptr; a.thh = nullptr; a.th = nullptr;
         LaunchScope ls(h, KC_SOLVE);
-        k_subst<<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
+        k_subst<<<dim3(col_grid(d), a.nchains - 1), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     {
@@ -539,6 +540,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.dinv[0] = dPO; a.dinv[1] = dCH; a.dinv[2] = nullptr;
         a.shift[0] = 0.0; a.shift[1] = c.lam_phi; a.shift[2] = 0.0;
         a.nchains = phase ? 2 : 1;
+        a.pair01 = 0;
         a.coef = h->at<cplx>(L.coef); a.wh = h->at<double>(L.wh); a.thh = h->at<double>(L.thh); a.th = TH;
         LaunchScope ls(h, KC_SOLVE);
         k_subst<<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
