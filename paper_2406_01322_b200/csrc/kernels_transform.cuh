@@ -57,6 +57,12 @@ __device__ __forceinline__ void load_twiddles(cplx *tw, const cplx *__restrict__
 // profiles/r1d: 35 % of the samples were long-scoreboard waits in the head pass).  Optional derived outputs i kx X and i ky X of one field (row a1:
 // the x / y derivatives of phi commute with the z transform, so they cost no transform of their own).
 // ------------------------------------------------------------------------------------------
+// fft_head with an explicit plan (the load functor type is deduced)
+template <int L, int NT, class P, class Load>
+__device__ __forceinline__ void fft_head_z(cplx *__restrict__ s, const cplx *__restrict__ tw, int tid, Load load) {
+    fft_head<L, -1, NT, Load, P>(s, tw, tid, load);
+}
+
 struct ZArgs {
     FieldPtrs f;
     int nf;     // fields
@@ -69,15 +75,20 @@ struct ZArgs {
     double kxf, kyf;
 };
 
+template <int N, bool FWD> struct ZPlan { typedef PlanF<N> type; };
+template <int N> struct ZPlan<N, false> { typedef PlanZB<N> type; };
+template <int N, bool FWD> __host__ __device__ constexpr int zpass_threads() { return fused_threads<N, typename ZPlan<N, FWD>::type>(); }
+
 template <int N, bool FWD> __host__ __device__ constexpr int zpass_smem_cplx() {
-    return N * TILE_LINES + N + (fused_threads<N>() / 32) * 8 + (N / 2 + 1) + (FWD ? 0 : (N / 2) * TILE_LINES);
+    return N * TILE_LINES + N + (zpass_threads<N, FWD>() / 32) * 8 + (N / 2 + 1) + (FWD ? 0 : (N / 2) * TILE_LINES);
 }
 
 template <int N, bool FWD>
-__global__ void __launch_bounds__(fused_threads<N>(), (N >= 512 ? 2 : 3)) k_zpass(const __grid_constant__ ZArgs a,
+__global__ void __launch_bounds__(zpass_threads<N, FWD>(), (N >= 512 ? 2 : 3)) k_zpass(const __grid_constant__ ZArgs a,
                                                                                const cplx *__restrict__ tw2n,
                                                                                const cplx *__restrict__ ctab_g) {
-    constexpr int NT = fused_threads<N>();
+    typedef typename ZPlan<N, FWD>::type ZP;
+    constexpr int NT = zpass_threads<N, FWD>();
     constexpr int NW = NT / 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
@@ -116,7 +127,7 @@ __global__ void __launch_bounds__(fused_threads<N>(), (N >= 512 ? 2 : 3)) k_zpas
         __syncthreads();                      // stage (and, first time, the tables) visible to all threads
         cplx h0 = make_double2(0.0, 0.0);
         // z_m = e_{2m} + i e_{2m+1}; for m >= N/2 the even extension folds back: e_j = a_{2N-j}
-        fft_head<N, -1, NT>(s, tw, tid, [&](int m) {
+        fft_head_z<N, NT, ZP>(s, tw, tid, [&](int m) {
             const int ne = (m < N / 2) ? 2 * m : 2 * N - 2 * m;
             const int no = (m < N / 2) ? 2 * m + 1 : 2 * N - 2 * m - 1;
             cplx e0 = make_double2(0.0, 0.0), e1 = e0;
@@ -135,7 +146,7 @@ __global__ void __launch_bounds__(fused_threads<N>(), (N >= 512 ? 2 : 3)) k_zpas
         if ((tid & 31) < 8) red[(tid >> 5) * 8 + line] = h0;
         __syncthreads();                      // head pass done: the stage is free
         prefetch(tile + gridDim.x);
-        fft_rest_inplace_nb<N, -1, NT>(s, tw, tid);
+        fft_rest_inplace_nb<N, -1, NT, ZP>(s, tw, tid);
         __syncthreads();
         // derived outputs: i kx E, i ky E of this column
         const bool der = !FWD && fld == a.dfield;
@@ -166,8 +177,8 @@ __global__ void __launch_bounds__(fused_threads<N>(), (N >= 512 ? 2 : 3)) k_zpas
                 emit(0, cscale(cadd(G0, H0), FWD ? 0.5 * sc : sc));
                 if (N < nout) emit(N, cscale(csub(G0, H0), FWD ? 0.5 * sc : sc));
             } else {
-                const cplx za = s[fft_pos_f<N>(k) * TILE_LINES + line];
-                const cplx zb = s[fft_pos_f<N>(kb) * TILE_LINES + line];
+                const cplx za = s[fft_pos_f<N, ZP>(k) * TILE_LINES + line];
+                const cplx zb = s[fft_pos_f<N, ZP>(kb) * TILE_LINES + line];
                 const cplx c = ctab[k];
                 const cplx d = csub(za, zb);
                 const cplx cd = make_double2(c.x * d.x - c.y * d.y, c.x * d.y + c.y * d.x);     // c_k d

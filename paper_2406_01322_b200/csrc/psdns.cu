@@ -254,8 +254,8 @@ cudaError_t launch_zpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, 
     LaunchScope ls(h, fwd ? KC_ZFWD : KC_ZBWD);
 #define ZH(NN)                                                                                           \
     {                                                                                                    \
-        if (fwd) k_zpass<NN, true><<<grid, fused_threads<NN>(), zpass_smem<NN, true>(), h->st>>>(a, tw, ct);   \
-        else k_zpass<NN, false><<<grid, fused_threads<NN>(), zpass_smem<NN, false>(), h->st>>>(a, tw, ct);      \
+        if (fwd) k_zpass<NN, true><<<grid, zpass_threads<NN, true>(), zpass_smem<NN, true>(), h->st>>>(a, tw, ct);   \
+        else k_zpass<NN, false><<<grid, zpass_threads<NN, false>(), zpass_smem<NN, false>(), h->st>>>(a, tw, ct);      \
     }
     DISPATCH_N(h->d.N, ZH)
 #undef ZH
@@ -299,8 +299,8 @@ cudaError_t setup_attrs(psdns_handle *h) {
 #define ZA(NN)                                                                                                         \
     {                                                                                                                  \
         CU0(set_smem(k_zpass<NN, true>, zpass_smem<NN, true>())); CU0(set_smem(k_zpass<NN, false>, zpass_smem<NN, false>()));        \
-        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_z[1], k_zpass<NN, true>, fused_threads<NN>(), zpass_smem<NN, true>()));  \
-        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_z[0], k_zpass<NN, false>, fused_threads<NN>(), zpass_smem<NN, false>())); \
+        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_z[1], k_zpass<NN, true>, zpass_threads<NN, true>(), zpass_smem<NN, true>()));  \
+        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_z[0], k_zpass<NN, false>, zpass_threads<NN, false>(), zpass_smem<NN, false>())); \
     }
 #define YA(LL)                                                                                                         \
     {                                                                                                                  \
