@@ -230,3 +230,38 @@ def test_navier_stokes_part_is_second_order_in_time():
         sols[n] = np.concatenate([f.ravel() for f in orc.get_state("spectral")])
     e = {n: np.linalg.norm(sols[n] - sols[256]) for n in (8, 16, 32)}
     assert 3.3 < e[8] / e[16] < 4.8 and 3.3 < e[16] / e[32] < 4.9, e
+
+
+def test_variable_viscosity_steady_layered_flow():
+    """Reading S14 (eta(phi) = 1 + (lambda - 1)(phi + 1)/2, viscous term split into implicit (1/Re) lap u and explicit
+    (1/Re) div[(eta - 1)(grad u + grad u^T)]) pinned against a closed form that does not use the split: for the layered
+    state phi = tanh(z/(sqrt2 Ch)) (Eq. 5), u = u(z), the x-momentum balance is d/dz(eta u') = -G Re, i.e.
+    eta u' = -G Re z + c with u(+-1) = 0 -- a quadrature.  That state must be steady under the scheme up to the
+    truncation error, which falls spectrally with resolution; a wrong sign or factor in the split leaves a tendency
+    of order G (lambda - 1) ~ 3e-2."""
+    from scipy.integrate import quad
+    re, lam, G, dt = 50.0, 0.3, 2.0 / 50.0, 1e-3
+
+    def tendency(nz, ch):
+        g = O.Grid(8, 8, nz, 4 * math.pi, 2 * math.pi)
+        z = O.cheb_nodes(g.N)
+        eta = lambda s: 1.0 + (lam - 1.0) * (math.tanh(s / (math.sqrt(2.0) * ch)) + 1.0) / 2.0
+        q = dict(epsabs=1e-13, epsrel=1e-13, limit=200)
+        c = -quad(lambda s: -G * re * s / eta(s), -1, 1, **q)[0] / quad(lambda s: 1.0 / eta(s), -1, 1, **q)[0]
+        u1 = np.array([quad(lambda s: (-G * re * s + c) / eta(s), -1, zz, **q)[0] for zz in z])
+        u = np.broadcast_to(u1[:, None, None], (nz, 8, 8)).copy()
+        phi = np.broadcast_to(np.tanh(z / (math.sqrt(2.0) * ch))[:, None, None], (nz, 8, 8)).copy()
+        orc = O.Oracle(g, O.Params(re=re, dt=dt, pe=1.0 / ch, ch=ch, we=1.0, gradp_x=G, visc_ratio=lam))
+        orc.set_state("physical", u, np.zeros_like(u), np.zeros_like(u), phi)
+        orc.step(2)
+        un, vn, wn, _ = orc.get_state("physical")
+        assert np.abs(vn).max() < 1e-12 and np.abs(wn).max() < 1e-12
+        return np.abs(un - u).max() / (2 * dt), np.abs(u1).max()
+
+    import warnings
+    with warnings.catch_warnings():
+        warnings.simplefilter("ignore")          # quad reports round-off at the 1e-13 request
+        t_coarse, umax = tendency(129, 0.1)
+        t_fine, _ = tendency(257, 0.07)
+    assert umax > 1.5                            # the low-viscosity layer speeds the flow up (lambda = 1: max u = 1)
+    assert t_coarse < 5e-6 and t_fine < 5e-8, (t_coarse, t_fine)
