@@ -32,7 +32,7 @@ def load_samples(k, nsteps):
     return norms, rows
 
 
-@pytest.mark.parametrize("k,nsteps", [(3, 1), (3, 3), (4, 1), (4, 2)])
+@pytest.mark.parametrize("k,nsteps", [(2, 100), (3, 1), (3, 3), (4, 1), (4, 2)])
 def test_config_full_grid_sampled(k, nsteps):
     import torch
     import paper_2406_01322_b200 as P
@@ -56,4 +56,31 @@ def test_config_full_grid_sampled(k, nsteps):
     for fi in range(4):
         got = float(torch.linalg.vector_norm(out[fi]))
         assert abs(got - norms[fi]) <= TOL * max(norms[fi], norms[0]), (fi, got, norms[fi])
+    s.close()
+
+
+@pytest.mark.parametrize("k", [2, 3, 4])
+def test_config_full_step_count_stays_bounded(k):
+    """BASELINE.json's full step counts (100 / 50 / 50) on the full grids: the state stays finite and bounded
+    (|phi| <= 1 + overshoot of the tanh profile, velocity of the order of the laminar centreline speed), mean(phi)
+    drifts only by the tau residual, and continuity holds algebraically at the end."""
+    import torch
+    import paper_2406_01322_b200 as P
+    c = I.CONFIGS[k]
+    st = I.channel_state(c)
+    s = solver_from_config(c)
+    s.set_state(P.PHYSICAL, *[to_dev(f) for f in st])
+    phi0 = s.get_state(P.SPECTRAL)[3][:, 0, 0].real.clone()
+    s.step(c.steps)
+    u, v, w, phi = s.get_state(P.PHYSICAL)
+    for t in (u, v, w, phi):
+        assert bool(torch.isfinite(t).all())
+    assert float(phi.abs().max()) < 1.2
+    assert float(u.abs().max()) < 2.0 and float(v.abs().max()) < 1.0 and float(w.abs().max()) < 1.0
+    # mean(phi) = 1/2 sum_{n even} phi^(0,0,n) 2/(1 - n^2)
+    n = torch.arange(c.nz, device="cuda", dtype=torch.float64)
+    wgt = torch.where(n.long() % 2 == 0, 1.0 / (1.0 - n * n), torch.zeros_like(n))
+    phi1 = s.get_state(P.SPECTRAL)[3][:, 0, 0].real
+    drift = abs(float((wgt * (phi1 - phi0)).sum()))
+    assert drift < 1e-4, drift
     s.close()
