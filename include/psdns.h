@@ -96,6 +96,19 @@ int psdns_step(psdns_handle *h, int nsteps);
  * zero in PSDNS_SPECTRAL).  d_phi may be NULL iff phase_field == 0. */
 int psdns_get_state(psdns_handle *h, int space, void *d_u, void *d_v, void *d_w, void *d_phi);
 
+/* Hidden state of the time integration, for an exact restart (SURVEY.md 8(b) "optional, for bit-exact restart";
+ * the paper's demo run "starts ... in a flow field previously obtained" from another run):
+ * theta^ = lap(w) carried from the last solve (reading S13), omega_z^, D phi^, the three Adams-Bashforth
+ * history spectra (N_omega, N_w, S_phi of step n-1, reading S7) and the step counter, as ONE opaque blob in the
+ * library's private layout.  Protocol: state = psdns_get_state(PSDNS_SPECTRAL), blob = psdns_get_history;
+ * later, on a handle of the same grid and params: psdns_set_state(PSDNS_SPECTRAL, state) then
+ * psdns_set_history(blob) - the following steps are bit-identical to the uninterrupted run.
+ * d_blob: DEVICE memory of psdns_history_bytes(h) bytes (256-byte aligned), owned by the caller.
+ * PSDNS_ESTATE before the first set_state; PSDNS_EINVAL on a null pointer or a size mismatch. */
+size_t psdns_history_bytes(const psdns_handle *h);
+int psdns_get_history(psdns_handle *h, void *d_blob, size_t bytes);
+int psdns_set_history(psdns_handle *h, const void *d_blob, size_t bytes);
+
 /* One forward+backward 3-D transform of a single field with dealiasing OFF (full sizes).
  * start_space = PSDNS_PHYSICAL: d_in physical -> (d_mid spectral, nullable) -> d_out physical.
  * start_space = PSDNS_SPECTRAL: d_in spectral -> (d_mid physical, nullable) -> d_out spectral.

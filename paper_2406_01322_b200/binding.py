@@ -12,6 +12,7 @@ EXPORTS = [
     "psdns_workspace_bytes", "psdns_init", "psdns_set_state", "psdns_step", "psdns_get_state",
     "psdns_transform_roundtrip", "psdns_run_host", "psdns_launch_count", "psdns_kernel_timing",
     "psdns_kernel_time_ms", "psdns_destroy", "psdns_last_error",
+    "psdns_history_bytes", "psdns_get_history", "psdns_set_history",
 ]
 
 
@@ -67,6 +68,12 @@ def load_library():
     lib.psdns_kernel_timing.argtypes = [vp, C.c_char_p, ci]
     lib.psdns_kernel_time_ms.restype = ci
     lib.psdns_kernel_time_ms.argtypes = [vp, C.POINTER(cd), C.POINTER(C.c_longlong)]
+    lib.psdns_history_bytes.restype = C.c_size_t
+    lib.psdns_history_bytes.argtypes = [vp]
+    lib.psdns_get_history.restype = ci
+    lib.psdns_get_history.argtypes = [vp, vp, C.c_size_t]
+    lib.psdns_set_history.restype = ci
+    lib.psdns_set_history.argtypes = [vp, vp, C.c_size_t]
     lib.psdns_destroy.restype = ci
     lib.psdns_destroy.argtypes = [vp]
     lib.psdns_last_error.restype = C.c_char_p
@@ -166,6 +173,16 @@ class Solver:
         pi = [C.c_void_p(t.data_ptr()) if t is not None else None for t in (list(h_in) + [None] * 4)[:4]]
         po = [C.c_void_p(t.data_ptr()) if t is not None else None for t in (list(h_out) + [None] * 4)[:4]]
         self._check(self.lib.psdns_run_host(self.handle, space, nsteps, *pi, *po))
+
+    def get_history(self):
+        """Opaque device blob with the hidden state of the time integration (exact restart)."""
+        n = int(self.lib.psdns_history_bytes(self.handle))
+        blob = self.torch.empty(n, dtype=self.torch.uint8, device=self.device)
+        self._check(self.lib.psdns_get_history(self.handle, _ptr(blob), n))
+        return blob
+
+    def set_history(self, blob):
+        self._check(self.lib.psdns_set_history(self.handle, _ptr(blob), blob.numel()))
 
     def launch_count(self):
         return int(self.lib.psdns_launch_count(self.handle))

@@ -847,6 +847,59 @@ int psdns_transform_roundtrip(psdns_handle *h, int start_space, const void *d_in
     return PSDNS_OK;
 }
 
+// hidden-state blob: theta | omega_z | D phi | N_omega | N_w | S_phi | (ab[2], counter) - each piece 256-byte aligned
+namespace {
+struct HistPiece { size_t off, bytes; };
+int hist_pieces(const psdns_handle *h, HistPiece *pc) {
+    const Dims &d = h->d;
+    const Layout &L = h->L;
+    int n = 0;
+    pc[n++] = {L.state[4], d.s_ret * sizeof(cplx)};
+    pc[n++] = {L.xom, d.s_ret * sizeof(cplx)};
+    pc[n++] = {L.derived[0], d.s_low * sizeof(cplx)};
+    for (int i = 0; i < 3; ++i) pc[n++] = {L.hist[i], d.s_low * sizeof(cplx)};
+    pc[n++] = {L.small, 64};
+    return n;
+}
+}  // namespace
+
+size_t psdns_history_bytes(const psdns_handle *h) {
+    if (!h) return 0;
+    HistPiece pc[8];
+    const int n = hist_pieces(h, pc);
+    size_t tot = 0;
+    for (int i = 0; i < n; ++i) tot += align_up(pc[i].bytes);
+    return tot;
+}
+
+int psdns_get_history(psdns_handle *h, void *d_blob, size_t bytes) {
+    if (!h) return PSDNS_EINVAL;
+    if (!d_blob || bytes != psdns_history_bytes(h)) { h->err = "psdns_get_history: null blob or size mismatch"; return PSDNS_EINVAL; }
+    if (!h->has_state) { h->err = "psdns_get_history: no state set"; return PSDNS_ESTATE; }
+    HistPiece pc[8];
+    const int n = hist_pieces(h, pc);
+    size_t o = 0;
+    for (int i = 0; i < n; ++i) {
+        CUDA_TRY(h, cudaMemcpyAsync((char *)d_blob + o, h->ws + pc[i].off, pc[i].bytes, cudaMemcpyDeviceToDevice, h->st));
+        o += align_up(pc[i].bytes);
+    }
+    return PSDNS_OK;
+}
+
+int psdns_set_history(psdns_handle *h, const void *d_blob, size_t bytes) {
+    if (!h) return PSDNS_EINVAL;
+    if (!d_blob || bytes != psdns_history_bytes(h)) { h->err = "psdns_set_history: null blob or size mismatch"; return PSDNS_EINVAL; }
+    if (!h->has_state) { h->err = "psdns_set_history: call psdns_set_state first"; return PSDNS_ESTATE; }
+    HistPiece pc[8];
+    const int n = hist_pieces(h, pc);
+    size_t o = 0;
+    for (int i = 0; i < n; ++i) {
+        CUDA_TRY(h, cudaMemcpyAsync(h->ws + pc[i].off, (const char *)d_blob + o, pc[i].bytes, cudaMemcpyDeviceToDevice, h->st));
+        o += align_up(pc[i].bytes);
+    }
+    return PSDNS_OK;
+}
+
 int psdns_run_host(psdns_handle *h, int space, int nsteps, const void *h_in_u, const void *h_in_v, const void *h_in_w,
                    const void *h_in_phi, void *h_out_u, void *h_out_v, void *h_out_w, void *h_out_phi) {
     if (!h) return PSDNS_EINVAL;
