@@ -445,7 +445,7 @@ struct RhsElimArgs {
 constexpr int RHS_COLS = 32;   // columns per CTA of k_rhs_elim (blockDim = 32 * number of chains)
 
 #ifndef RHS_MINB
-#define RHS_MINB 3
+#define RHS_MINB 4
 #endif
 __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
     const ColGeom &g = a.g;
