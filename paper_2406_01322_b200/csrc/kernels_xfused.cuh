@@ -195,6 +195,15 @@ __device__ __forceinline__ void nl_store(cplx *__restrict__ s, int t, const doub
     s[xidx(2 * t + 1, Q)] = make_double2(o00 - o10, o01 - o11);
 }
 
+// the four products of output field q at the four points of a row pair (q is a compile-time constant after unrolling)
+template <bool PHASE>
+__device__ __forceinline__ void nl_quad(int q, const double (&p00)[8], const double (&p01)[8], const double (&p10)[8],
+                                        const double (&p11)[8], double cs, double &o00, double &o01, double &o10, double &o11) {
+#define NLQ(Q) case Q: o00 = nl_out<Q, PHASE>(p00, cs); o01 = nl_out<Q, PHASE>(p01, cs); o10 = nl_out<Q, PHASE>(p10, cs); o11 = nl_out<Q, PHASE>(p11, cs); break;
+    switch (q) { NLQ(0) NLQ(1) NLQ(2) NLQ(3) NLQ(4) NLQ(5) default: NLQ(6) }
+#undef NLQ
+}
+
 struct XFArgs {
     const cplx *in[6];      // Y arrays: u v w [phi phy phz]
     cplx *out[8];           // Y arrays: Txx-Tzz Txy Txz Tyy-Tzz Tyz [Q C]
@@ -380,6 +389,231 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
             }
         }
         __syncthreads();
+    }
+}
+
+// ====================================================================================================
+// Warp-per-field form of the fused x kernel (the one psdns_step launches).
+//
+// Every stage except the pointwise one is independent per field, so a WARP owns one field: its 32 lanes are
+// the (up to) 32 butterflies of a pass.  Consequences (profiles/r1e: the field-interleaved form above ran its
+// FP64 pipe 48 % and its shared-memory pipe 73 % busy, in lockstep between eight CTA-wide barriers per line):
+//   * stages A -> B and D -> E -> F need only __syncwarp: three CTA-wide barriers per line (stage ready,
+//     before and after the pointwise stage), so the field warps drift apart and FP64 work of one overlaps
+//     the shared-memory traffic of another;
+//   * 7 fields = 7 working warps: the eighth field slot costs no work any more (it was 1/8 of all lanes); the
+//     eighth warp is a service warp (derives the i kx phi row, issues the TMA copies of the next line);
+//   * the j = 1 twiddles of the inner radix-R2 passes move into the pointwise stage (a thread there owns
+//     rows 2t, 2t+1 of all fields and needs ONE loop-invariant twiddle), so the inner passes have none and
+//     no lane diverges.
+// Tile index: the field slot is XOR-swizzled with row bits chosen so that a quarter-warp is conflict free in
+// every stage: 8 consecutive rows of one field (A, E: bits 0-2), 4 blocks x 2 classes of the inner pass
+// (B, D: bit 0 and the two bits above log2(2 R2)), 8 consecutive row pairs (pointwise: bits 1-3).
+// ====================================================================================================
+template <int LOG2LS>
+__device__ __forceinline__ int widx(int row, int f) {
+    const int sw = (row & 7) ^ ((row >> 3) & 1) ^ (((row >> LOG2LS) & 3) << 1);
+    return row * TILE_LINES + ((f ^ sw) & (TILE_LINES - 1));
+}
+__host__ __device__ constexpr int ilog2(int x) { return x <= 1 ? 0 : 1 + ilog2(x / 2); }
+
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+constexpr int XFW_THREADS = 256;   // 8 warps: one per field slot
+
+template <int L, bool PHASE>
+__global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 512 ? 2 : 3))) k_xfusedw(const __grid_constant__ XFArgs a,
+                                                                             const cplx *__restrict__ twx) {
+    constexpr int H = L / 2;
+    constexpr int R1 = XPlan<H>::R1, R2 = XPlan<H>::R2;
+    constexpr int NT = XFW_THREADS;
+    constexpr int S1 = H / R1;              // butterflies per field of pass R1 (<= 32)
+    constexpr int LS = 2 * R2;              // sub-length of the inner pass
+    constexpr int NB2 = H / R2;             // butterflies per field of the inner pass (<= 32)
+    constexpr int LG = ilog2(LS) < 3 ? 3 : ilog2(LS);
+    constexpr int NIN = PHASE ? 7 : 3, NOUT = PHASE ? 7 : 5;
+    constexpr int NTMA = PHASE ? 6 : 3;
+    constexpr int NST = xf_nstage<PHASE>();
+    static_assert(R1 * R2 * 2 == H && S1 <= 32 && NB2 <= 32, "plan");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx *s = reinterpret_cast<cplx *>(smem_raw);
+    cplx *stage = s + H * TILE_LINES;
+    const int kxp = a.kxp, nkx = a.nkx;
+    const int spitch = xf_spitch(nkx);
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)NST * spitch);
+    unsigned long long *bar_free = bar + 1;         // stage consumed by every input-field warp
+    const int tid = threadIdx.x, f = tid >> 5, lane = tid & 31;
+    const bool service = (f == TILE_LINES - 1);     // eighth warp
+    cplx *outf = a.out[f < NOUT ? f : 0];
+    const double sc = 0.5 / L;
+    const unsigned row_bytes = (unsigned)(nkx * sizeof(cplx));
+    auto issue = [&](int line) {
+        mbar_expect_tx(bar, row_bytes * NTMA);
+#pragma unroll
+        for (int q = 0; q < NTMA; ++q) bulk_g2s(stage + (size_t)q * spitch, a.in[q] + (size_t)line * kxp, row_bytes, bar);
+    };
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        mbar_init(bar_free, NIN);
+        if ((int)blockIdx.x < a.nlines) issue(blockIdx.x);
+    }
+    __syncthreads();
+    const int j = lane;                             // butterfly of passes A, E, F
+    const bool itemA = j < S1;
+    cplx wj = twx[itemA ? j : 0];                   // w_L^j
+    // pointwise-stage twiddle of this thread's row pair: w_LS^(t mod R2) = w_L^((t mod R2) L / LS)
+    cplx wc = twx[(tid % R2) * (L / LS)];
+    unsigned parity = 0;
+    // field -> staged row: u v w phi phx phy phz  <-  0 1 2 3 6 4 5
+    const int srow = !PHASE ? (f < NST ? f : 0) : (f < 4 ? f : (f == 4 ? 6 : (f < NIN ? f - 1 : 0)));
+    const cplx *sf = stage + (size_t)srow * spitch;
+    for (int line = blockIdx.x; line < a.nlines; line += gridDim.x) {
+        const size_t base = (size_t)line * kxp;
+        mbar_wait(bar, parity);
+        if constexpr (PHASE) {
+            if (service) {                          // row a1: phx^ = i kx phi^
+                for (int k = lane; k < nkx; k += 32) {
+                    const cplx p = stage[3 * spitch + k];
+                    const double kk = a.kxf * (double)k;
+                    stage[6 * spitch + k] = make_double2(-kk * p.y, kk * p.x);
+                }
+            }
+            __syncthreads();
+        }
+        asm volatile("" : "+d"(wj.x), "+d"(wj.y), "+d"(wc.x), "+d"(wc.y));
+        if (f < NIN) {
+            // ---- A: pre-twiddle from the staged rows + DIF pass R1 (inverse transform, sign +) ----
+            if (itemA) {
+                const int jj = opaque(j);
+                cplx v[R1];
+#pragma unroll
+                for (int m = 0; m < R1; ++m) {
+                    if (m && (m & 3) == 0) asm volatile("" ::: "memory");
+                    const int k = jj + S1 * m, kb = H - k;
+                    cplx xa = make_double2(0.0, 0.0), xb = xa;
+                    if (k < nkx) xa = sf[k];
+                    if (kb < nkx) xb = sf[kb];
+                    if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
+                    const cplx w = m ? cmul(wj, make_double2(wc_re<2 * R1>(m), wc_im<2 * R1>(m))) : wj;
+                    const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
+                    v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
+                }
+                RegFFT<R1, +1>::run(v);
+                TwPow<R1> tp;
+                tp.init(cmul(wj, wj));
+                s[widx<LG>(jj, f)] = v[0];
+                tp.each([&](int q, cplx wq) { s[widx<LG>(jj + S1 * q, f)] = cmultw<+1>(v[q], wq); });
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_free);   // this field's staged row is consumed
+            // ---- B: DIF pass R2, no twiddles (they are applied in the pointwise stage) ----
+            if constexpr (R2 > 1) {
+                if (lane < NB2) {
+                    const int b = opaque(lane), row0 = (b >> 1) * LS + (b & 1);
+                    cplx v[R2];
+#pragma unroll
+                    for (int m = 0; m < R2; ++m) v[m] = s[widx<LG>(row0 + 2 * m, f)];
+                    RegFFT<R2, +1>::run(v);
+#pragma unroll
+                    for (int q = 0; q < R2; ++q) s[widx<LG>(row0 + 2 * q, f)] = v[q];
+                }
+            }
+        } else if (service) {
+            if (lane == 0) {                        // all input warps are done with the stage: prefetch the next line
+                mbar_wait(bar_free, parity);
+                if (line + (int)gridDim.x < a.nlines) {
+                    fence_proxy_async();
+                    issue(line + gridDim.x);
+                }
+            }
+        }
+        parity ^= 1;
+        __syncthreads();
+        // ---- C: last DIF radix 2 (with the inner pass's twiddle), pointwise products, first DIT radix 2 ----
+        for (int t = opaque(tid); t < H / 2; t += NT) {
+            double p00[8], p01[8], p10[8], p11[8];
+#pragma unroll
+            for (int q = 0; q < NIN; ++q) {
+                const cplx p = s[widx<LG>(2 * t, q)];
+                cplx m = s[widx<LG>(2 * t + 1, q)];
+                if (R2 > 1) m = cmultw<+1>(m, wc);
+                p00[q] = p.x + m.x; p01[q] = p.y + m.y;
+                p10[q] = p.x - m.x; p11[q] = p.y - m.y;
+            }
+#pragma unroll
+            for (int q = 0; q < NOUT; ++q) {
+                double o00, o01, o10, o11;
+                nl_quad<PHASE>(q, p00, p01, p10, p11, a.cs, o00, o01, o10, o11);
+                s[widx<LG>(2 * t, q)] = make_double2(o00 + o10, o01 + o11);
+                cplx m = make_double2(o00 - o10, o01 - o11);
+                if (R2 > 1) m = cmultw<-1>(m, wc);
+                s[widx<LG>(2 * t + 1, q)] = m;
+            }
+        }
+        __syncthreads();
+        if (f < NOUT) {
+            // ---- D: DIT pass R2 (forward transform, sign -), no twiddles ----
+            if constexpr (R2 > 1) {
+                if (lane < NB2) {
+                    const int b = opaque(lane), row0 = (b >> 1) * LS + (b & 1);
+                    cplx v[R2];
+#pragma unroll
+                    for (int m = 0; m < R2; ++m) v[m] = s[widx<LG>(row0 + 2 * m, f)];
+                    RegFFT<R2, -1>::run(v);
+#pragma unroll
+                    for (int q = 0; q < R2; ++q) s[widx<LG>(row0 + 2 * q, f)] = v[q];
+                }
+                __syncwarp();
+            }
+            // ---- E: DIT pass R1; results stay in registers, only the rows a partner needs go to the tile ----
+            cplx v[R1];
+            if (itemA) {
+                const int jj = opaque(j);
+                TwPow<R1> tp;
+                tp.init(cmul(wj, wj));
+                v[0] = s[widx<LG>(jj, f)];
+                tp.each([&](int m, cplx wq) { v[m] = cmultw<-1>(s[widx<LG>(jj + S1 * m, f)], wq); });
+                RegFFT<R1, -1>::run(v);
+#pragma unroll
+                for (int q = 0; q < R1; ++q) {
+                    const int r = jj + S1 * q;
+                    if (r > H - nkx) s[widx<LG>(r, f)] = v[q];
+                }
+            }
+            __syncwarp();
+            // ---- F: post-twiddle of row k against the partner row H - k, truncated store ----
+            if (itemA) {
+                const int jj = opaque(j);
+                cplx *o = outf + base;
+#pragma unroll
+                for (int q0 = 0; q0 < R1; q0 += 4) {
+                    if (S1 * q0 < kxp) {
+                        cplx zb[4];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const int k = jj + S1 * (q0 + i);
+                            zb[i] = s[widx<LG>((H - k) & (H - 1), f)];
+                        }
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const int q = q0 + i, k = jj + S1 * q;
+                            if (q < R1 && k < nkx) {
+                                const cplx za = v[q];
+                                const cplx zp = k ? zb[i] : za;
+                                const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
+                                const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
+                                stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
+                            } else if (q < R1 && k < kxp) {
+                                stg(o + k, make_double2(0.0, 0.0));
+                            }
+                        }
+                    }
+                }
+            }
+            __syncwarp();     // this warp's F reads are done before its next stage A overwrites the field
+        }
     }
 }
 
