@@ -567,8 +567,10 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 512 
                 }
                 __syncwarp();
             }
-            // ---- E: DIT pass R1; results stay in registers, only the rows a partner needs go to the tile ----
+            // ---- E: DIT pass R1; the results stay in registers ----
             cplx v[R1];
+#pragma unroll
+            for (int q = 0; q < R1; ++q) v[q] = make_double2(0.0, 0.0);
             if (itemA) {
                 const int jj = opaque(j);
                 TwPow<R1> tp;
@@ -576,38 +578,30 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 512 
                 v[0] = s[widx<LG>(jj, f)];
                 tp.each([&](int m, cplx wq) { v[m] = cmultw<-1>(s[widx<LG>(jj + S1 * m, f)], wq); });
                 RegFFT<R1, -1>::run(v);
-#pragma unroll
-                for (int q = 0; q < R1; ++q) {
-                    const int r = jj + S1 * q;
-                    if (r > H - nkx) s[widx<LG>(r, f)] = v[q];
-                }
             }
-            __syncwarp();
-            // ---- F: post-twiddle of row k against the partner row H - k, truncated store ----
-            if (itemA) {
-                const int jj = opaque(j);
+            // ---- F: post-twiddle of row k = j + S1 q against its partner row H - k, truncated store.  The partner
+            // is output R1 - 1 - q of butterfly S1 - j (output R1 - q of butterfly 0 for j = 0): a register of another
+            // lane of THIS warp, fetched by shuffle - no shared-memory exchange and no barrier.
+            {
+                const int src = (S1 - j) & (S1 - 1);
                 cplx *o = outf + base;
 #pragma unroll
-                for (int q0 = 0; q0 < R1; q0 += 4) {
-                    if (S1 * q0 < kxp) {
-                        cplx zb[4];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const int k = jj + S1 * (q0 + i);
-                            zb[i] = s[widx<LG>((H - k) & (H - 1), f)];
-                        }
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const int q = q0 + i, k = jj + S1 * q;
-                            if (q < R1 && k < nkx) {
-                                const cplx za = v[q];
-                                const cplx zp = k ? zb[i] : za;
-                                const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
-                                const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
-                                stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
-                            } else if (q < R1 && k < kxp) {
-                                stg(o + k, make_double2(0.0, 0.0));
-                            }
+                for (int q = 0; q < R1; ++q) {
+                    if (S1 * q < kxp) {                        // CTA-uniform: no row of this q is kept otherwise
+                        const cplx mine = (j == 0) ? v[(R1 - q) & (R1 - 1)] : v[R1 - 1 - q];
+                        cplx zp;
+                        zp.x = __shfl_sync(0xffffffffu, mine.x, src);
+                        zp.y = __shfl_sync(0xffffffffu, mine.y, src);
+                        const int k = j + S1 * q;
+                        if (itemA && k < nkx) {
+                            const cplx za = v[q];
+                            if (k == 0) zp = za;               // k = 0 is its own partner
+                            const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
+                            const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
+                            // X_k = (S - i w D) / (2 L)
+                            stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
+                        } else if (itemA && k < kxp) {
+                            stg(o + k, make_double2(0.0, 0.0));
                         }
                     }
                 }
