@@ -79,7 +79,6 @@ struct psdns_handle {
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tevents;
     int nf_in, nf_out;
     bool use_xfused;
-    bool xf_warp;               // warp-per-field form of the fused x kernel (default; PSDNS_XF_OLD=1: field-interleaved form)
     int xf_occ, n_sm;
     int occ_z[2], occ_y[2];     // resident CTAs per SM of the persistent z / y passes, [fwd]
 
@@ -317,20 +316,12 @@ cudaError_t setup_attrs(psdns_handle *h) {
     {                                                                                                        \
         const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                               \
         int occ = 0;                                                                                         \
-        if (h->xf_warp) {                                                                                    \
-            if (h->p.phase_field) {                                                                          \
-                CU0(set_smem(k_xfusedw<LL, true>, sm));                                                      \
-                CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, true>, XFW_THREADS, sm)); \
-            } else {                                                                                         \
-                CU0(set_smem(k_xfusedw<LL, false>, sm));                                                     \
-                CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, false>, XFW_THREADS, sm)); \
-            }                                                                                                \
-        } else if (h->p.phase_field) {                                                                       \
-            CU0(set_smem(k_xfused<LL, true>, sm));                                                           \
-            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfused<LL, true>, xf_threads<LL>(), sm)); \
+        if (h->p.phase_field) {                                                                              \
+            CU0(set_smem(k_xfusedw<LL, true>, sm));                                                          \
+            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, true>, XFW_THREADS, sm));  \
         } else {                                                                                             \
-            CU0(set_smem(k_xfused<LL, false>, sm));                                                          \
-            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfused<LL, false>, xf_threads<LL>(), sm)); \
+            CU0(set_smem(k_xfusedw<LL, false>, sm));                                                         \
+            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, false>, XFW_THREADS, sm)); \
         }                                                                                                    \
         h->xf_occ = occ;                                                                                     \
     }
@@ -350,11 +341,8 @@ cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
 #define XF(LL)                                                                                               \
     {                                                                                                        \
         const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                               \
-        if (h->xf_warp) {                                                                                    \
-            if (h->p.phase_field) k_xfusedw<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);              \
-            else k_xfusedw<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                              \
-        } else if (h->p.phase_field) k_xfused<LL, true><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);       \
-        else k_xfused<LL, false><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);                              \
+        if (h->p.phase_field) k_xfusedw<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                  \
+        else k_xfusedw<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                                  \
     }
     DISPATCH_L(h->d.nx, XF)
 #undef XF
@@ -684,7 +672,6 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->has_state = false; h->graph = nullptr; h->graph_ready = false;
     h->use_graph = std::getenv("PSDNS_NO_GRAPH") == nullptr;
     h->use_xfused = std::getenv("PSDNS_NO_XFUSE") == nullptr;
-    h->xf_warp = std::getenv("PSDNS_XF_OLD") == nullptr;
     h->launches = 0; h->per_step = 0; h->timed_class = -1;
     const bool phase = params->phase_field != 0;
     const bool visc = phase && params->visc_ratio != 1.0;
