@@ -21,6 +21,7 @@ struct ColGeom {
     int N;       // nz - 1
     int nkz;     // retained Chebyshev planes (K + 1)
     double kxf, kyf;  // 2 pi / Lx, 2 pi / Ly
+    int pf, pf_rhs;   // L2 prefetch distances in rows
 };
 
 __device__ __forceinline__ void col_wavenumbers(const ColGeom &g, int col, double &kx, double &ky) {
@@ -41,14 +42,8 @@ __device__ __forceinline__ void pf_l2(const void *p) { asm volatile("prefetch.gl
 // Distances measured on B200 at 1024x512x513: the substitution / second-elimination / finish kernels keep every column
 // resident at once, so rows x arrays x 1.9 MB of prefetched data must stay well inside the 126 MB L2 (6 rows ahead thrashed
 // it: +2 GB of re-reads per kernel); k_rhs_elim has 12 % of the columns resident and likes a longer distance.
-#ifndef PF_ROWS_N
-#define PF_ROWS_N 2
-#endif
-#ifndef PF_ROWS_RHS_N
-#define PF_ROWS_RHS_N 4
-#endif
-constexpr int PF_ROWS = PF_ROWS_N;
-constexpr int PF_ROWS_RHS = PF_ROWS_RHS_N;
+// The distance is a run-time number in ColGeom (pf for the sweeps that keep every column resident, pf_rhs for
+// k_rhs_elim), set by the host (psdns.cu geom()): 2 / 4 rows.
 
 // ---- layout conversion ---------------------------------------------------------------------
 // Both sides are cplx [n][rows][pitch]; a side is described by (rows, pitch, jpos, nkx):
@@ -503,7 +498,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
         for (int n = N; n >= 0; --n) {
             const RowIn r = nx;
             if (n > 0) nx = load(n - 1);
-            const int np = n - PF_ROWS_RHS;
+            const int np = n - g.pf_rhs;
             if (np >= 0 && c == 0) {
                 pf_l2(a.om + col + np * st); pf_l2(a.th + col + np * st);
                 if (np < nkz) {
@@ -581,7 +576,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
         for (int n = N; n >= 0; --n) {
             const RowIn r = nx;
             if (n > 0) nx = load(n - 1);
-            const int np = n - PF_ROWS_RHS;
+            const int np = n - g.pf_rhs;
             if (np >= 0) {
                 pf_l2(x + np * st);
                 if (np < nkz) { pf_l2(qq + np * st); pf_l2(cc + np * st); pf_l2(hist + np * st); }
@@ -640,7 +635,7 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
         cplx um2 = x0[0], um1 = x0[st], vm2 = x1[0], vm1 = x1[st];
 #pragma unroll 4
         for (int k = 2; k <= N; ++k) {
-            const int kp = k + PF_ROWS;
+            const int kp = k + g.pf;
             if (kp <= N) { pf_l2(x0 + kp * st); pf_l2(x1 + kp * st); pf_l2(dinv + kp * st); }
             const double ak = -sigma * helm_p(k), di = dinv[k * st];
             const cplx u = cscale(cfma(-ak, um2, x0[k * st]), di);
@@ -665,7 +660,7 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
     }
 #pragma unroll 4
     for (int k = 2; k <= N; ++k) {
-        const int kp = k + PF_ROWS;
+        const int kp = k + g.pf;
         if (kp <= N) {
             pf_l2(x + kp * st); pf_l2(dinv + kp * st);
             if (corr) { pf_l2(a.wh + kp * st + col); pf_l2(a.thh + kp * st + col); pf_l2(a.th + kp * st + col); }
@@ -717,7 +712,7 @@ __global__ void __launch_bounds__(NT_COL, 5) k_elim2(const __grid_constant__ Eli
         pv.init();
 #pragma unroll 4
         for (int k = N; k >= 2; --k) {
-            const int kp = k - PF_ROWS;
+            const int kp = k - g.pf;
             if (kp >= 2) pf_l2(in + (kp - 2) * st);
             out[k * st] = el.row<false, true>(k, N, k2, in[(k - 2) * st], pv.step(k, N, k2));
         }
@@ -736,7 +731,7 @@ __global__ void __launch_bounds__(NT_COL, 5) k_elim2(const __grid_constant__ Eli
         pv.init();
 #pragma unroll 4
         for (int k = N; k >= 2; --k) {
-            const int kp = k - PF_ROWS;
+            const int kp = k - g.pf;
             if (kp >= 2) pf_l2(x + (kp - 2) * st);
             const cplx fm2 = x[(k - 2) * st];
             x[k * st] = el.row<true, false>(k, N, sigma, fm2, pv.step(k, N, sigma));
@@ -791,7 +786,7 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
     cW.init(); cP.init();
     for (int n = g.N; n >= 0; --n) {
         const size_t o = n * st + col;
-        const int np = n - PF_ROWS;
+        const int np = n - g.pf;
         if (np >= 0) {
             const size_t op = np * st + col;
             pf_l2(a.w + op); pf_l2(a.om + op);

@@ -79,6 +79,8 @@ struct psdns_handle {
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tevents;
     int nf_in, nf_out;
     bool use_xfused;
+    bool xf_warp;               // fused x kernel: warp-per-field form (nx = 1024: 32 butterflies per pass = one per lane) or
+                                // thread = (butterfly, field) form (smaller nx, where a warp per field would leave lanes idle)
     int xf_occ, n_sm;
     int occ_z[2], occ_y[2];     // resident CTAs per SM of the persistent z / y passes, [fwd]
 
@@ -191,6 +193,12 @@ ColGeom geom(const psdns_handle *h) {
     g.ncols = (int)d.ncols; g.kxp = d.kxp; g.nkx = d.nkx; g.nky = d.nky; g.jpos = d.jpos;
     g.N = d.N; g.nkz = d.nkz;
     g.kxf = 2.0 * M_PI / h->g.lx; g.kyf = 2.0 * M_PI / h->g.ly;
+    // L2 prefetch distances in rows (kernels_spectral.cuh).  Measured on B200: 2 (4 for k_rhs_elim) is best at 117 k
+    // columns, where 6 thrashed the L2, and longer distances do not help the latency-bound small grids either
+    // (256x256x257: solve 0.82 ms at 2 rows, 0.84 at 12, 0.90 at 24).
+    static const char *e_pf = std::getenv("PSDNS_PF"), *e_pfr = std::getenv("PSDNS_PF_RHS");
+    g.pf = e_pf ? std::atoi(e_pf) : 2;
+    g.pf_rhs = e_pfr ? std::atoi(e_pfr) : 4;
     return g;
 }
 
@@ -316,12 +324,20 @@ cudaError_t setup_attrs(psdns_handle *h) {
     {                                                                                                        \
         const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                               \
         int occ = 0;                                                                                         \
-        if (h->p.phase_field) {                                                                              \
-            CU0(set_smem(k_xfusedw<LL, true>, sm));                                                          \
-            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, true>, XFW_THREADS, sm));  \
+        if (h->xf_warp) {                                                                                    \
+            if (h->p.phase_field) {                                                                          \
+                CU0(set_smem(k_xfusedw<LL, true>, sm));                                                      \
+                CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, true>, XFW_THREADS, sm)); \
+            } else {                                                                                         \
+                CU0(set_smem(k_xfusedw<LL, false>, sm));                                                     \
+                CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, false>, XFW_THREADS, sm)); \
+            }                                                                                                \
+        } else if (h->p.phase_field) {                                                                       \
+            CU0(set_smem(k_xfused<LL, true>, sm));                                                           \
+            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfused<LL, true>, xf_threads<LL>(), sm)); \
         } else {                                                                                             \
-            CU0(set_smem(k_xfusedw<LL, false>, sm));                                                         \
-            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, false>, XFW_THREADS, sm)); \
+            CU0(set_smem(k_xfused<LL, false>, sm));                                                          \
+            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfused<LL, false>, xf_threads<LL>(), sm)); \
         }                                                                                                    \
         h->xf_occ = occ;                                                                                     \
     }
@@ -341,8 +357,11 @@ cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
 #define XF(LL)                                                                                               \
     {                                                                                                        \
         const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                               \
-        if (h->p.phase_field) k_xfusedw<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                  \
-        else k_xfusedw<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                                  \
+        if (h->xf_warp) {                                                                                    \
+            if (h->p.phase_field) k_xfusedw<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);              \
+            else k_xfusedw<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                              \
+        } else if (h->p.phase_field) k_xfused<LL, true><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);       \
+        else k_xfused<LL, false><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);                              \
     }
     DISPATCH_L(h->d.nx, XF)
 #undef XF
@@ -672,6 +691,10 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->has_state = false; h->graph = nullptr; h->graph_ready = false;
     h->use_graph = std::getenv("PSDNS_NO_GRAPH") == nullptr;
     h->use_xfused = std::getenv("PSDNS_NO_XFUSE") == nullptr;
+    {   // measured on B200: warp-per-field 8.2 vs 10.6 ms at nx = 1024, but 1.89 vs 1.27 ms at nx = 512 and 1.11 vs 0.65 ms at 256
+        const char *e = std::getenv("PSDNS_XF_WARP");
+        h->xf_warp = e ? std::atoi(e) != 0 : grid->nx >= 1024;
+    }
     h->launches = 0; h->per_step = 0; h->timed_class = -1;
     const bool phase = params->phase_field != 0;
     const bool visc = phase && params->visc_ratio != 1.0;
