@@ -619,6 +619,12 @@ struct SubstArgs {
     cplx *th;
 };
 
+// The sweeps work in place, so the compiler cannot move the load of row k + 1 above the store of row k (same
+// pointer, run-time stride): every row then costs a full memory latency, which dominates on small grids (few
+// columns, little parallelism).  The loops below therefore load a GROUP of LOOKAHEAD rows into registers before the
+// previous group's results are stored (different rows: no hazard).
+constexpr int LOOKAHEAD = 4;
+
 __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstArgs a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
@@ -628,20 +634,43 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
     col_wavenumbers(g, col, kx, ky);
     const size_t st = g.ncols;
     const int N = g.N;
+    constexpr int G = LOOKAHEAD;
     if (a.pair01 && blockIdx.y == 0) {      // omega_z and theta: same recurrence coefficients, two right-hand sides
         const double sigma = kx * kx + ky * ky + a.shift[0];
         cplx *x0 = a.x[0] + col, *x1 = a.x[1] + col;
         const double *__restrict__ dinv = a.dinv[0] + col;
         cplx um2 = x0[0], um1 = x0[st], vm2 = x1[0], vm1 = x1[st];
-#pragma unroll 4
-        for (int k = 2; k <= N; ++k) {
-            const int kp = k + g.pf;
-            if (kp <= N) { pf_l2(x0 + kp * st); pf_l2(x1 + kp * st); pf_l2(dinv + kp * st); }
-            const double ak = -sigma * helm_p(k), di = dinv[k * st];
-            const cplx u = cscale(cfma(-ak, um2, x0[k * st]), di);
-            const cplx v = cscale(cfma(-ak, vm2, x1[k * st]), di);
-            um2 = um1; um1 = u; vm2 = vm1; vm1 = v;
-            x0[k * st] = u; x1[k * st] = v;
+        cplx q0[G], q1[G];
+        double dq[G];
+        auto load = [&](int k0, cplx (&p0)[G], cplx (&p1)[G], double (&d)[G]) {
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const int k = k0 + i;
+                if (k <= N) { p0[i] = x0[k * st]; p1[i] = x1[k * st]; d[i] = dinv[k * st]; }
+            }
+        };
+        load(2, q0, q1, dq);
+        for (int k0 = 2; k0 <= N; k0 += G) {
+            cplx n0[G], n1[G];
+            double dn[G];
+            load(k0 + G, n0, n1, dn);
+            const int kp = k0 + 2 * G + g.pf;
+#pragma unroll
+            for (int i = 0; i < G; ++i)
+                if (kp + i <= N) { pf_l2(x0 + (kp + i) * st); pf_l2(x1 + (kp + i) * st); pf_l2(dinv + (kp + i) * st); }
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const int k = k0 + i;
+                if (k <= N) {
+                    const double ak = -sigma * helm_p(k);
+                    const cplx u = cscale(cfma(-ak, um2, q0[i]), dq[i]);
+                    const cplx v = cscale(cfma(-ak, vm2, q1[i]), dq[i]);
+                    um2 = um1; um1 = u; vm2 = vm1; vm1 = v;
+                    x0[k * st] = u; x1[k * st] = v;
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < G; ++i) { q0[i] = n0[i]; q1[i] = n1[i]; dq[i] = dn[i]; }
         }
         return;
     }
@@ -658,24 +687,48 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
         a.th[col] = cfma(a.thh[col], Ae, a.th[col]);
         a.th[st + col] = cfma(a.thh[st + col], Ao, a.th[st + col]);
     }
-#pragma unroll 4
-    for (int k = 2; k <= N; ++k) {
-        const int kp = k + g.pf;
-        if (kp <= N) {
-            pf_l2(x + kp * st); pf_l2(dinv + kp * st);
-            if (corr) { pf_l2(a.wh + kp * st + col); pf_l2(a.thh + kp * st + col); pf_l2(a.th + kp * st + col); }
+    struct Row { cplx x, th; double di, wh, thh; };
+    auto load = [&](int k0, Row (&r)[G]) {
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            const int k = k0 + i;
+            if (k <= N) {
+                r[i].x = x[k * st]; r[i].di = dinv[k * st];
+                if (corr) { const size_t o = k * st + col; r[i].wh = a.wh[o]; r[i].thh = a.thh[o]; r[i].th = a.th[o]; }
+            }
         }
-        const double ak = -sigma * helm_p(k);
-        const cplx u = cscale(cfma(-ak, um2, x[k * st]), dinv[k * st]);
-        um2 = um1; um1 = u;
-        if (corr) {
-            const size_t o = k * st + col;
-            const cplx A = (k & 1) ? Ao : Ae;
-            x[k * st] = cfma(a.wh[o], A, u);
-            a.th[o] = cfma(a.thh[o], A, a.th[o]);
-        } else {
-            x[k * st] = u;
+    };
+    Row q[G];
+    load(2, q);
+    for (int k0 = 2; k0 <= N; k0 += G) {
+        Row nx[G];
+        load(k0 + G, nx);
+        const int kp = k0 + 2 * G + g.pf;
+#pragma unroll
+        for (int i = 0; i < G; ++i)
+            if (kp + i <= N) {
+                pf_l2(x + (kp + i) * st); pf_l2(dinv + (kp + i) * st);
+                if (corr) { pf_l2(a.wh + (kp + i) * st + col); pf_l2(a.thh + (kp + i) * st + col); pf_l2(a.th + (kp + i) * st + col); }
+            }
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            const int k = k0 + i;
+            if (k <= N) {
+                const double ak = -sigma * helm_p(k);
+                const cplx u = cscale(cfma(-ak, um2, q[i].x), q[i].di);
+                um2 = um1; um1 = u;
+                if (corr) {
+                    const size_t o = k * st + col;
+                    const cplx A = (k & 1) ? Ao : Ae;
+                    x[k * st] = cfma(q[i].wh, A, u);
+                    a.th[o] = cfma(q[i].thh, A, q[i].th);
+                } else {
+                    x[k * st] = u;
+                }
+            }
         }
+#pragma unroll
+        for (int i = 0; i < G; ++i) q[i] = nx[i];
     }
 }
 
@@ -693,7 +746,7 @@ struct Elim2Args {
     int phase;
 };
 
-__global__ void __launch_bounds__(NT_COL, 5) k_elim2(const __grid_constant__ Elim2Args a) {
+__global__ void __launch_bounds__(NT_COL, 3) k_elim2(const __grid_constant__ Elim2Args a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= g.ncols) return;
@@ -710,11 +763,26 @@ __global__ void __launch_bounds__(NT_COL, 5) k_elim2(const __grid_constant__ Eli
         cplx *__restrict__ out = a.w + col;
         PivotDown pv;
         pv.init();
-#pragma unroll 4
-        for (int k = N; k >= 2; --k) {
-            const int kp = k - g.pf;
-            if (kp >= 2) pf_l2(in + (kp - 2) * st);
-            out[k * st] = el.row<false, true>(k, N, k2, in[(k - 2) * st], pv.step(k, N, k2));
+        constexpr int G = LOOKAHEAD;
+        cplx q[G];
+        auto load = [&](int k0, cplx (&r)[G]) {          // rows k0, k0 - 1, .. (descending)
+#pragma unroll
+            for (int i = 0; i < G; ++i) if (k0 - i >= 2) r[i] = in[(k0 - i - 2) * st];
+        };
+        load(N, q);
+        for (int k0 = N; k0 >= 2; k0 -= G) {
+            cplx nx[G];
+            load(k0 - G, nx);
+            const int kp = k0 - 2 * G - g.pf;
+#pragma unroll
+            for (int i = 0; i < G; ++i) if (kp - i >= 2) pf_l2(in + (kp - i - 2) * st);
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const int k = k0 - i;
+                if (k >= 2) out[k * st] = el.row<false, true>(k, N, k2, q[i], pv.step(k, N, k2));
+            }
+#pragma unroll
+            for (int i = 0; i < G; ++i) q[i] = nx[i];
         }
         cplx u0, u1, de, dodd;
         el.finish<false>(k2, 0.0, 0.0, u0, u1);
@@ -729,12 +797,28 @@ __global__ void __launch_bounds__(NT_COL, 5) k_elim2(const __grid_constant__ Eli
         cplx *x = a.phi + col;
         PivotDown pv;
         pv.init();
-#pragma unroll 4
-        for (int k = N; k >= 2; --k) {
-            const int kp = k - g.pf;
-            if (kp >= 2) pf_l2(x + (kp - 2) * st);
-            const cplx fm2 = x[(k - 2) * st];
-            x[k * st] = el.row<true, false>(k, N, sigma, fm2, pv.step(k, N, sigma));
+        // in place: row k - 2 is read (as the right-hand side of row k) before it is overwritten by row k - 2's result,
+        // LOOKAHEAD >= 2 rows later in this loop order; the register look-ahead reads it even earlier
+        constexpr int G = LOOKAHEAD;
+        cplx q[G];
+        auto load = [&](int k0, cplx (&r)[G]) {
+#pragma unroll
+            for (int i = 0; i < G; ++i) if (k0 - i >= 2) r[i] = x[(k0 - i - 2) * st];
+        };
+        load(N, q);
+        for (int k0 = N; k0 >= 2; k0 -= G) {
+            cplx nx[G];
+            load(k0 - G, nx);
+            const int kp = k0 - 2 * G - g.pf;
+#pragma unroll
+            for (int i = 0; i < G; ++i) if (kp - i >= 2) pf_l2(x + (kp - i - 2) * st);
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const int k = k0 - i;
+                if (k >= 2) x[k * st] = el.row<true, false>(k, N, sigma, q[i], pv.step(k, N, sigma));
+            }
+#pragma unroll
+            for (int i = 0; i < G; ++i) q[i] = nx[i];
         }
         cplx u0, u1;
         el.finish<true>(sigma, 0.0, 0.0, u0, u1);
@@ -784,26 +868,56 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
     const bool phase = a.phi != nullptr;
     Chain1 cW, cP;
     cW.init(); cP.init();
-    for (int n = g.N; n >= 0; --n) {
-        const size_t o = n * st + col;
-        const int np = n - g.pf;
-        if (np >= 0) {
-            const size_t op = np * st + col;
-            pf_l2(a.w + op); pf_l2(a.om + op);
-            if (phase && np < g.nkz) pf_l2(a.phi + op);
+    constexpr int G = LOOKAHEAD;
+    struct Row { cplx w, om, phi; };
+    auto load = [&](int n0, Row (&r)[G]) {               // rows n0, n0 - 1, .. (descending)
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            const int n = n0 - i;
+            if (n >= 0) {
+                const size_t o = n * st + col;
+                r[i].w = a.w[o];
+                r[i].om = a.om[o];
+                if (phase && n < g.nkz) r[i].phi = a.phi[o];
+                if (mean) r[i].w = a.th[o];              // column (0,0): v-bar lives in the theta slot
+            }
         }
-        const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
-        if (phase && n < g.nkz) a.phz[o] = cP.step(a.phi[o], f, h);   // D of the truncated phi^ (P first, then D)
-        if (mean) {   // mean flow: u-bar from the omega slot, v-bar from the theta slot, w = 0 (reading S12)
-            a.u[o] = a.om[o];
-            a.v[o] = a.th[o];
-            a.w[o] = cz();
-        } else {
-            const cplx dw = cW.step(a.w[o], f, h);
-            const cplx om = a.om[o];
-            a.u[o] = cscale(ci(cadd(cscale(dw, kx), cscale(om, ky))), ik2);
-            a.v[o] = cscale(ci(csub(cscale(dw, ky), cscale(om, kx))), ik2);
+    };
+    Row q[G];
+    load(g.N, q);
+    for (int n0 = g.N; n0 >= 0; n0 -= G) {
+        Row nx[G];
+        load(n0 - G, nx);
+        const int np0 = n0 - 2 * G - g.pf;
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            const int np = np0 - i;
+            if (np >= 0) {
+                const size_t op = np * st + col;
+                pf_l2(a.w + op); pf_l2(a.om + op);
+                if (phase && np < g.nkz) pf_l2(a.phi + op);
+            }
         }
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            const int n = n0 - i;
+            if (n < 0) continue;
+            const size_t o = n * st + col;
+            const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
+            if (phase && n < g.nkz) a.phz[o] = cP.step(q[i].phi, f, h);   // D of the truncated phi^ (P first, then D)
+            if (mean) {   // mean flow: u-bar from the omega slot, v-bar from the theta slot, w = 0 (reading S12)
+                a.u[o] = q[i].om;
+                a.v[o] = q[i].w;
+                a.w[o] = cz();
+            } else {
+                const cplx dw = cW.step(q[i].w, f, h);
+                const cplx om = q[i].om;
+                a.u[o] = cscale(ci(cadd(cscale(dw, kx), cscale(om, ky))), ik2);
+                a.v[o] = cscale(ci(csub(cscale(dw, ky), cscale(om, kx))), ik2);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < G; ++i) q[i] = nx[i];
     }
 }
 
