@@ -623,7 +623,10 @@ struct SubstArgs {
 // pointer, run-time stride): every row then costs a full memory latency, which dominates on small grids (few
 // columns, little parallelism).  The loops below therefore load a GROUP of LOOKAHEAD rows into registers before the
 // previous group's results are stored (different rows: no hazard).
-constexpr int LOOKAHEAD = 4;
+#ifndef LOOKAHEAD_N
+#define LOOKAHEAD_N 4
+#endif
+constexpr int LOOKAHEAD = LOOKAHEAD_N;
 
 __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstArgs a) {
     const ColGeom &g = a.g;
