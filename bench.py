@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py - psdns_step throughput on B200 (grid-point-steps/s, ms/step, FP64) with roofline.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 5c|5b|5a|cfg3|fig3] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 5c|5b|5a|cfg1|cfg2|cfg3|cfg4|fig3] [--impl reference]
 
 One "step" = one pass of the whole hot path (rows a1-a11 of DESIGN.md) over the state.
 Default workload = BASELINE.json config 5 on the 1024x512x513 grid (the grid the >= 60 % HBM
@@ -43,8 +43,8 @@ def workload(tag: str):
     elif tag == "cfg3":
         c = I.CONFIGS[3]
         kind = "channel-state"
-    elif tag == "cfg2":
-        c = I.CONFIGS[2]
+    elif tag in ("cfg1", "cfg2", "cfg4"):
+        c = I.CONFIGS[int(tag[3])]
         kind = "channel-state"
     elif tag == "fig3":   # the paper's Fig. 3 shape: single-phase 256x256x257
         c = I.Config("fig3", 256, 256, 257, re=3000.0, ch=1.0, pe=1.0, we=1.0, dt=2e-5, steps=10, seed=1006,
@@ -72,9 +72,9 @@ def algorithmic_bytes(c):
     # field counts of the pipeline AS BUILT: matched viscosity sends 5 spectra through the
     # backward z pass (u v w phi Dphi; i ky phi is a second output of the phi columns), 6 through the backward y
     # pass (i kx phi is formed inside the fused x kernel) and 7 deviatoric products through the forward passes
-    # (T_zz is subtracted pointwise).  Variable viscosity: 10 / 12 / 12 backward, unfused x passes.
+    # (T_zz is subtracted pointwise).  Variable viscosity: 10 / 11 / 11 backward (5 strain spectra more), fused 16-slot x kernel.
     if phase:
-        nzr, nzw, nyb, nfw = (10, 12, 12, 7) if visc else (5, 6, 6, 7)
+        nzr, nzw, nyb, nfw = (10, 11, 11, 7) if visc else (5, 6, 6, 7)
     else:
         nzr, nzw, nyb, nfw = 3, 3, 3, 5
     per_kernel = {

@@ -17,6 +17,7 @@
 #include "kernels_spectral.cuh"
 #include "kernels_transform.cuh"
 #include "kernels_xfused.cuh"
+#include "kernels_xfused_visc.cuh"
 
 using namespace psdns;
 
@@ -81,7 +82,7 @@ struct psdns_handle {
     bool use_xfused;
     bool xf_warp;               // fused x kernel: warp-per-field form (nx = 1024: 32 butterflies per pass = one per lane) or
                                 // thread = (butterfly, field) form (smaller nx, where a warp per field would leave lanes idle)
-    int xf_occ, n_sm;
+    int xf_occ, xfv_occ, n_sm;
     int occ_z[2], occ_y[2];     // resident CTAs per SM of the persistent z / y passes, [fwd]
 
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
@@ -209,6 +210,9 @@ size_t fft_smem() { return (size_t)(L * TILE_LINES + L) * sizeof(cplx); }
 // tile + stage [nst][spitch] + mbarrier
 template <int L>
 size_t xfused_smem(int nkx, int nst) { return (size_t)((L / 2) * TILE_LINES + nst * xf_spitch(nkx)) * sizeof(cplx) + 16; }
+
+template <int L>
+size_t xfusedv_smem(int nkx) { return (size_t)((L / 2) * XV_SLOTS + XV_NST * xf_spitch(nkx)) * sizeof(cplx) + 16; }
 
 template <class K>
 cudaError_t set_smem(K kern, size_t bytes) {
@@ -343,6 +347,16 @@ cudaError_t setup_attrs(psdns_handle *h) {
     }
     if (h->nf_in <= 7) { DISPATCH_L(h->d.nx, XFA) }
 #undef XFA
+#define XFVA(LL)                                                                                             \
+    {                                                                                                        \
+        const size_t sm = xfusedv_smem<LL>(h->d.nkx);                                                        \
+        int occ = 0;                                                                                         \
+        CU0(set_smem(k_xfusedv<LL>, sm));                                                                    \
+        CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedv<LL>, xv_threads<LL>(), sm));       \
+        h->xfv_occ = occ;                                                                                    \
+    }
+    if (h->nf_in > 7) { DISPATCH_L(h->d.nx, XFVA) }
+#undef XFVA
 #undef ZA
 #undef YA
 #undef XA
@@ -365,6 +379,16 @@ cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
     }
     DISPATCH_L(h->d.nx, XF)
 #undef XF
+    return cudaGetLastError();
+}
+
+cudaError_t launch_xfusedv(psdns_handle *h, const XFVArgs &a) {
+    const cplx *tw = h->at<cplx>(h->L.tw_x);
+    const int grid = std::min(a.nlines, h->n_sm * std::max(h->xfv_occ, 1));   // persistent: one wave
+    LaunchScope ls(h, KC_XFUSED);
+#define XFV(LL) k_xfusedv<LL><<<grid, xv_threads<LL>(), xfusedv_smem<LL>(h->d.nkx), h->st>>>(a, tw);
+    DISPATCH_L(h->d.nx, XFV)
+#undef XFV
     return cudaGetLastError();
 }
 
@@ -457,8 +481,13 @@ cudaError_t enqueue_step(psdns_handle *h) {
         if (visc) {
             for (int i = 0; i < 5; ++i) src[5 + i] = h->at<cplx>(L.derived[1 + i]);
             nz_f = 10;
-            zd.dfield = 3; zd.out_dx = h->at<cplx>(L.zb[10]); zd.out_dy = h->at<cplx>(L.zb[11]);
-            ny_f = 12;
+            if (h->use_xfused) {   // fused: i kx phi is derived in the x kernel's stage; Z / Y array 10 = i ky phi
+                zd.dfield = 3; zd.out_dx = nullptr; zd.out_dy = h->at<cplx>(L.zb[10]);
+                ny_f = 11;
+            } else {
+                zd.dfield = 3; zd.out_dx = h->at<cplx>(L.zb[10]); zd.out_dy = h->at<cplx>(L.zb[11]);
+                ny_f = 12;
+            }
         } else {
             const bool fused = h->use_xfused;
             zd.dfield = 3; zd.out_dx = fused ? nullptr : h->at<cplx>(L.zb[6]); zd.out_dy = h->at<cplx>(L.zb[5]);
@@ -474,7 +503,16 @@ cudaError_t enqueue_step(psdns_handle *h) {
         gy.in[i] = h->at<cplx>(L.yb[i]); gy.out[i] = h->at<cplx>(L.zb[i]);
         gz.in[i] = gy.out[i]; gz.out[i] = h->at<cplx>(L.prod[i]);
     }
-    if (h->use_xfused && !visc) {
+    if (h->use_xfused && visc) {
+        // a4 + a5 + a6 fused, 16-slot tile (kernels_xfused_visc.cuh); Y arrays: u v w phi phz exx eyy exy exz eyz phy
+        XFVArgs a;
+        const int stage_src[XV_NTMA] = {0, 1, 2, 3, 10, 4, 5, 6, 7, 8, 9};   // u v w phi phy phz exx eyy exy exz eyz
+        for (int i = 0; i < XV_NTMA; ++i) a.in[i] = h->at<cplx>(L.yb[stage_src[i]]);
+        for (int i = 0; i < XV_NOUT; ++i) a.out[i] = h->at<cplx>(L.yb[i]);
+        a.kxp = d.kxp; a.nkx = d.nkx; a.nlines = d.nz * d.ny;
+        a.cs = c.cs; a.kxf = 2.0 * M_PI / h->g.lx; a.eta_c = (p.visc_ratio - 1.0) / (2.0 * p.re);
+        CU(launch_xfusedv(h, a));
+    } else if (h->use_xfused && !visc) {
         // a4 + a5 + a6 fused: physical space never leaves the SM; in place on the Y arrays
         XFArgs a;
         const int stage_src[6] = {0, 1, 2, 3, 5, 4};   // u v w phi phy phz  <-  Y arrays u v w phi phz phy
@@ -700,7 +738,7 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     const bool visc = phase && params->visc_ratio != 1.0;
     h->nf_in = phase ? (visc ? 12 : 7) : 3;
     h->nf_out = phase ? 7 : 5;
-    h->xf_occ = 1; h->n_sm = 148;
+    h->xf_occ = 1; h->xfv_occ = 1; h->n_sm = 148;
     h->occ_z[0] = h->occ_z[1] = h->occ_y[0] = h->occ_y[1] = 1;
     {
         int dev = 0, nsm = 0;

@@ -68,6 +68,15 @@ def test_variable_viscosity():
         assert ev < TOL and ep < TOL, (k, ev, ep)
 
 
+def test_variable_viscosity_wide_and_ragged():
+    """The 16-slot fused x kernel of the variable-viscosity step at other radix plans, incl. nx = 1024."""
+    for (nx, ny, nz) in [(16, 32, 17), (128, 16, 17), (512, 16, 9), (1024, 16, 9)]:
+        c = I.small_config(nx=nx, ny=ny, nz=nz, visc_ratio=0.3)
+        errs, *_ = run_both(c, [2])
+        for k, (ev, ep) in errs.items():
+            assert ev < TOL and ep < TOL, (nx, k, ev, ep)
+
+
 def test_ragged_shapes():
     """nx != ny != nz-1, padded kx pitch (nkx = 6 -> 8, 22 -> 24) and several column tiles."""
     for (nx, ny, nz) in [(16, 64, 17), (64, 16, 65)]:
