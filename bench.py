@@ -359,7 +359,7 @@ def run_ours(args):
     # under profiles/; null for workloads that were not captured)
     traffic = {}
     try:
-        tj = json.load(open(os.path.join(ROOT, "profiles", "r1f_traffic_5c.json")))
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r1g_traffic_5c.json")))
         if tj.get("workload") == args.workload:
             traffic = tj["bytes_per_launch"]
     except Exception:
