@@ -393,7 +393,8 @@ __global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_
 }
 
 // ====================================================================================================
-// Warp-per-field form of the fused x kernel (the one psdns_step launches).
+// Warp-per-field form of the fused x kernel (psdns_step launches it when nx = 1024, where a pass has 32 butterflies
+// per field = one per lane; k_xfused above serves the smaller nx, where a warp per field would leave lanes idle).
 //
 // Every stage except the pointwise one is independent per field, so a WARP owns one field: its 32 lanes are
 // the (up to) 32 butterflies of a pass.  Consequences (profiles/r1e: the field-interleaved form above ran its
