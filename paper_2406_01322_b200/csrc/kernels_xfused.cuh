@@ -13,9 +13,9 @@
 //   B  DIF pass R2                                                   tile -> tile
 //   C  DIF radix 2 + pointwise products + DIT radix 2 (a thread owns two rows x all 8 fields)
 //   D  DIT pass R2                                                   tile -> tile
-//   E  DIT pass R1, results kept in registers and published to the tile
-//   F  post-twiddle with the partner row H-k read from the tile, truncated store to HBM
-// i.e. 5 tile round trips per line instead of 9.  The backward FFT is decimation in frequency, the
+//   E  DIT pass R1, results kept in registers
+//   F  post-twiddle against the partner row H-k (a register of another lane: warp shuffle), truncated store
+// i.e. 4 tile exchanges per line instead of 9.  The backward FFT is decimation in frequency, the
 // products are elementwise, the forward FFT is decimation in time: no reordering anywhere.
 #pragma once
 #include "fft_tile.cuh"
@@ -69,27 +69,6 @@ template <> struct XPlan<128> { static constexpr int R1 = 8,  R2 = 8; };
 template <> struct XPlan<256> { static constexpr int R1 = 16, R2 = 8; };
 template <> struct XPlan<512> { static constexpr int R1 = 16, R2 = 16; };
 
-// threads per CTA: one thread per (butterfly of pass R1, field)
-template <int L> __host__ __device__ constexpr int xf_threads() {
-    return (8 * (L / 2) / XPlan<L / 2>::R1) > 64 ? (8 * (L / 2) / XPlan<L / 2>::R1) : 64;
-}
-
-// tile index: the field slot is rotated by row/2, so that (i) a quarter-warp that touches one row with its
-// 8 fields and (ii) 8 consecutive threads that each touch their own row PAIR (2t, 2t+1) at the same field
-// both cover all eight 16-byte bank groups: conflict free in every stage.
-__device__ __forceinline__ int xidx(int row, int f) { return row * TILE_LINES + ((f + (row >> 1)) & (TILE_LINES - 1)); }
-
-// w_H^i = w_L^{2i} from the table tw[k] = w_L^k, k < H (w_L^{k+H} = -w_L^k), 0 <= i < H
-template <int H>
-__device__ __forceinline__ cplx tw_half(const cplx *__restrict__ tw, int i) {
-    const int idx = 2 * i;
-    cplx w = tw[idx & (H - 1)];
-    const int sgn = (idx & H) ? (int)0x80000000 : 0;
-    w.x = __hiloint2double(__double2hiint(w.x) ^ sgn, __double2loint(w.x));
-    w.y = __hiloint2double(__double2hiint(w.y) ^ sgn, __double2loint(w.y));
-    return w;
-}
-
 // compile-time twiddle w_LS^q = exp(-2 pi i q / LS) for LS in {4, 8, 16, 32}, 0 <= q < LS/2
 __device__ __forceinline__ constexpr double cos32(int i) {   // cos(2 pi i / 32), 0 <= i <= 16
     constexpr double C[9] = {1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708,
@@ -102,36 +81,6 @@ __device__ __forceinline__ constexpr double wc_re(int q) { return cos32(q * (32 
 template <int LS>
 __device__ __forceinline__ constexpr double wc_im(int q) {   // -sin(2 pi q / LS)
     return q * (32 / LS) <= 8 ? -cos32(8 - q * (32 / LS)) : -cos32(q * (32 / LS) - 8);
-}
-
-// In-place pass of sub-length LS = 2 R (stride 2) on the x tile.  The two twiddle classes j = 0 (no twiddle)
-// and j = 1 (w_LS^q, compile-time constants) are assigned to different WARPS, so that no twiddle is ever
-// loaded from shared memory (a broadcast LDS.128 costs as many wavefronts as a data access).
-template <int H, int R, int SIGN, int NT, bool DIT>
-__device__ __forceinline__ void xpass_mid(cplx *__restrict__ s, int tid) {
-    tid = opaque(tid);
-    constexpr int LS = 2 * R;
-    constexpr int NBLK = H / LS;           // blocks per field; items per field = 2 * NBLK
-    static_assert(NBLK % 4 == 0, "j must be uniform over a warp (4 butterflies x 8 fields)");
-    const int f = tid & (TILE_LINES - 1);
-    for (int b = tid >> 3; b < 2 * NBLK; b += NT / TILE_LINES) {
-        const int j = b / NBLK, blk = b % NBLK;
-        const int row0 = blk * LS + j;
-        cplx v[R];
-#pragma unroll
-        for (int m = 0; m < R; ++m) v[m] = s[xidx(row0 + 2 * m, f)];
-        if (DIT && j) {
-#pragma unroll
-            for (int m = 1; m < R; ++m) v[m] = cmultw<SIGN>(v[m], make_double2(wc_re<LS>(m), wc_im<LS>(m)));
-        }
-        RegFFT<R, SIGN>::run(v);
-        if (!DIT && j) {
-#pragma unroll
-            for (int q = 1; q < R; ++q) v[q] = cmultw<SIGN>(v[q], make_double2(wc_re<LS>(q), wc_im<LS>(q)));
-        }
-#pragma unroll
-        for (int q = 0; q < R; ++q) s[xidx(row0 + 2 * q, f)] = v[q];
-    }
 }
 
 // Powers w^1 .. w^{R-1} of a per-thread base twiddle from the loop-invariant set {w, w^2, w^4, w^8}:
@@ -184,17 +133,6 @@ __device__ __forceinline__ double nl_out(const double (&in)[8], double cs) {
     return in[3] * in[3] * in[3];
 }
 
-// one output field of the row pair (2t, 2t+1): the products at the four points held by this thread, recombined
-// by the first DIT radix-2 butterfly and stored; inputs stay in registers, outputs never accumulate
-template <int Q, bool PHASE>
-__device__ __forceinline__ void nl_store(cplx *__restrict__ s, int t, const double (&p00)[8], const double (&p01)[8],
-                                         const double (&p10)[8], const double (&p11)[8], double cs) {
-    const double o00 = nl_out<Q, PHASE>(p00, cs), o01 = nl_out<Q, PHASE>(p01, cs);
-    const double o10 = nl_out<Q, PHASE>(p10, cs), o11 = nl_out<Q, PHASE>(p11, cs);
-    s[xidx(2 * t, Q)] = make_double2(o00 + o10, o01 + o11);
-    s[xidx(2 * t + 1, Q)] = make_double2(o00 - o10, o01 - o11);
-}
-
 // the four products of output field q at the four points of a row pair (q is a compile-time constant after unrolling)
 template <bool PHASE>
 __device__ __forceinline__ void nl_quad(int q, const double (&p00)[8], const double (&p01)[8], const double (&p10)[8],
@@ -215,189 +153,23 @@ struct XFArgs {
 // stage pitch (cplx): odd, so that the 8 fields of one k sit in 8 different 16-byte bank groups
 __host__ __device__ inline int xf_spitch(int nkx) { return nkx | 1; }
 
-// shared memory: tile [H][8] | stage [NST][spitch] | mbarrier.  The stage receives the NEXT line's spectra rows
-// by TMA bulk copies while the current line is transformed; with the phase field its last row is derived in
-// place: i kx phi^ (row a1), so that the x derivative of phi costs no FP64 work in the butterfly warps.
+// shared memory: tile [LPI H][8] | stage [LPI][NST][spitch] | mbarriers.  The stage receives the NEXT iteration's
+// spectra rows by TMA bulk copies while the current lines are transformed; with the phase field its last row is
+// derived in place: i kx phi^ (row a1).
 // Register budget (128 at 2 CTAs/SM): only the thread's base twiddle w_L^j is carried across the line loop;
-// its powers are re-derived per stage and nothing is held in registers across a barrier (profiles/r1d: the
-// previous form spilled 456 B/thread, 8 GB of extra DRAM writes per step and 15 % of the time in LDL waits).
+// its powers are re-derived per stage (profiles/r1c: an earlier form spilled 456 B/thread, 8 GB of extra DRAM
+// writes per step and 15 % of the time in local-memory waits).
 #ifndef XF_MINB
 #define XF_MINB 2
 #endif
 template <bool PHASE> __host__ __device__ constexpr int xf_nstage() { return PHASE ? 7 : 3; }
 
-template <int L, bool PHASE>
-__global__ void __launch_bounds__(xf_threads<L>(), (L >= 1024 ? XF_MINB : 3)) k_xfused(const __grid_constant__ XFArgs a,
-                                                                               const cplx *__restrict__ twx) {
-    constexpr int H = L / 2;
-    constexpr int R1 = XPlan<H>::R1, R2 = XPlan<H>::R2;
-    constexpr int NT = xf_threads<L>();
-    constexpr int S1 = H / R1;              // stride of pass R1 = number of its butterflies per field
-    constexpr int NIN = PHASE ? 7 : 3, NOUT = PHASE ? 7 : 5;   // fields through the backward / forward FFT
-    constexpr int NTMA = PHASE ? 6 : 3;                        // rows staged by TMA: u v w [phi phy phz]
-    constexpr int NST = xf_nstage<PHASE>();                    // + derived row i kx phi
-    static_assert(R1 * R2 * 2 == H, "plan");
-    static_assert(S1 * TILE_LINES <= NT, "one (butterfly, field) item per thread in stages A and E");
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx *s = reinterpret_cast<cplx *>(smem_raw);
-    cplx *stage = s + H * TILE_LINES;
-    const int kxp = a.kxp, nkx = a.nkx;
-    const int spitch = xf_spitch(nkx);
-    unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)NST * spitch);
-    const int tid = threadIdx.x, f = tid & 7, j = tid >> 3;
-    const bool item = j < S1;               // this thread owns butterfly j of field f in stages A, E, F
-    cplx *outf = a.out[f < NOUT ? f : 0];
-    const double sc = 0.5 / L;
-    const unsigned row_bytes = (unsigned)(nkx * sizeof(cplx));
-    auto issue = [&](int line) {   // one thread: arm the barrier and launch the bulk copies
-        mbar_expect_tx(bar, row_bytes * NTMA);
-#pragma unroll
-        for (int q = 0; q < NTMA; ++q) bulk_g2s(stage + (size_t)q * spitch, a.in[q] + (size_t)line * kxp, row_bytes, bar);
-    };
-    if (tid == 0) {
-        mbar_init(bar, 1);
-        if ((int)blockIdx.x < a.nlines) issue(blockIdx.x);
-    }
-    __syncthreads();
-    // w_L^k for k = j + S1 m is w_L^j times the compile-time constant w_{2 R1}^m; the pass twiddles are powers
-    // of w_H^j = (w_L^j)^2: no table look-up per element
-    cplx wj = twx[item ? j : 0];
-    unsigned parity = 0;
-    // field -> staged row: u v w phi phx phy phz  <-  0 1 2 3 6 4 5
-    const int srow = !PHASE ? (f < NST ? f : 0) : (f < 4 ? f : (f == 4 ? 6 : (f < NIN ? f - 1 : 0)));
-    const cplx *sf = stage + (size_t)srow * spitch;
-    for (int line = blockIdx.x; line < a.nlines; line += gridDim.x) {
-        const size_t base = (size_t)line * kxp;
-        mbar_wait(bar, parity);
-        parity ^= 1;
-        if constexpr (PHASE) {              // row a1: phx^ = i kx phi^
-            for (int k = tid; k < nkx; k += NT) {
-                const cplx p = stage[3 * spitch + k];
-                const double kk = a.kxf * (double)k;
-                stage[6 * spitch + k] = make_double2(-kk * p.y, kk * p.x);
-            }
-            __syncthreads();
-        }
-        // keep the compiler from hoisting per-line derived twiddles out of the line loop (they would be spilled)
-        asm volatile("" : "+d"(wj.x), "+d"(wj.y));
-        // ---- A: pre-twiddle from the staged rows + DIF pass R1 (inverse transform, sign +) ----
-        if (item) {
-            const int j = opaque(tid) >> 3;
-            cplx v[R1];
-#pragma unroll
-            for (int m = 0; m < R1; ++m) {
-                if (m && (m & 3) == 0) asm volatile("" ::: "memory");   // at most 4 elements' staged loads in flight
-                const int k = j + S1 * m, kb = H - k;
-                cplx xa = make_double2(0.0, 0.0), xb = xa;
-                if (f < NIN) {
-                    if (k < nkx) xa = sf[k];
-                    if (kb < nkx) xb = sf[kb];
-                }
-                if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
-                const cplx w = m ? cmul(wj, make_double2(wc_re<2 * R1>(m), wc_im<2 * R1>(m))) : wj;
-                const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
-                // Z = S + i conj(w) D
-                v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
-            }
-            RegFFT<R1, +1>::run(v);
-            TwPow<R1> tp;
-            tp.init(cmul(wj, wj));
-            s[xidx(j, f)] = v[0];
-            tp.each([&](int q, cplx wq) { s[xidx(j + S1 * q, f)] = cmultw<+1>(v[q], wq); });
-        }
-        __syncthreads();
-        if (tid == 0 && line + (int)gridDim.x < a.nlines) {   // stage is free: prefetch the next line
-            fence_proxy_async();
-            issue(line + gridDim.x);
-        }
-        // ---- B: DIF pass R2 ----
-        if constexpr (R2 > 1) {
-            xpass_mid<H, R2, +1, NT, false>(s, tid);
-            __syncthreads();
-        }
-        // ---- C: last DIF radix 2, pointwise products, first DIT radix 2: rows (2t, 2t+1) x all fields ----
-        for (int t = opaque(tid); t < H / 2; t += NT) {
-            double p00[8], p01[8], p10[8], p11[8];   // the four grid points of this row pair, all input fields
-#pragma unroll
-            for (int q = 0; q < NIN; ++q) {
-                const cplx p = s[xidx(2 * t, q)], m = s[xidx(2 * t + 1, q)];
-                p00[q] = p.x + m.x; p01[q] = p.y + m.y;
-                p10[q] = p.x - m.x; p11[q] = p.y - m.y;
-            }
-            nl_store<0, PHASE>(s, t, p00, p01, p10, p11, a.cs);
-            nl_store<1, PHASE>(s, t, p00, p01, p10, p11, a.cs);
-            nl_store<2, PHASE>(s, t, p00, p01, p10, p11, a.cs);
-            nl_store<3, PHASE>(s, t, p00, p01, p10, p11, a.cs);
-            nl_store<4, PHASE>(s, t, p00, p01, p10, p11, a.cs);
-            if (PHASE) {
-                nl_store<5, PHASE>(s, t, p00, p01, p10, p11, a.cs);
-                nl_store<6, PHASE>(s, t, p00, p01, p10, p11, a.cs);
-            }
-        }
-        __syncthreads();
-        // ---- D: DIT pass R2 (forward transform, sign -) ----
-        if constexpr (R2 > 1) {
-            xpass_mid<H, R2, -1, NT, true>(s, tid);
-            __syncthreads();
-        }
-        // ---- E: DIT pass R1; the results stay in registers, only the rows some partner needs go to the tile ----
-        asm volatile("" : "+d"(wj.x), "+d"(wj.y));
-        cplx v[R1];
-        if (item) {
-            const int j = opaque(tid) >> 3;
-            TwPow<R1> tp;
-            tp.init(cmul(wj, wj));
-            v[0] = s[xidx(j, f)];
-            tp.each([&](int m, cplx wq) { v[m] = cmultw<-1>(s[xidx(j + S1 * m, f)], wq); });
-            RegFFT<R1, -1>::run(v);
-            // in place: a thread reads and writes the same rows j + S1 m of its own field
-#pragma unroll
-            for (int q = 0; q < R1; ++q) {     // row r is read as the partner H - k of some kept k < nkx iff r > H - nkx
-                const int r = j + S1 * q;
-                if (r > H - nkx) s[xidx(r, f)] = v[q];
-            }
-        }
-        __syncthreads();
-        // ---- F: post-twiddle of row k against the partner row H - k, truncated store ----
-        if (item && f < NOUT) {
-            const int j = opaque(tid) >> 3;
-            cplx *o = outf + base;
-#pragma unroll
-            for (int q0 = 0; q0 < R1; q0 += 4) {          // four rows' partner loads in flight, then their stores
-                if (S1 * q0 < kxp) {                       // CTA-uniform: no row of this group is kept otherwise
-                    cplx zb[4];
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int k = j + S1 * (q0 + i);
-                        zb[i] = s[xidx((H - k) & (H - 1), f)];   // every row exists: no predicate on the loads
-                    }
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int q = q0 + i, k = j + S1 * q;
-                        if (k < nkx) {
-                            const cplx za = v[q];
-                            const cplx zp = k ? zb[i] : za;      // k = 0 is its own partner (row 0 was not republished)
-                            const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
-                            const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
-                            // X_k = (S - i w D) / (2 L)
-                            stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
-                        } else if (k < kxp) {
-                            stg(o + k, make_double2(0.0, 0.0));
-                        }
-                    }
-                }
-            }
-        }
-        __syncthreads();
-    }
-}
-
 // ====================================================================================================
-// Warp-per-field form of the fused x kernel (psdns_step launches it when nx = 1024, where a pass has 32 butterflies
-// per field = one per lane; k_xfused above serves the smaller nx, where a warp per field would leave lanes idle).
+// Warp-per-field organisation of the stages above (k_xfusedw: nx = 1024, where a pass has 32 butterflies per field =
+// one per lane; k_xfusedwm further down: smaller nx, several lines per iteration fill the warp).
 //
 // Every stage except the pointwise one is independent per field, so a WARP owns one field: its 32 lanes are
-// the (up to) 32 butterflies of a pass.  Consequences (profiles/r1e: the field-interleaved form above ran its
+// the (up to) 32 butterflies of a pass.  Consequences (profiles/r1e: an earlier field-interleaved form (thread = (butterfly, field)) ran its
 // FP64 pipe 48 % and its shared-memory pipe 73 % busy, in lockstep between eight CTA-wide barriers per line):
 //   * stages A -> B and D -> E -> F need only __syncwarp: three CTA-wide barriers per line (stage ready,
 //     before and after the pointwise stage), so the field warps drift apart and FP64 work of one overlaps
@@ -423,6 +195,10 @@ __device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
 }
 
 constexpr int XFW_THREADS = 256;   // 8 warps: one per field slot
+// lines per CTA iteration: a warp's 32 lanes = LPI lines x S1 butterflies of its field (1 at nx = 1024, 2 at nx = 512 ..)
+template <int L> __host__ __device__ constexpr int xfw_lpi() {
+    return ((L / 2) / XPlan<L / 2>::R1) >= 32 ? 1 : 32 / ((L / 2) / XPlan<L / 2>::R1);
+}
 
 template <int L, bool PHASE>
 __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 512 ? 2 : 3))) k_xfusedw(const __grid_constant__ XFArgs a,
@@ -585,6 +361,215 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 512 
             // lane of THIS warp, fetched by shuffle - no shared-memory exchange and no barrier.
             {
                 const int src = (S1 - j) & (S1 - 1);
+                cplx *o = outf + base;
+#pragma unroll
+                for (int q = 0; q < R1; ++q) {
+                    if (S1 * q < kxp) {                        // CTA-uniform: no row of this q is kept otherwise
+                        const cplx mine = (j == 0) ? v[(R1 - q) & (R1 - 1)] : v[R1 - 1 - q];
+                        cplx zp;
+                        zp.x = __shfl_sync(0xffffffffu, mine.x, src);
+                        zp.y = __shfl_sync(0xffffffffu, mine.y, src);
+                        const int k = j + S1 * q;
+                        if (itemA && k < nkx) {
+                            const cplx za = v[q];
+                            if (k == 0) zp = za;               // k = 0 is its own partner
+                            const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
+                            const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
+                            // X_k = (S - i w D) / (2 L)
+                            stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
+                        } else if (itemA && k < kxp) {
+                            stg(o + k, make_double2(0.0, 0.0));
+                        }
+                    }
+                }
+            }
+            __syncwarp();     // this warp's F reads are done before its next stage A overwrites the field
+        }
+    }
+}
+
+// Multi-line generalisation for nx < 1024, where a pass has fewer than 32 butterflies per field: the 32 lanes of a
+// field warp are LPI lines x S1 butterflies (LPI = 2 at nx = 512 and 256, 4 at 128, ..), the tile holds LPI lines.
+// Kept as a second kernel: folded to LPI = 1 it is the kernel above instruction for instruction, yet measured 3 %
+// slower at nx = 1024 (8.4 vs 8.16 ms), so nx = 1024 keeps the single-line form.
+template <int L, bool PHASE>
+__global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 128 ? 2 : 3))) k_xfusedwm(const __grid_constant__ XFArgs a,
+                                                                             const cplx *__restrict__ twx) {
+    constexpr int H = L / 2;
+    constexpr int R1 = XPlan<H>::R1, R2 = XPlan<H>::R2;
+    constexpr int NT = XFW_THREADS;
+    constexpr int S1 = H / R1;              // butterflies per field of pass R1 (<= 32)
+    constexpr int LS = 2 * R2;              // sub-length of the inner pass
+    constexpr int NB2 = H / R2;             // butterflies per field of the inner pass (<= 32)
+    constexpr int LG = ilog2(LS) < 3 ? 3 : ilog2(LS);
+    constexpr int NIN = PHASE ? 7 : 3, NOUT = PHASE ? 7 : 5;
+    constexpr int NTMA = PHASE ? 6 : 3;
+    constexpr int NST = xf_nstage<PHASE>();
+    constexpr int LPI = xfw_lpi<L>();       // lines per iteration
+    static_assert(R1 * R2 * 2 == H && S1 * LPI == 32, "plan");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx *s = reinterpret_cast<cplx *>(smem_raw);
+    cplx *stage = s + LPI * H * TILE_LINES;         // [LPI][NST][spitch]
+    const int kxp = a.kxp, nkx = a.nkx;
+    const int spitch = xf_spitch(nkx);
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)LPI * NST * spitch);
+    unsigned long long *bar_free = bar + 1;         // stage consumed by every input-field warp
+    const int tid = threadIdx.x, f = tid >> 5, lane = tid & 31;
+    const bool service = (f == TILE_LINES - 1);     // eighth warp
+    cplx *outf = a.out[f < NOUT ? f : 0];
+    const double sc = 0.5 / L;
+    const unsigned row_bytes = (unsigned)(nkx * sizeof(cplx));
+    const int ngroups = a.nlines / LPI;             // nlines = nz * ny is a multiple of LPI (ny >= 16, power of two)
+    auto issue = [&](int grp) {
+        mbar_expect_tx(bar, row_bytes * NTMA * LPI);
+#pragma unroll
+        for (int l = 0; l < LPI; ++l)
+#pragma unroll
+            for (int q = 0; q < NTMA; ++q)
+                bulk_g2s(stage + (size_t)(l * NST + q) * spitch, a.in[q] + (size_t)(grp * LPI + l) * kxp, row_bytes, bar);
+    };
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        mbar_init(bar_free, NIN);
+        if ((int)blockIdx.x < ngroups) issue(blockIdx.x);
+    }
+    __syncthreads();
+    const int j = LPI == 1 ? lane : (lane & (S1 - 1)), ln = LPI == 1 ? 0 : lane / S1;   // butterfly of passes A, E, F; its line
+    constexpr bool itemA = true;                    // S1 * LPI = 32: every lane owns a butterfly
+    const int lrow = ln * H;                        // first tile row of that line
+    cplx wj = twx[j];                               // w_L^j
+    // pointwise-stage twiddle of this thread's row pair: w_LS^(t mod R2) = w_L^((t mod R2) L / LS)
+    cplx wc = twx[(tid % R2) * (L / LS)];
+    unsigned parity = 0;
+    // field -> staged row: u v w phi phx phy phz  <-  0 1 2 3 6 4 5
+    const int srow = !PHASE ? (f < NST ? f : 0) : (f < 4 ? f : (f == 4 ? 6 : (f < NIN ? f - 1 : 0)));
+    const cplx *sf = stage + (size_t)(ln * NST + srow) * spitch;
+    for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        const size_t base = (size_t)(grp * LPI + ln) * kxp;
+        mbar_wait(bar, parity);
+        if constexpr (PHASE) {
+            if (service) {                          // row a1: phx^ = i kx phi^
+#pragma unroll
+                for (int l = 0; l < LPI; ++l)
+                    for (int k = lane; k < nkx; k += 32) {
+                        const cplx p = stage[(l * NST + 3) * spitch + k];
+                        const double kk = a.kxf * (double)k;
+                        stage[(l * NST + 6) * spitch + k] = make_double2(-kk * p.y, kk * p.x);
+                    }
+            }
+            __syncthreads();
+        }
+        asm volatile("" : "+d"(wj.x), "+d"(wj.y), "+d"(wc.x), "+d"(wc.y));
+        if (f < NIN) {
+            // ---- A: pre-twiddle from the staged rows + DIF pass R1 (inverse transform, sign +) ----
+            if (itemA) {
+                const int jj = opaque(j);
+                cplx v[R1];
+#pragma unroll
+                for (int m = 0; m < R1; ++m) {
+                    if (m && (m & 3) == 0) asm volatile("" ::: "memory");
+                    const int k = jj + S1 * m, kb = H - k;
+                    cplx xa = make_double2(0.0, 0.0), xb = xa;
+                    if (k < nkx) xa = sf[k];
+                    if (kb < nkx) xb = sf[kb];
+                    if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
+                    const cplx w = m ? cmul(wj, make_double2(wc_re<2 * R1>(m), wc_im<2 * R1>(m))) : wj;
+                    const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
+                    v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
+                }
+                RegFFT<R1, +1>::run(v);
+                TwPow<R1> tp;
+                tp.init(cmul(wj, wj));
+                s[widx<LG>(lrow + jj, f)] = v[0];
+                tp.each([&](int q, cplx wq) { s[widx<LG>(lrow + jj + S1 * q, f)] = cmultw<+1>(v[q], wq); });
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_free);   // this field's staged row is consumed
+            // ---- B: DIF pass R2, no twiddles (they are applied in the pointwise stage) ----
+            if constexpr (R2 > 1) {
+#pragma unroll
+                for (int it = 0; it < (LPI * NB2 + 31) / 32; ++it) {
+                    const int b0 = opaque(lane) + 32 * it;
+                    if (b0 < LPI * NB2) {
+                        const int b = b0 % NB2, row0 = (b0 / NB2) * H + (b >> 1) * LS + (b & 1);
+                        cplx v[R2];
+#pragma unroll
+                        for (int m = 0; m < R2; ++m) v[m] = s[widx<LG>(row0 + 2 * m, f)];
+                        RegFFT<R2, +1>::run(v);
+#pragma unroll
+                        for (int q = 0; q < R2; ++q) s[widx<LG>(row0 + 2 * q, f)] = v[q];
+                    }
+                }
+            }
+        } else if (service) {
+            if (lane == 0) {                        // all input warps are done with the stage: prefetch the next line
+                mbar_wait(bar_free, parity);
+                if (grp + (int)gridDim.x < ngroups) {
+                    fence_proxy_async();
+                    issue(grp + gridDim.x);
+                }
+            }
+        }
+        parity ^= 1;
+        __syncthreads();
+        // ---- C: last DIF radix 2 (with the inner pass's twiddle), pointwise products, first DIT radix 2 ----
+        for (int t0 = opaque(tid); t0 < LPI * (H / 2); t0 += NT) {
+            const int t = t0;                                // row pair (2t, 2t+1) of the LPI-line tile (line l starts at row l H)
+            double p00[8], p01[8], p10[8], p11[8];
+#pragma unroll
+            for (int q = 0; q < NIN; ++q) {
+                const cplx p = s[widx<LG>(2 * t, q)];
+                cplx m = s[widx<LG>(2 * t + 1, q)];
+                if (R2 > 1) m = cmultw<+1>(m, wc);
+                p00[q] = p.x + m.x; p01[q] = p.y + m.y;
+                p10[q] = p.x - m.x; p11[q] = p.y - m.y;
+            }
+#pragma unroll
+            for (int q = 0; q < NOUT; ++q) {
+                double o00, o01, o10, o11;
+                nl_quad<PHASE>(q, p00, p01, p10, p11, a.cs, o00, o01, o10, o11);
+                s[widx<LG>(2 * t, q)] = make_double2(o00 + o10, o01 + o11);
+                cplx m = make_double2(o00 - o10, o01 - o11);
+                if (R2 > 1) m = cmultw<-1>(m, wc);
+                s[widx<LG>(2 * t + 1, q)] = m;
+            }
+        }
+        __syncthreads();
+        if (f < NOUT) {
+            // ---- D: DIT pass R2 (forward transform, sign -), no twiddles ----
+            if constexpr (R2 > 1) {
+#pragma unroll
+                for (int it = 0; it < (LPI * NB2 + 31) / 32; ++it) {
+                    const int b0 = opaque(lane) + 32 * it;
+                    if (b0 < LPI * NB2) {
+                        const int b = b0 % NB2, row0 = (b0 / NB2) * H + (b >> 1) * LS + (b & 1);
+                        cplx v[R2];
+#pragma unroll
+                        for (int m = 0; m < R2; ++m) v[m] = s[widx<LG>(row0 + 2 * m, f)];
+                        RegFFT<R2, -1>::run(v);
+#pragma unroll
+                        for (int q = 0; q < R2; ++q) s[widx<LG>(row0 + 2 * q, f)] = v[q];
+                    }
+                }
+                __syncwarp();
+            }
+            // ---- E: DIT pass R1; the results stay in registers ----
+            cplx v[R1];
+#pragma unroll
+            for (int q = 0; q < R1; ++q) v[q] = make_double2(0.0, 0.0);
+            if (itemA) {
+                const int jj = opaque(j);
+                TwPow<R1> tp;
+                tp.init(cmul(wj, wj));
+                v[0] = s[widx<LG>(lrow + jj, f)];
+                tp.each([&](int m, cplx wq) { v[m] = cmultw<-1>(s[widx<LG>(lrow + jj + S1 * m, f)], wq); });
+                RegFFT<R1, -1>::run(v);
+            }
+            // ---- F: post-twiddle of row k = j + S1 q against its partner row H - k, truncated store.  The partner
+            // is output R1 - 1 - q of butterfly S1 - j (output R1 - q of butterfly 0 for j = 0): a register of another
+            // lane of THIS warp, fetched by shuffle - no shared-memory exchange and no barrier.
+            {
+                const int src = ln * S1 + ((S1 - j) & (S1 - 1));
                 cplx *o = outf + base;
 #pragma unroll
                 for (int q = 0; q < R1; ++q) {

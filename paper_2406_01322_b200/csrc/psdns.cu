@@ -80,8 +80,6 @@ struct psdns_handle {
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tevents;
     int nf_in, nf_out;
     bool use_xfused;
-    bool xf_warp;               // fused x kernel: warp-per-field form (nx = 1024: 32 butterflies per pass = one per lane) or
-                                // thread = (butterfly, field) form (smaller nx, where a warp per field would leave lanes idle)
     int xf_occ, xfv_occ, n_sm;
     int occ_z[2], occ_y[2];     // resident CTAs per SM of the persistent z / y passes, [fwd]
 
@@ -207,12 +205,13 @@ ColGeom geom(const psdns_handle *h) {
 template <int L>
 size_t fft_smem() { return (size_t)(L * TILE_LINES + L) * sizeof(cplx); }
 
-// tile + stage [nst][spitch] + mbarrier
-template <int L>
-size_t xfused_smem(int nkx, int nst) { return (size_t)((L / 2) * TILE_LINES + nst * xf_spitch(nkx)) * sizeof(cplx) + 16; }
-
 template <int L>
 size_t xfusedv_smem(int nkx) { return (size_t)((L / 2) * XV_SLOTS + XV_NST * xf_spitch(nkx)) * sizeof(cplx) + 16; }
+
+template <int L>
+size_t xfusedw_smem(int nkx, int nst) {
+    return (size_t)(xfw_lpi<L>() * ((L / 2) * TILE_LINES + nst * xf_spitch(nkx))) * sizeof(cplx) + 32;
+}
 
 template <class K>
 cudaError_t set_smem(K kern, size_t bytes) {
@@ -326,22 +325,24 @@ cudaError_t setup_attrs(psdns_handle *h) {
     DISPATCH_L(h->d.nx, XA)
 #define XFA(LL)                                                                                              \
     {                                                                                                        \
-        const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                               \
+        const size_t sm = xfusedw_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                              \
         int occ = 0;                                                                                         \
-        if (h->xf_warp) {                                                                                    \
-            if (h->p.phase_field) {                                                                          \
-                CU0(set_smem(k_xfusedw<LL, true>, sm));                                                      \
-                CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, true>, XFW_THREADS, sm)); \
+        {                                                                                                    \
+            if (xfw_lpi<LL>() == 1) {                                                                        \
+                if (h->p.phase_field) {                                                                      \
+                    CU0(set_smem(k_xfusedw<LL, true>, sm));                                                  \
+                    CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, true>, XFW_THREADS, sm)); \
+                } else {                                                                                     \
+                    CU0(set_smem(k_xfusedw<LL, false>, sm));                                                 \
+                    CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, false>, XFW_THREADS, sm)); \
+                }                                                                                            \
+            } else if (h->p.phase_field) {                                                                   \
+                CU0(set_smem(k_xfusedwm<LL, true>, sm));                                                     \
+                CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedwm<LL, true>, XFW_THREADS, sm)); \
             } else {                                                                                         \
-                CU0(set_smem(k_xfusedw<LL, false>, sm));                                                     \
-                CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, false>, XFW_THREADS, sm)); \
+                CU0(set_smem(k_xfusedwm<LL, false>, sm));                                                    \
+                CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedwm<LL, false>, XFW_THREADS, sm)); \
             }                                                                                                \
-        } else if (h->p.phase_field) {                                                                       \
-            CU0(set_smem(k_xfused<LL, true>, sm));                                                           \
-            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfused<LL, true>, xf_threads<LL>(), sm)); \
-        } else {                                                                                             \
-            CU0(set_smem(k_xfused<LL, false>, sm));                                                          \
-            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfused<LL, false>, xf_threads<LL>(), sm)); \
         }                                                                                                    \
         h->xf_occ = occ;                                                                                     \
     }
@@ -370,12 +371,14 @@ cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
     LaunchScope ls(h, KC_XFUSED);
 #define XF(LL)                                                                                               \
     {                                                                                                        \
-        const size_t sm = xfused_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                               \
-        if (h->xf_warp) {                                                                                    \
-            if (h->p.phase_field) k_xfusedw<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);              \
-            else k_xfusedw<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                              \
-        } else if (h->p.phase_field) k_xfused<LL, true><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);       \
-        else k_xfused<LL, false><<<grid, xf_threads<LL>(), sm, h->st>>>(a, tw);                              \
+        const size_t sm = xfusedw_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                              \
+        {                                                                                                    \
+            if (xfw_lpi<LL>() == 1) {                                                                        \
+                if (h->p.phase_field) k_xfusedw<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);          \
+                else k_xfusedw<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                          \
+            } else if (h->p.phase_field) k_xfusedwm<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);      \
+            else k_xfusedwm<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                             \
+        }                                                                                                    \
     }
     DISPATCH_L(h->d.nx, XF)
 #undef XF
@@ -729,10 +732,6 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->has_state = false; h->graph = nullptr; h->graph_ready = false;
     h->use_graph = std::getenv("PSDNS_NO_GRAPH") == nullptr;
     h->use_xfused = std::getenv("PSDNS_NO_XFUSE") == nullptr;
-    {   // measured on B200: warp-per-field 8.2 vs 10.6 ms at nx = 1024, but 1.89 vs 1.27 ms at nx = 512 and 1.11 vs 0.65 ms at 256
-        const char *e = std::getenv("PSDNS_XF_WARP");
-        h->xf_warp = e ? std::atoi(e) != 0 : grid->nx >= 1024;
-    }
     h->launches = 0; h->per_step = 0; h->timed_class = -1;
     const bool phase = params->phase_field != 0;
     const bool visc = phase && params->visc_ratio != 1.0;

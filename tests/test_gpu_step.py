@@ -164,8 +164,8 @@ def test_exact_restart_through_history_blob():
     assert r.lib.psdns_set_history(r.handle, None, 0) == -1
 
 
-def test_nx1024_uses_warp_per_field_x_kernel():
-    """nx = 1024 selects the warp-per-field fused x kernel (the one the 1024x512x513 bench runs): element-by-element
+def test_nx1024_single_line_x_kernel():
+    """nx = 1024 runs the single-line warp-per-field fused x kernel (the one the 1024x512x513 bench runs): element-by-element
     parity on a grid that is wide in x only, with and without the phase field."""
     for phase in (1, 0):
         c = I.small_config(nx=1024, ny=16, nz=9, phase_field=phase)
@@ -174,11 +174,10 @@ def test_nx1024_uses_warp_per_field_x_kernel():
             assert ev < TOL and ep < TOL, (phase, k, ev, ep)
 
 
-def test_warp_per_field_x_kernel_on_small_grids(monkeypatch):
-    """The same kernel forced on grids where it is not the default (fewer than 32 butterflies per pass: idle lanes,
-    other radix plans): PSDNS_XF_WARP=1 is read by psdns_init."""
-    monkeypatch.setenv("PSDNS_XF_WARP", "1")
-    for (nx, ny, nz) in [(32, 16, 17), (256, 16, 9), (512, 16, 9)]:
+def test_multi_line_x_kernel_plans():
+    """nx < 1024 runs the multi-line warp-per-field kernel (k_xfusedwm): 16, 4, 2, 2 lines per CTA iteration and the
+    radix plans 16 | 8*4*2 | 8*8*2 | 16*8*2."""
+    for (nx, ny, nz) in [(32, 16, 17), (128, 32, 9), (256, 16, 9), (512, 16, 9)]:
         c = I.small_config(nx=nx, ny=ny, nz=nz)
         errs, *_ = run_both(c, [2])
         for k, (ev, ep) in errs.items():
