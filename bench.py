@@ -359,9 +359,11 @@ def run_ours(args):
     # under profiles/; null for workloads that were not captured)
     traffic = {}
     try:
-        tj = json.load(open(os.path.join(ROOT, "profiles", "r1g_traffic_5c.json")))
-        if tj.get("workload") == args.workload:
-            traffic = tj["bytes_per_launch"]
+        if args.workload == "5c":
+            with open(os.path.join(ROOT, "profiles", "r1g_traffic_5c.csv")) as fh:
+                for ln in fh.read().strip().splitlines()[1:]:
+                    kname, val = ln.split(",")
+                    traffic[kname] = float(val)
     except Exception:
         pass
 
