@@ -1,7 +1,8 @@
 // Fused x pass for the variable-viscosity step (BASELINE.json config 4, reading S14): rows a4 + a5 + a6 with
 // 12 fields backward (u v w phi phx phy phz exx eyy exy exz eyz) and 7 forward, in a tile of SIXTEEN field slots.
-// Same stages as k_xfused (kernels_xfused.cuh): thread = (butterfly, field slot), half-length real transform,
-// TMA-staged spectra rows, DIF backward / DIT forward with the radix-2 + pointwise stage in the middle.
+// Same stages A-F as the matched-viscosity kernels of kernels_xfused.cuh (half-length real transform, TMA-staged
+// spectra rows, DIF backward / DIT forward with the radix-2 + pointwise stage in the middle), here in the
+// thread = (butterfly, field slot) organisation with CTA-wide barriers between the stages.
 //   T_ij = -u_i u_j + cs (|grad phi|^2 delta_ij - phi_i phi_j) + eta1(phi) E_ij,  eta1 = eta_c (phi + 1),
 //   eta_c = (lambda - 1) / (2 Re);  E_zz = -E_xx - E_yy;  only T_ij - T_zz delta_ij is transformed (see psdns.cu).
 // Without it the variable-viscosity step runs three kernels with 19 physical-space arrays in HBM
