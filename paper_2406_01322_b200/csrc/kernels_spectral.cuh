@@ -621,13 +621,12 @@ struct SubstArgs {
 
 // The sweeps work in place, so the compiler cannot move the load of row k + 1 above the store of row k (same
 // pointer, run-time stride): every row then costs a full memory latency, which dominates on small grids (few
-// columns, little parallelism).  The loops below therefore load a GROUP of LOOKAHEAD rows into registers before the
-// previous group's results are stored (different rows: no hazard).
-#ifndef LOOKAHEAD_N
-#define LOOKAHEAD_N 4
-#endif
-constexpr int LOOKAHEAD = LOOKAHEAD_N;
+// columns, little parallelism).  The loops below therefore load a GROUP of G rows into registers before the
+// previous group's results are stored (different rows: no hazard).  G is a template parameter chosen by the host:
+// 4 on small grids (latency-bound), 2 above 60 k columns (DRAM-bound: more resident threads win; measured at
+// 1024x512x513: solve 4.23 ms with 2, 4.36 with 4, 4.51 with 8; at 256x256x257: 0.43 with 4, 0.42 with 8).
 
+template <int G>
 __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstArgs a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
@@ -637,7 +636,6 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
     col_wavenumbers(g, col, kx, ky);
     const size_t st = g.ncols;
     const int N = g.N;
-    constexpr int G = LOOKAHEAD;
     if (a.pair01 && blockIdx.y == 0) {      // omega_z and theta: same recurrence coefficients, two right-hand sides
         const double sigma = kx * kx + ky * ky + a.shift[0];
         cplx *x0 = a.x[0] + col, *x1 = a.x[1] + col;
@@ -749,6 +747,7 @@ struct Elim2Args {
     int phase;
 };
 
+template <int G>
 __global__ void __launch_bounds__(NT_COL, 3) k_elim2(const __grid_constant__ Elim2Args a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
@@ -766,8 +765,7 @@ __global__ void __launch_bounds__(NT_COL, 3) k_elim2(const __grid_constant__ Eli
         cplx *__restrict__ out = a.w + col;
         PivotDown pv;
         pv.init();
-        constexpr int G = LOOKAHEAD;
-        cplx q[G];
+            cplx q[G];
         auto load = [&](int k0, cplx (&r)[G]) {          // rows k0, k0 - 1, .. (descending)
 #pragma unroll
             for (int i = 0; i < G; ++i) if (k0 - i >= 2) r[i] = in[(k0 - i - 2) * st];
@@ -801,9 +799,8 @@ __global__ void __launch_bounds__(NT_COL, 3) k_elim2(const __grid_constant__ Eli
         PivotDown pv;
         pv.init();
         // in place: row k - 2 is read (as the right-hand side of row k) before it is overwritten by row k - 2's result,
-        // LOOKAHEAD >= 2 rows later in this loop order; the register look-ahead reads it even earlier
-        constexpr int G = LOOKAHEAD;
-        cplx q[G];
+        // G >= 2 rows later in this loop order; the register look-ahead reads it even earlier
+            cplx q[G];
         auto load = [&](int k0, cplx (&r)[G]) {
 #pragma unroll
             for (int i = 0; i < G; ++i) if (k0 - i >= 2) r[i] = x[(k0 - i - 2) * st];
@@ -858,6 +855,7 @@ struct FinishArgs {
     cplx *phz;         // [nkz][ncols]: D phi^, truncated (operator P)
 };
 
+template <int G>
 __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ FinishArgs a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
@@ -871,7 +869,6 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
     const bool phase = a.phi != nullptr;
     Chain1 cW, cP;
     cW.init(); cP.init();
-    constexpr int G = LOOKAHEAD;
     struct Row { cplx w, om, phi; };
     auto load = [&](int n0, Row (&r)[G]) {               // rows n0, n0 - 1, .. (descending)
 #pragma unroll

@@ -554,6 +554,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
     // a9 + first elimination (K_A), substitution (K_B), second elimination (K_C), substitution +
     // influence-matrix correction (K_D), velocity recovery (a11)
     const double inv_g = 1.0 / c.gamma;
+    const bool la2 = d.ncols > 60000;   // register look-ahead depth of the solver sweeps (kernels_spectral.cuh)
     const double *dNS = h->at<double>(L.dinv[0]), *dPO = h->at<double>(L.dinv[1]), *dCH = h->at<double>(L.dinv[2]);
     {
         RhsElimArgs a;
@@ -582,7 +583,8 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.pair01 = 1;
         a.coef = nullptr; a.wh = nullptr; a.thh = nullptr; a.th = nullptr;
         LaunchScope ls(h, KC_SOLVE);
-        k_subst<<<dim3(col_grid(d), a.nchains - 1), NT_COL, 0, h->st>>>(a);
+        if (la2) k_subst<2><<<dim3(col_grid(d), a.nchains - 1), NT_COL, 0, h->st>>>(a);
+        else k_subst<4><<<dim3(col_grid(d), a.nchains - 1), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     {
@@ -590,7 +592,8 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.g = geom(h); a.th = TH; a.w = W; a.phi = PHI; a.dinv_po = dPO; a.dinv_ch = dCH;
         a.hw = h->at<double>(L.hw); a.coef = h->at<cplx>(L.coef); a.lam_phi = c.lam_phi; a.phase = phase;
         LaunchScope ls(h, KC_SOLVE);
-        k_elim2<<<dim3(col_grid(d), phase ? 2 : 1), NT_COL, 0, h->st>>>(a);
+        if (la2) k_elim2<2><<<dim3(col_grid(d), phase ? 2 : 1), NT_COL, 0, h->st>>>(a);
+        else k_elim2<4><<<dim3(col_grid(d), phase ? 2 : 1), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     {
@@ -603,7 +606,8 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.pair01 = 0;
         a.coef = h->at<cplx>(L.coef); a.wh = h->at<double>(L.wh); a.thh = h->at<double>(L.thh); a.th = TH;
         LaunchScope ls(h, KC_SOLVE);
-        k_subst<<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
+        if (la2) k_subst<2><<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
+        else k_subst<4><<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     // a11: u^, v^ (and D phi^ for the next step)
@@ -612,7 +616,8 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.g = geom(h); a.om = OM; a.th = TH; a.u = U; a.v = V; a.w = W;
         a.phi = phase ? PHI : nullptr; a.phz = PHZ;
         LaunchScope ls(h, KC_SOLVE);
-        k_finish<<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        if (la2) k_finish<2><<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        else k_finish<4><<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     return cudaSuccess;
