@@ -360,7 +360,7 @@ def run_ours(args):
     traffic = {}
     try:
         if args.workload == "5c":
-            with open(os.path.join(ROOT, "profiles", "r1g_traffic_5c.csv")) as fh:
+            with open(os.path.join(ROOT, "profiles", "r1h_traffic_5c.csv")) as fh:
                 for ln in fh.read().strip().splitlines()[1:]:
                     kname, val = ln.split(",")
                     traffic[kname] = float(val)
