@@ -31,10 +31,12 @@ Pins (tests/test_oracle_*.py, all `-m "not gpu"`): Chebyshev transform of T_m an
 D T_3 = 3 T_0 + 6 T_2, equality with the length-2N DFT of the even extension (L178),
 plane waves / Parseval / shift theorem, dealiased product == exact truncated convolution,
 manufactured Helmholtz and biharmonic solutions, coupled-vs-influence-matrix w solve,
-Crank-Nicolson decay factor of a Stokes mode, steady Poiseuille flow, algebraic
+Crank-Nicolson decay factor of Stokes modes (omega_z mode with w = 0; clamped eigenmodes of the
+4th-order w equation, which pin H_w of Eq. 15), steady Poiseuille flow, algebraic
 divergence-freeness, the split-CH operator identity, the tanh equilibrium profile (Eq. 5),
+mean(phi) of an off-centre interface (closed form; drift falling spectrally with N),
 an independent sympy-differentiated manufactured RHS, and a brute-force all-dense
-re-formulation of one step on a tiny grid.
+re-formulation of the step on tiny grids (tests/test_oracle_bruteforce.py).
 Parity unpinned (no statement in the paper to pin against): the variable-viscosity term
 (reading S14) beyond its lambda=1 limit and the 1-D steady-state quadrature check.
 """
@@ -222,15 +224,6 @@ def boundary_rows(N: int, bc: int) -> np.ndarray:
     if bc == DIRICHLET:
         return np.stack([np.ones(N + 1), sgn])
     return np.stack([n * n, -sgn * n * n])
-
-
-def tau_matrix(N: int, sigma: float, bc: int) -> np.ndarray:
-    """(N+1)x(N+1) tau matrix of (D^2 - sigma) a = f: rows 0..N-2 of the operator, then the
-    two boundary rows (S11)."""
-    D = cheb_deriv_matrix(N)
-    A = D @ D - sigma * np.eye(N + 1)
-    A[N - 1:, :] = boundary_rows(N, bc)
-    return A
 
 
 def helmholtz_solve(f: np.ndarray, sigma: np.ndarray, bc: int,

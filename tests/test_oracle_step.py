@@ -1,5 +1,6 @@
 """Pins for the oracle's time step (not gpu): closed forms of the scheme and invariants.
- * Stokes mode decays by the Crank-Nicolson factor (channel version of exp(-nu k^2 t));
+ * Stokes mode decays by the Crank-Nicolson factor (channel version of exp(-nu k^2 t)), both for a mode that
+   lives in omega_z (w = 0) and for the clamped eigenmodes of the 4th-order w equation (w != 0: pins H_w, Eq. 15);
  * laminar Poiseuille flow is steady with G = 2/Re;
  * the new velocity is divergence-free algebraically;
  * the split Cahn-Hilliard solve satisfies the 4th-order operator identity (S8) and the
@@ -37,6 +38,56 @@ def test_stokes_mode_crank_nicolson_factor():
         assert np.abs(un - fac ** n * u).max() < 1e-12
         assert np.abs(vn).max() < 1e-13 and np.abs(wn).max() < 1e-13
     # and it approaches the viscous decay exp(-kappa^2 t / Re)
+    assert abs(fac ** 3 - math.exp(-kap2 * 3 * p.dt / p.re)) < 1e-9
+
+
+@pytest.mark.parametrize("parity", ["even", "odd"])
+def test_stokes_eigenmode_of_the_w_equation(parity):
+    """Pins the Crank-Nicolson right-hand side of Eq. 15, H_w = theta + gamma (D^2 - k^2) theta + dt NL_w
+    (reading S13), with w != 0.  Linearised Eq. 15: d/dt lap(w) = (1/Re) lap(lap(w)), w = dw/dz = 0 at z = +-1.  Eigenmodes:
+        even: W = cosh(kz)/cosh k - cos(mu z)/cos mu,  k tanh k + mu tan mu = 0
+        odd : W = sinh(kz)/sinh k - sin(mu z)/sin mu,  k coth k - mu cot mu = 0
+    (both give W(+-1) = W'(+-1) = 0; lap W = (k^2 + mu^2) x the trigonometric part, an eigenfunction of lap with
+    eigenvalue -(k^2 + mu^2)).  One step of the scheme multiplies w, theta = lap w and (through Eqs. 6, 16) u, v by
+    g = (1 - gamma kappa^2)/(1 + gamma kappa^2), kappa^2 = k^2 + mu^2, exactly in time and to spectral accuracy in z.
+    A single Fourier mode of amplitude A feeds back on itself only at O(A^3 dt), so A = 1e-3 leaves the non-linear
+    terms below rounding.  A wrong sign or factor on gamma lap(theta) gives g = 1 or worse: off by 4e-4 per step."""
+    from scipy.optimize import brentq
+    g = O.Grid(8, 8, 33)
+    p = O.Params(re=50.0, dt=2e-3, phase_field=0)
+    ii, jj = 2, 1
+    kx, ky = 2 * np.pi / g.lx * ii, 2 * np.pi / g.ly * jj
+    k = math.hypot(kx, ky)
+    if parity == "even":
+        mu = brentq(lambda m: k * math.tanh(k) + m * math.tan(m), math.pi / 2 + 1e-9, math.pi - 1e-9)
+        W = lambda z: np.cosh(k * z) / math.cosh(k) - np.cos(mu * z) / math.cos(mu)
+        dW = lambda z: k * np.sinh(k * z) / math.cosh(k) + mu * np.sin(mu * z) / math.cos(mu)
+    else:
+        mu = brentq(lambda m: k / math.tanh(k) - m / math.tan(m), math.pi + 1e-9, 1.5 * math.pi - 1e-9)
+        W = lambda z: np.sinh(k * z) / math.sinh(k) - np.sin(mu * z) / math.sin(mu)
+        dW = lambda z: k * np.cosh(k * z) / math.sinh(k) - mu * np.cos(mu * z) / math.sin(mu)
+    assert abs(W(1.0)) < 1e-12 and abs(dW(1.0)) < 1e-10 and abs(W(-1.0)) < 1e-12 and abs(dW(-1.0)) < 1e-10
+    z = O.cheb_nodes(g.N)[:, None, None]
+    x = g.lx / g.nx * np.arange(g.nx)[None, None, :]
+    y = g.ly / g.ny * np.arange(g.ny)[None, :, None]
+    A = 1e-3
+    ph = kx * x + ky * y
+    w = A * W(z) * np.cos(ph)
+    u = -(kx / k ** 2) * A * dW(z) * np.sin(ph)        # continuity (Eq. 6) with omega_z = 0 (Eq. 16)
+    v = -(ky / k ** 2) * A * dW(z) * np.sin(ph)
+    orc = O.Oracle(g, p)
+    orc.set_state("physical", u, v, w)
+    s0 = orc.state
+    w0, th0, u0, v0 = (f[:, jj, ii].copy() for f in (s0.w, s0.theta, s0.u, s0.v))
+    gam = p.dt / (2 * p.re)
+    kap2 = k * k + mu * mu
+    fac = (1 - gam * kap2) / (1 + gam * kap2)
+    assert 1e-4 < 1 - fac < 1e-2
+    for n in range(1, 4):
+        orc.step(1)
+        s = orc.state
+        for got, ref, tol in ((s.w, w0, 1e-12), (s.theta, th0, 1e-10), (s.u, u0, 1e-12), (s.v, v0, 1e-12)):
+            assert np.abs(got[:, jj, ii] - fac ** n * ref).max() < tol * np.abs(ref).max(), (parity, n)
     assert abs(fac ** 3 - math.exp(-kap2 * 3 * p.dt / p.re)) < 1e-9
 
 
@@ -136,6 +187,24 @@ def test_tanh_equilibrium_profile_is_stationary():
     u, v, w, _ = orc.get_state("physical")
     assert max(np.abs(u).max(), np.abs(v).max(), np.abs(w).max()) < 1e-9   # no spurious flow in x,y; 1-D
     assert abs(m1 - m0) < 1e-13                                           # z-odd profile: mean conserved
+
+
+def test_mean_phi_of_an_off_centre_interface():
+    """mean(phi) (Eq. 1 is a conservation law: d/dt int phi = (1/Pe) [d mu/dz] at the walls = 0 with the no-flux
+    conditions of reading S10) for an interface at z0 = 0.2, which is NOT z-odd:
+      * `mean_phi` equals the closed form (1/2) int tanh((z - z0)/w) dz = (w/2) ln[cosh((1 - z0)/w)/cosh((1 + z0)/w)];
+      * the tau scheme conserves it only up to the tau residual of the psi problem, which falls spectrally with
+        resolution (SURVEY 8(c) "mean(phi)": measured there 4e-5 at N = 128, Ch = 0.05 ... 2e-9 at N = 256, Ch = 0.07 over
+        10 steps): drift over 10 steps < 1e-8 at N = 256, Ch = 0.07, and >= 1000 x smaller than at N = 128."""
+    ch, z0 = 0.07, 0.2
+    w = math.sqrt(2) * ch
+    drift = {}
+    for N in (128, 256):
+        phi0, phi1, m0, m1, orc = _ch_1d(N, ch, 10, lambda z: np.tanh((z - z0) / w))
+        exact = 0.5 * w * (np.log(np.cosh((1 - z0) / w)) - np.log(np.cosh((1 + z0) / w)))
+        assert abs(m0 - exact) < 1e-12, (N, m0, exact)
+        drift[N] = abs(m1 - m0)
+    assert drift[256] < 1e-8 and drift[256] < 1e-3 * drift[128] and drift[128] < 1e-4, drift
 
 
 def test_non_equilibrium_profile_relaxes_towards_tanh():
