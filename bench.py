@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py - psdns_step throughput on B200 (grid-point-steps/s, ms/step, FP64) with roofline.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 5c|5b|5a|cfg1|cfg2|cfg3|cfg4|fig3] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 5c-channel|5c|5b|5a|cfg1|cfg2|cfg3|cfg4|fig3] [--impl reference]
 
 One "step" = one pass of the whole hot path (rows a1-a11 of DESIGN.md) over the state.
 Default workload = BASELINE.json config 5 on the 1024x512x513 grid (the grid the >= 60 % HBM
@@ -31,6 +31,7 @@ import numpy as np  # noqa: E402
 import psdns_inputs as I  # noqa: E402
 
 METRIC = "grid-point-steps/s"
+TRAFFIC_CSV = "r1h_traffic_5c.csv"   # ncu dram bytes per launch and kernel class, written from the --set full capture
 
 
 # ------------------------------------------------------------------------------------------------
@@ -40,6 +41,17 @@ def workload(tag: str):
     if tag in I.SCALING_GRIDS:
         c = I.scaling_config(tag)
         kind = "random-spectra"
+    elif tag.endswith("-channel") and tag[:-8] in I.SCALING_GRIDS:
+        # config-3 recipe (channel state: Poiseuille + solenoidal k^-5/3 perturbation + 64 drops, Ch = 0.025, We = 3,
+        # dt = 2e-5) on a config-5 grid.  SURVEY 8(d): "if the timed steps go non-finite, time the step on the config-3
+        # recipe at these grids instead and say so" - the random-spectra state blows up at 1024x512x513 with dt = 2e-5
+        # (an explicit-coupling time-step limit of the method at that resolution), so this is the
+        # default workload
+        nx, ny, nz = I.SCALING_GRIDS[tag[:-8]]
+        k3 = I.CONFIGS[3]
+        c = I.Config("cfg" + tag, nx, ny, nz, re=k3.re, ch=k3.ch, pe=k3.pe, we=k3.we, dt=k3.dt, steps=k3.steps,
+                     ndrops=k3.ndrops, radius=k3.radius, seed=k3.seed)
+        kind = "channel-state, config-3 recipe"
     elif tag == "cfg3":
         c = I.CONFIGS[3]
         kind = "channel-state"
@@ -53,6 +65,12 @@ def workload(tag: str):
     else:
         raise SystemExit(f"unknown workload {tag}")
     return c, kind
+
+
+def workload_string(c, kind) -> str:
+    """One string for both arms (ours and --impl reference), so the driver sees the same config."""
+    return (f"{c.name} psdns_step {c.nx}x{c.ny}x{c.nz} ({kind}), phase_field={c.phase_field}, "
+            f"visc_ratio={c.visc_ratio}")
 
 
 def algorithmic_bytes(c):
@@ -86,7 +104,14 @@ def algorithmic_bytes(c):
         "yfwd": nfw * (S_pyz + S_ppz),
         "zfwd": nfw * (S_ppz + S_ppp),
         "xfused": (nyb + nfw) * S_pyz,
+        # solver stage, column-resident bound (every array crosses HBM once): k_rhs_elim reads the nfw product spectra,
+        # the three AB2 history spectra and omega_z^, theta^, phi^ (all nz modes), writes the history; the sweeps that
+        # follow write u^ v^ w^ phi^ theta^ omega_z^ (all nz modes) and D phi^.  The g' arrays between the down and up
+        # sweeps of a solve are NOT algorithmic: whatever they add shows up as frac < 1.
+        "rhs": (nfw + 3) * S_ppp + 3 * S_ppz + 3 * S_ppp,
+        "solve": 6 * S_ppz + S_ppp,
     }
+    per_kernel["solver"] = per_kernel["rhs"] + per_kernel["solve"]
     # fused-pipeline figure of SURVEY 8(d) (7 in / 8 out fields; the contract figure, about 310 B per grid point):
     # physical-space arrays never leave the SM
     step_fused = (4 * S_ppp + nin * S_ppz) + nin * (S_ppz + S_pyz) + (nin + nout) * S_pyz \
@@ -240,7 +265,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": METRIC, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{c.name} psdns_step {c.nx}x{c.ny}x{c.nz} ({kind})"},
+        "config": {"workload": workload_string(c, kind)},
         "cpu_baseline": {"value": val, "unit": METRIC, "cores": threads, "kind": "oracle", "sample": desc},
         "e2e": {"value": val, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -325,6 +350,13 @@ def run_ours(args):
     finite = all(bool(torch.isfinite(torch.view_as_real(t)).all()) for t in out)
     maxabs = [float(torch.view_as_real(t).abs().max()) for t in out]
     del out
+    if not finite:
+        # a timing of kernels processing NaN / Inf is not a measurement of this workload: no metric line, non-zero exit
+        sys.stderr.write(f"bench.py: state of workload {args.workload} is non-finite after {args.warmup} + {args.steps} steps "
+                         f"(max-abs {maxabs}); refusing to report a value\n")
+        if world > 1:
+            dist.destroy_process_group()
+        raise SystemExit(3)
     ms_max = reduce_max_ms(ms, world, "cuda")
     value = aggregate_value(M, args.steps, ms_max, world)
 
@@ -354,13 +386,19 @@ def run_ours(args):
                 ent["gbs"] = per_kernel[name] / (tot / ksteps * 1e-3) / 1e9 if tot > 0 else None
                 ent["frac"] = ent["gbs"] / peak if tot > 0 else None
             kernels[name] = ent
-    dominant = max((k for k in kernels if k in per_kernel), key=lambda k: kernels[k]["ms_per_step"], default=None)
+    if "rhs" in kernels and "solve" in kernels:
+        tms = kernels["rhs"]["ms_per_step"] + kernels["solve"]["ms_per_step"]
+        kernels["solver"] = {"ms_per_step": tms, "launches_per_step": kernels["rhs"]["launches_per_step"] + kernels["solve"]["launches_per_step"],
+                             "alg_bytes_per_step": per_kernel["solver"], "gbs": per_kernel["solver"] / (tms * 1e-3) / 1e9,
+                             "frac": per_kernel["solver"] / (tms * 1e-3) / 1e9 / peak,
+                             "note": "rhs + solve classes together (k_rhs_elim ... k_finish), column-resident bound"}
+    dominant = max((k for k in kernels if k in per_kernel and k != "solver"), key=lambda k: kernels[k]["ms_per_step"], default=None)
     # measured DRAM traffic per launch from the committed ncu --set full capture of this workload (text summary
     # under profiles/; null for workloads that were not captured)
     traffic = {}
     try:
-        if args.workload == "5c":
-            with open(os.path.join(ROOT, "profiles", "r1h_traffic_5c.csv")) as fh:
+        if args.workload in ("5c", "5c-channel"):     # same grid, same kernels: DRAM traffic does not depend on the data
+            with open(os.path.join(ROOT, "profiles", TRAFFIC_CSV)) as fh:
                 for ln in fh.read().strip().splitlines()[1:]:
                     kname, val = ln.split(",")
                     traffic[kname] = float(val)
@@ -384,6 +422,43 @@ def run_ours(args):
     e2e_max = reduce_max_ms(e2e_ms, world, "cuda")
     e2e_val = aggregate_value(M, esteps, e2e_max, world)
     e2e_finite = all(bool(torch.isfinite(torch.view_as_real(t) if t.is_complex() else t).all()) for t in pinned_out)
+    if not e2e_finite:
+        sys.stderr.write("bench.py: end-to-end output is non-finite; refusing to report a value\n")
+        raise SystemExit(3)
+    del pinned_out
+
+    # ---- forward + backward transform round trip of one field, dealiasing off (BASELINE.json config 5) ----------
+    roundtrip = None
+    if rank == 0:
+        R = 8 * M
+        S_full = 16 * (c.nx // 2 + 1) * c.ny * c.nz
+        xin = torch.from_numpy(I.random_physical_field(c.nx, c.ny, c.nz, seed=5)).cuda()
+        rt = solver.transform_roundtrip(P.PHYSICAL, xin)           # warm-up, and the identity check
+        rt_err = float(torch.linalg.vector_norm(rt - xin) / torch.linalg.vector_norm(xin))
+        del rt
+        rsteps = max(1, min(args.steps, 5))
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        r0.record()
+        for _ in range(rsteps):
+            rt = solver.transform_roundtrip(P.PHYSICAL, xin)
+        r1.record()
+        torch.cuda.synchronize()
+        rt_ms = r0.elapsed_time(r1) / rsteps
+        del rt, xin
+        # each of the 3 + 3 one-dimensional passes reads and writes its array once (x: R <-> S_full, y and z: S_full <->
+        # S_full), and the boundary-layout copy on either side of the spectrum moves S_full twice more
+        passes = 2 * R + 10 * S_full
+        roundtrip = {"ms": rt_ms, "rel_l2_identity_error": rt_err, "fields": 1, "dealias": 0,
+                     "alg_bytes_min": 2 * (R + S_full), "gbs_min": 2 * (R + S_full) / (rt_ms * 1e-3) / 1e9,
+                     "alg_bytes_passes": passes, "gbs_passes": passes / (rt_ms * 1e-3) / 1e9,
+                     "frac_passes": passes / (rt_ms * 1e-3) / 1e9 / peak,
+                     "note": "psdns_transform_roundtrip PHYSICAL -> SPECTRAL -> PHYSICAL, full (unpruned) sizes; "
+                             "alg_bytes_min = read R, write S, read S, write R; alg_bytes_passes = six 1-D passes each "
+                             "reading and writing its array once"}
+        if rt_err > 1e-11:
+            sys.stderr.write(f"bench.py: transform round trip error {rt_err:.2e} > 1e-11\n")
+            raise SystemExit(3)
 
     if rank == 0:
         roof = None
@@ -402,8 +477,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{c.name} psdns_step {c.nx}x{c.ny}x{c.nz} ({kind}), phase_field={c.phase_field}, "
-                                   f"visc_ratio={c.visc_ratio}", "grid": [c.nx, c.ny, c.nz],
+            "config": {"workload": workload_string(c, kind), "grid": [c.nx, c.ny, c.nz],
                        "l2": "inputs larger than L2 (state and intermediates >> 126 MB)" if M > 4e6 else "small grid: L2-resident, no roofline claim",
                        "parallelism": "replicas only" if world > 1 else "single GPU", "finite": finite, "max_abs": maxabs},
             "clocks": clocks,
@@ -416,6 +490,7 @@ def run_ours(args):
                               "achieved_gbs": step_fused_bytes / (ms_max / args.steps * 1e-3) / 1e9,
                               "frac": step_fused_bytes / (ms_max / args.steps * 1e-3) / 1e9 / peak},
             "kernels": kernels,
+            "roundtrip": roundtrip,
             "cpu_baseline": cpu,
         }
         print(json.dumps(line))
@@ -429,7 +504,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="5c")
+    ap.add_argument("--workload", default="5c-channel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -135,6 +135,38 @@ long long psdns_launch_count(const psdns_handle *h);
 int psdns_kernel_timing(psdns_handle *h, const char *name, int enable);
 int psdns_kernel_time_ms(psdns_handle *h, double *ms_total, long long *launches);
 
+/* Diagnostics of the current state, computed on the device from the resident spectra (the fields a run
+ * monitors) - no host round trip, asynchronous on the stream.  d_out: DEVICE memory, 8 doubles:
+ *   [0] mean(phi)          volume average, 1/2 sum_{n even} phi^(0,0,n) 2/(1 - n^2)   (0 when phase_field == 0)
+ *   [1] max |div u|        max over all retained coefficients of |i kx u^ + i ky v^ + D w^|  (Eq. 6)
+ *   [2] kinetic energy     1/2 <u^2 + v^2 + w^2>: mean over x, y (Parseval over the retained modes), Clenshaw-Curtis
+ *                          quadrature over the collocation points z_k, divided by the channel height 2
+ *   [3] [4] wall shear     d u-bar/dz at z = +1 and at z = -1 (mean streamwise velocity, column (0,0))
+ *   [5] bulk velocity      1/2 int u-bar dz
+ *   [6] [7]                reserved, written as 0
+ * Uses the transform scratch (not the state).  PSDNS_ESTATE before the first set_state. */
+int psdns_diagnostics(psdns_handle *h, double *d_out);
+
+/* Tuning and test switches.  None is needed for normal use; the defaults are the product path.  Changing an option
+ * drops the captured CUDA graph of the step (it is re-captured by the next psdns_step).
+ *   "graph"    1 (default) / 0 : replay one captured CUDA graph per step / launch the kernels directly
+ *   "xfuse"    1 (default) / 0 : fused x kernel (rows a4-a6 in one kernel, physical space never in HBM) / the three-kernel
+ *                                cross-check path x-backward -> pointwise -> x-forward through physical-space arrays;
+ *                                0 needs a workspace of psdns_workspace_bytes_unfused() bytes at init, else PSDNS_ENOMEM
+ *   "grid_cap" n >= 0          : upper bound on the grid of every persistent kernel (z, y, fused x passes); 0 = none.
+ *                                Tests use a small cap so that each CTA walks many tiles / lines of a small grid.
+ *   "pf", "pf_rhs" n >= 0      : L2 prefetch distance, in rows, of the solver sweeps (defaults 2 and 4)
+ * PSDNS_EINVAL on an unknown name or a bad value. */
+int psdns_set_option(psdns_handle *h, const char *name, double value);
+
+/* Workspace size that also holds the physical-space arrays of the unfused cross-check path ("xfuse" 0). */
+size_t psdns_workspace_bytes_unfused(const psdns_grid *grid, const psdns_params *params);
+
+/* Introspection for tests and bench.py; -1 on an unknown name.  "<class>_grid" / "<class>_items": grid size and number
+ * of work items (tiles or lines) of the last launch of the persistent kernel class <class> = zbwd | ybwd | xfused |
+ * yfwd | zfwd; "n_sm"; "workspace_bytes"; "launches_per_step" (kernels in the captured graph of one step). */
+double psdns_get_info(const psdns_handle *h, const char *name);
+
 /* Release the handle (host memory only; the workspace stays the caller's). */
 int psdns_destroy(psdns_handle *h);
 

@@ -540,6 +540,40 @@ def mean_phi(g: Grid, phi_hat):
     return float(np.real(np.sum(phi_hat[n, 0, 0] * (2.0 / (1.0 - n.astype(np.float64) ** 2)))) * 0.5)
 
 
+def clenshaw_curtis_weights(N: int) -> np.ndarray:
+    """Quadrature weights on z_k = cos(pi k/N) that integrate every polynomial of degree <= N exactly over
+    [-1, 1]: int f dz = sum_{n even} a_n 2/(1 - n^2) with a = forward Chebyshev transform of f, hence
+    w_k = sum_{n even} 2/(1 - n^2) Cf[n, k]."""
+    n = np.arange(0, N + 1, 2)
+    return (2.0 / (1.0 - n.astype(np.float64) ** 2)) @ cheb_fwd_matrix(N)[n, :]
+
+
+def kinetic_energy(g: Grid, u_hat, v_hat, w_hat) -> float:
+    """Volume-averaged kinetic energy (1/2) <u^2 + v^2 + w^2> of the diagnostics row,
+    evaluated the plain way: fields in physical space, mean over the periodic x, y points, Clenshaw-Curtis quadrature
+    over the collocation points in z, divided by the channel height 2."""
+    e = sum(backward_transform(a, g) ** 2 for a in (u_hat, v_hat, w_hat))
+    return float(0.25 * np.sum(clenshaw_curtis_weights(g.N) * e.mean(axis=(1, 2))))
+
+
+def wall_shear(g: Grid, u_hat):
+    """d u-bar/dz of the mean streamwise velocity (the (0,0) column) at z = +1 and z = -1:
+    T_n'(+-1) = (+-1)^(n+1) n^2."""
+    n = np.arange(g.nz, dtype=np.float64)
+    a = np.real(u_hat[:, 0, 0])
+    return float(np.sum(n * n * a)), float(np.sum(np.where(np.arange(g.nz) % 2 == 0, -1.0, 1.0) * n * n * a))
+
+
+def bulk_velocity(g: Grid, u_hat) -> float:
+    """(1/2) int u-bar dz, same quadrature as mean_phi."""
+    return mean_phi(g, u_hat)
+
+
+def max_divergence(g: Grid, u, v, w) -> float:
+    """max over the spectrum of |i kx u^ + i ky v^ + D w^|."""
+    return float(np.abs(divergence_spectrum(g, u, v, w)).max())
+
+
 def rel_l2(a, b):
     """||a - b||_2 / ||b||_2 over all entries."""
     a, b = np.asarray(a), np.asarray(b)

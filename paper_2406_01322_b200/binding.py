@@ -13,6 +13,7 @@ EXPORTS = [
     "psdns_transform_roundtrip", "psdns_run_host", "psdns_launch_count", "psdns_kernel_timing",
     "psdns_kernel_time_ms", "psdns_destroy", "psdns_last_error",
     "psdns_history_bytes", "psdns_get_history", "psdns_set_history",
+    "psdns_set_option", "psdns_get_info", "psdns_workspace_bytes_unfused", "psdns_diagnostics",
 ]
 
 
@@ -74,6 +75,14 @@ def load_library():
     lib.psdns_get_history.argtypes = [vp, vp, C.c_size_t]
     lib.psdns_set_history.restype = ci
     lib.psdns_set_history.argtypes = [vp, vp, C.c_size_t]
+    lib.psdns_diagnostics.restype = ci
+    lib.psdns_diagnostics.argtypes = [vp, vp]
+    lib.psdns_set_option.restype = ci
+    lib.psdns_set_option.argtypes = [vp, C.c_char_p, cd]
+    lib.psdns_get_info.restype = cd
+    lib.psdns_get_info.argtypes = [vp, C.c_char_p]
+    lib.psdns_workspace_bytes_unfused.restype = C.c_size_t
+    lib.psdns_workspace_bytes_unfused.argtypes = [C.POINTER(psdns_grid), C.POINTER(psdns_params)]
     lib.psdns_destroy.restype = ci
     lib.psdns_destroy.argtypes = [vp]
     lib.psdns_last_error.restype = C.c_char_p
@@ -96,7 +105,7 @@ class Solver:
     include/psdns.h: PHYSICAL float64 [nz, ny, nx]; SPECTRAL complex128 [nz, ny, nx//2+1]."""
 
     def __init__(self, nx, ny, nz, lx, ly, *, re, dt, pe=1.0, ch=1.0, we=1.0, gradp_x=0.0,
-                 visc_ratio=1.0, phase_field=1, dealias=1, device="cuda:0"):
+                 visc_ratio=1.0, phase_field=1, dealias=1, device="cuda:0", unfused_workspace=False):
         import torch
         self.torch = torch
         self.lib = load_library()
@@ -107,7 +116,8 @@ class Solver:
         self.params = psdns_params(re, pe, ch, we, dt, gradp_x, visc_ratio, phase_field, dealias)
         self.nx, self.ny, self.nz = nx, ny, nz
         self.phase = bool(phase_field)
-        nbytes = self.lib.psdns_workspace_bytes(C.byref(self.grid), C.byref(self.params))
+        wsfn = self.lib.psdns_workspace_bytes_unfused if unfused_workspace else self.lib.psdns_workspace_bytes
+        nbytes = wsfn(C.byref(self.grid), C.byref(self.params))
         if nbytes == 0:
             raise PsdnsError("psdns_workspace_bytes: invalid grid/params")
         self.workspace_bytes = nbytes
@@ -194,6 +204,20 @@ class Solver:
         ms, n = C.c_double(), C.c_longlong()
         self._check(self.lib.psdns_kernel_time_ms(self.handle, C.byref(ms), C.byref(n)))
         return ms.value, n.value
+
+    DIAG_NAMES = ("mean_phi", "max_div", "kinetic_energy", "shear_top", "shear_bottom", "bulk_velocity")
+
+    def diagnostics(self):
+        """psdns_diagnostics into a fresh device tensor of 8 doubles (asynchronous; index with DIAG_NAMES order)."""
+        out = self.torch.empty(8, dtype=self.torch.float64, device=self.device)
+        self._check(self.lib.psdns_diagnostics(self.handle, _ptr(out)))
+        return out
+
+    def set_option(self, name, value):
+        self._check(self.lib.psdns_set_option(self.handle, name.encode(), float(value)))
+
+    def get_info(self, name):
+        return float(self.lib.psdns_get_info(self.handle, name.encode()))
 
     def close(self):
         if getattr(self, "handle", None):

@@ -18,6 +18,7 @@
 #include "kernels_transform.cuh"
 #include "kernels_xfused.cuh"
 #include "kernels_xfused_visc.cuh"
+#include "kernels_diag.cuh"
 
 using namespace psdns;
 
@@ -47,6 +48,7 @@ struct Dims {
 struct Layout {
     size_t tw_x, tw_y, tw_z;
     size_t ctab_z;                     // c_k of the half-length Chebyshev transform, k <= N/2
+    size_t ccw;                        // Clenshaw-Curtis weights on z_k (diagnostics), nz doubles
     size_t state[5];                   // u v w phi theta
     size_t hist[3];
     size_t dinv[3];                    // NS (beta^2), PO (k^2), CH (k^2 + lambda)
@@ -58,7 +60,7 @@ struct Layout {
     size_t zb[MAXF], yb[MAXF], ph[MAXF];
     size_t small;                      // ab[2] doubles + counter
     size_t stage[4];                   // host-staging device buffers (boundary layout)
-    size_t total;
+    size_t total, total_unfused;
 };
 
 }  // namespace
@@ -79,9 +81,21 @@ struct psdns_handle {
     int timed_class;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tevents;
     int nf_in, nf_out;
-    bool use_xfused;
+    bool use_xfused, has_unfused_ws;
     int xf_occ, xfv_occ, n_sm;
     int occ_z[2], occ_y[2];     // resident CTAs per SM of the persistent z / y passes, [fwd]
+    int yx_chunk;               // psdns_set_option("yx_chunk"): z planes per chunk of the y -> x -> y sequence (0 = whole grid)
+    int l2_window;              // psdns_set_option("l2_window"): 1 = persisting-L2 access window over the Y ring
+    int grid_cap;               // psdns_set_option("grid_cap"): upper bound on the grid of every persistent kernel (0 = none)
+    int pf, pf_rhs;             // L2 prefetch distances of the column sweeps, in rows
+    long long last_grid[KC_COUNT], last_items[KC_COUNT];   // grid / work items of the last launch of each persistent class
+
+    int persistent_grid(int kc, long long items, int occ) {
+        long long g = std::min<long long>(items, (long long)n_sm * std::max(occ, 1));
+        if (grid_cap > 0) g = std::min<long long>(g, grid_cap);
+        last_grid[kc] = g; last_items[kc] = items;
+        return (int)g;
+    }
 
     template <class T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
 };
@@ -127,6 +141,7 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.tw_y = take(d.ny * C);
     L.tw_z = take(2 * d.N * C);
     L.ctab_z = take((d.N / 2 + 1) * C);
+    L.ccw = take(d.nz * sizeof(double));
     for (int i = 0; i < 5; ++i) L.state[i] = take(d.s_ret * C);
     for (int i = 0; i < 3; ++i) L.hist[i] = take(d.s_low * C);
     for (int i = 0; i < 3; ++i) L.dinv[i] = take(d.s_ret * sizeof(double));
@@ -148,11 +163,14 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     for (int i = 0; i < nf; ++i) { L.yb[i] = take(d.s_y * C); zy_bytes += align_up(d.s_y * C); }
     const size_t need_full = 3 * align_up(d.s_full * C);
     if (zy_bytes < need_full) take(need_full - zy_bytes);
-    for (int i = 0; i < nf; ++i) L.ph[i] = take(d.s_p * sizeof(double));
     L.small = take(64);
     const size_t stage_bytes = std::max(d.s_p * sizeof(double), d.s_bspec * C);
     for (int i = 0; i < 4; ++i) L.stage[i] = take(stage_bytes);
     L.total = o;
+    // physical-space arrays of the UNFUSED x path (psdns_set_option "xfuse" 0, a cross-check): behind the product's
+    // workspace, present only when the caller passed psdns_workspace_bytes_unfused() bytes to psdns_init
+    for (int i = 0; i < nf; ++i) L.ph[i] = take(d.s_p * sizeof(double));
+    L.total_unfused = o;
     return L;
 }
 
@@ -195,9 +213,8 @@ ColGeom geom(const psdns_handle *h) {
     // L2 prefetch distances in rows (kernels_spectral.cuh).  Measured on B200: 2 (4 for k_rhs_elim) is best at 117 k
     // columns, where 6 thrashed the L2, and longer distances do not help the latency-bound small grids either
     // (256x256x257: solve 0.82 ms at 2 rows, 0.84 at 12, 0.90 at 24).
-    static const char *e_pf = std::getenv("PSDNS_PF"), *e_pfr = std::getenv("PSDNS_PF_RHS");
-    g.pf = e_pf ? std::atoi(e_pf) : 2;
-    g.pf_rhs = e_pfr ? std::atoi(e_pfr) : 4;
+    g.pf = h->pf;
+    g.pf_rhs = h->pf_rhs;
     return g;
 }
 
@@ -261,7 +278,7 @@ cudaError_t launch_zpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, 
     const cplx *tw = h->at<cplx>(h->L.tw_z);
     const cplx *ct = h->at<cplx>(h->L.ctab_z);
     const long long ntiles = (long long)(ncols / 8) * nf;
-    const int grid = (int)std::min<long long>(ntiles, (long long)h->n_sm * std::max(h->occ_z[fwd], 1));
+    const int grid = h->persistent_grid(fwd ? KC_ZFWD : KC_ZBWD, ntiles, h->occ_z[fwd]);
     LaunchScope ls(h, fwd ? KC_ZFWD : KC_ZBWD);
 #define ZH(NN)                                                                                           \
     {                                                                                                    \
@@ -273,11 +290,12 @@ cudaError_t launch_zpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, 
     return cudaGetLastError();
 }
 
-cudaError_t launch_ypass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, int kxp, int nky, int jpos) {
-    YArgs a; a.f = f; a.nf = nf; a.nz = h->d.nz; a.kxp = kxp; a.nky = nky; a.jpos = jpos;
+cudaError_t launch_ypass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, int kxp, int nky, int jpos, int nplanes = -1) {
+    if (nplanes < 0) nplanes = h->d.nz;
+    YArgs a; a.f = f; a.nf = nf; a.nz = nplanes; a.kxp = kxp; a.nky = nky; a.jpos = jpos;
     const cplx *tw = h->at<cplx>(h->L.tw_y);
-    const long long ntiles = (long long)(kxp / 8) * h->d.nz * nf;
-    const int grid = (int)std::min<long long>(ntiles, (long long)h->n_sm * std::max(h->occ_y[fwd], 1));
+    const long long ntiles = (long long)(kxp / 8) * nplanes * nf;
+    const int grid = h->persistent_grid(fwd ? KC_YFWD : KC_YBWD, ntiles, h->occ_y[fwd]);
     LaunchScope ls(h, fwd ? KC_YFWD : KC_YBWD);
 #define YL(LL)                                                                                          \
     {                                                                                                   \
@@ -367,7 +385,7 @@ cudaError_t setup_attrs(psdns_handle *h) {
 
 cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
     const cplx *tw = h->at<cplx>(h->L.tw_x);
-    const int grid = std::min(a.nlines, h->n_sm * std::max(h->xf_occ, 1));   // persistent: one wave
+    const int grid = h->persistent_grid(KC_XFUSED, a.nlines, h->xf_occ);   // persistent: one wave
     LaunchScope ls(h, KC_XFUSED);
 #define XF(LL)                                                                                               \
     {                                                                                                        \
@@ -387,7 +405,7 @@ cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
 
 cudaError_t launch_xfusedv(psdns_handle *h, const XFVArgs &a) {
     const cplx *tw = h->at<cplx>(h->L.tw_x);
-    const int grid = std::min(a.nlines, h->n_sm * std::max(h->xfv_occ, 1));   // persistent: one wave
+    const int grid = h->persistent_grid(KC_XFUSED, a.nlines, h->xfv_occ);   // persistent: one wave
     LaunchScope ls(h, KC_XFUSED);
 #define XFV(LL) k_xfusedv<LL><<<grid, xv_threads<LL>(), xfusedv_smem<LL>(h->d.nkx), h->st>>>(a, tw);
     DISPATCH_L(h->d.nx, XFV)
@@ -397,7 +415,7 @@ cudaError_t launch_xfusedv(psdns_handle *h, const XFVArgs &a) {
 
 cudaError_t launch_relayout(psdns_handle *h, cplx *dst, const cplx *src, SpecSide ds, SpecSide ss, int nplanes) {
     const size_t total = (size_t)nplanes * ds.rows * ds.pitch;
-    const int blocks = (int)std::min<size_t>((total + 255) / 256, 148 * 16);
+    const int blocks = (int)std::min<size_t>((total + 255) / 256, (size_t)h->n_sm * 16);
     LaunchScope ls(h, KC_MISC);
     k_relayout<<<blocks, 256, 0, h->st>>>(dst, src, ds, ss, nplanes);
     return cudaGetLastError();
@@ -439,6 +457,28 @@ Coefs coefs(const psdns_params &p) {
         cudaError_t e__ = (expr);                 \
         if (e__ != cudaSuccess) return e__;       \
     } while (0)
+
+// Persisting-L2 access window over the Y ring of the chunked y -> x -> y sequence (psdns_set_option "l2_window" 1):
+// accesses to the ring are marked persisting (they stay in the set-aside part of the L2), everything else streaming.
+cudaError_t apply_l2_window(psdns_handle *h, cudaStream_t st) {
+    if (!h->l2_window || h->yx_chunk <= 0) return cudaSuccess;
+    const Dims &d = h->d;
+    const size_t ring_bytes = (size_t)h->nf_out * h->yx_chunk * d.ny * d.kxp * sizeof(cplx);
+    int dev = 0, max_persist = 0, max_win = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev));
+    CU(cudaDeviceGetAttribute(&max_win, cudaDevAttrMaxAccessPolicyWindowSize, dev));
+    const size_t set_aside = std::min<size_t>(ring_bytes, (size_t)max_persist);
+    CU(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, set_aside));
+    cudaStreamAttrValue v;
+    std::memset(&v, 0, sizeof(v));
+    v.accessPolicyWindow.base_ptr = h->ws + h->L.yb[0];
+    v.accessPolicyWindow.num_bytes = std::min<size_t>(ring_bytes, (size_t)max_win);
+    v.accessPolicyWindow.hitRatio = (float)std::min(1.0, (double)set_aside / (double)v.accessPolicyWindow.num_bytes);
+    v.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    v.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+    return cudaStreamSetAttribute(st, cudaStreamAttributeAccessPolicyWindow, &v);
+}
 
 // ---- one time step (rows a1-a11) ------------------------------------------------------------------
 // Field bookkeeping (matched viscosity, phase field on):
@@ -500,7 +540,8 @@ cudaError_t enqueue_step(psdns_handle *h) {
     for (int i = 0; i < nz_f; ++i) { fz.in[i] = src[i]; fz.out[i] = h->at<cplx>(L.zb[i]); }
     for (int i = 0; i < ny_f; ++i) { fy.in[i] = h->at<cplx>(L.zb[i]); fy.out[i] = h->at<cplx>(L.yb[i]); }
     CU(launch_zpass(h, false, fz, nz_f, d.ncols, d.nkz, d.kxp, d.nky, d.jpos, zd));
-    CU(launch_ypass(h, false, fy, ny_f, d.kxp, d.nky, d.jpos));
+    const bool chunked = h->yx_chunk > 0 && h->use_xfused && !visc;
+    if (!chunked) CU(launch_ypass(h, false, fy, ny_f, d.kxp, d.nky, d.jpos));
     FieldPtrs gy{}, gz{};
     for (int i = 0; i < nout; ++i) {
         gy.in[i] = h->at<cplx>(L.yb[i]); gy.out[i] = h->at<cplx>(L.zb[i]);
@@ -515,6 +556,29 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.kxp = d.kxp; a.nkx = d.nkx; a.nlines = d.nz * d.ny;
         a.cs = c.cs; a.kxf = 2.0 * M_PI / h->g.lx; a.eta_c = (p.visc_ratio - 1.0) / (2.0 * p.re);
         CU(launch_xfusedv(h, a));
+    } else if (chunked) {
+        // a3 .. a7 in chunks of yx_chunk z planes through a small RING of Y arrays (the first planes of the Y region,
+        // fields back to back), so that the Y arrays live in the 126 MB L2 between the y-backward pass, the fused x
+        // kernel and the y-forward pass of a chunk instead of crossing HBM four times
+        const int C = h->yx_chunk;
+        const size_t ring_field = (size_t)C * d.ny * d.kxp;           // cplx per field in the ring
+        cplx *ring = h->at<cplx>(L.yb[0]);
+        const int stage_src[6] = {0, 1, 2, 3, 5, 4};   // u v w phi phy phz  <-  Y arrays u v w phi phz phy
+        for (int z0 = 0; z0 < d.nz; z0 += C) {
+            const int np = std::min(C, d.nz - z0);
+            const size_t zoff = (size_t)z0 * d.nky * d.kxp;
+            FieldPtrs cy{}, dy{};
+            for (int i = 0; i < ny_f; ++i) { cy.in[i] = h->at<cplx>(L.zb[i]) + zoff; cy.out[i] = ring + i * ring_field; }
+            CU(launch_ypass(h, false, cy, ny_f, d.kxp, d.nky, d.jpos, np));
+            XFArgs a;
+            for (int i = 0; i < 6; ++i) a.in[i] = ring + (phase ? stage_src[i] : (i < 3 ? i : 0)) * ring_field;
+            for (int i = 0; i < 8; ++i) a.out[i] = ring + (i < nout ? i : 0) * ring_field;
+            a.kxp = d.kxp; a.nkx = d.nkx; a.nlines = np * d.ny;
+            a.cs = c.cs; a.kxf = 2.0 * M_PI / h->g.lx;
+            CU(launch_xfused(h, a));
+            for (int i = 0; i < nout; ++i) { dy.in[i] = ring + i * ring_field; dy.out[i] = h->at<cplx>(L.zb[i]) + zoff; }
+            CU(launch_ypass(h, true, dy, nout, d.kxp, d.nky, d.jpos, np));
+        }
     } else if (h->use_xfused && !visc) {
         // a4 + a5 + a6 fused: physical space never leaves the SM; in place on the Y arrays
         XFArgs a;
@@ -525,7 +589,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.cs = c.cs; a.kxf = 2.0 * M_PI / h->g.lx;
         CU(launch_xfused(h, a));
     } else {
-        // unfused path (variable viscosity, or PSDNS_NO_XFUSE): a4, a5, a6 as separate kernels
+        // unfused cross-check path (psdns_set_option "xfuse" 0): a4, a5, a6 as separate kernels
         FieldPtrs fx{}, gx{};
         const int nx_f = ny_f;
         for (int i = 0; i < nx_f; ++i) { fx.in[i] = h->at<cplx>(L.yb[i]); fx.out[i] = h->at<double>(L.ph[i]); }
@@ -542,14 +606,14 @@ cudaError_t enqueue_step(psdns_handle *h) {
             a.n = d.s_p; a.cs = c.cs; a.eta_c = (p.visc_ratio - 1.0) / (2.0 * p.re);
             a.phase = phase; a.visc = visc;
             LaunchScope ls(h, KC_PW);
-            k_pointwise<<<148 * 8, 256, 0, h->st>>>(a);
+            k_pointwise<<<h->n_sm * 8, 256, 0, h->st>>>(a);
             CU(cudaGetLastError());
         }
         for (int i = 0; i < nout; ++i) { gx.in[i] = h->at<double>(L.ph[i]); gx.out[i] = h->at<cplx>(L.yb[i]); }
         CU(launch_xpass(h, true, gx, nout, d.kxp, d.nkx));
     }
     // a7-a8: forward y, z with truncation
-    CU(launch_ypass(h, true, gy, nout, d.kxp, d.nky, d.jpos));
+    if (!chunked) CU(launch_ypass(h, true, gy, nout, d.kxp, d.nky, d.jpos));
     CU(launch_zpass(h, true, gz, nout, d.ncols, d.nkz, d.kxp, d.nky, d.jpos));
     // a9 + first elimination (K_A), substitution (K_B), second elimination (K_C), substitution +
     // influence-matrix correction (K_D), velocity recovery (a11)
@@ -654,6 +718,20 @@ cudaError_t build_tables(psdns_handle *h) {
         CU(cudaMemcpyAsync(h->ws + L.ctab_z, t.data(), t.size() * sizeof(cplx), cudaMemcpyHostToDevice, h->st));
         CU(cudaStreamSynchronize(h->st));
     }
+    {   // Clenshaw-Curtis weights w_k = (c_k / N) [1 - sum_{j=1}^{N/2} b_j cos(2 j k pi / N) / (4 j^2 - 1)], b_{N/2} = 1 else 2,
+        // c_0 = c_N = 1 else 2 (N even): exact for polynomials of degree <= N on the Gauss-Lobatto points
+        std::vector<double> t(d.nz);
+        const long double pi = 3.14159265358979323846264338327950288L;
+        for (int k = 0; k <= d.N; ++k) {
+            long double acc = 1.0L;
+            for (int j = 1; j <= d.N / 2; ++j)
+                acc -= (j == d.N / 2 ? 1.0L : 2.0L) * cosl(2.0L * pi * (long double)j * (long double)k / (long double)d.N) /
+                       (4.0L * (long double)j * (long double)j - 1.0L);
+            t[k] = (double)(((k == 0 || k == d.N) ? 1.0L : 2.0L) * acc / (long double)d.N);
+        }
+        CU(cudaMemcpyAsync(h->ws + L.ccw, t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
+        CU(cudaStreamSynchronize(h->st));
+    }
     {   // p_k, q_k, r_k of the quasi-tridiagonal recurrence (kernels_spectral.cuh), k-only: constant memory
         static double hp[HELM_KMAX + 1], hq[HELM_KMAX + 1], hr[HELM_KMAX + 1];
         for (int k = 0; k <= HELM_KMAX; ++k) { hp[k] = helm_p_host(k); hq[k] = helm_q_host(k); hr[k] = helm_r_host(k); }
@@ -723,6 +801,11 @@ size_t psdns_workspace_bytes(const psdns_grid *grid, const psdns_params *params)
     return make_layout(make_dims(*grid), *params).total;
 }
 
+size_t psdns_workspace_bytes_unfused(const psdns_grid *grid, const psdns_params *params) {
+    if (!validate(grid, params)) return 0;
+    return make_layout(make_dims(*grid), *params).total_unfused;
+}
+
 int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_workspace, size_t bytes, void *cuda_stream,
                psdns_handle **out) {
     if (!out) return PSDNS_EINVAL;
@@ -735,8 +818,10 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->L = make_layout(h->d, *params);
     h->ws = (char *)d_workspace;
     h->has_state = false; h->graph = nullptr; h->graph_ready = false;
-    h->use_graph = std::getenv("PSDNS_NO_GRAPH") == nullptr;
-    h->use_xfused = std::getenv("PSDNS_NO_XFUSE") == nullptr;
+    h->use_graph = true;
+    h->use_xfused = true;
+    h->grid_cap = 0; h->pf = 2; h->pf_rhs = 4; h->yx_chunk = 0; h->l2_window = 0;
+    for (int i = 0; i < KC_COUNT; ++i) { h->last_grid[i] = 0; h->last_items[i] = 0; }
     h->launches = 0; h->per_step = 0; h->timed_class = -1;
     const bool phase = params->phase_field != 0;
     const bool visc = phase && params->visc_ratio != 1.0;
@@ -750,6 +835,7 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
             h->n_sm = nsm;
     }
     if (bytes < h->L.total || ((uintptr_t)d_workspace % ALIGN) != 0) { delete h; return PSDNS_ENOMEM; }
+    h->has_unfused_ws = bytes >= h->L.total_unfused;
     cudaError_t e = setup_attrs(h);
     if (e == cudaSuccess) e = build_tables(h);
     if (e != cudaSuccess) {
@@ -828,6 +914,7 @@ int psdns_step(psdns_handle *h, int nsteps) {
     if (!h->has_state) { h->err = "psdns_step: no state set"; return PSDNS_ESTATE; }
     const bool direct = !h->use_graph || h->timed_class >= 0;
     if (direct) {
+        CUDA_TRY(h, apply_l2_window(h, h->st));
         for (int i = 0; i < nsteps; ++i) CUDA_TRY(h, enqueue_step(h));
         return PSDNS_OK;
     }
@@ -839,7 +926,8 @@ int psdns_step(psdns_handle *h, int nsteps) {
         cudaGraph_t graph = nullptr;
         h->st = cap;
         const long long before = h->launches;
-        cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+        cudaError_t e = apply_l2_window(h, cap);
+        if (e == cudaSuccess) e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
         if (e == cudaSuccess) e = enqueue_step(h);
         cudaError_t e2 = cudaStreamEndCapture(cap, &graph);
         h->st = user;
@@ -1015,6 +1103,74 @@ int psdns_kernel_time_ms(psdns_handle *h, double *ms_total, long long *launches)
     *ms_total = tot;
     *launches = (long long)h->tevents.size();
     return PSDNS_OK;
+}
+
+int psdns_diagnostics(psdns_handle *h, double *d_out) {
+    if (!h) return PSDNS_EINVAL;
+    if (!d_out) { h->err = "psdns_diagnostics: null output pointer"; return PSDNS_EINVAL; }
+    if (!h->has_state) { h->err = "psdns_diagnostics: no state set"; return PSDNS_ESTATE; }
+    const Dims &d = h->d;
+    const Layout &L = h->L;
+    const bool phase = h->p.phase_field != 0;
+    const cplx *U = h->at<cplx>(L.state[0]), *V = h->at<cplx>(L.state[1]), *W = h->at<cplx>(L.state[2]);
+    // partial results live behind the three Z arrays the energy pass needs (transform scratch is free between steps)
+    double *part_max = h->at<double>(L.zb[3]);
+    const int nb_cols = (int)((d.ncols + DIAG_NT - 1) / DIAG_NT);
+    const int nb_en = h->n_sm * 8;
+    double *part_sum = part_max + nb_cols;
+    {
+        LaunchScope ls(h, KC_MISC);
+        k_diag_columns<<<nb_cols, DIAG_NT, 0, h->st>>>(geom(h), U, V, W, phase ? h->at<cplx>(L.state[3]) : nullptr, part_max, d_out);
+        CUDA_TRY(h, cudaGetLastError());
+    }
+    FieldPtrs fz{};
+    for (int i = 0; i < 3; ++i) { fz.in[i] = h->at<cplx>(L.state[i]); fz.out[i] = h->at<cplx>(L.zb[i]); }
+    CUDA_TRY(h, launch_zpass(h, false, fz, 3, d.ncols, d.nz, d.kxp, d.nky, d.jpos));
+    {
+        LaunchScope ls(h, KC_MISC);
+        k_diag_energy<<<nb_en, DIAG_NT, 0, h->st>>>(h->at<cplx>(L.zb[0]), h->at<cplx>(L.zb[1]), h->at<cplx>(L.zb[2]),
+                                                     h->at<double>(L.ccw), d.nz, (int)d.ncols, d.kxp, part_sum);
+        CUDA_TRY(h, cudaGetLastError());
+    }
+    {
+        LaunchScope ls(h, KC_MISC);
+        k_diag_final<<<1, DIAG_NT, 0, h->st>>>(part_max, nb_cols, part_sum, nb_en, d_out);
+        CUDA_TRY(h, cudaGetLastError());
+    }
+    return PSDNS_OK;
+}
+
+int psdns_set_option(psdns_handle *h, const char *name, double value) {
+    if (!h || !name) return PSDNS_EINVAL;
+    const std::string n(name);
+    const int iv = (int)value;
+    if (n == "graph") h->use_graph = iv != 0;
+    else if (n == "xfuse") {
+        if (!iv && !h->has_unfused_ws) { h->err = "psdns_set_option: xfuse = 0 needs psdns_workspace_bytes_unfused() bytes at init"; return PSDNS_ENOMEM; }
+        h->use_xfused = iv != 0;
+    }
+    else if (n == "grid_cap" && iv >= 0) h->grid_cap = iv;
+    else if (n == "yx_chunk" && iv >= 0) h->yx_chunk = iv;
+    else if (n == "l2_window" && iv >= 0) h->l2_window = iv;
+    else if (n == "pf" && iv >= 0) h->pf = iv;
+    else if (n == "pf_rhs" && iv >= 0) h->pf_rhs = iv;
+    else { h->err = "psdns_set_option: unknown option or bad value: " + n; return PSDNS_EINVAL; }
+    if (h->graph) { cudaGraphExecDestroy(h->graph); h->graph = nullptr; }   // the captured step bakes the options in
+    h->graph_ready = false;
+    return PSDNS_OK;
+}
+
+double psdns_get_info(const psdns_handle *h, const char *name) {
+    if (!h || !name) return -1.0;
+    const std::string n(name);
+    for (int i = 0; i < KC_COUNT; ++i) {
+        if (n == std::string(kclass_names[i]) + "_grid") return (double)h->last_grid[i];
+        if (n == std::string(kclass_names[i]) + "_items") return (double)h->last_items[i];
+    }
+    if (n == "n_sm") return (double)h->n_sm;
+    if (n == "workspace_bytes") return (double)h->L.total;
+    if (n == "launches_per_step") return (double)h->per_step;
+    return -1.0;
 }
 
 int psdns_destroy(psdns_handle *h) {
