@@ -155,6 +155,11 @@ int psdns_diagnostics(psdns_handle *h, double *d_out);
  *                                0 needs a workspace of psdns_workspace_bytes_unfused() bytes at init, else PSDNS_ENOMEM
  *   "grid_cap" n >= 0          : upper bound on the grid of every persistent kernel (z, y, fused x passes); 0 = none.
  *                                Tests use a small cap so that each CTA walks many tiles / lines of a small grid.
+ *   "ztma"     1 (default) / 0 : z passes fed by 2-D TMA tensor loads into a two-deep shared-memory stage (k_zpass_tma)
+ *                                / by per-thread strided loads (k_zpass); same arithmetic at N < 512, radix plan differs
+ *                                in the forward pass at N = 512
+ *   "zgemm"    0 (default) / 1 : nz <= 65 only: Chebyshev transform as a dense FP64 matrix product on the tensor cores
+ *                                (k_zgemm, DMMA) instead of the FFT path - kept for the measurement of SURVEY 8(f)-1
  *   "pf", "pf_rhs" n >= 0      : L2 prefetch distance, in rows, of the solver sweeps (defaults 2 and 4)
  * PSDNS_EINVAL on an unknown name or a bad value. */
 int psdns_set_option(psdns_handle *h, const char *name, double value);

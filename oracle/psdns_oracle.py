@@ -84,6 +84,13 @@ class Params:
     visc_ratio: float = 1.0
     phase_field: int = 1
     dealias: int = 1
+    # "no-slip or free-slip [walls], or a combination of them".  0 = no-slip (u = v = w = 0),
+    # 1 = free-slip (w = 0, du/dz = dv/dz = 0), for the wall z = +1 (top) and z = -1 (bottom); reading S10b of DESIGN.md
+    wall_top: int = 0
+    wall_bottom: int = 0
+
+
+NO_SLIP, FREE_SLIP = 0, 1
 
 
 def cheb_nodes(N: int) -> np.ndarray:
@@ -214,16 +221,27 @@ def truncation_mask(g: Grid, dealias: int = 1, z: bool = True) -> np.ndarray:
 
 DIRICHLET = 0
 NEUMANN = 1
+SECOND_DERIVATIVE = 2
 
 
-def boundary_rows(N: int, bc: int) -> np.ndarray:
-    """Two rows acting on Chebyshev coefficients.  Dirichlet: value at z=+1 (sum a_n) and
-    at z=-1 (sum (-1)^n a_n).  Neumann: T_n'(+-1) = (+-1)^(n+1) n^2."""
+def wall_row(N: int, kind: int, wall: int) -> np.ndarray:
+    """Row acting on Chebyshev coefficients that evaluates, at the wall z = wall (+1 or -1):
+    the value T_n(+-1) = (+-1)^n (DIRICHLET), the first derivative T_n'(+-1) = (+-1)^(n+1) n^2 (NEUMANN) or the
+    second derivative T_n''(+-1) = (+-1)^n n^2 (n^2 - 1) / 3 (SECOND_DERIVATIVE)."""
     n = np.arange(N + 1, dtype=np.float64)
-    sgn = np.where(np.arange(N + 1) % 2 == 0, 1.0, -1.0)
-    if bc == DIRICHLET:
-        return np.stack([np.ones(N + 1), sgn])
-    return np.stack([n * n, -sgn * n * n])
+    sgn = np.ones(N + 1) if wall > 0 else np.where(np.arange(N + 1) % 2 == 0, 1.0, -1.0)
+    if kind == DIRICHLET:
+        return sgn
+    if kind == NEUMANN:
+        return (sgn if wall > 0 else -sgn) * n * n
+    return sgn * n * n * (n * n - 1.0) / 3.0
+
+
+def boundary_rows(N: int, bc) -> np.ndarray:
+    """Two rows acting on Chebyshev coefficients, first the wall z = +1, then z = -1.  bc: one kind for both walls, or a
+    pair (kind at z = +1, kind at z = -1) for mixed walls."""
+    bp, bm = (bc, bc) if np.isscalar(bc) else bc
+    return np.stack([wall_row(N, bp, +1), wall_row(N, bm, -1)])
 
 
 def helmholtz_solve(f: np.ndarray, sigma: np.ndarray, bc: int,
@@ -254,12 +272,13 @@ def helmholtz_solve(f: np.ndarray, sigma: np.ndarray, bc: int,
 
 
 def coupled_w_solve(hw: np.ndarray, beta2: np.ndarray, k2: np.ndarray, gamma: float,
-                    chunk: int = 64):
+                    chunk: int = 64, walls=(NO_SLIP, NO_SLIP)):
     """The 4th-order wall-normal velocity problem as two coupled Helmholtz problems
     (readings S10, S11, S13):
         (D^2 - beta2) theta = -hw / gamma     rows 0..N-2, no condition on theta
         (D^2 - k2) w - theta = 0              rows 0..N-2
-        w(+-1) = 0, Dw(+-1) = 0
+        w(+-1) = 0, and per wall Dw = 0 (no-slip) or D^2 w = 0 (free-slip: du/dz = dv/dz = 0 and continuity,
+        PAPER.md L52; walls = (kind at z = +1, kind at z = -1))
     assembled as one (2N+2)x(2N+2) dense system per column.  Returns (theta, w)."""
     N = hw.shape[0] - 1
     M = hw.shape[1]
@@ -267,7 +286,7 @@ def coupled_w_solve(hw: np.ndarray, beta2: np.ndarray, k2: np.ndarray, gamma: fl
     D2 = D @ D
     eye = np.eye(N + 1)
     bd = boundary_rows(N, DIRICHLET)
-    bn = boundary_rows(N, NEUMANN)
+    bn = boundary_rows(N, tuple(SECOND_DERIVATIVE if k == FREE_SLIP else NEUMANN for k in walls))
     theta = np.empty((N + 1, M), dtype=np.complex128)
     w = np.empty((N + 1, M), dtype=np.complex128)
     n1 = N + 1
@@ -478,11 +497,14 @@ class Oracle:
         # -- wall-normal vorticity, Eq. 14, Crank-Nicolson
         om = ikx * s.v - iky * s.u                                   # Eq. 16
         H_om = om + gamma * self._lap(om) + dt * NL["om"]
-        om_new = helmholtz_solve(-H_om[:, jn, in_] / gamma, beta2, DIRICHLET)
+        # walls: no-slip u = v = 0 gives omega_z = 0; free-slip du/dz = dv/dz = 0 gives d omega_z/dz = 0
+        walls = (p.wall_top, p.wall_bottom)
+        bc_h = tuple(NEUMANN if k == FREE_SLIP else DIRICHLET for k in walls)
+        om_new = helmholtz_solve(-H_om[:, jn, in_] / gamma, beta2, bc_h)
 
         # -- wall-normal velocity, Eq. 15, Crank-Nicolson, two Helmholtz problems (L140)
         H_w = s.theta + gamma * self._lap(s.theta) + dt * NL["w"]
-        th_new, w_new = coupled_w_solve(H_w[:, jn, in_], beta2, k2n, gamma)
+        th_new, w_new = coupled_w_solve(H_w[:, jn, in_], beta2, k2n, gamma, walls=walls)
 
         # -- u, v from continuity (Eq. 6) and the vorticity definition (Eq. 16): row a11
         Dcol = self.D.astype(np.complex128)
@@ -504,7 +526,7 @@ class Oracle:
         for name, F in (("ubar", s.u), ("vbar", s.v)):
             m = F[:, 0, 0]
             H = m + gamma * (self.D2 @ m) + dt * NL[name]
-            sol = helmholtz_solve((-H / gamma)[:, None], np.array([1.0 / gamma]), DIRICHLET)
+            sol = helmholtz_solve((-H / gamma)[:, None], np.array([1.0 / gamma]), bc_h)
             (U if name == "ubar" else V)[:, 0, 0] = sol[:, 0]
 
         # -- Cahn-Hilliard, Eq. 17, implicit Euler, two Helmholtz problems (L142)

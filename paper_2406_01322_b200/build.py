@@ -7,7 +7,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "psdns.cu")
-DEPS = [os.path.join(HERE, "csrc", f) for f in ("psdns.cu", "fft_tile.cuh", "fft_fused.cuh", "kernels_transform.cuh", "kernels_spectral.cuh", "kernels_xfused.cuh", "kernels_xfused_visc.cuh")]
+DEPS = sorted(os.path.join(HERE, "csrc", f) for f in os.listdir(os.path.join(HERE, "csrc")) if f.endswith((".cu", ".cuh")))
 DEPS.append(os.path.join(os.path.dirname(HERE), "include", "psdns.h"))
 LIB = os.path.join(HERE, "libpsdns.so")
 

@@ -19,6 +19,10 @@
 #include "kernels_xfused.cuh"
 #include "kernels_xfused_visc.cuh"
 #include "kernels_diag.cuh"
+#include "kernels_ztma.cuh"
+#include "kernels_zgemm.cuh"
+
+#include <cudaTypedefs.h>
 
 using namespace psdns;
 
@@ -46,8 +50,9 @@ struct Dims {
 };
 
 struct Layout {
-    size_t tw_x, tw_y, tw_z;
+    size_t tw_x, tw_y, tw_z, tw_zn;    // tw_zn: exp(-2 pi i k / N), k < N (the z passes' FFT length)
     size_t ctab_z;                     // c_k of the half-length Chebyshev transform, k <= N/2
+    size_t zg_b, zg_f;                 // GEMM-form Chebyshev matrices [ZG_MP][ZG_KP] (N <= 64 only)
     size_t ccw;                        // Clenshaw-Curtis weights on z_k (diagnostics), nz doubles
     size_t state[5];                   // u v w phi theta
     size_t hist[3];
@@ -84,8 +89,10 @@ struct psdns_handle {
     bool use_xfused, has_unfused_ws;
     int xf_occ, xfv_occ, n_sm;
     int occ_z[2], occ_y[2];     // resident CTAs per SM of the persistent z / y passes, [fwd]
-    int yx_chunk;               // psdns_set_option("yx_chunk"): z planes per chunk of the y -> x -> y sequence (0 = whole grid)
-    int l2_window;              // psdns_set_option("l2_window"): 1 = persisting-L2 access window over the Y ring
+    int use_zgemm;              // psdns_set_option("zgemm"): GEMM-form Chebyshev on the FP64 tensor cores for N <= 64
+    int use_ztma;               // psdns_set_option("ztma"): z passes with TMA tensor loads (k_zpass_tma) / register-fed (k_zpass)
+    int occ_zt[2][2];           // resident CTAs per SM of k_zpass_tma, [fwd][full-length input]
+    PFN_cuTensorMapEncodeTiled encode_tiled;
     int grid_cap;               // psdns_set_option("grid_cap"): upper bound on the grid of every persistent kernel (0 = none)
     int pf, pf_rhs;             // L2 prefetch distances of the column sweeps, in rows
     long long last_grid[KC_COUNT], last_items[KC_COUNT];   // grid / work items of the last launch of each persistent class
@@ -140,8 +147,11 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.tw_x = take(d.nx * C);
     L.tw_y = take(d.ny * C);
     L.tw_z = take(2 * d.N * C);
+    L.tw_zn = take(d.N * C);
     L.ctab_z = take((d.N / 2 + 1) * C);
     L.ccw = take(d.nz * sizeof(double));
+    L.zg_b = L.zg_f = 0;
+    if (d.N <= 64) { L.zg_b = take(ZG_MP * ZG_KP * sizeof(double)); L.zg_f = take(ZG_MP * ZG_KP * sizeof(double)); }
     for (int i = 0; i < 5; ++i) L.state[i] = take(d.s_ret * C);
     for (int i = 0; i < 3; ++i) L.hist[i] = take(d.s_low * C);
     for (int i = 0; i < 3; ++i) L.dinv[i] = take(d.s_ret * sizeof(double));
@@ -269,8 +279,65 @@ struct ZDerived {
     cplx *out_dx = nullptr, *out_dy = nullptr;
 };
 
+// input rows of a z-pass tile -> (number of TMA boxes, rows per box); a box has at most 256 rows
+inline std::pair<int, int> ztma_rows(int nin) {
+    const int nb = (nin + 255) / 256;
+    return {nb, (nin + nb - 1) / nb};
+}
+
+cudaError_t launch_zpass_tma(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, size_t ncols, int nk, int kxp, int nky,
+                             int jpos, const ZDerived &zd) {
+    ZTArgs a;
+    const int N = h->d.N;
+    const int nin = fwd ? N + 1 : nk;
+    const auto rb = ztma_rows(nin);
+    a.nf = nf; a.ncols = (int)ncols; a.nk = nk; a.nboxes = rb.first; a.box_rows = rb.second;
+    a.dfield = fwd ? -1 : zd.dfield; a.out_dx = zd.out_dx; a.out_dy = zd.out_dy;
+    a.kxp = kxp; a.nky = nky; a.jpos = jpos;
+    a.kxf = 2.0 * M_PI / h->g.lx; a.kyf = 2.0 * M_PI / h->g.ly;
+    for (int i = 0; i < nf; ++i) {
+        a.out[i] = f.out[i];
+        const cuuint64_t gdim[2] = {(cuuint64_t)(2 * ncols), (cuuint64_t)nin};
+        const cuuint64_t gstr[1] = {(cuuint64_t)(ncols * sizeof(cplx))};
+        const cuuint32_t box[2] = {16u, (cuuint32_t)rb.second};
+        const cuuint32_t estr[2] = {1u, 1u};
+        const CUresult r = h->encode_tiled(&a.in_map[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(f.in[i]), gdim, gstr,
+                                           box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    }
+    const cplx *tw = h->at<cplx>(h->L.tw_zn);
+    const cplx *ct = h->at<cplx>(h->L.ctab_z);
+    const long long ntiles = (long long)(ncols / 8) * nf;
+    const int srows = rb.first * rb.second;
+    const int grid = h->persistent_grid(fwd ? KC_ZFWD : KC_ZBWD, ntiles, h->occ_zt[fwd][nin == N + 1]);
+    LaunchScope ls(h, fwd ? KC_ZFWD : KC_ZBWD);
+#define ZT(NN)                                                                                                         \
+    {                                                                                                                  \
+        if (fwd) k_zpass_tma<NN, true><<<grid, ztma_threads<NN>(), ztma_smem_bytes<NN>(srows), h->st>>>(a, tw, ct);    \
+        else k_zpass_tma<NN, false><<<grid, ztma_threads<NN>(), ztma_smem_bytes<NN>(srows), h->st>>>(a, tw, ct);       \
+    }
+    DISPATCH_N(N, ZT)
+#undef ZT
+    return cudaGetLastError();
+}
+
 cudaError_t launch_zpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, size_t ncols, int nk, int kxp, int nky,
                          int jpos, const ZDerived &zd = ZDerived()) {
+    if (h->use_zgemm && h->d.N <= 64 && !(zd.dfield >= 0 && zd.out_dx)) {
+        // GEMM form on the FP64 tensor cores (kernels_zgemm.cuh), short columns only
+        ZGArgs g; g.f = f; g.nf = nf; g.ncols = (int)ncols;
+        g.nrow_in = fwd ? h->d.N + 1 : nk; g.nrow_out = fwd ? nk : h->d.N + 1;
+        g.mat = h->at<double>(fwd ? h->L.zg_f : h->L.zg_b);
+        g.dfield = fwd ? -1 : zd.dfield; g.out_dy = zd.out_dy; g.kxp = kxp; g.nky = nky; g.jpos = jpos;
+        g.kyf = 2.0 * M_PI / h->g.ly;
+        const long long nblk = ((2 * (long long)ncols + ZG_COLS - 1) / ZG_COLS) * nf;
+        const int grid = h->persistent_grid(fwd ? KC_ZFWD : KC_ZBWD, nblk, 2);
+        LaunchScope ls(h, fwd ? KC_ZFWD : KC_ZBWD);
+        k_zgemm<<<grid, ZG_NT, ZG_SMEM, h->st>>>(g);
+        return cudaGetLastError();
+    }
+    if (h->use_ztma && h->encode_tiled) return launch_zpass_tma(h, fwd, f, nf, ncols, nk, kxp, nky, jpos, zd);
     ZArgs a; a.f = f; a.nf = nf; a.ncols = (int)ncols; a.nk = nk;
     a.dfield = fwd ? -1 : zd.dfield; a.out_dx = zd.out_dx; a.out_dy = zd.out_dy;
     a.kxp = kxp; a.nky = nky; a.jpos = jpos;
@@ -339,6 +406,20 @@ cudaError_t setup_attrs(psdns_handle *h) {
     }
 #define XA(LL) { CU0(set_smem(k_xpass<LL, true>, fft_smem<LL>())); CU0(set_smem(k_xpass<LL, false>, fft_smem<LL>())); }
     DISPATCH_N(h->d.N, ZA)
+#define ZTA(NN)                                                                                                        \
+    {                                                                                                                  \
+        const auto rf = ztma_rows(NN + 1);                                                                             \
+        const size_t big = ztma_smem_bytes<NN>(rf.first * rf.second);                                                  \
+        CU0(set_smem(k_zpass_tma<NN, true>, big)); CU0(set_smem(k_zpass_tma<NN, false>, big));                          \
+        for (int full = 0; full < 2; ++full) {                                                                         \
+            const auto rb = ztma_rows(full ? NN + 1 : h->d.nkz);                                                       \
+            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_zt[0][full], k_zpass_tma<NN, false>, ztma_threads<NN>(), ztma_smem_bytes<NN>(rb.first * rb.second))); \
+            CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->occ_zt[1][full], k_zpass_tma<NN, true>, ztma_threads<NN>(), big)); \
+        }                                                                                                              \
+    }
+    DISPATCH_N(h->d.N, ZTA)
+    CU0(set_smem(k_zgemm, ZG_SMEM));
+#undef ZTA
     DISPATCH_L(h->d.ny, YA)
     DISPATCH_L(h->d.nx, XA)
 #define XFA(LL)                                                                                              \
@@ -458,28 +539,6 @@ Coefs coefs(const psdns_params &p) {
         if (e__ != cudaSuccess) return e__;       \
     } while (0)
 
-// Persisting-L2 access window over the Y ring of the chunked y -> x -> y sequence (psdns_set_option "l2_window" 1):
-// accesses to the ring are marked persisting (they stay in the set-aside part of the L2), everything else streaming.
-cudaError_t apply_l2_window(psdns_handle *h, cudaStream_t st) {
-    if (!h->l2_window || h->yx_chunk <= 0) return cudaSuccess;
-    const Dims &d = h->d;
-    const size_t ring_bytes = (size_t)h->nf_out * h->yx_chunk * d.ny * d.kxp * sizeof(cplx);
-    int dev = 0, max_persist = 0, max_win = 0;
-    CU(cudaGetDevice(&dev));
-    CU(cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev));
-    CU(cudaDeviceGetAttribute(&max_win, cudaDevAttrMaxAccessPolicyWindowSize, dev));
-    const size_t set_aside = std::min<size_t>(ring_bytes, (size_t)max_persist);
-    CU(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, set_aside));
-    cudaStreamAttrValue v;
-    std::memset(&v, 0, sizeof(v));
-    v.accessPolicyWindow.base_ptr = h->ws + h->L.yb[0];
-    v.accessPolicyWindow.num_bytes = std::min<size_t>(ring_bytes, (size_t)max_win);
-    v.accessPolicyWindow.hitRatio = (float)std::min(1.0, (double)set_aside / (double)v.accessPolicyWindow.num_bytes);
-    v.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
-    v.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
-    return cudaStreamSetAttribute(st, cudaStreamAttributeAccessPolicyWindow, &v);
-}
-
 // ---- one time step (rows a1-a11) ------------------------------------------------------------------
 // Field bookkeeping (matched viscosity, phase field on):
 //   backward: 5 z transforms (u, v, w, phi, D phi) whose epilogue also emits i ky phi (row a1), 6 y
@@ -540,8 +599,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
     for (int i = 0; i < nz_f; ++i) { fz.in[i] = src[i]; fz.out[i] = h->at<cplx>(L.zb[i]); }
     for (int i = 0; i < ny_f; ++i) { fy.in[i] = h->at<cplx>(L.zb[i]); fy.out[i] = h->at<cplx>(L.yb[i]); }
     CU(launch_zpass(h, false, fz, nz_f, d.ncols, d.nkz, d.kxp, d.nky, d.jpos, zd));
-    const bool chunked = h->yx_chunk > 0 && h->use_xfused && !visc;
-    if (!chunked) CU(launch_ypass(h, false, fy, ny_f, d.kxp, d.nky, d.jpos));
+    CU(launch_ypass(h, false, fy, ny_f, d.kxp, d.nky, d.jpos));
     FieldPtrs gy{}, gz{};
     for (int i = 0; i < nout; ++i) {
         gy.in[i] = h->at<cplx>(L.yb[i]); gy.out[i] = h->at<cplx>(L.zb[i]);
@@ -556,29 +614,6 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.kxp = d.kxp; a.nkx = d.nkx; a.nlines = d.nz * d.ny;
         a.cs = c.cs; a.kxf = 2.0 * M_PI / h->g.lx; a.eta_c = (p.visc_ratio - 1.0) / (2.0 * p.re);
         CU(launch_xfusedv(h, a));
-    } else if (chunked) {
-        // a3 .. a7 in chunks of yx_chunk z planes through a small RING of Y arrays (the first planes of the Y region,
-        // fields back to back), so that the Y arrays live in the 126 MB L2 between the y-backward pass, the fused x
-        // kernel and the y-forward pass of a chunk instead of crossing HBM four times
-        const int C = h->yx_chunk;
-        const size_t ring_field = (size_t)C * d.ny * d.kxp;           // cplx per field in the ring
-        cplx *ring = h->at<cplx>(L.yb[0]);
-        const int stage_src[6] = {0, 1, 2, 3, 5, 4};   // u v w phi phy phz  <-  Y arrays u v w phi phz phy
-        for (int z0 = 0; z0 < d.nz; z0 += C) {
-            const int np = std::min(C, d.nz - z0);
-            const size_t zoff = (size_t)z0 * d.nky * d.kxp;
-            FieldPtrs cy{}, dy{};
-            for (int i = 0; i < ny_f; ++i) { cy.in[i] = h->at<cplx>(L.zb[i]) + zoff; cy.out[i] = ring + i * ring_field; }
-            CU(launch_ypass(h, false, cy, ny_f, d.kxp, d.nky, d.jpos, np));
-            XFArgs a;
-            for (int i = 0; i < 6; ++i) a.in[i] = ring + (phase ? stage_src[i] : (i < 3 ? i : 0)) * ring_field;
-            for (int i = 0; i < 8; ++i) a.out[i] = ring + (i < nout ? i : 0) * ring_field;
-            a.kxp = d.kxp; a.nkx = d.nkx; a.nlines = np * d.ny;
-            a.cs = c.cs; a.kxf = 2.0 * M_PI / h->g.lx;
-            CU(launch_xfused(h, a));
-            for (int i = 0; i < nout; ++i) { dy.in[i] = ring + i * ring_field; dy.out[i] = h->at<cplx>(L.zb[i]) + zoff; }
-            CU(launch_ypass(h, true, dy, nout, d.kxp, d.nky, d.jpos, np));
-        }
     } else if (h->use_xfused && !visc) {
         // a4 + a5 + a6 fused: physical space never leaves the SM; in place on the Y arrays
         XFArgs a;
@@ -613,7 +648,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
         CU(launch_xpass(h, true, gx, nout, d.kxp, d.nkx));
     }
     // a7-a8: forward y, z with truncation
-    if (!chunked) CU(launch_ypass(h, true, gy, nout, d.kxp, d.nky, d.jpos));
+    CU(launch_ypass(h, true, gy, nout, d.kxp, d.nky, d.jpos));
     CU(launch_zpass(h, true, gz, nout, d.ncols, d.nkz, d.kxp, d.nky, d.jpos));
     // a9 + first elimination (K_A), substitution (K_B), second elimination (K_C), substitution +
     // influence-matrix correction (K_D), velocity recovery (a11)
@@ -707,6 +742,7 @@ cudaError_t build_tables(psdns_handle *h) {
     CU(fill(L.tw_x, d.nx));
     CU(fill(L.tw_y, d.ny));
     CU(fill(L.tw_z, 2 * d.N));
+    CU(fill(L.tw_zn, d.N));
     {   // c_k = -(1 + sin t)/(2 sin t) + i cos t/(2 sin t), t = pi k / N  (kernels_transform.cuh, k_zpass_h)
         std::vector<cplx> t(d.N / 2 + 1);
         t[0] = make_double2(0.0, 0.0);
@@ -716,6 +752,20 @@ cudaError_t build_tables(psdns_handle *h) {
             t[k] = make_double2((double)(-(1.0L + sn) / (2.0L * sn)), (double)(cs / (2.0L * sn)));
         }
         CU(cudaMemcpyAsync(h->ws + L.ctab_z, t.data(), t.size() * sizeof(cplx), cudaMemcpyHostToDevice, h->st));
+        CU(cudaStreamSynchronize(h->st));
+    }
+    if (d.N <= 64) {   // GEMM-form Chebyshev matrices (kernels_zgemm.cuh), long double on the host
+        std::vector<double> mb(ZG_MP * ZG_KP, 0.0), mf(ZG_MP * ZG_KP, 0.0);
+        const long double pi = 3.14159265358979323846264338327950288L;
+        for (int k = 0; k <= d.N; ++k)
+            for (int n = 0; n <= d.N; ++n) {
+                const long double cs = cosl(pi * (long double)((long long)n * k % (2 * d.N)) / (long double)d.N);
+                mb[k * ZG_KP + n] = (double)cs;                                              // f_k = sum_n a_n cos(pi n k / N)
+                const long double cn = (n == 0 || n == d.N) ? 2.0L : 1.0L, ck = (k == 0 || k == d.N) ? 2.0L : 1.0L;
+                mf[n * ZG_KP + k] = (double)(2.0L * cs / ((long double)d.N * cn * ck));      // a_n = 2/(N c_n) sum_k f_k cos / c_k
+            }
+        CU(cudaMemcpyAsync(h->ws + L.zg_b, mb.data(), mb.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
+        CU(cudaMemcpyAsync(h->ws + L.zg_f, mf.data(), mf.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
         CU(cudaStreamSynchronize(h->st));
     }
     {   // Clenshaw-Curtis weights w_k = (c_k / N) [1 - sum_{j=1}^{N/2} b_j cos(2 j k pi / N) / (4 j^2 - 1)], b_{N/2} = 1 else 2,
@@ -820,7 +870,18 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->has_state = false; h->graph = nullptr; h->graph_ready = false;
     h->use_graph = true;
     h->use_xfused = true;
-    h->grid_cap = 0; h->pf = 2; h->pf_rhs = 4; h->yx_chunk = 0; h->l2_window = 0;
+    h->grid_cap = 0; h->pf = 2; h->pf_rhs = 4;
+    h->use_ztma = 1; h->encode_tiled = nullptr; h->use_zgemm = 0;
+    for (int i = 0; i < 4; ++i) (&h->occ_zt[0][0])[i] = 1;
+    {   // driver entry point of the tensor-map encoder (no link-time dependency on libcuda)
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            h->encode_tiled = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(fn);
+        else
+            cudaGetLastError();
+    }
     for (int i = 0; i < KC_COUNT; ++i) { h->last_grid[i] = 0; h->last_items[i] = 0; }
     h->launches = 0; h->per_step = 0; h->timed_class = -1;
     const bool phase = params->phase_field != 0;
@@ -914,7 +975,6 @@ int psdns_step(psdns_handle *h, int nsteps) {
     if (!h->has_state) { h->err = "psdns_step: no state set"; return PSDNS_ESTATE; }
     const bool direct = !h->use_graph || h->timed_class >= 0;
     if (direct) {
-        CUDA_TRY(h, apply_l2_window(h, h->st));
         for (int i = 0; i < nsteps; ++i) CUDA_TRY(h, enqueue_step(h));
         return PSDNS_OK;
     }
@@ -926,8 +986,7 @@ int psdns_step(psdns_handle *h, int nsteps) {
         cudaGraph_t graph = nullptr;
         h->st = cap;
         const long long before = h->launches;
-        cudaError_t e = apply_l2_window(h, cap);
-        if (e == cudaSuccess) e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+        cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
         if (e == cudaSuccess) e = enqueue_step(h);
         cudaError_t e2 = cudaStreamEndCapture(cap, &graph);
         h->st = user;
@@ -1150,8 +1209,8 @@ int psdns_set_option(psdns_handle *h, const char *name, double value) {
         h->use_xfused = iv != 0;
     }
     else if (n == "grid_cap" && iv >= 0) h->grid_cap = iv;
-    else if (n == "yx_chunk" && iv >= 0) h->yx_chunk = iv;
-    else if (n == "l2_window" && iv >= 0) h->l2_window = iv;
+    else if (n == "ztma") h->use_ztma = iv != 0;
+    else if (n == "zgemm") h->use_zgemm = iv != 0;
     else if (n == "pf" && iv >= 0) h->pf = iv;
     else if (n == "pf_rhs" && iv >= 0) h->pf_rhs = iv;
     else { h->err = "psdns_set_option: unknown option or bad value: " + n; return PSDNS_EINVAL; }

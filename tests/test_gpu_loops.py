@@ -153,3 +153,51 @@ def test_fused_equals_unfused_x_path():
     with pytest.raises(P.PsdnsError):
         s.set_option("xfuse", 0)          # the lean workspace has no physical-space arrays
     s.close()
+
+
+@pytest.mark.parametrize("form", [1, 0])
+@pytest.mark.parametrize("nx,ny,nz,kind", [(32, 32, 33, "channel"), (16, 16, 513, "random"), (64, 16, 129, "random"),
+                                           (16, 64, 17, "channel")])
+def test_tma_z_pass_matches_oracle(nx, ny, nz, kind, form):
+    """k_zpass_tma (2-D TMA box loads into a two-deep mbarrier stage) against the live oracle, capped grid so that
+    both stages and both barrier parities are reused many times; N = 512 takes three boxes (forward) / two (backward)."""
+    import paper_2406_01322_b200 as P
+    c = scaling_like(nx, ny, nz) if kind == "random" else I.small_config(nx=nx, ny=ny, nz=nz)
+    space, st = state_of(c, kind)
+    orc, g = oracle_from_config(c)
+    orc.set_state(space, *st)
+    orc.step(2)
+    s = solver_from_config(c)
+    s.set_option("ztma", form)               # 1: TMA-fed k_zpass_tma (the default); 0: register-fed k_zpass
+    s.set_option("grid_cap", 3)
+    s.set_state(P.SPECTRAL if space == "spectral" else P.PHYSICAL, *[to_dev(f) for f in st])
+    s.step(2)
+    for k in ("zbwd", "zfwd"):
+        assert s.get_info(k + "_items") >= 3 * s.get_info(k + "_grid") > 0, k
+    assert_parity([to_np(t) for t in s.get_state(P.SPECTRAL)], orc.get_state("spectral"), TOL, tag=("ztma", nx, ny, nz))
+    # physical-space get_state runs the full-length backward z pass (nk = nz) through the TMA kernel as well
+    ev = [np.abs(to_np(a) - b).max() / np.abs(b).max() for a, b in zip(s.get_state(P.PHYSICAL), orc.get_state("physical"))]
+    assert max(ev) < TOL, ev
+    s.close()
+
+
+@pytest.mark.parametrize("nx,ny,nz,phase", [(32, 32, 33, 1), (64, 16, 65, 1), (16, 64, 17, 0)])
+def test_gemm_form_chebyshev_matches_oracle(nx, ny, nz, phase):
+    """Row f1: the GEMM form of the Chebyshev transform on the FP64 tensor cores (k_zgemm, mma.sync m8n8k4, N <= 64)
+    drives the whole step (backward with the i ky phi by-product, forward with truncation) and the physical-space
+    get_state (full-length backward)."""
+    import paper_2406_01322_b200 as P
+    c = I.small_config(nx=nx, ny=ny, nz=nz, phase_field=phase)
+    space, st = state_of(c, "channel")
+    orc, g = oracle_from_config(c)
+    orc.set_state(space, *st)
+    orc.step(2)
+    s = solver_from_config(c)
+    s.set_option("zgemm", 1)
+    s.set_option("grid_cap", 3)
+    s.set_state(P.PHYSICAL, *[to_dev(f) for f in st])          # forward z pass with nk = nz
+    s.step(2)
+    assert_parity([to_np(t) for t in s.get_state(P.SPECTRAL)], orc.get_state("spectral"), TOL, tag=("zgemm", nx, ny, nz))
+    ev = [np.abs(to_np(a) - b).max() / np.abs(b).max() for a, b in zip(s.get_state(P.PHYSICAL), orc.get_state("physical"))]
+    assert max(ev) < TOL, ev
+    s.close()
