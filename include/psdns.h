@@ -45,6 +45,9 @@ typedef struct {
  * visc_ratio: lambda, viscosity ratio; 1.0 = matched; != 1 evaluates the
  *             explicit variable-viscosity stress pointwise (reading S14)
  * phase_field: 0 = single-phase Navier-Stokes only (the Fig. 3 workload, L231), 1 = + Cahn-Hilliard
+ * wall_top, wall_bottom: velocity condition at z = +1 / z = -1.  Free-slip turns the condition on
+ *             omega_z (and the mean flow) into d/dz = 0 and the second condition on w into d^2 w/dz^2 = 0 (continuity);
+ *             phi keeps d phi/dz = d psi/dz = 0.  Zero-initialised structs give the no-slip channel.
  * dealias   : must be 1 for psdns_step (2/3 rule in x, y, z; reading S3).  The round-trip
  *             call always runs with dealiasing off. */
 typedef struct {
@@ -53,6 +56,8 @@ typedef struct {
     double visc_ratio;
     int phase_field;
     int dealias;
+    int wall_top;    /* wall z = +1: 0 = no-slip (u = v = w = 0), 1 = free-slip (w = 0, du/dz = dv/dz = 0) - PAPER.md L52 */
+    int wall_bottom; /* wall z = -1, same codes; "a combination of them" (L52) = different values at the two walls */
 } psdns_params;
 
 enum { PSDNS_PHYSICAL = 0, PSDNS_SPECTRAL = 1 };

@@ -336,13 +336,14 @@ struct ElimDown {
     double dp2, dp1;          // 1/d'_{k+2}, 1/d'_{k+1}
     double zp2, zp1;          // boundary-row adjoint weights z_{k+2}, z_{k+1}
     double yp2, yp1;          // second functional (weights k^2)
-    cplx Je, Jo, Ke, Ko;
+    double xp2, xp1;          // third functional (weights k^2 (k^2 - 1) / 3: T_k''(+-1), free-slip walls)
+    cplx Je, Jo, Ke, Ko, Me, Mo;
     __device__ __forceinline__ void init() {
-        fp2 = fp1 = f0 = fm1 = gp2 = gp1 = Je = Jo = Ke = Ko = cz();
-        dp2 = dp1 = zp2 = zp1 = yp2 = yp1 = 0.0;
+        fp2 = fp1 = f0 = fm1 = gp2 = gp1 = Je = Jo = Ke = Ko = Me = Mo = cz();
+        dp2 = dp1 = zp2 = zp1 = yp2 = yp1 = xp2 = xp1 = 0.0;
     }
     // row k (N >= k >= 2): fm2 = F(k-2) (scaled RHS, zero-extended above N-2), di = 1/d'_k.  Returns g'_k.
-    template <bool NEU, bool SECOND>
+    template <bool NEU, bool SECOND, bool THIRD = false>
     __device__ __forceinline__ cplx row(int k, int N, double sigma, cplx fm2, double di) {
         cplx g = cfma(helm_p(k), fm2, cfma(helm_q(k), f0, cscale(fp2, helm_r(k))));
         if (k + 4 <= N) g = cfma(sigma * helm_r(k) * dp2, gp2, g);   // g - (c_k/d'_{k+2}) g'_{k+2}, c_k = -sigma r_k
@@ -354,6 +355,12 @@ struct ElimDown {
             const double y = ((double)k * k + sp * yp2) * di;
             if (k & 1) Ko = cfma(y, g, Ko); else Ke = cfma(y, g, Ke);
             yp2 = yp1; yp1 = y;
+        }
+        if (THIRD) {
+            const double k2 = (double)k * k;
+            const double x = (k2 * (k2 - 1.0) * (1.0 / 3.0) + sp * xp2) * di;
+            if (k & 1) Mo = cfma(x, g, Mo); else Me = cfma(x, g, Me);
+            xp2 = xp1; xp1 = x;
         }
         zp2 = zp1; zp1 = z;
         gp2 = gp1; gp1 = g;
@@ -374,20 +381,46 @@ struct ElimDown {
         de = cfma(sigma * helm_p(2) * yp1, u0, Ke);                    // 0^2 u_0 + K_e + u_0 sum k^2 beta_k
         dodd = cadd(u1, cfma(sigma * helm_p(3) * yp2, u1, Ko));          // 1^2 u_1 + K_o + u_1 sum k^2 beta_k
     }
+    // sum_{k in parity} k^2 (k^2 - 1)/3 u_k of the finished solution (needs THIRD); the weights of k = 0, 1 vanish
+    __device__ __forceinline__ void third(double sigma, cplx u0, cplx u1, cplx &me, cplx &mo) const {
+        me = cfma(sigma * helm_p(2) * xp1, u0, Me);
+        mo = cfma(sigma * helm_p(3) * xp2, u1, Mo);
+    }
 };
+
+// Boundary closure of one Helmholtz solve for any pair of wall conditions (no-slip, free-slip or a
+// combination; kind 0 = value prescribed (Dirichlet), 1 = first derivative (Neumann), homogeneous).  With
+// u_k = alpha_k + beta_k u_par the four parity sums of the solution are
+//   S_e = Sa_e + se u_0,  S_o = Sa_o + so u_1   (weights 1),      K_e = Ka_e + ke u_0,  K_o = Ka_o + ko u_1   (weights k^2)
+// and T_k(+-1) = (+-1)^k, T_k'(+-1) = (+-1)^(k+1) k^2 give the value / derivative at z = +1 as S_e + S_o / K_e + K_o and
+// at z = -1 as S_e - S_o / -K_e + K_o.  Equal kinds decouple by parity; mixed kinds leave a 2 x 2 system.
+__device__ __forceinline__ void wall_closure(int top, int bot, double Sae, double Sao, double Kae, double Kao, double se,
+                                             double so, double ke, double ko, double &u0, double &u1) {
+    if (top == 0 && bot == 0) { u0 = -Sae / se; u1 = -Sao / so; return; }
+    if (top == 1 && bot == 1) { u0 = -Kae / ke; u1 = -Kao / ko; return; }
+    double a11, a12, b1, a21, a22, b2;
+    if (top == 1) { a11 = ke; a12 = ko; b1 = -(Kae + Kao); a21 = se; a22 = -so; b2 = -(Sae - Sao); }     // N at +1, D at -1
+    else          { a11 = se; a12 = so; b1 = -(Sae + Sao); a21 = -ke; a22 = ko; b2 = Kae - Kao; }        // D at +1, N at -1
+    const double idet = 1.0 / (a11 * a22 - a12 * a21);
+    u0 = (b1 * a22 - a12 * b2) * idet;
+    u1 = (a11 * b2 - a21 * b1) * idet;
+}
 
 // Real-component form of ElimDown for TWO right-hand sides that share sigma, the pivots and the Dirichlet adjoint
 // weights (the omega_z and theta problems of one column: both sigma = k^2 + 1/gamma).  The tau system has real
 // coefficients, so the real and imaginary parts of a column are two independent real problems.
+template <bool GEN = false>   // GEN: also the k^2-weighted functional, for walls that are not both no-slip
 struct ElimDown2R {
     double fp2[2], fp1[2], f0[2], fm1[2];   // F(k+2), F(k+1), F(k), F(k-1) of the next row k, per right-hand side
     double gp2[2], gp1[2];                  // g'_{k+2}, g'_{k+1}
     double Je[2], Jo[2];
+    double Ke[2], Ko[2];                    // GEN only
     double dp2, dp1, zp2, zp1;
+    double yp2, yp1;                        // GEN only
     __device__ __forceinline__ void init() {
 #pragma unroll
-        for (int i = 0; i < 2; ++i) fp2[i] = fp1[i] = f0[i] = fm1[i] = gp2[i] = gp1[i] = Je[i] = Jo[i] = 0.0;
-        dp2 = dp1 = zp2 = zp1 = 0.0;
+        for (int i = 0; i < 2; ++i) fp2[i] = fp1[i] = f0[i] = fm1[i] = gp2[i] = gp1[i] = Je[i] = Jo[i] = Ke[i] = Ko[i] = 0.0;
+        dp2 = dp1 = zp2 = zp1 = yp2 = yp1 = 0.0;
     }
     __device__ __forceinline__ void row(int k, int N, double sigma, double fa, double fb, double di, double &ga, double &gb) {
         const double pk = helm_p(k), qk = helm_q(k), rk = helm_r(k);
@@ -396,14 +429,17 @@ struct ElimDown2R {
         const double m = (k + 4 <= N) ? sigma * rk * dp2 : 0.0;
         const double sp = (k + 2 <= N) ? sigma * helm_p(k + 2) : 0.0;
         const double z = (1.0 + sp * zp2) * di;
+        const double y = GEN ? ((double)k * k + sp * yp2) * di : 0.0;
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             g[i] = fma(pk, fm2[i], fma(qk, f0[i], fp2[i] * rk));
             g[i] = fma(m, gp2[i], g[i]);
             if (k & 1) Jo[i] = fma(z, g[i], Jo[i]); else Je[i] = fma(z, g[i], Je[i]);
+            if (GEN) { if (k & 1) Ko[i] = fma(y, g[i], Ko[i]); else Ke[i] = fma(y, g[i], Ke[i]); }
             gp2[i] = gp1[i]; gp1[i] = g[i];
             fp2[i] = fp1[i]; fp1[i] = f0[i]; f0[i] = fm1[i]; fm1[i] = fm2[i];
         }
+        if (GEN) { yp2 = yp1; yp1 = y; }
         zp2 = zp1; zp1 = z;
         dp2 = dp1; dp1 = di;
         ga = g[0]; gb = g[1];
@@ -414,6 +450,12 @@ struct ElimDown2R {
         const double so = 1.0 + sigma * helm_p(3) * zp2;
         u0 = -Je[i] / se;
         u1 = -Jo[i] / so;
+    }
+    // any pair of homogeneous wall conditions (GEN): kinds 0 = value, 1 = derivative, at z = +1 / z = -1
+    __device__ __forceinline__ void finish_walls(double sigma, int i, int top, int bot, double &u0, double &u1) const {
+        const double se = 1.0 + sigma * helm_p(2) * zp1, so = 1.0 + sigma * helm_p(3) * zp2;
+        const double ke = sigma * helm_p(2) * yp1, ko = 1.0 + sigma * helm_p(3) * yp2;
+        wall_closure(top, bot, Je[i], Jo[i], Ke[i], Ko[i], se, so, ke, ko, u0, u1);
     }
 };
 
@@ -435,6 +477,7 @@ struct RhsElimArgs {
     const double *ab;
     double dt, gamma, inv_pe, e_phi, gradp, lam_phi, gam_phi;
     int phase;
+    int wall_top, wall_bot;           // 0 = no-slip, 1 = free-slip
 };
 
 constexpr int RHS_COLS = 32;   // columns per CTA of k_rhs_elim (blockDim = 32 * number of chains)
@@ -442,6 +485,7 @@ constexpr int RHS_COLS = 32;   // columns per CTA of k_rhs_elim (blockDim = 32 *
 #ifndef RHS_MINB
 #define RHS_MINB 4
 #endif
+template <bool GEN>   // GEN: walls that are not both no-slip (row f3); false = the no-slip product path, unchanged
 __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
     const ColGeom &g = a.g;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -492,7 +536,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
         double Aa1 = 0, Ab1 = 0, Ab2 = 0, Ac1 = 0, Ac2 = 0;             // D^2 A
         double Oa1 = 0, Ob1 = 0, Ob2 = 0, Oc1 = 0, Oc2 = 0;             // D^2 omega
         double Ta1 = 0, Tb1 = 0, Tb2 = 0, Tc1 = 0, Tc2 = 0;             // D^2 theta
-        ElimDown2R el;
+        ElimDown2R<GEN> el;
         el.init();
         RowIn nx = load(N);
         for (int n = N; n >= 0; --n) {
@@ -549,10 +593,19 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
             }
         }
         double u0, u1;
-        el.finish(sigma, 0, u0, u1);
-        xo[0] = u0; xo[st2] = u1;
-        el.finish(sigma, 1, u0, u1);
-        xt[0] = u0; xt[st2] = u1;
+        if (GEN) {
+            // omega_z (column 0: u-bar): value at a no-slip wall, derivative at a free-slip wall.  theta_p: value at both
+            // walls (the influence matrix closes the w problem); column 0 carries v-bar there, with u-bar's conditions
+            el.finish_walls(sigma, 0, a.wall_top, a.wall_bot, u0, u1);
+            xo[0] = u0; xo[st2] = u1;
+            el.finish_walls(sigma, 1, mean ? a.wall_top : 0, mean ? a.wall_bot : 0, u0, u1);
+            xt[0] = u0; xt[st2] = u1;
+        } else {
+            el.finish(sigma, 0, u0, u1);
+            xo[0] = u0; xo[st2] = u1;
+            el.finish(sigma, 1, u0, u1);
+            xt[0] = u0; xt[st2] = u1;
+        }
     } else {
         const double sigma = k2 + a.lam_phi, fs = 1.0 / a.gam_phi;
         const cplx *__restrict__ qq = a.q + col, *__restrict__ cc = a.c + col;
@@ -741,13 +794,14 @@ struct Elim2Args {
     const cplx *th;   cplx *w;      // chain 0
     cplx *phi;                      // chain 1 (in place)
     const double *dinv_po, *dinv_ch;
-    const double *hw;               // [2][ncols]: sum_{even} k^2 w_h, sum_{odd} k^2 w_h
+    const double *hw;               // [4][ncols]: sum_{even}, sum_{odd} of k^2 w_h, then of k^2 (k^2 - 1)/3 w_h
     cplx *coef;                     // [2][ncols] out
     double lam_phi;
     int phase;
+    int wall_top, wall_bot;         // 0 = no-slip (Dw = 0), 1 = free-slip (D^2 w = 0)
 };
 
-template <int G>
+template <int G, bool GEN>
 __global__ void __launch_bounds__(NT_COL, 3) k_elim2(const __grid_constant__ Elim2Args a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
@@ -780,7 +834,7 @@ __global__ void __launch_bounds__(NT_COL, 3) k_elim2(const __grid_constant__ Eli
 #pragma unroll
             for (int i = 0; i < G; ++i) {
                 const int k = k0 - i;
-                if (k >= 2) out[k * st] = el.row<false, true>(k, N, k2, q[i], pv.step(k, N, k2));
+                if (k >= 2) out[k * st] = el.row<false, true, GEN>(k, N, k2, q[i], pv.step(k, N, k2));
             }
 #pragma unroll
             for (int i = 0; i < G; ++i) q[i] = nx[i];
@@ -790,8 +844,30 @@ __global__ void __launch_bounds__(NT_COL, 3) k_elim2(const __grid_constant__ Eli
         el.second(k2, u0, u1, de, dodd);
         out[0] = u0; out[st] = u1;
         const bool off = (col == 0);
-        a.coef[col] = off ? cz() : cscale(de, -1.0 / a.hw[col]);
-        a.coef[st + col] = off ? cz() : cscale(dodd, -1.0 / a.hw[st + col]);
+        if (!GEN) {
+            a.coef[col] = off ? cz() : cscale(de, -1.0 / a.hw[col]);
+            a.coef[st + col] = off ? cz() : cscale(dodd, -1.0 / a.hw[st + col]);
+        } else {
+            // w = w_p + A_e w_h,e + A_o w_h,o with, per wall, Dw = 0 (no-slip) or D^2 w = 0 (free-slip):
+            //   T_k'(+-1) = (+-1)^(k+1) k^2       -> Dw(+1) = K_e + K_o,    Dw(-1) = -K_e + K_o
+            //   T_k''(+-1) = (+-1)^k k^2(k^2-1)/3 -> D^2 w(+1) = M_e + M_o, D^2 w(-1) = M_e - M_o
+            cplx me, mo;
+            el.third(k2, u0, u1, me, mo);
+            const double Keh = a.hw[col], Koh = a.hw[st + col], Meh = a.hw[2 * st + col], Moh = a.hw[3 * st + col];
+            cplx Ae, Ao;
+            if (a.wall_top == 1 && a.wall_bot == 1) { Ae = cscale(me, -1.0 / Meh); Ao = cscale(mo, -1.0 / Moh); }
+            else {
+                double a11, a12, a21, a22;
+                cplx b1, b2;
+                if (a.wall_top == 1) { a11 = Meh; a12 = Moh; b1 = cscale(cadd(me, mo), -1.0); a21 = -Keh; a22 = Koh; b2 = csub(de, dodd); }
+                else                 { a11 = Keh; a12 = Koh; b1 = cscale(cadd(de, dodd), -1.0); a21 = Meh; a22 = -Moh; b2 = cscale(csub(me, mo), -1.0); }
+                const double idet = 1.0 / (a11 * a22 - a12 * a21);
+                Ae = cscale(csub(cscale(b1, a22), cscale(b2, a12)), idet);
+                Ao = cscale(csub(cscale(b2, a11), cscale(b1, a21)), idet);
+            }
+            a.coef[col] = off ? cz() : Ae;
+            a.coef[st + col] = off ? cz() : Ao;
+        }
     } else {
         if (!a.phase) return;
         const double sigma = k2 + a.lam_phi;
@@ -833,16 +909,19 @@ __global__ void __launch_bounds__(NT_COL) k_hom_tables(const __grid_constant__ C
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= g.ncols) return;
     const size_t st = g.ncols;
-    double he = 0.0, ho = 0.0;
+    double he = 0.0, ho = 0.0, me = 0.0, mo = 0.0;
     for (int k = 0; k <= g.N; ++k) {
         const size_t o = k * st + col;
         const double w = wh_c[o].x;
         thh[o] = thh_c[o].x;
         wh[o] = w;
-        if (k & 1) ho += (double)k * k * w; else he += (double)k * k * w;
+        const double k2 = (double)k * k, m = k2 * (k2 - 1.0) * (1.0 / 3.0);
+        if (k & 1) { ho += k2 * w; mo += m * w; } else { he += k2 * w; me += m * w; }
     }
     hw[col] = he;
     hw[st + col] = ho;
+    hw[2 * st + col] = me;      // free-slip walls (row f3): sums of T_k''(1) w_h,k per parity
+    hw[3 * st + col] = mo;
 }
 
 // ---- row a11: velocity recovery, plus D phi^ for the next step's grad(phi) (row a1) -----------------------

@@ -117,6 +117,7 @@ bool validate(const psdns_grid *g, const psdns_params *p) {
     if (!(g->lx > 0) || !(g->ly > 0)) return false;
     if (!(p->re > 0) || !(p->dt > 0)) return false;
     if (p->phase_field != 0 && p->phase_field != 1) return false;
+    if ((p->wall_top != 0 && p->wall_top != 1) || (p->wall_bottom != 0 && p->wall_bottom != 1)) return false;
     if (p->phase_field && (!(p->pe > 0) || !(p->ch > 0) || !(p->we > 0) || !(p->visc_ratio > 0))) return false;
     return true;
 }
@@ -157,7 +158,7 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     for (int i = 0; i < 3; ++i) L.dinv[i] = take(d.s_ret * sizeof(double));
     L.thh = take(d.s_ret * sizeof(double));
     L.wh = take(d.s_ret * sizeof(double));
-    L.hw = take(2 * d.ncols * sizeof(double));
+    L.hw = take(4 * d.ncols * sizeof(double));
     L.coef = take(2 * d.ncols * C);
     L.xom = take(d.s_ret * C);
     const bool visc_l = p.phase_field && p.visc_ratio != 1.0;
@@ -654,6 +655,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
     // influence-matrix correction (K_D), velocity recovery (a11)
     const double inv_g = 1.0 / c.gamma;
     const bool la2 = d.ncols > 60000;   // register look-ahead depth of the solver sweeps (kernels_spectral.cuh)
+    const bool walls_gen = p.wall_top != 0 || p.wall_bottom != 0;   // free-slip or mixed walls (row f3)
     const double *dNS = h->at<double>(L.dinv[0]), *dPO = h->at<double>(L.dinv[1]), *dCH = h->at<double>(L.dinv[2]);
     {
         RhsElimArgs a;
@@ -667,9 +669,11 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.ab = ab; a.dt = p.dt; a.gamma = c.gamma; a.inv_pe = phase ? 1.0 / p.pe : 0.0;
         a.e_phi = 1.0 + c.s_coef * p.ch * p.ch;
         a.gradp = p.gradp_x; a.lam_phi = c.lam_phi; a.gam_phi = c.gam_phi; a.phase = phase;
+        a.wall_top = p.wall_top; a.wall_bot = p.wall_bottom;
         const int grid = (int)((d.ncols + RHS_COLS - 1) / RHS_COLS);
         LaunchScope ls(h, KC_RHS);
-        k_rhs_elim<<<grid, 32 * (phase ? 3 : 2), 0, h->st>>>(a);
+        if (walls_gen) k_rhs_elim<true><<<grid, 32 * (phase ? 3 : 2), 0, h->st>>>(a);
+        else k_rhs_elim<false><<<grid, 32 * (phase ? 3 : 2), 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     {
@@ -690,9 +694,12 @@ cudaError_t enqueue_step(psdns_handle *h) {
         Elim2Args a;
         a.g = geom(h); a.th = TH; a.w = W; a.phi = PHI; a.dinv_po = dPO; a.dinv_ch = dCH;
         a.hw = h->at<double>(L.hw); a.coef = h->at<cplx>(L.coef); a.lam_phi = c.lam_phi; a.phase = phase;
+        a.wall_top = p.wall_top; a.wall_bot = p.wall_bottom;
         LaunchScope ls(h, KC_SOLVE);
-        if (la2) k_elim2<2><<<dim3(col_grid(d), phase ? 2 : 1), NT_COL, 0, h->st>>>(a);
-        else k_elim2<4><<<dim3(col_grid(d), phase ? 2 : 1), NT_COL, 0, h->st>>>(a);
+        const dim3 g2(col_grid(d), phase ? 2 : 1);
+        if (walls_gen) { if (la2) k_elim2<2, true><<<g2, NT_COL, 0, h->st>>>(a); else k_elim2<4, true><<<g2, NT_COL, 0, h->st>>>(a); }
+        else if (la2) k_elim2<2, false><<<g2, NT_COL, 0, h->st>>>(a);
+        else k_elim2<4, false><<<g2, NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     {
