@@ -331,7 +331,16 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident timing -------------------------------------------------------------------
+    # step i) of the algorithm on the device: set_state (forward transform of the four fields when the
+    # workload is a physical-space state), timed on its own (warm call first)
     solver.set_state(space, *dev)
+    torch.cuda.synchronize()
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s0.record()
+    solver.set_state(space, *dev)
+    s1.record()
+    torch.cuda.synchronize()
+    set_state_ms = s0.elapsed_time(s1)
     solver.step(args.warmup)
     barrier()
     sampler = ClockSampler(local)
@@ -350,6 +359,16 @@ def run_ours(args):
     finite = all(bool(torch.isfinite(torch.view_as_real(t)).all()) for t in out)
     maxabs = [float(torch.view_as_real(t).abs().max()) for t in out]
     del out
+    # device-side diagnostics (psdns_diagnostics: mean phi, max |div u|, kinetic energy, wall shear, bulk velocity)
+    solver.diagnostics()
+    torch.cuda.synchronize()
+    d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    d0.record()
+    diag = solver.diagnostics()
+    d1.record()
+    torch.cuda.synchronize()
+    diag_ms = d0.elapsed_time(d1)
+    diag = dict(zip(P.Solver.DIAG_NAMES, [float(x) for x in diag.cpu().numpy()]))
     if not finite:
         # a timing of kernels processing NaN / Inf is not a measurement of this workload: no metric line, non-zero exit
         sys.stderr.write(f"bench.py: state of workload {args.workload} is non-finite after {args.warmup} + {args.steps} steps "
@@ -491,6 +510,10 @@ def run_ours(args):
                               "frac": step_fused_bytes / (ms_max / args.steps * 1e-3) / 1e9 / peak},
             "kernels": kernels,
             "roundtrip": roundtrip,
+            "step_i": {"call": f"psdns_set_state({space_name.upper()})", "ms": set_state_ms, "fields": len(dev),
+                       "note": "PAPER.md L138 step i): one full forward transform per field (x, y, z) when the input is "
+                               "physical, a re-layout when it is spectral; plus the hidden state theta^, omega_z^, D phi^"},
+            "diagnostics": {"ms": diag_ms, **diag},
             "cpu_baseline": cpu,
         }
         print(json.dumps(line))

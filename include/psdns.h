@@ -152,6 +152,28 @@ int psdns_kernel_time_ms(psdns_handle *h, double *ms_total, long long *launches)
  * Uses the transform scratch (not the state).  PSDNS_ESTATE before the first set_state. */
 int psdns_diagnostics(psdns_handle *h, double *d_out);
 
+/* Iso-surface ray-caster (Fig. 5: the drops are rendered as the iso-surface phi = 0).
+ * Pure compute into headless DEVICE buffers, no graphics API.  One ray per pixel:
+ *   camera : f = unit(target - eye), r = unit(f x up), v = r x f; pixel (px, py), py = 0 the top row:
+ *            sx = (2 (px + 1/2)/width - 1) tan(fov_y/2) width/height, sy = (1 - 2 (py + 1/2)/height) tan(fov_y/2),
+ *            direction = unit(f + sx r + sy v)
+ *   box    : slab intersection with [0, lx] x [0, ly] x [-1, 1]; a miss gives intensity 0, depth -1
+ *   field  : trilinear interpolation on the grid (periodic in x, y; z clamped to the Gauss-Lobatto points)
+ *   march  : samples at t0 + i step (last one at the exit point); the first sign change of field - iso is refined by
+ *            24 bisections; depth = ray parameter of the midpoint of the last bracket
+ *   shade  : intensity = 0.2 + 0.8 |unit(grad) . unit(light)|, grad by central differences with steps (lx/nx, ly/ny, 1/N)
+ * d_field: DEVICE double [nz][ny][nx] (PSDNS_PHYSICAL layout), or NULL = the current phase field phi of the state
+ * (needs phase_field = 1 and a state).  d_intensity, d_depth: DEVICE double [height][width], fully overwritten. */
+typedef struct {
+    double eye[3], target[3], up[3];
+    double fov_y_deg;
+    int width, height;
+    double step;
+    double light[3];
+} psdns_camera;
+int psdns_render_isosurface(psdns_handle *h, const psdns_camera *cam, double iso, const void *d_field,
+                            void *d_intensity, void *d_depth);
+
 /* Tuning and test switches.  None is needed for normal use; the defaults are the product path.  Changing an option
  * drops the captured CUDA graph of the step (it is re-captured by the next psdns_step).
  *   "graph"    1 (default) / 0 : replay one captured CUDA graph per step / launch the kernels directly

@@ -14,6 +14,7 @@ EXPORTS = [
     "psdns_kernel_time_ms", "psdns_destroy", "psdns_last_error",
     "psdns_history_bytes", "psdns_get_history", "psdns_set_history",
     "psdns_set_option", "psdns_get_info", "psdns_workspace_bytes_unfused", "psdns_diagnostics",
+    "psdns_render_isosurface",
 ]
 
 
@@ -23,6 +24,11 @@ class PsdnsError(RuntimeError):
 
 class psdns_grid(C.Structure):
     _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("lx", C.c_double), ("ly", C.c_double)]
+
+
+class psdns_camera(C.Structure):
+    _fields_ = [("eye", C.c_double * 3), ("target", C.c_double * 3), ("up", C.c_double * 3), ("fov_y_deg", C.c_double),
+                ("width", C.c_int), ("height", C.c_int), ("step", C.c_double), ("light", C.c_double * 3)]
 
 
 class psdns_params(C.Structure):
@@ -77,6 +83,8 @@ def load_library():
     lib.psdns_set_history.argtypes = [vp, vp, C.c_size_t]
     lib.psdns_diagnostics.restype = ci
     lib.psdns_diagnostics.argtypes = [vp, vp]
+    lib.psdns_render_isosurface.restype = ci
+    lib.psdns_render_isosurface.argtypes = [vp, C.POINTER(psdns_camera), cd, vp, vp, vp]
     lib.psdns_set_option.restype = ci
     lib.psdns_set_option.argtypes = [vp, C.c_char_p, cd]
     lib.psdns_get_info.restype = cd
@@ -213,6 +221,18 @@ class Solver:
         out = self.torch.empty(8, dtype=self.torch.float64, device=self.device)
         self._check(self.lib.psdns_diagnostics(self.handle, _ptr(out)))
         return out
+
+    def render_isosurface(self, eye, target, up=(0.0, 0.0, 1.0), fov_y_deg=40.0, width=64, height=48, step=0.02,
+                          light=(0.3, -0.5, 0.8), iso=0.0, field=None):
+        """psdns_render_isosurface: (intensity, depth) device tensors [height, width]; field = None renders the state's phi."""
+        if field is not None:
+            self._chk_field(field, PHYSICAL)
+        v3 = C.c_double * 3
+        cam = psdns_camera(v3(*eye), v3(*target), v3(*up), fov_y_deg, width, height, step, v3(*light))
+        inten = self.torch.empty((height, width), dtype=self.torch.float64, device=self.device)
+        depth = self.torch.empty((height, width), dtype=self.torch.float64, device=self.device)
+        self._check(self.lib.psdns_render_isosurface(self.handle, C.byref(cam), float(iso), _ptr(field), _ptr(inten), _ptr(depth)))
+        return inten, depth
 
     def set_option(self, name, value):
         self._check(self.lib.psdns_set_option(self.handle, name.encode(), float(value)))

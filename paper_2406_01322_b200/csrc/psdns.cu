@@ -21,6 +21,7 @@
 #include "kernels_diag.cuh"
 #include "kernels_ztma.cuh"
 #include "kernels_zgemm.cuh"
+#include "kernels_raycast.cuh"
 
 #include <cudaTypedefs.h>
 
@@ -53,6 +54,7 @@ struct Layout {
     size_t tw_x, tw_y, tw_z, tw_zn;    // tw_zn: exp(-2 pi i k / N), k < N (the z passes' FFT length)
     size_t ctab_z;                     // c_k of the half-length Chebyshev transform, k <= N/2
     size_t zg_b, zg_f;                 // GEMM-form Chebyshev matrices [ZG_MP][ZG_KP] (N <= 64 only)
+    size_t znodes;                     // z_k = cos(pi k / N) (ray-caster), nz doubles
     size_t ccw;                        // Clenshaw-Curtis weights on z_k (diagnostics), nz doubles
     size_t state[5];                   // u v w phi theta
     size_t hist[3];
@@ -151,6 +153,7 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.tw_zn = take(d.N * C);
     L.ctab_z = take((d.N / 2 + 1) * C);
     L.ccw = take(d.nz * sizeof(double));
+    L.znodes = take(d.nz * sizeof(double));
     L.zg_b = L.zg_f = 0;
     if (d.N <= 64) { L.zg_b = take(ZG_MP * ZG_KP * sizeof(double)); L.zg_f = take(ZG_MP * ZG_KP * sizeof(double)); }
     for (int i = 0; i < 5; ++i) L.state[i] = take(d.s_ret * C);
@@ -775,6 +778,13 @@ cudaError_t build_tables(psdns_handle *h) {
         CU(cudaMemcpyAsync(h->ws + L.zg_f, mf.data(), mf.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
         CU(cudaStreamSynchronize(h->st));
     }
+    {   // Gauss-Lobatto points z_k = cos(pi k / N) (ray-caster)
+        std::vector<double> t(d.nz);
+        for (int k = 0; k <= d.N; ++k) t[k] = (double)cosl(3.14159265358979323846264338327950288L * (long double)k / (long double)d.N);
+        t[0] = 1.0; t[d.N] = -1.0; t[d.N / 2] = 0.0;
+        CU(cudaMemcpyAsync(h->ws + L.znodes, t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
+        CU(cudaStreamSynchronize(h->st));
+    }
     {   // Clenshaw-Curtis weights w_k = (c_k / N) [1 - sum_{j=1}^{N/2} b_j cos(2 j k pi / N) / (4 j^2 - 1)], b_{N/2} = 1 else 2,
         // c_0 = c_N = 1 else 2 (N even): exact for polynomials of degree <= N on the Gauss-Lobatto points
         std::vector<double> t(d.nz);
@@ -1203,6 +1213,52 @@ int psdns_diagnostics(psdns_handle *h, double *d_out) {
         k_diag_final<<<1, DIAG_NT, 0, h->st>>>(part_max, nb_cols, part_sum, nb_en, d_out);
         CUDA_TRY(h, cudaGetLastError());
     }
+    return PSDNS_OK;
+}
+
+int psdns_render_isosurface(psdns_handle *h, const psdns_camera *cam, double iso, const void *d_field, void *d_intensity,
+                            void *d_depth) {
+    if (!h) return PSDNS_EINVAL;
+    if (!cam || !d_intensity || !d_depth || cam->width <= 0 || cam->height <= 0 || !(cam->step > 0) ||
+        !(cam->fov_y_deg > 0) || !(cam->fov_y_deg < 180)) {
+        h->err = "psdns_render_isosurface: null pointer or bad camera";
+        return PSDNS_EINVAL;
+    }
+    const Dims &d = h->d;
+    const Layout &L = h->L;
+    const double *field = (const double *)d_field;
+    if (!field) {   // the current phase field, brought to physical space in the staging buffer
+        if (!h->p.phase_field) { h->err = "psdns_render_isosurface: no phase field and no d_field"; return PSDNS_EINVAL; }
+        if (!h->has_state) { h->err = "psdns_render_isosurface: no state set"; return PSDNS_ESTATE; }
+        FieldPtrs fz{}, fy{}, fx{};
+        fz.in[0] = h->at<cplx>(L.state[3]); fz.out[0] = h->at<cplx>(L.zb[0]);
+        fy.in[0] = fz.out[0]; fy.out[0] = h->at<cplx>(L.yb[0]);
+        fx.in[0] = fy.out[0]; fx.out[0] = h->ws + L.stage[3];
+        CUDA_TRY(h, launch_zpass(h, false, fz, 1, d.ncols, d.nz, d.kxp, d.nky, d.jpos));
+        CUDA_TRY(h, launch_ypass(h, false, fy, 1, d.kxp, d.nky, d.jpos));
+        CUDA_TRY(h, launch_xpass(h, false, fx, 1, d.kxp, d.nkx));
+        field = h->at<double>(L.stage[3]);
+    }
+    auto unit = [](const double *v, double *o) { const double n = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]); for (int c = 0; c < 3; ++c) o[c] = v[c] / n; };
+    auto cross = [](const double *a, const double *b, double *o) { o[0] = a[1] * b[2] - a[2] * b[1]; o[1] = a[2] * b[0] - a[0] * b[2]; o[2] = a[0] * b[1] - a[1] * b[0]; };
+    RayArgs a;
+    a.phi = field; a.zn = h->at<double>(L.znodes);
+    a.intensity = (double *)d_intensity; a.depth = (double *)d_depth;
+    a.nx = d.nx; a.ny = d.ny; a.nz = d.nz; a.lx = h->g.lx; a.ly = h->g.ly;
+    double f[3] = {cam->target[0] - cam->eye[0], cam->target[1] - cam->eye[1], cam->target[2] - cam->eye[2]}, r[3];
+    unit(f, a.fwd);
+    cross(a.fwd, cam->up, r);
+    if (!(r[0] * r[0] + r[1] * r[1] + r[2] * r[2] > 0)) { h->err = "psdns_render_isosurface: up is parallel to the view direction"; return PSDNS_EINVAL; }
+    unit(r, a.right);
+    cross(a.right, a.fwd, a.upv);
+    unit(cam->light, a.light);
+    for (int c = 0; c < 3; ++c) a.eye[c] = cam->eye[c];
+    a.tan_half = std::tan(cam->fov_y_deg * M_PI / 180.0 / 2.0);
+    a.aspect = (double)cam->width / (double)cam->height;
+    a.step = cam->step; a.iso = iso; a.width = cam->width; a.height = cam->height;
+    LaunchScope ls(h, KC_MISC);
+    k_raycast<<<(cam->width * cam->height + 127) / 128, 128, 0, h->st>>>(a);
+    CUDA_TRY(h, cudaGetLastError());
     return PSDNS_OK;
 }
 
