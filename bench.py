@@ -31,7 +31,7 @@ import numpy as np  # noqa: E402
 import psdns_inputs as I  # noqa: E402
 
 METRIC = "grid-point-steps/s"
-TRAFFIC_CSV = "r1h_traffic_5c.csv"   # ncu dram bytes per launch and kernel class, written from the --set full capture
+TRAFFIC_CSV = "r2a_traffic_5c.csv"   # ncu dram bytes per launch and kernel class, written from the --set full capture
 
 
 # ------------------------------------------------------------------------------------------------
@@ -62,6 +62,12 @@ def workload(tag: str):
         c = I.Config("fig3", 256, 256, 257, re=3000.0, ch=1.0, pe=1.0, we=1.0, dt=2e-5, steps=10, seed=1006,
                      phase_field=0)
         kind = "channel-state"
+    elif tag.count("x") == 2 and all(t.isdigit() for t in tag.split("x")):
+        # config-5 recipe (random spectra, SURVEY 8(d) step parameters) on any supported grid, e.g. 512x256x65
+        nx, ny, nz = (int(t) for t in tag.split("x"))
+        k5 = I.scaling_config("5a")
+        c = I.Config("cfg5-" + tag, nx, ny, nz, re=k5.re, ch=k5.ch, pe=k5.pe, we=k5.we, dt=k5.dt, steps=k5.steps, seed=k5.seed)
+        kind = "random-spectra"
     else:
         raise SystemExit(f"unknown workload {tag}")
     return c, kind
@@ -319,7 +325,13 @@ def run_ours(args):
     space_name, host = make_state(c, kind)
     space = P.SPECTRAL if space_name == "spectral" else P.PHYSICAL
     solver = P.Solver(c.nx, c.ny, c.nz, c.lx, c.ly, re=c.re, dt=c.dt, pe=c.pe, ch=c.ch, we=c.we, gradp_x=c.gradp_x,
-                      visc_ratio=c.visc_ratio, phase_field=c.phase_field, device=f"cuda:{local}")
+                      visc_ratio=c.visc_ratio, phase_field=c.phase_field, device=f"cuda:{local}",
+                      unfused_workspace=any(kv.startswith("xfuse=0") for kv in args.option))
+    options = {}
+    for kv in args.option:
+        name, val = kv.split("=")
+        solver.set_option(name, float(val))
+        options[name] = float(val)
     pinned_in = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in host]
     del host
     dev = [t.cuda(non_blocking=True) for t in pinned_in]
@@ -416,7 +428,7 @@ def run_ours(args):
     # under profiles/; null for workloads that were not captured)
     traffic = {}
     try:
-        if args.workload in ("5c", "5c-channel"):     # same grid, same kernels: DRAM traffic does not depend on the data
+        if args.workload in ("5c", "5c-channel") and not options:   # same grid, same kernels: traffic does not depend on the data
             with open(os.path.join(ROOT, "profiles", TRAFFIC_CSV)) as fh:
                 for ln in fh.read().strip().splitlines()[1:]:
                     kname, val = ln.split(",")
@@ -498,7 +510,8 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_string(c, kind), "grid": [c.nx, c.ny, c.nz],
                        "l2": "inputs larger than L2 (state and intermediates >> 126 MB)" if M > 4e6 else "small grid: L2-resident, no roofline claim",
-                       "parallelism": "replicas only" if world > 1 else "single GPU", "finite": finite, "max_abs": maxabs},
+                       "parallelism": "replicas only" if world > 1 else "single GPU", "finite": finite, "max_abs": maxabs,
+                       "options": options},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": METRIC, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                     "ms_per_step": e2e_max / esteps, "steps": esteps, "finite": e2e_finite},
@@ -529,6 +542,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="5c-channel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
+                    help="psdns_set_option before the run (A/B measurements: ztma=0, zgemm=1, xfuse=0, graph=0, ...)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -393,6 +393,38 @@ cudaError_t launch_xpass(psdns_handle *h, bool fwd, const FieldPtrs &f, int nf, 
     return cudaGetLastError();
 }
 
+// fused x kernel of one line length: the single-line warp-per-field kernel where a pass fills a warp (nx = 1024), the
+// multi-line one below that.  Templates, so that only the kernel actually used for a line length is instantiated.
+template <int LL>
+cudaError_t setup_xfused_L(psdns_handle *h) {
+    const size_t sm = xfusedw_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);
+    int occ = 0;
+    cudaError_t e = cudaSuccess;
+    auto prep = [&](auto kern) {
+        e = set_smem(kern, sm);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, XFW_THREADS, sm);
+    };
+    if constexpr (xfw_lpi<LL>() == 1) {
+        if (h->p.phase_field) prep(k_xfusedw<LL, true>); else prep(k_xfusedw<LL, false>);
+    } else {
+        if (h->p.phase_field) prep(k_xfusedwm<LL, true>); else prep(k_xfusedwm<LL, false>);
+    }
+    h->xf_occ = occ;
+    return e;
+}
+
+template <int LL>
+void launch_xfused_L(psdns_handle *h, const XFArgs &a, const cplx *tw, int grid) {
+    const size_t sm = xfusedw_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);
+    if constexpr (xfw_lpi<LL>() == 1) {
+        if (h->p.phase_field) k_xfusedw<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);
+        else k_xfusedw<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);
+    } else {
+        if (h->p.phase_field) k_xfusedwm<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);
+        else k_xfusedwm<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);
+    }
+}
+
 // opt-in to > 48 KB dynamic shared memory once, at init (not inside graph capture), and size the persistent grids
 cudaError_t setup_attrs(psdns_handle *h) {
 #define CU0(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) return e__; } while (0)
@@ -426,29 +458,7 @@ cudaError_t setup_attrs(psdns_handle *h) {
 #undef ZTA
     DISPATCH_L(h->d.ny, YA)
     DISPATCH_L(h->d.nx, XA)
-#define XFA(LL)                                                                                              \
-    {                                                                                                        \
-        const size_t sm = xfusedw_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                              \
-        int occ = 0;                                                                                         \
-        {                                                                                                    \
-            if (xfw_lpi<LL>() == 1) {                                                                        \
-                if (h->p.phase_field) {                                                                      \
-                    CU0(set_smem(k_xfusedw<LL, true>, sm));                                                  \
-                    CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, true>, XFW_THREADS, sm)); \
-                } else {                                                                                     \
-                    CU0(set_smem(k_xfusedw<LL, false>, sm));                                                 \
-                    CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedw<LL, false>, XFW_THREADS, sm)); \
-                }                                                                                            \
-            } else if (h->p.phase_field) {                                                                   \
-                CU0(set_smem(k_xfusedwm<LL, true>, sm));                                                     \
-                CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedwm<LL, true>, XFW_THREADS, sm)); \
-            } else {                                                                                         \
-                CU0(set_smem(k_xfusedwm<LL, false>, sm));                                                    \
-                CU0(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfusedwm<LL, false>, XFW_THREADS, sm)); \
-            }                                                                                                \
-        }                                                                                                    \
-        h->xf_occ = occ;                                                                                     \
-    }
+#define XFA(LL) { CU0(setup_xfused_L<LL>(h)); }
     if (h->nf_in <= 7) { DISPATCH_L(h->d.nx, XFA) }
 #undef XFA
 #define XFVA(LL)                                                                                             \
@@ -472,17 +482,7 @@ cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
     const cplx *tw = h->at<cplx>(h->L.tw_x);
     const int grid = h->persistent_grid(KC_XFUSED, a.nlines, h->xf_occ);   // persistent: one wave
     LaunchScope ls(h, KC_XFUSED);
-#define XF(LL)                                                                                               \
-    {                                                                                                        \
-        const size_t sm = xfusedw_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);                              \
-        {                                                                                                    \
-            if (xfw_lpi<LL>() == 1) {                                                                        \
-                if (h->p.phase_field) k_xfusedw<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);          \
-                else k_xfusedw<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                          \
-            } else if (h->p.phase_field) k_xfusedwm<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);      \
-            else k_xfusedwm<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);                             \
-        }                                                                                                    \
-    }
+#define XF(LL) launch_xfused_L<LL>(h, a, tw, grid);
     DISPATCH_L(h->d.nx, XF)
 #undef XF
     return cudaGetLastError();
