@@ -10,7 +10,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 
 EXPORTS = [
     "psdns_workspace_bytes", "psdns_init", "psdns_set_state", "psdns_step", "psdns_get_state",
-    "psdns_transform_roundtrip", "psdns_run_host", "psdns_launch_count", "psdns_kernel_timing",
+    "psdns_transform_roundtrip", "psdns_run_host", "psdns_run_host_wait", "psdns_launch_count", "psdns_kernel_timing",
     "psdns_kernel_time_ms", "psdns_destroy", "psdns_last_error",
     "psdns_history_bytes", "psdns_get_history", "psdns_set_history",
     "psdns_set_option", "psdns_get_info", "psdns_workspace_bytes_unfused", "psdns_diagnostics",
@@ -69,6 +69,8 @@ def load_library():
     lib.psdns_transform_roundtrip.argtypes = [vp, ci, vp, vp, vp]
     lib.psdns_run_host.restype = ci
     lib.psdns_run_host.argtypes = [vp, ci, ci] + [vp] * 8
+    lib.psdns_run_host_wait.restype = ci
+    lib.psdns_run_host_wait.argtypes = [vp]
     lib.psdns_launch_count.restype = C.c_longlong
     lib.psdns_launch_count.argtypes = [vp]
     lib.psdns_kernel_timing.restype = ci
@@ -188,10 +190,14 @@ class Solver:
         return (out, mid) if want_mid else out
 
     def run_host(self, space, nsteps, h_in, h_out):
-        """h_in / h_out: lists of pinned host tensors (boundary layout).  Asynchronous."""
+        """h_in / h_out: lists of pinned host tensors (boundary layout).  Asynchronous: h_out is valid after run_host_wait()."""
         pi = [C.c_void_p(t.data_ptr()) if t is not None else None for t in (list(h_in) + [None] * 4)[:4]]
         po = [C.c_void_p(t.data_ptr()) if t is not None else None for t in (list(h_out) + [None] * 4)[:4]]
         self._check(self.lib.psdns_run_host(self.handle, space, nsteps, *pi, *po))
+
+    def run_host_wait(self):
+        """Blocks until the device -> host copies of the last run_host have landed in h_out."""
+        self._check(self.lib.psdns_run_host_wait(self.handle))
 
     def get_history(self):
         """Opaque device blob with the hidden state of the time integration (exact restart)."""

@@ -66,7 +66,8 @@ struct Layout {
     size_t prod[8];                    // txx-tzz txy txz tyy-tzz tyz q c
     size_t zb[MAXF], yb[MAXF], ph[MAXF];
     size_t small;                      // ab[2] doubles + counter
-    size_t stage[4];                   // host-staging device buffers (boundary layout)
+    size_t stage[4];                   // host-staging device buffers (boundary layout): inputs of psdns_run_host
+    size_t stage_out[4];               // outputs of psdns_run_host (copied back on the side stream while the next call runs)
     size_t total, total_unfused;
 };
 
@@ -89,6 +90,9 @@ struct psdns_handle {
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tevents;
     int nf_in, nf_out;
     bool use_xfused, has_unfused_ws;
+    cudaStream_t copy_st;        // side stream of psdns_run_host's device -> host copies
+    cudaEvent_t ev_out_ready, ev_d2h_done;
+    bool d2h_pending;
     int xf_occ, xfv_occ, n_sm;
     int occ_z[2], occ_y[2];     // resident CTAs per SM of the persistent z / y passes, [fwd]
     int use_zgemm;              // psdns_set_option("zgemm"): GEMM-form Chebyshev on the FP64 tensor cores for N <= 64
@@ -180,6 +184,7 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.small = take(64);
     const size_t stage_bytes = std::max(d.s_p * sizeof(double), d.s_bspec * C);
     for (int i = 0; i < 4; ++i) L.stage[i] = take(stage_bytes);
+    for (int i = 0; i < 4; ++i) L.stage_out[i] = take(stage_bytes);
     L.total = o;
     // physical-space arrays of the UNFUSED x path (psdns_set_option "xfuse" 0, a cross-check): behind the product's
     // workspace, present only when the caller passed psdns_workspace_bytes_unfused() bytes to psdns_init
@@ -887,6 +892,7 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->has_state = false; h->graph = nullptr; h->graph_ready = false;
     h->use_graph = true;
     h->use_xfused = true;
+    h->copy_st = nullptr; h->ev_out_ready = nullptr; h->ev_d2h_done = nullptr; h->d2h_pending = false;
     h->grid_cap = 0; h->pf = 2; h->pf_rhs = 4;
     h->use_ztma = 1; h->encode_tiled = nullptr; h->use_zgemm = 0;
     for (int i = 0; i < 4; ++i) (&h->occ_zt[0][0])[i] = 1;
@@ -1144,13 +1150,34 @@ int psdns_run_host(psdns_handle *h, int space, int nsteps, const void *h_in_u, c
     void *hout[4] = {h_out_u, h_out_v, h_out_w, h_out_phi};
     void *dev[4];
     const int nf = phase ? 4 : 3;
-    for (int i = 0; i < 4; ++i) dev[i] = h->ws + h->L.stage[i];
+    void *dout[4];
+    for (int i = 0; i < 4; ++i) { dev[i] = h->ws + h->L.stage[i]; dout[i] = h->ws + h->L.stage_out[i]; }
+    if (!h->copy_st) {   // side stream and events of the device -> host leg, created on first use
+        CUDA_TRY(h, cudaStreamCreateWithFlags(&h->copy_st, cudaStreamNonBlocking));
+        CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_out_ready, cudaEventDisableTiming));
+        CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_d2h_done, cudaEventDisableTiming));
+    }
     for (int i = 0; i < nf; ++i) CUDA_TRY(h, cudaMemcpyAsync(dev[i], hin[i], bytes, cudaMemcpyHostToDevice, h->st));
     int rc = psdns_set_state(h, space, dev[0], dev[1], dev[2], phase ? dev[3] : nullptr);
     if (rc != PSDNS_OK) return rc;
     if ((rc = psdns_step(h, nsteps)) != PSDNS_OK) return rc;
-    if ((rc = psdns_get_state(h, space, dev[0], dev[1], dev[2], phase ? dev[3] : nullptr)) != PSDNS_OK) return rc;
-    for (int i = 0; i < nf; ++i) CUDA_TRY(h, cudaMemcpyAsync(hout[i], dev[i], bytes, cudaMemcpyDeviceToHost, h->st));
+    // the output staging buffers are still being read by the previous call's device -> host copies
+    if (h->d2h_pending) CUDA_TRY(h, cudaStreamWaitEvent(h->st, h->ev_d2h_done, 0));
+    if ((rc = psdns_get_state(h, space, dout[0], dout[1], dout[2], phase ? dout[3] : nullptr)) != PSDNS_OK) return rc;
+    CUDA_TRY(h, cudaEventRecord(h->ev_out_ready, h->st));
+    CUDA_TRY(h, cudaStreamWaitEvent(h->copy_st, h->ev_out_ready, 0));
+    for (int i = 0; i < nf; ++i) CUDA_TRY(h, cudaMemcpyAsync(hout[i], dout[i], bytes, cudaMemcpyDeviceToHost, h->copy_st));
+    CUDA_TRY(h, cudaEventRecord(h->ev_d2h_done, h->copy_st));
+    h->d2h_pending = true;
+    return PSDNS_OK;
+}
+
+int psdns_run_host_wait(psdns_handle *h) {
+    if (!h) return PSDNS_EINVAL;
+    if (h->d2h_pending) {
+        CUDA_TRY(h, cudaEventSynchronize(h->ev_d2h_done));
+        h->d2h_pending = false;
+    }
     return PSDNS_OK;
 }
 
@@ -1298,6 +1325,7 @@ double psdns_get_info(const psdns_handle *h, const char *name) {
 int psdns_destroy(psdns_handle *h) {
     if (!h) return PSDNS_EINVAL;
     if (h->graph) cudaGraphExecDestroy(h->graph);
+    if (h->copy_st) { cudaStreamSynchronize(h->copy_st); cudaStreamDestroy(h->copy_st); cudaEventDestroy(h->ev_out_ready); cudaEventDestroy(h->ev_d2h_done); }
     for (auto &pr : h->tevents) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
     delete h;
     return PSDNS_OK;

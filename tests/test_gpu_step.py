@@ -182,3 +182,29 @@ def test_multi_line_x_kernel_plans():
         errs, *_ = run_both(c, [2])
         for k, (ev, ep) in errs.items():
             assert ev < TOL and ep < TOL, (nx, k, ev, ep)
+
+
+def test_run_host_pipelined_calls_match_device_path():
+    """psdns_run_host: three back-to-back calls with different inputs and separate output buffers (the copy-back of one
+    call runs on the side stream while the next call uploads and computes) give exactly what set_state / step / get_state
+    give on device buffers."""
+    import torch
+    import paper_2406_01322_b200 as P
+    c = I.small_config(nx=32, ny=32, nz=33)
+    base = [f for f in I.channel_state(c)]
+    s = solver_from_config(c)
+    ins, outs, refs = [], [], []
+    for k in range(3):
+        st = [np.ascontiguousarray(f * (1.0 + 0.1 * k)) for f in base]
+        ins.append([torch.from_numpy(a).pin_memory() for a in st])
+        outs.append([torch.empty_like(t).pin_memory() for t in ins[-1]])
+        s.set_state(P.PHYSICAL, *[t.cuda() for t in ins[-1]])
+        s.step(2)
+        refs.append([t.cpu() for t in s.get_state(P.PHYSICAL)])
+    for k in range(3):
+        s.run_host(P.PHYSICAL, 2, ins[k], outs[k])
+    s.run_host_wait()
+    for k in range(3):
+        for a, b in zip(outs[k], refs[k]):
+            assert torch.equal(a, b), k
+    s.close()
