@@ -48,6 +48,10 @@ typedef struct {
  * wall_top, wall_bottom: velocity condition at z = +1 / z = -1.  Free-slip turns the condition on
  *             omega_z (and the mean flow) into d/dz = 0 and the second condition on w into d^2 w/dz^2 = 0 (continuity);
  *             phi keeps d phi/dz = d psi/dz = 0.  Zero-initialised structs give the no-slip channel.
+ * surface_tension_form: 1 evaluates the surface tension as a force vector instead of a stress tensor.  The two differ by
+ *             a gradient that Eqs. 14-15 annihilate, in the discrete problem only to truncation error, so it is a switch
+ *             and not an optimisation; it costs one more backward field (lap phi) and three more forward fields, runs the
+ *             three-kernel x path through physical-space arrays (part of its workspace) and is slower than form 0.
  * dealias   : must be 1 for psdns_step (2/3 rule in x, y, z; reading S3).  The round-trip
  *             call always runs with dealiasing off. */
 typedef struct {
@@ -58,6 +62,8 @@ typedef struct {
     int dealias;
     int wall_top;    /* wall z = +1: 0 = no-slip (u = v = w = 0), 1 = free-slip (w = 0, du/dz = dv/dz = 0) - PAPER.md L52 */
     int wall_bottom; /* wall z = -1, same codes; "a combination of them" (L52) = different values at the two walls */
+    int surface_tension_form; /* 0 = divergence of the Korteweg tensor, Eq. 8 as written (reading S5); 1 = the force
+                               * -c_sigma lap(phi) grad(phi): needs phase_field = 1, visc_ratio = 1 */
 } psdns_params;
 
 enum { PSDNS_PHYSICAL = 0, PSDNS_SPECTRAL = 1 };

@@ -88,6 +88,11 @@ class Params:
     # 1 = free-slip (w = 0, du/dz = dv/dz = 0), for the wall z = +1 (top) and z = -1 (bottom); reading S10b of DESIGN.md
     wall_top: int = 0
     wall_bottom: int = 0
+    # Form of the surface-tension term (reading S5): 0 = divergence of the Korteweg tensor, Eq. 8 as
+    # written (tensor in physical space, divergence in spectral space); 1 = the force -c_sigma lap(phi) grad(phi), which
+    # differs from Eq. 8 by the gradient c_sigma grad(|grad phi|^2)/2 - annihilated by the curl formulation of Eqs. 14-15
+    # in the continuous problem, to truncation error in the discrete one
+    surface_tension_form: int = 0
 
 
 NO_SLIP, FREE_SLIP = 0, 1
@@ -315,7 +320,7 @@ def coupled_w_solve(hw: np.ndarray, beta2: np.ndarray, k2: np.ndarray, gamma: fl
 # --------------------------------------------------------------------------------------
 
 
-def pointwise_terms(p: Params, u, v, w, phi=None, phx=None, phy=None, phz=None, strain=None):
+def pointwise_terms(p: Params, u, v, w, phi=None, phx=None, phy=None, phz=None, strain=None, lap_phi=None):
     """Physical-space products.  Returns dict with the symmetric flux tensor
     T_ij = -u_i u_j + c_sigma ( |grad phi|^2 delta_ij - phi_i phi_j ) [+ (eta-1)/Re E_ij]
     (divergence form of Eq. 7's convective term, reading S4; Korteweg tensor of Eq. 8,
@@ -328,13 +333,17 @@ def pointwise_terms(p: Params, u, v, w, phi=None, phx=None, phy=None, phz=None, 
     out = {"T": T}
     if p.phase_field:
         cs = 3.0 / math.sqrt(8.0) * p.ch / p.we
-        g2 = phx * phx + phy * phy + phz * phz
-        T["xx"] = T["xx"] + cs * (g2 - phx * phx)
-        T["yy"] = T["yy"] + cs * (g2 - phy * phy)
-        T["zz"] = T["zz"] + cs * (g2 - phz * phz)
-        T["xy"] = T["xy"] - cs * phx * phy
-        T["xz"] = T["xz"] - cs * phx * phz
-        T["yz"] = T["yz"] - cs * phy * phz
+        if p.surface_tension_form == 0:
+            g2 = phx * phx + phy * phy + phz * phz
+            T["xx"] = T["xx"] + cs * (g2 - phx * phx)
+            T["yy"] = T["yy"] + cs * (g2 - phy * phy)
+            T["zz"] = T["zz"] + cs * (g2 - phz * phz)
+            T["xy"] = T["xy"] - cs * phx * phy
+            T["xz"] = T["xz"] - cs * phx * phz
+            T["yz"] = T["yz"] - cs * phy * phz
+        else:
+            # force form: f = -c_sigma lap(phi) grad(phi), a vector added to S = div T (not a divergence itself)
+            out["F"] = {"x": -cs * lap_phi * phx, "y": -cs * lap_phi * phy, "z": -cs * lap_phi * phz}
         out["Q"] = u * phx + v * phy + w * phz
         out["C"] = phi * phi * phi
         if p.visc_ratio != 1.0:
@@ -430,6 +439,8 @@ class Oracle:
         if p.phase_field:
             phP = np.where(P, s.phi, 0.0)
             spec += [phP, 1j * self.KX * phP, 1j * self.KY * phP, self._Dz(phP)]
+            if p.surface_tension_form == 1:
+                lap_spec = np.where(P, self._lap(phP), 0.0)      # lap of the truncated phi, truncated again (operator P)
             if p.visc_ratio != 1.0:
                 spec += [2j * self.KX * uP, 2j * self.KY * vP,
                          1j * self.KY * uP + 1j * self.KX * vP,
@@ -438,7 +449,8 @@ class Oracle:
         phys = [backward_transform(a, g) for a in spec]
         if p.phase_field:
             strain = phys[7:12] if p.visc_ratio != 1.0 else None
-            pw = pointwise_terms(p, phys[0], phys[1], phys[2], phys[3], phys[4], phys[5], phys[6], strain)
+            lap_phys = backward_transform(lap_spec, g) if p.surface_tension_form == 1 else None
+            pw = pointwise_terms(p, phys[0], phys[1], phys[2], phys[3], phys[4], phys[5], phys[6], strain, lap_phys)
         else:
             pw = pointwise_terms(p, phys[0], phys[1], phys[2])
         out = {k: np.where(P, forward_transform(t, g), 0.0) for k, t in pw["T"].items()}
@@ -446,6 +458,9 @@ class Oracle:
             out["Q"] = np.where(P, forward_transform(pw["Q"], g), 0.0)
             out["C"] = np.where(P, forward_transform(pw["C"], g), 0.0)
             out["phP"] = phP
+            if "F" in pw:
+                for k, t in pw["F"].items():
+                    out["F" + k] = np.where(P, forward_transform(t, g), 0.0)
         return out
 
     def explicit_terms(self):
@@ -456,6 +471,8 @@ class Oracle:
         Sx = ikx * t["xx"] + iky * t["xy"] + self._Dz(t["xz"])
         Sy = ikx * t["xy"] + iky * t["yy"] + self._Dz(t["yz"])
         Sz = ikx * t["xz"] + iky * t["yz"] + self._Dz(t["zz"])
+        if "Fx" in t:                                              # force form of the surface tension (8(f)-4)
+            Sx, Sy, Sz = Sx + t["Fx"], Sy + t["Fy"], Sz + t["Fz"]
         Sx[0, 0, 0] += p.gradp_x                                   # S12
         N = {}
         N["om"] = ikx * Sy - iky * Sx                              # Eq. 14

@@ -103,51 +103,6 @@ __global__ void __launch_bounds__(NT_COL) k_hidden_state(const __grid_constant__
     }
 }
 
-// ---- row a1: derived spectra that need a z derivative ----------------------------------------------------
-// phz = D phi^ (only at set_state: k_finish maintains it afterwards); the five strain spectra of the
-// variable-viscosity term (config 4, reading S14).  i kx phi^ and i ky phi^ are formed inside the z pass.
-struct PrepArgs {
-    ColGeom g;
-    const cplx *u, *v, *w, *phi;
-    cplx *phz;
-    cplx *exx, *eyy, *exy, *exz, *eyz;
-    int do_phz, visc;
-};
-
-__global__ void __launch_bounds__(NT_COL) k_prep(const __grid_constant__ PrepArgs a) {
-    const ColGeom &g = a.g;
-    const int col = blockIdx.x * blockDim.x + threadIdx.x;
-    if (col >= g.ncols) return;
-    double kx, ky;
-    col_wavenumbers(g, col, kx, ky);
-    const size_t st = g.ncols;
-    cplx p1 = cz(), dp1 = cz(), dp2 = cz();
-    cplx u1 = cz(), du1 = cz(), du2 = cz(), v1 = cz(), dv1 = cz(), dv2 = cz();
-    // every derivative is taken of the TRUNCATED field (P first, then D; SURVEY 8(c) step 1)
-    for (int n = g.nkz - 1; n >= 0; --n) {
-        const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
-        const size_t o = n * st + col;
-        if (a.do_phz) {
-            const cplx pn = a.phi[o];
-            const cplx dpn = cscale(cfma(f, p1, dp2), h);
-            a.phz[o] = dpn;
-            p1 = pn; dp2 = dp1; dp1 = dpn;
-        }
-        if (a.visc) {
-            const cplx un = a.u[o], vn = a.v[o], wn = a.w[o];
-            const cplx dun = cscale(cfma(f, u1, du2), h);
-            const cplx dvn = cscale(cfma(f, v1, dv2), h);
-            a.exx[o] = cscale(ci(un), 2.0 * kx);
-            a.eyy[o] = cscale(ci(vn), 2.0 * ky);
-            a.exy[o] = cadd(cscale(ci(un), ky), cscale(ci(vn), kx));
-            a.exz[o] = cadd(dun, cscale(ci(wn), kx));
-            a.eyz[o] = cadd(dvn, cscale(ci(wn), ky));
-            u1 = un; du2 = du1; du1 = dun;
-            v1 = vn; dv2 = dv1; dv1 = dvn;
-        }
-    }
-}
-
 // ---- derivative recurrences fed top-down (used by rows a1, a9, a11) ------------------------------------
 struct Chain1 {  // first derivative of a sequence fed top-down
     cplx a1, b1, b2;
@@ -168,6 +123,60 @@ struct Chain2 {  // second derivative
         return cn;
     }
 };
+
+// ---- row a1: derived spectra that need a z derivative ----------------------------------------------------
+// phz = D phi^ (only at set_state: k_finish maintains it afterwards); the five strain spectra of the
+// variable-viscosity term (config 4, reading S14).  i kx phi^ and i ky phi^ are formed inside the z pass.
+struct PrepArgs {
+    ColGeom g;
+    const cplx *u, *v, *w, *phi;
+    cplx *phz;
+    cplx *exx, *eyy, *exy, *exz, *eyz;
+    int do_phz, visc;
+    cplx *lap;       // do_lap: (D^2 - k^2) of the truncated phi^ (force form of the surface tension)
+    int do_lap;
+};
+
+__global__ void __launch_bounds__(NT_COL) k_prep(const __grid_constant__ PrepArgs a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const size_t st = g.ncols;
+    cplx p1 = cz(), dp1 = cz(), dp2 = cz();
+    cplx u1 = cz(), du1 = cz(), du2 = cz(), v1 = cz(), dv1 = cz(), dv2 = cz();
+    Chain2 cL;
+    cL.init();
+    const double k2 = kx * kx + ky * ky;
+    // every derivative is taken of the TRUNCATED field (P first, then D; SURVEY 8(c) step 1)
+    for (int n = g.nkz - 1; n >= 0; --n) {
+        const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
+        const size_t o = n * st + col;
+        if (a.do_lap) {
+            const cplx pn = a.phi[o];
+            a.lap[o] = cfma(-k2, pn, cL.step(pn, f, h));
+        }
+        if (a.do_phz) {
+            const cplx pn = a.phi[o];
+            const cplx dpn = cscale(cfma(f, p1, dp2), h);
+            a.phz[o] = dpn;
+            p1 = pn; dp2 = dp1; dp1 = dpn;
+        }
+        if (a.visc) {
+            const cplx un = a.u[o], vn = a.v[o], wn = a.w[o];
+            const cplx dun = cscale(cfma(f, u1, du2), h);
+            const cplx dvn = cscale(cfma(f, v1, dv2), h);
+            a.exx[o] = cscale(ci(un), 2.0 * kx);
+            a.eyy[o] = cscale(ci(vn), 2.0 * ky);
+            a.exy[o] = cadd(cscale(ci(un), ky), cscale(ci(vn), kx));
+            a.exz[o] = cadd(dun, cscale(ci(wn), kx));
+            a.eyz[o] = cadd(dvn, cscale(ci(wn), ky));
+            u1 = un; du2 = du1; du1 = dun;
+            v1 = vn; dv2 = dv1; dv1 = dvn;
+        }
+    }
+}
 
 // ---- row a10: quasi-tridiagonal Chebyshev-tau Helmholtz solve ---------------------------------------
 // (D^2 - sigma) u = f in rows 0..N-2 plus two boundary rows (reading S11).  In coefficient space,
@@ -471,6 +480,7 @@ struct ElimDown2R {
 struct RhsElimArgs {
     ColGeom g;
     const cplx *txx, *txy, *txz, *tyy, *tyz, *q, *c;   // txx, tyy hold the deviatoric T_xx - T_zz, T_yy - T_zz
+    const cplx *fx, *fy, *fz;         // FORCE only: the surface-tension force -c lap(phi) grad(phi), added to S = div T
     cplx *om, *th, *phi;              // in: omega^n, theta^n, phi^n; out: g' arrays (slots 0,1 = u_0, u_1)
     cplx *h_om, *h_w, *h_phi;
     const double *dinv_ns, *dinv_ch;
@@ -485,8 +495,11 @@ constexpr int RHS_COLS = 32;   // columns per CTA of k_rhs_elim (blockDim = 32 *
 #ifndef RHS_MINB
 #define RHS_MINB 4
 #endif
-template <bool GEN>   // GEN: walls that are not both no-slip (row f3); false = the no-slip product path, unchanged
-__global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
+// GEN: walls that are not both no-slip (row f3).  FORCE: the surface tension enters as a force vector F next to the flux
+// tensor: N_omega += i (kx F_y - ky F_x), N_w += -k^2 F_z - D (i kx F_x + i ky F_y), S-bar += F(0,0).
+// <false, false> is the product path, unchanged.
+template <bool GEN, bool FORCE>
+__global__ void __launch_bounds__(96, (FORCE ? 3 : RHS_MINB)) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
     const ColGeom &g = a.g;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const bool nschain = warp < 2;
@@ -513,7 +526,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
         double *xo = reinterpret_cast<double *>(a.om + col) + c, *xt = reinterpret_cast<double *>(a.th + col) + c;
         double *ho = reinterpret_cast<double *>(a.h_om + col) + c, *hw = reinterpret_cast<double *>(a.h_w + col) + c;
         const size_t st2 = 2 * st;
-        struct RowIn { double xo, xt, ho, hw, t0, t1, t3; cplx t2, t4; };
+        struct RowIn { double xo, xt, ho, hw, t0, t1, t3; cplx t2, t4; cplx f0, f1; double f2; };
         PivotDown pv;
         pv.init();
         auto load = [&](int n) {
@@ -527,6 +540,10 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
                 r.t1 = reinterpret_cast<const double *>(txy + o)[c];
                 r.t3 = reinterpret_cast<const double *>(tyy + o)[c];
                 r.t2 = txz[o]; r.t4 = tyz[o];
+                if (FORCE) {
+                    r.f0 = a.fx[col + o]; r.f1 = a.fy[col + o];
+                    r.f2 = reinterpret_cast<const double *>(a.fz + col + o)[c];
+                }
             }
             return r;
         };
@@ -567,6 +584,17 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
                     B = r.t0 * (kx * kx) + r.t1 * (2.0 * kx * ky) + r.t3 * (ky * ky);
                 }
             }
+            double extra_w = 0.0;
+            if (FORCE && low) {
+                const double f0c = c ? r.f0.y : r.f0.x, f0o = c ? r.f0.x : r.f0.y;
+                const double f1c = c ? r.f1.y : r.f1.x, f1o = c ? r.f1.x : r.f1.y;
+                if (mean) { P = f0c; extra_w = f1c; }                     // S-bar_x += F_x(0,0), S-bar_y += F_y(0,0)
+                else {
+                    P += sg * (kx * f1o - ky * f0o);                      // i (kx F_y - ky F_x)
+                    B -= sg * (kx * f0o + ky * f1o);                      // -D (i kx F_x + i ky F_y): B is differentiated once
+                    extra_w = -k2 * r.f2;                                 // -k^2 F_z
+                }
+            }
             const double dR = fma(f, Ra1, Rb2) * h; Ra1 = R; Rb2 = Rb1; Rb1 = dR;
             const double dB = fma(f, Ba1, Bb2) * h; Ba1 = B; Bb2 = Bb1; Bb1 = dB;
             const double dA = fma(f, Aa1, Ab2) * h, ddA = fma(f, Ab1, Ac2) * h;
@@ -577,7 +605,7 @@ __global__ void __launch_bounds__(96, RHS_MINB) k_rhs_elim(const __grid_constant
             Ta1 = r.xt; Tb2 = Tb1; Tb1 = dT; Tc2 = Tc1; Tc1 = ddT;
             double nl_o = P + dR;
             if (mean && n == 0 && c == 0) nl_o += a.gradp;
-            const double nl_w = (dB - ddA) + A * (-k2);
+            const double nl_w = (dB - ddA) + A * (-k2) + extra_w;
             double so = nl_o * ab0, sw = nl_w * ab0;
             if (low) {
                 so = fma(ab1, r.ho, so); sw = fma(ab1, r.hw, sw);

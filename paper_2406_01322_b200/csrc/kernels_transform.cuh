@@ -334,11 +334,12 @@ __global__ void __launch_bounds__(tile_threads<L>()) k_xpass(const __grid_consta
 // ------------------------------------------------------------------------------------------
 struct PwArgs {
     const double *b[MAXF];
-    double *o[8];
+    double *o[10];
     size_t n;
     double cs;        // 3/sqrt(8) Ch/We
     double eta_c;     // (lambda - 1) / (2 Re)
     int phase, visc;
+    int force;        // surface tension as the force -cs lap(phi) grad(phi) (b[7] = lap phi, o[7..9] = F) instead of the Korteweg tensor
 };
 
 __global__ void __launch_bounds__(256) k_pointwise(const __grid_constant__ PwArgs a) {
@@ -350,11 +351,16 @@ __global__ void __launch_bounds__(256) k_pointwise(const __grid_constant__ PwArg
         if (a.phase) {
             const double ph = a.b[3][i], px = a.b[4][i], py = a.b[5][i], pz = a.b[6][i];
             const double cs = a.cs;
-            dxx += cs * (pz * pz - px * px);
-            dyy += cs * (pz * pz - py * py);
-            txy -= cs * px * py;
-            txz -= cs * px * pz;
-            tyz -= cs * py * pz;
+            if (a.force) {
+                const double m = -cs * a.b[7][i];
+                a.o[7][i] = m * px; a.o[8][i] = m * py; a.o[9][i] = m * pz;
+            } else {
+                dxx += cs * (pz * pz - px * px);
+                dyy += cs * (pz * pz - py * py);
+                txy -= cs * px * py;
+                txz -= cs * px * pz;
+                tyz -= cs * py * pz;
+            }
             if (a.visc) {
                 const double e1 = a.eta_c * (ph + 1.0);
                 const double exx = a.b[7][i], eyy = a.b[8][i], exy = a.b[9][i], exz = a.b[10][i], eyz = a.b[11][i];

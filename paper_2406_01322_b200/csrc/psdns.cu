@@ -63,7 +63,7 @@ struct Layout {
     size_t hw, coef;                   // [2][ncols] doubles / cplx
     size_t xom;
     size_t derived[8];                 // phz [exx eyy exy exz eyz]
-    size_t prod[8];                    // txx-tzz txy txz tyy-tzz tyz q c
+    size_t prod[10];                   // txx-tzz txy txz tyy-tzz tyz q c [fx fy fz: force form of the surface tension]
     size_t zb[MAXF], yb[MAXF], ph[MAXF];
     size_t small;                      // ab[2] doubles + counter
     size_t stage[4];                   // host-staging device buffers (boundary layout): inputs of psdns_run_host
@@ -123,6 +123,8 @@ bool validate(const psdns_grid *g, const psdns_params *p) {
     if (!(g->lx > 0) || !(g->ly > 0)) return false;
     if (!(p->re > 0) || !(p->dt > 0)) return false;
     if (p->phase_field != 0 && p->phase_field != 1) return false;
+    if (p->surface_tension_form != 0 && p->surface_tension_form != 1) return false;
+    if (p->surface_tension_form == 1 && (!p->phase_field || p->visc_ratio != 1.0)) return false;   // force form: matched viscosity only
     if ((p->wall_top != 0 && p->wall_top != 1) || (p->wall_bottom != 0 && p->wall_bottom != 1)) return false;
     if (p->phase_field && (!(p->pe > 0) || !(p->ch > 0) || !(p->we > 0) || !(p->visc_ratio > 0))) return false;
     return true;
@@ -170,10 +172,11 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.xom = take(d.s_ret * C);
     const bool visc_l = p.phase_field && p.visc_ratio != 1.0;
     for (int i = 0; i < 8; ++i) L.derived[i] = 0;
-    for (int i = 0; i < (visc_l ? 6 : 1); ++i) L.derived[i] = take(d.s_low * C);   // phz [+ 5 strains]
-    for (int i = 0; i < 8; ++i) L.prod[i] = 0;
-    for (int i = 0; i < 7; ++i) L.prod[i] = take(d.s_low * C);
-    const int nf = visc_l ? 12 : 7;
+    const bool force_l = p.phase_field && p.surface_tension_form == 1;
+    for (int i = 0; i < (visc_l ? 6 : (force_l ? 2 : 1)); ++i) L.derived[i] = take(d.s_low * C);   // phz [+ 5 strains | + lap phi]
+    for (int i = 0; i < 10; ++i) L.prod[i] = 0;
+    for (int i = 0; i < (force_l ? 10 : 7); ++i) L.prod[i] = take(d.s_low * C);
+    const int nf = visc_l ? 12 : (force_l ? 10 : 7);
     // Z / Y arrays double as the full-size round-trip scratch (3 arrays of s_full each)
     size_t zy_bytes = 0;
     for (int i = 0; i < MAXF; ++i) { L.zb[i] = 0; L.yb[i] = 0; L.ph[i] = 0; }
@@ -185,10 +188,12 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     const size_t stage_bytes = std::max(d.s_p * sizeof(double), d.s_bspec * C);
     for (int i = 0; i < 4; ++i) L.stage[i] = take(stage_bytes);
     for (int i = 0; i < 4; ++i) L.stage_out[i] = take(stage_bytes);
+    // the force form of the surface tension runs the three-kernel x path: its physical arrays are product state
+    if (force_l) for (int i = 0; i < nf; ++i) L.ph[i] = take(d.s_p * sizeof(double));
     L.total = o;
     // physical-space arrays of the UNFUSED x path (psdns_set_option "xfuse" 0, a cross-check): behind the product's
     // workspace, present only when the caller passed psdns_workspace_bytes_unfused() bytes to psdns_init
-    for (int i = 0; i < nf; ++i) L.ph[i] = take(d.s_p * sizeof(double));
+    if (!force_l) for (int i = 0; i < nf; ++i) L.ph[i] = take(d.s_p * sizeof(double));
     L.total_unfused = o;
     return L;
 }
@@ -563,6 +568,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
     const Coefs c = coefs(p);
     const bool phase = p.phase_field != 0;
     const bool visc = phase && p.visc_ratio != 1.0;
+    const bool force = phase && p.surface_tension_form == 1;
     const int nout = h->nf_out;
     cplx *U = h->at<cplx>(L.state[0]), *V = h->at<cplx>(L.state[1]), *W = h->at<cplx>(L.state[2]);
     cplx *PHI = h->at<cplx>(L.state[3]), *TH = h->at<cplx>(L.state[4]), *OM = h->at<cplx>(L.xom);
@@ -573,11 +579,19 @@ cudaError_t enqueue_step(psdns_handle *h) {
 
     // a1 (variable viscosity only): strain spectra
     if (visc) {
-        PrepArgs a;
+        PrepArgs a{};
         a.g = geom(h); a.u = U; a.v = V; a.w = W; a.phi = PHI; a.phz = PHZ;
         a.exx = h->at<cplx>(L.derived[1]); a.eyy = h->at<cplx>(L.derived[2]); a.exy = h->at<cplx>(L.derived[3]);
         a.exz = h->at<cplx>(L.derived[4]); a.eyz = h->at<cplx>(L.derived[5]);
         a.do_phz = 0; a.visc = 1;
+        LaunchScope ls(h, KC_RHS);
+        k_prep<<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        CU(cudaGetLastError());
+    }
+    if (force) {   // row a1, force form: lap(phi)^ = (D^2 - k^2) P phi^, the 8th backward field
+        PrepArgs a{};
+        a.g = geom(h); a.phi = PHI; a.lap = h->at<cplx>(L.derived[1]);
+        a.do_phz = 0; a.visc = 0; a.do_lap = 1;
         LaunchScope ls(h, KC_RHS);
         k_prep<<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
@@ -599,6 +613,11 @@ cudaError_t enqueue_step(psdns_handle *h) {
                 zd.dfield = 3; zd.out_dx = h->at<cplx>(L.zb[10]); zd.out_dy = h->at<cplx>(L.zb[11]);
                 ny_f = 12;
             }
+        } else if (force) {   // Z arrays: u v w phi phz lap | i ky phi | i kx phi
+            src[5] = h->at<cplx>(L.derived[1]);
+            nz_f = 6;
+            zd.dfield = 3; zd.out_dy = h->at<cplx>(L.zb[6]); zd.out_dx = h->at<cplx>(L.zb[7]);
+            ny_f = 8;
         } else {
             const bool fused = h->use_xfused;
             zd.dfield = 3; zd.out_dx = fused ? nullptr : h->at<cplx>(L.zb[6]); zd.out_dy = h->at<cplx>(L.zb[5]);
@@ -644,11 +663,12 @@ cudaError_t enqueue_step(psdns_handle *h) {
             //                                                            (matched viscosity: 0 1 2 3 6 5 4)
             const int order_v[MAXF] = {0, 1, 2, 3, 10, 11, 4, 5, 6, 7, 8, 9};
             const int order_m[MAXF] = {0, 1, 2, 3, 6, 5, 4, 0, 0, 0, 0, 0};
+            const int order_f[MAXF] = {0, 1, 2, 3, 7, 6, 4, 5, 0, 0, 0, 0};   // force form: .. phx phy phz lap
             for (int i = 0; i < MAXF; ++i)
-                a.b[i] = h->at<double>(L.ph[phase ? (visc ? order_v[i] : order_m[i]) : (i < 3 ? i : 0)]);
-            for (int i = 0; i < 8; ++i) a.o[i] = h->at<double>(L.ph[i < nout ? i : 0]);
+                a.b[i] = h->at<double>(L.ph[phase ? (visc ? order_v[i] : (force ? order_f[i] : order_m[i])) : (i < 3 ? i : 0)]);
+            for (int i = 0; i < 10; ++i) a.o[i] = h->at<double>(L.ph[i < nout ? i : 0]);
             a.n = d.s_p; a.cs = c.cs; a.eta_c = (p.visc_ratio - 1.0) / (2.0 * p.re);
-            a.phase = phase; a.visc = visc;
+            a.phase = phase; a.visc = visc; a.force = force;
             LaunchScope ls(h, KC_PW);
             k_pointwise<<<h->n_sm * 8, 256, 0, h->st>>>(a);
             CU(cudaGetLastError());
@@ -671,6 +691,8 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.txx = h->at<cplx>(L.prod[0]); a.txy = h->at<cplx>(L.prod[1]); a.txz = h->at<cplx>(L.prod[2]);
         a.tyy = h->at<cplx>(L.prod[3]); a.tyz = h->at<cplx>(L.prod[4]);
         a.q = h->at<cplx>(L.prod[5]); a.c = h->at<cplx>(L.prod[6]);
+        a.fx = force ? h->at<cplx>(L.prod[7]) : nullptr; a.fy = force ? h->at<cplx>(L.prod[8]) : nullptr;
+        a.fz = force ? h->at<cplx>(L.prod[9]) : nullptr;
         a.om = OM; a.th = TH; a.phi = PHI;
         a.h_om = h->at<cplx>(L.hist[0]); a.h_w = h->at<cplx>(L.hist[1]); a.h_phi = h->at<cplx>(L.hist[2]);
         a.dinv_ns = dNS; a.dinv_ch = dCH;
@@ -680,8 +702,10 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.wall_top = p.wall_top; a.wall_bot = p.wall_bottom;
         const int grid = (int)((d.ncols + RHS_COLS - 1) / RHS_COLS);
         LaunchScope ls(h, KC_RHS);
-        if (walls_gen) k_rhs_elim<true><<<grid, 32 * (phase ? 3 : 2), 0, h->st>>>(a);
-        else k_rhs_elim<false><<<grid, 32 * (phase ? 3 : 2), 0, h->st>>>(a);
+        const int nt = 32 * (phase ? 3 : 2);
+        if (force) { if (walls_gen) k_rhs_elim<true, true><<<grid, nt, 0, h->st>>>(a); else k_rhs_elim<false, true><<<grid, nt, 0, h->st>>>(a); }
+        else if (walls_gen) k_rhs_elim<true, false><<<grid, nt, 0, h->st>>>(a);
+        else k_rhs_elim<false, false><<<grid, nt, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     {
@@ -909,8 +933,10 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->launches = 0; h->per_step = 0; h->timed_class = -1;
     const bool phase = params->phase_field != 0;
     const bool visc = phase && params->visc_ratio != 1.0;
-    h->nf_in = phase ? (visc ? 12 : 7) : 3;
-    h->nf_out = phase ? 7 : 5;
+    const bool force = phase && params->surface_tension_form == 1;
+    h->nf_in = phase ? (visc ? 12 : (force ? 8 : 7)) : 3;
+    h->nf_out = phase ? (force ? 10 : 7) : 5;
+    if (force) h->use_xfused = false;   // three-kernel x path (k_xpass, k_pointwise, k_xpass): 10 forward fields exceed the fused tile
     h->xf_occ = 1; h->xfv_occ = 1; h->n_sm = 148;
     h->occ_z[0] = h->occ_z[1] = h->occ_y[0] = h->occ_y[1] = 1;
     {
@@ -919,7 +945,7 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
             h->n_sm = nsm;
     }
     if (bytes < h->L.total || ((uintptr_t)d_workspace % ALIGN) != 0) { delete h; return PSDNS_ENOMEM; }
-    h->has_unfused_ws = bytes >= h->L.total_unfused;
+    h->has_unfused_ws = bytes >= h->L.total_unfused || force;
     cudaError_t e = setup_attrs(h);
     if (e == cudaSuccess) e = build_tables(h);
     if (e != cudaSuccess) {
@@ -1294,6 +1320,10 @@ int psdns_set_option(psdns_handle *h, const char *name, double value) {
     const std::string n(name);
     const int iv = (int)value;
     if (n == "graph") h->use_graph = iv != 0;
+    else if (n == "xfuse" && iv && h->p.phase_field && h->p.surface_tension_form == 1) {
+        h->err = "psdns_set_option: the force form of the surface tension has no fused x kernel";
+        return PSDNS_EINVAL;
+    }
     else if (n == "xfuse") {
         if (!iv && !h->has_unfused_ws) { h->err = "psdns_set_option: xfuse = 0 needs psdns_workspace_bytes_unfused() bytes at init"; return PSDNS_ENOMEM; }
         h->use_xfused = iv != 0;

@@ -218,10 +218,12 @@ def test_non_equilibrium_profile_relaxes_towards_tanh():
     assert d1 < d0
 
 
-def test_explicit_terms_match_symbolic_continuous_formulas():
+@pytest.mark.parametrize("form", [0, 1])
+def test_explicit_terms_match_symbolic_continuous_formulas(form):
+    """form 0: Korteweg tensor (Eq. 8 as written); form 1: the force -c_sigma lap(phi) grad(phi)."""
     import sympy as sp
     g = O.Grid(16, 16, 65)
-    p = O.Params(re=80.0, dt=1e-3, pe=3.0, ch=0.3, we=1.3, gradp_x=0.04, visc_ratio=0.3)
+    p = O.Params(re=80.0, dt=1e-3, pe=3.0, ch=0.3, we=1.3, gradp_x=0.04, visc_ratio=0.3, surface_tension_form=form)
     x, y, z = sp.symbols("x y z", real=True)
     kx, ky = sp.Rational(1, 2), 1                         # fundamental wavenumbers of 4pi x 2pi
     q = 1 - z ** 2
@@ -242,9 +244,11 @@ def test_explicit_terms_match_symbolic_continuous_formulas():
     T = sp.zeros(3, 3)
     for a in range(3):
         for b in range(3):
-            T[a, b] = (-U[a] * U[b] + cs * ((gp.dot(gp) if a == b else 0) - gp[a] * gp[b])
+            T[a, b] = (-U[a] * U[b] + (cs * ((gp.dot(gp) if a == b else 0) - gp[a] * gp[b]) if form == 0 else 0)
                        + eta1 * (sp.diff(U[b], X[a]) + sp.diff(U[a], X[b])))
     S = sp.Matrix([sum(sp.diff(T[a, b], X[b]) for b in range(3)) for a in range(3)])
+    if form == 1:
+        S = S - cs * lap(phi) * gp
     S[0] = S[0] + sp.Float(p.gradp_x)
     divS = sum(sp.diff(S[a], X[a]) for a in range(3))
     N_om = curl(S)[2]                                              # Eq. 14
@@ -334,3 +338,30 @@ def test_variable_viscosity_steady_layered_flow():
         t_fine, _ = tendency(257, 0.07)
     assert umax > 1.5                            # the low-viscosity layer speeds the flow up (lambda = 1: max u = 1)
     assert t_coarse < 5e-6 and t_fine < 5e-8, (t_coarse, t_fine)
+
+
+def test_surface_tension_forms_differ_by_a_gradient_only():
+    """Korteweg divergence (form 0) and the force -c lap(phi) grad(phi) (form 1) differ by grad(c |grad phi|^2 / 2), which
+    the curl (Eq. 14) and the lap S_z - d/dz div S combination (Eq. 15) annihilate: N_omega and N_w of the two forms agree
+    to truncation error on a resolved state - but not to rounding (they are different discrete operators), which is why
+    the form is a switch of the oracle and not a free choice of the kernels.  S_phi does not contain the term at all."""
+    g = O.Grid(16, 16, 49)
+    z = O.cheb_nodes(g.N)[:, None, None]
+    x = g.lx / g.nx * np.arange(g.nx)[None, None, :]
+    y = g.ly / g.ny * np.arange(g.ny)[None, :, None]
+    q = 1 - z * z
+    phi = 0.3 * q ** 4 * np.cos(0.5 * x) * np.cos(y) + 0.2 * z * np.sin(y) - 0.1 + 0 * x
+    u = 0.5 * q * np.ones_like(phi)
+    zero = np.zeros_like(phi)
+    out = []
+    for form in (0, 1):
+        p = O.Params(re=80.0, dt=1e-3, pe=3.0, ch=0.3, we=1.3, surface_tension_form=form)
+        orc = O.Oracle(g, p)
+        orc.set_state("physical", u, zero, zero, phi)
+        out.append(orc.explicit_terms())
+    for key in ("om", "w"):
+        d = O.rel_l2(out[1][key], out[0][key])
+        assert 1e-15 < d < 1e-7, (key, d)
+    assert np.array_equal(out[0]["phi"], out[1]["phi"])
+    # the mean-flow forcing S-bar_x differs by d/dx of a mean: nothing
+    assert np.abs(out[0]["ubar"] - out[1]["ubar"]).max() < 1e-12
