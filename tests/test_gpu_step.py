@@ -86,6 +86,15 @@ def test_ragged_shapes():
             assert ev < TOL and ep < TOL, (nx, ny, nz, k, ev, ep)
 
 
+def test_extreme_supported_sizes():
+    """Smallest and largest supported line lengths (R4): ny = 1024 (one-CTA-per-SM y pass), nx = ny = 16, nz = 9."""
+    for (nx, ny, nz) in [(16, 1024, 9), (16, 16, 9), (1024, 16, 9)]:
+        c = I.small_config(nx=nx, ny=ny, nz=nz, band=2)
+        errs, *_ = run_both(c, [2])
+        for k, (ev, ep) in errs.items():
+            assert ev < TOL and ep < TOL, (nx, ny, nz, k, ev, ep)
+
+
 def test_spectral_set_state_equals_physical():
     import paper_2406_01322_b200 as P
     c = I.small_config()
