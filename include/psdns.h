@@ -48,6 +48,8 @@ typedef struct {
  * wall_top, wall_bottom: velocity condition at z = +1 / z = -1.  Free-slip turns the condition on
  *             omega_z (and the mean flow) into d/dz = 0 and the second condition on w into d^2 w/dz^2 = 0 (continuity);
  *             phi keeps d phi/dz = d psi/dz = 0.  Zero-initialised structs give the no-slip channel.
+ * convection_form: 1 evaluates the convective term as u x omega (vorticity of the truncated velocity formed in spectral
+ *             space, three more backward fields); differs from form 0 by grad(|u|^2 / 2), see surface_tension_form.
  * surface_tension_form: 1 evaluates the surface tension as a force vector instead of a stress tensor.  The two differ by
  *             a gradient that Eqs. 14-15 annihilate, in the discrete problem only to truncation error, so it is a switch
  *             and not an optimisation; it costs one more backward field (lap phi) and three more forward fields, runs the
@@ -64,6 +66,8 @@ typedef struct {
     int wall_bottom; /* wall z = -1, same codes; "a combination of them" (L52) = different values at the two walls */
     int surface_tension_form; /* 0 = divergence of the Korteweg tensor, Eq. 8 as written (reading S5); 1 = the force
                                * -c_sigma lap(phi) grad(phi): needs phase_field = 1, visc_ratio = 1 */
+    int convection_form;      /* 0 = divergence form -div(u u) (reading S4); 1 = rotational form u x omega;
+                               * not together with visc_ratio != 1 */
 } psdns_params;
 
 enum { PSDNS_PHYSICAL = 0, PSDNS_SPECTRAL = 1 };

@@ -93,6 +93,9 @@ class Params:
     # differs from Eq. 8 by the gradient c_sigma grad(|grad phi|^2)/2 - annihilated by the curl formulation of Eqs. 14-15
     # in the continuous problem, to truncation error in the discrete one
     surface_tension_form: int = 0
+    # Form of the convective term (reading S4): 0 = divergence form -div(u u); 1 = rotational form u x omega
+    # (the two differ by grad(|u|^2 / 2), which Eqs. 14-15 annihilate - to truncation error in the discrete problem)
+    convection_form: int = 0
 
 
 NO_SLIP, FREE_SLIP = 0, 1
@@ -320,17 +323,24 @@ def coupled_w_solve(hw: np.ndarray, beta2: np.ndarray, k2: np.ndarray, gamma: fl
 # --------------------------------------------------------------------------------------
 
 
-def pointwise_terms(p: Params, u, v, w, phi=None, phx=None, phy=None, phz=None, strain=None, lap_phi=None):
+def pointwise_terms(p: Params, u, v, w, phi=None, phx=None, phy=None, phz=None, strain=None, lap_phi=None, vort=None):
     """Physical-space products.  Returns dict with the symmetric flux tensor
     T_ij = -u_i u_j + c_sigma ( |grad phi|^2 delta_ij - phi_i phi_j ) [+ (eta-1)/Re E_ij]
     (divergence form of Eq. 7's convective term, reading S4; Korteweg tensor of Eq. 8,
     c_sigma = 3/sqrt(8) Ch/We, reading S5; variable viscosity reading S14) and, with the
     phase field on, Q = u . grad phi (Eq. 1) and C = phi^3 (Eq. 4)."""
-    T = {
-        "xx": -u * u, "xy": -u * v, "xz": -u * w,
-        "yy": -v * v, "yz": -v * w, "zz": -w * w,
-    }
-    out = {"T": T}
+    if p.convection_form == 0:
+        T = {
+            "xx": -u * u, "xy": -u * v, "xz": -u * w,
+            "yy": -v * v, "yz": -v * w, "zz": -w * w,
+        }
+        out = {"T": T}
+    else:
+        # rotational form: -(u . grad) u = u x omega - grad(|u|^2 / 2); the gradient is dropped, u x omega is a force vector
+        zero = np.zeros_like(u)
+        T = {k: zero.copy() for k in ("xx", "xy", "xz", "yy", "yz", "zz")}
+        ox, oy, oz = vort
+        out = {"T": T, "F": {"x": v * oz - w * oy, "y": w * ox - u * oz, "z": u * oy - v * ox}}
     if p.phase_field:
         cs = 3.0 / math.sqrt(8.0) * p.ch / p.we
         if p.surface_tension_form == 0:
@@ -343,7 +353,8 @@ def pointwise_terms(p: Params, u, v, w, phi=None, phx=None, phy=None, phz=None, 
             T["yz"] = T["yz"] - cs * phy * phz
         else:
             # force form: f = -c_sigma lap(phi) grad(phi), a vector added to S = div T (not a divergence itself)
-            out["F"] = {"x": -cs * lap_phi * phx, "y": -cs * lap_phi * phy, "z": -cs * lap_phi * phz}
+            fs = {"x": -cs * lap_phi * phx, "y": -cs * lap_phi * phy, "z": -cs * lap_phi * phz}
+            out["F"] = {k: out["F"][k] + fs[k] for k in fs} if "F" in out else fs
         out["Q"] = u * phx + v * phy + w * phz
         out["C"] = phi * phi * phi
         if p.visc_ratio != 1.0:
@@ -447,20 +458,24 @@ class Oracle:
                          self._Dz(uP) + 1j * self.KX * wP,
                          self._Dz(vP) + 1j * self.KY * wP]
         phys = [backward_transform(a, g) for a in spec]
+        vort = None
+        if p.convection_form == 1:   # vorticity of the truncated velocity, in spectral space, then to physical space
+            vs = [1j * self.KY * wP - self._Dz(vP), self._Dz(uP) - 1j * self.KX * wP, 1j * self.KX * vP - 1j * self.KY * uP]
+            vort = [backward_transform(a, g) for a in vs]
         if p.phase_field:
             strain = phys[7:12] if p.visc_ratio != 1.0 else None
             lap_phys = backward_transform(lap_spec, g) if p.surface_tension_form == 1 else None
-            pw = pointwise_terms(p, phys[0], phys[1], phys[2], phys[3], phys[4], phys[5], phys[6], strain, lap_phys)
+            pw = pointwise_terms(p, phys[0], phys[1], phys[2], phys[3], phys[4], phys[5], phys[6], strain, lap_phys, vort)
         else:
-            pw = pointwise_terms(p, phys[0], phys[1], phys[2])
+            pw = pointwise_terms(p, phys[0], phys[1], phys[2], vort=vort)
         out = {k: np.where(P, forward_transform(t, g), 0.0) for k, t in pw["T"].items()}
         if p.phase_field:
             out["Q"] = np.where(P, forward_transform(pw["Q"], g), 0.0)
             out["C"] = np.where(P, forward_transform(pw["C"], g), 0.0)
             out["phP"] = phP
-            if "F" in pw:
-                for k, t in pw["F"].items():
-                    out["F" + k] = np.where(P, forward_transform(t, g), 0.0)
+        if "F" in pw:
+            for k, t in pw["F"].items():
+                out["F" + k] = np.where(P, forward_transform(t, g), 0.0)
         return out
 
     def explicit_terms(self):

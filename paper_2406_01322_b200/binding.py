@@ -35,7 +35,7 @@ class psdns_params(C.Structure):
     _fields_ = [("re", C.c_double), ("pe", C.c_double), ("ch", C.c_double), ("we", C.c_double),
                 ("dt", C.c_double), ("gradp_x", C.c_double), ("visc_ratio", C.c_double),
                 ("phase_field", C.c_int), ("dealias", C.c_int), ("wall_top", C.c_int), ("wall_bottom", C.c_int),
-                ("surface_tension_form", C.c_int)]
+                ("surface_tension_form", C.c_int), ("convection_form", C.c_int)]
 
 
 def lib_path() -> str:
@@ -117,7 +117,7 @@ class Solver:
 
     def __init__(self, nx, ny, nz, lx, ly, *, re, dt, pe=1.0, ch=1.0, we=1.0, gradp_x=0.0,
                  visc_ratio=1.0, phase_field=1, dealias=1, device="cuda:0", unfused_workspace=False,
-                 wall_top=0, wall_bottom=0, surface_tension_form=0):
+                 wall_top=0, wall_bottom=0, surface_tension_form=0, convection_form=0):
         import torch
         self.torch = torch
         self.lib = load_library()
@@ -126,7 +126,7 @@ class Solver:
         self.device = torch.device(device)
         self.grid = psdns_grid(nx, ny, nz, lx, ly)
         self.params = psdns_params(re, pe, ch, we, dt, gradp_x, visc_ratio, phase_field, dealias, wall_top, wall_bottom,
-                                   surface_tension_form)
+                                   surface_tension_form, convection_form)
         self.nx, self.ny, self.nz = nx, ny, nz
         self.phase = bool(phase_field)
         wsfn = self.lib.psdns_workspace_bytes_unfused if unfused_workspace else self.lib.psdns_workspace_bytes

@@ -135,6 +135,8 @@ struct PrepArgs {
     int do_phz, visc;
     cplx *lap;       // do_lap: (D^2 - k^2) of the truncated phi^ (force form of the surface tension)
     int do_lap;
+    cplx *wx, *wy, *wz;   // do_vort: vorticity of the truncated velocity (rotational form of convection)
+    int do_vort;
 };
 
 __global__ void __launch_bounds__(NT_COL) k_prep(const __grid_constant__ PrepArgs a) {
@@ -156,6 +158,16 @@ __global__ void __launch_bounds__(NT_COL) k_prep(const __grid_constant__ PrepArg
         if (a.do_lap) {
             const cplx pn = a.phi[o];
             a.lap[o] = cfma(-k2, pn, cL.step(pn, f, h));
+        }
+        if (a.do_vort) {   // omega = curl u: (i ky w - D v, D u - i kx w, i kx v - i ky u); column (0,0) included (omega_z = 0 there)
+            const cplx un = a.u[o], vn = a.v[o], wn = a.w[o];
+            const cplx dun = cscale(cfma(f, u1, du2), h);
+            const cplx dvn = cscale(cfma(f, v1, dv2), h);
+            a.wx[o] = csub(cscale(ci(wn), ky), dvn);
+            a.wy[o] = csub(dun, cscale(ci(wn), kx));
+            a.wz[o] = csub(cscale(ci(vn), kx), cscale(ci(un), ky));
+            u1 = un; du2 = du1; du1 = dun;
+            v1 = vn; dv2 = dv1; dv1 = dvn;
         }
         if (a.do_phz) {
             const cplx pn = a.phi[o];

@@ -339,7 +339,9 @@ struct PwArgs {
     double cs;        // 3/sqrt(8) Ch/We
     double eta_c;     // (lambda - 1) / (2 Re)
     int phase, visc;
-    int force;        // surface tension as the force -cs lap(phi) grad(phi) (b[7] = lap phi, o[7..9] = F) instead of the Korteweg tensor
+    int force;        // a force vector F = o[7..9] next to the flux tensor (alternative non-linear forms):
+    int st_force;     //   surface tension as -cs lap(phi) grad(phi) (b[7] = lap phi) instead of the Korteweg tensor
+    int rot;          //   convection as u x omega (b[8..10] = omega) instead of -div(u u)
 };
 
 __global__ void __launch_bounds__(256) k_pointwise(const __grid_constant__ PwArgs a) {
@@ -348,12 +350,18 @@ __global__ void __launch_bounds__(256) k_pointwise(const __grid_constant__ PwArg
         const double u = a.b[0][i], v = a.b[1][i], w = a.b[2][i];
         double dxx = w * w - u * u, dyy = w * w - v * v, txy = -u * v, txz = -u * w, tyz = -v * w;
         double q = 0.0, c3 = 0.0;
+        double fx = 0.0, fy = 0.0, fz = 0.0;
+        if (a.rot) {
+            const double ox = a.b[8][i], oy = a.b[9][i], oz = a.b[10][i];
+            dxx = dyy = txy = txz = tyz = 0.0;
+            fx = v * oz - w * oy; fy = w * ox - u * oz; fz = u * oy - v * ox;
+        }
         if (a.phase) {
             const double ph = a.b[3][i], px = a.b[4][i], py = a.b[5][i], pz = a.b[6][i];
             const double cs = a.cs;
-            if (a.force) {
+            if (a.st_force) {
                 const double m = -cs * a.b[7][i];
-                a.o[7][i] = m * px; a.o[8][i] = m * py; a.o[9][i] = m * pz;
+                fx += m * px; fy += m * py; fz += m * pz;
             } else {
                 dxx += cs * (pz * pz - px * px);
                 dyy += cs * (pz * pz - py * py);
@@ -374,7 +382,8 @@ __global__ void __launch_bounds__(256) k_pointwise(const __grid_constant__ PwArg
             c3 = ph * ph * ph;
         }
         a.o[0][i] = dxx; a.o[1][i] = txy; a.o[2][i] = txz; a.o[3][i] = dyy; a.o[4][i] = tyz;
-        if (a.phase) { a.o[5][i] = q; a.o[6][i] = c3; }
+        if (a.phase || a.force) { a.o[5][i] = q; a.o[6][i] = c3; }
+        if (a.force) { a.o[7][i] = fx; a.o[8][i] = fy; a.o[9][i] = fz; }
     }
 }
 

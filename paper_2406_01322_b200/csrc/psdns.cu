@@ -125,6 +125,8 @@ bool validate(const psdns_grid *g, const psdns_params *p) {
     if (p->phase_field != 0 && p->phase_field != 1) return false;
     if (p->surface_tension_form != 0 && p->surface_tension_form != 1) return false;
     if (p->surface_tension_form == 1 && (!p->phase_field || p->visc_ratio != 1.0)) return false;   // force form: matched viscosity only
+    if (p->convection_form != 0 && p->convection_form != 1) return false;
+    if (p->convection_form == 1 && p->phase_field && p->visc_ratio != 1.0) return false;
     if ((p->wall_top != 0 && p->wall_top != 1) || (p->wall_bottom != 0 && p->wall_bottom != 1)) return false;
     if (p->phase_field && (!(p->pe > 0) || !(p->ch > 0) || !(p->we > 0) || !(p->visc_ratio > 0))) return false;
     return true;
@@ -172,11 +174,11 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.xom = take(d.s_ret * C);
     const bool visc_l = p.phase_field && p.visc_ratio != 1.0;
     for (int i = 0; i < 8; ++i) L.derived[i] = 0;
-    const bool force_l = p.phase_field && p.surface_tension_form == 1;
-    for (int i = 0; i < (visc_l ? 6 : (force_l ? 2 : 1)); ++i) L.derived[i] = take(d.s_low * C);   // phz [+ 5 strains | + lap phi]
+    const bool force_l = (p.phase_field && p.surface_tension_form == 1) || p.convection_form == 1;   // a force vector next to T
+    for (int i = 0; i < (visc_l ? 6 : (force_l ? 5 : 1)); ++i) L.derived[i] = take(d.s_low * C);   // phz [+ 5 strains | + lap phi, 3 vorticity]
     for (int i = 0; i < 10; ++i) L.prod[i] = 0;
     for (int i = 0; i < (force_l ? 10 : 7); ++i) L.prod[i] = take(d.s_low * C);
-    const int nf = visc_l ? 12 : (force_l ? 10 : 7);
+    const int nf = (visc_l || force_l) ? 12 : 7;
     // Z / Y arrays double as the full-size round-trip scratch (3 arrays of s_full each)
     size_t zy_bytes = 0;
     for (int i = 0; i < MAXF; ++i) { L.zb[i] = 0; L.yb[i] = 0; L.ph[i] = 0; }
@@ -568,7 +570,9 @@ cudaError_t enqueue_step(psdns_handle *h) {
     const Coefs c = coefs(p);
     const bool phase = p.phase_field != 0;
     const bool visc = phase && p.visc_ratio != 1.0;
-    const bool force = phase && p.surface_tension_form == 1;
+    const bool st_force = phase && p.surface_tension_form == 1;   // surface tension as a force vector
+    const bool rot = p.convection_form == 1;                     // convection as u x omega
+    const bool force = st_force || rot;                          // a force vector F next to the flux tensor (row f4)
     const int nout = h->nf_out;
     cplx *U = h->at<cplx>(L.state[0]), *V = h->at<cplx>(L.state[1]), *W = h->at<cplx>(L.state[2]);
     cplx *PHI = h->at<cplx>(L.state[3]), *TH = h->at<cplx>(L.state[4]), *OM = h->at<cplx>(L.xom);
@@ -588,10 +592,11 @@ cudaError_t enqueue_step(psdns_handle *h) {
         k_prep<<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
-    if (force) {   // row a1, force form: lap(phi)^ = (D^2 - k^2) P phi^, the 8th backward field
+    if (force) {   // row a1, alternative forms: lap(phi)^ = (D^2 - k^2) P phi^ and / or the vorticity spectra of P u^
         PrepArgs a{};
-        a.g = geom(h); a.phi = PHI; a.lap = h->at<cplx>(L.derived[1]);
-        a.do_phz = 0; a.visc = 0; a.do_lap = 1;
+        a.g = geom(h); a.u = U; a.v = V; a.w = W; a.phi = PHI; a.lap = h->at<cplx>(L.derived[1]);
+        a.wx = h->at<cplx>(L.derived[2]); a.wy = h->at<cplx>(L.derived[3]); a.wz = h->at<cplx>(L.derived[4]);
+        a.do_lap = st_force; a.do_vort = rot;
         LaunchScope ls(h, KC_RHS);
         k_prep<<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
@@ -601,6 +606,10 @@ cudaError_t enqueue_step(psdns_handle *h) {
     ZDerived zd;
     int nz_f = 3, ny_f = 3;   // fields through the z pass / the y pass
     const cplx *src[MAXF] = {U, V, W, PHI, PHZ};
+    if (!phase && rot) {   // single-phase, rotational form: u v w wx wy wz
+        for (int i = 0; i < 3; ++i) src[3 + i] = h->at<cplx>(L.derived[2 + i]);
+        nz_f = 6; ny_f = 6;
+    }
     if (phase) {
         nz_f = 5;
         if (visc) {
@@ -613,11 +622,12 @@ cudaError_t enqueue_step(psdns_handle *h) {
                 zd.dfield = 3; zd.out_dx = h->at<cplx>(L.zb[10]); zd.out_dy = h->at<cplx>(L.zb[11]);
                 ny_f = 12;
             }
-        } else if (force) {   // Z arrays: u v w phi phz lap | i ky phi | i kx phi
-            src[5] = h->at<cplx>(L.derived[1]);
-            nz_f = 6;
-            zd.dfield = 3; zd.out_dy = h->at<cplx>(L.zb[6]); zd.out_dx = h->at<cplx>(L.zb[7]);
-            ny_f = 8;
+        } else if (force) {   // Z arrays: u v w phi phz [lap] [wx wy wz] | i ky phi | i kx phi
+            nz_f = 5;
+            if (st_force) src[nz_f++] = h->at<cplx>(L.derived[1]);
+            if (rot) for (int i = 0; i < 3; ++i) src[nz_f++] = h->at<cplx>(L.derived[2 + i]);
+            zd.dfield = 3; zd.out_dy = h->at<cplx>(L.zb[nz_f]); zd.out_dx = h->at<cplx>(L.zb[nz_f + 1]);
+            ny_f = nz_f + 2;
         } else {
             const bool fused = h->use_xfused;
             zd.dfield = 3; zd.out_dx = fused ? nullptr : h->at<cplx>(L.zb[6]); zd.out_dy = h->at<cplx>(L.zb[5]);
@@ -663,12 +673,23 @@ cudaError_t enqueue_step(psdns_handle *h) {
             //                                                            (matched viscosity: 0 1 2 3 6 5 4)
             const int order_v[MAXF] = {0, 1, 2, 3, 10, 11, 4, 5, 6, 7, 8, 9};
             const int order_m[MAXF] = {0, 1, 2, 3, 6, 5, 4, 0, 0, 0, 0, 0};
-            const int order_f[MAXF] = {0, 1, 2, 3, 7, 6, 4, 5, 0, 0, 0, 0};   // force form: .. phx phy phz lap
+            // alternative forms: u v w phi phx phy phz lap wx wy wz  <-  Z/Y/physical buffers as laid out above
+            int order_f[MAXF] = {0, 1, 2, 3, 0, 0, 4, 0, 0, 0, 0, 0};
+            if (force) {
+                if (phase) {
+                    int nb = 5;
+                    if (st_force) order_f[7] = nb++;
+                    if (rot) for (int i = 0; i < 3; ++i) order_f[8 + i] = nb++;
+                    order_f[5] = nb; order_f[4] = nb + 1;       // i ky phi, i kx phi
+                } else {
+                    for (int i = 0; i < 3; ++i) order_f[8 + i] = 3 + i;
+                }
+            }
             for (int i = 0; i < MAXF; ++i)
-                a.b[i] = h->at<double>(L.ph[phase ? (visc ? order_v[i] : (force ? order_f[i] : order_m[i])) : (i < 3 ? i : 0)]);
+                a.b[i] = h->at<double>(L.ph[force ? order_f[i] : (phase ? (visc ? order_v[i] : order_m[i]) : (i < 3 ? i : 0))]);
             for (int i = 0; i < 10; ++i) a.o[i] = h->at<double>(L.ph[i < nout ? i : 0]);
             a.n = d.s_p; a.cs = c.cs; a.eta_c = (p.visc_ratio - 1.0) / (2.0 * p.re);
-            a.phase = phase; a.visc = visc; a.force = force;
+            a.phase = phase; a.visc = visc; a.force = force; a.st_force = st_force; a.rot = rot;
             LaunchScope ls(h, KC_PW);
             k_pointwise<<<h->n_sm * 8, 256, 0, h->st>>>(a);
             CU(cudaGetLastError());
@@ -933,9 +954,9 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->launches = 0; h->per_step = 0; h->timed_class = -1;
     const bool phase = params->phase_field != 0;
     const bool visc = phase && params->visc_ratio != 1.0;
-    const bool force = phase && params->surface_tension_form == 1;
-    h->nf_in = phase ? (visc ? 12 : (force ? 8 : 7)) : 3;
-    h->nf_out = phase ? (force ? 10 : 7) : 5;
+    const bool force = (phase && params->surface_tension_form == 1) || params->convection_form == 1;
+    h->nf_in = phase ? (visc ? 12 : (force ? 11 : 7)) : (force ? 6 : 3);
+    h->nf_out = phase ? (force ? 10 : 7) : (force ? 10 : 5);
     if (force) h->use_xfused = false;   // three-kernel x path (k_xpass, k_pointwise, k_xpass): 10 forward fields exceed the fused tile
     h->xf_occ = 1; h->xfv_occ = 1; h->n_sm = 148;
     h->occ_z[0] = h->occ_z[1] = h->occ_y[0] = h->occ_y[1] = 1;
@@ -1320,8 +1341,8 @@ int psdns_set_option(psdns_handle *h, const char *name, double value) {
     const std::string n(name);
     const int iv = (int)value;
     if (n == "graph") h->use_graph = iv != 0;
-    else if (n == "xfuse" && iv && h->p.phase_field && h->p.surface_tension_form == 1) {
-        h->err = "psdns_set_option: the force form of the surface tension has no fused x kernel";
+    else if (n == "xfuse" && iv && ((h->p.phase_field && h->p.surface_tension_form == 1) || h->p.convection_form == 1)) {
+        h->err = "psdns_set_option: the alternative non-linear forms have no fused x kernel";
         return PSDNS_EINVAL;
     }
     else if (n == "xfuse") {

@@ -13,10 +13,11 @@ TOL = 1e-9
 
 def run(c, nsteps, **over):
     import paper_2406_01322_b200 as P
-    st = I.channel_state(c)
-    orc, g = oracle_from_config(c, surface_tension_form=1, **over)
+    st = [f for f in I.channel_state(c) if f is not None]
+    over.setdefault("surface_tension_form", 1)
+    orc, g = oracle_from_config(c, **over)
     orc.set_state("physical", *st)
-    s = solver_from_config(c, surface_tension_form=1, **over)
+    s = solver_from_config(c, **over)
     s.set_state(P.PHYSICAL, *[to_dev(f) for f in st])
     done = 0
     for n in nsteps:
@@ -58,13 +59,26 @@ def test_force_form_differs_from_the_tensor_form_and_config2_grid():
     assert 1e-13 < d < 1e-3, d
 
 
+@pytest.mark.parametrize("st_form,phase", [(0, 1), (1, 1), (0, 0)])
+def test_rotational_form_of_convection(st_form, phase):
+    """convection_form = 1 (u x omega; vorticity spectra from k_prep, three more backward fields), alone, together with the
+    force form of the surface tension (then the flux tensor is empty), and single-phase; ragged grid and mixed walls too."""
+    for (nx, ny, nz, kw) in [(32, 32, 33, {}), (16, 64, 17, {}), (64, 16, 65, dict(wall_top=1))]:
+        c = I.small_config(nx=nx, ny=ny, nz=nz, phase_field=phase)
+        s, _ = run(c, [1, 3], convection_form=1, surface_tension_form=st_form, **kw)
+        s.close()
+
+
 def test_force_form_rejects_unsupported_combinations():
     import paper_2406_01322_b200 as P
     with pytest.raises(P.PsdnsError):
         P.Solver(16, 16, 17, 1.0, 1.0, re=10.0, dt=1e-3, phase_field=0, surface_tension_form=1)
     with pytest.raises(P.PsdnsError):
         P.Solver(16, 16, 17, 1.0, 1.0, re=10.0, dt=1e-3, pe=1.0, ch=0.2, we=1.0, visc_ratio=0.5, surface_tension_form=1)
-    s = P.Solver(16, 16, 17, 1.0, 1.0, re=10.0, dt=1e-3, pe=1.0, ch=0.2, we=1.0, surface_tension_form=1)
     with pytest.raises(P.PsdnsError):
-        s.set_option("xfuse", 1)
-    s.close()
+        P.Solver(16, 16, 17, 1.0, 1.0, re=10.0, dt=1e-3, pe=1.0, ch=0.2, we=1.0, visc_ratio=0.5, convection_form=1)
+    for kw in (dict(surface_tension_form=1), dict(convection_form=1)):
+        s = P.Solver(16, 16, 17, 1.0, 1.0, re=10.0, dt=1e-3, pe=1.0, ch=0.2, we=1.0, **kw)
+        with pytest.raises(P.PsdnsError):
+            s.set_option("xfuse", 1)
+        s.close()

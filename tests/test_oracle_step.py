@@ -218,12 +218,14 @@ def test_non_equilibrium_profile_relaxes_towards_tanh():
     assert d1 < d0
 
 
-@pytest.mark.parametrize("form", [0, 1])
-def test_explicit_terms_match_symbolic_continuous_formulas(form):
-    """form 0: Korteweg tensor (Eq. 8 as written); form 1: the force -c_sigma lap(phi) grad(phi)."""
+@pytest.mark.parametrize("form,conv", [(0, 0), (1, 0), (0, 1), (1, 1)])
+def test_explicit_terms_match_symbolic_continuous_formulas(form, conv):
+    """form 0: Korteweg tensor (Eq. 8 as written); form 1: the force -c_sigma lap(phi) grad(phi); conv 0: -div(u u) (S4);
+    conv 1: the rotational form u x omega - each against ITS OWN continuous expression."""
     import sympy as sp
     g = O.Grid(16, 16, 65)
-    p = O.Params(re=80.0, dt=1e-3, pe=3.0, ch=0.3, we=1.3, gradp_x=0.04, visc_ratio=0.3, surface_tension_form=form)
+    p = O.Params(re=80.0, dt=1e-3, pe=3.0, ch=0.3, we=1.3, gradp_x=0.04, visc_ratio=0.3, surface_tension_form=form,
+                 convection_form=conv)
     x, y, z = sp.symbols("x y z", real=True)
     kx, ky = sp.Rational(1, 2), 1                         # fundamental wavenumbers of 4pi x 2pi
     q = 1 - z ** 2
@@ -244,11 +246,13 @@ def test_explicit_terms_match_symbolic_continuous_formulas(form):
     T = sp.zeros(3, 3)
     for a in range(3):
         for b in range(3):
-            T[a, b] = (-U[a] * U[b] + (cs * ((gp.dot(gp) if a == b else 0) - gp[a] * gp[b]) if form == 0 else 0)
+            T[a, b] = ((-U[a] * U[b] if conv == 0 else 0) + (cs * ((gp.dot(gp) if a == b else 0) - gp[a] * gp[b]) if form == 0 else 0)
                        + eta1 * (sp.diff(U[b], X[a]) + sp.diff(U[a], X[b])))
     S = sp.Matrix([sum(sp.diff(T[a, b], X[b]) for b in range(3)) for a in range(3)])
     if form == 1:
         S = S - cs * lap(phi) * gp
+    if conv == 1:
+        S = S + U.cross(curl(U))
     S[0] = S[0] + sp.Float(p.gradp_x)
     divS = sum(sp.diff(S[a], X[a]) for a in range(3))
     N_om = curl(S)[2]                                              # Eq. 14
@@ -365,3 +369,20 @@ def test_surface_tension_forms_differ_by_a_gradient_only():
     assert np.array_equal(out[0]["phi"], out[1]["phi"])
     # the mean-flow forcing S-bar_x differs by d/dx of a mean: nothing
     assert np.abs(out[0]["ubar"] - out[1]["ubar"]).max() < 1e-12
+
+
+def test_convection_forms_differ_by_a_gradient_only():
+    """Divergence form -div(u u) and rotational form u x omega differ by grad(|u|^2 / 2) for a solenoidal field: N_omega,
+    N_w and the mean-flow forcing agree to truncation error on a resolved solenoidal state, not to rounding."""
+    c = I.small_config(nx=16, ny=16, nz=49, band=2, phase_field=0)
+    g = O.Grid(c.nx, c.ny, c.nz, c.lx, c.ly)
+    st = I.channel_state(c)[:3]
+    out = []
+    for conv in (0, 1):
+        orc = O.Oracle(g, O.Params(re=c.re, dt=c.dt, gradp_x=c.gradp_x, phase_field=0, convection_form=conv))
+        orc.set_state("physical", *st)
+        out.append(orc.explicit_terms())
+    for key in ("om", "w"):
+        d = O.rel_l2(out[1][key], out[0][key])
+        assert 1e-16 < d < 1e-8, (key, d)
+    assert np.abs(out[0]["ubar"] - out[1]["ubar"]).max() < 1e-10 * np.abs(out[0]["ubar"]).max() + 1e-13
