@@ -482,7 +482,7 @@ def run_ours(args):
         rt_ms = r0.elapsed_time(r1) / rsteps
         del rt, xin
         # each of the 3 + 3 one-dimensional passes reads and writes its array once (x: R <-> S_full, y and z: S_full <->
-        # S_full), and the boundary-layout copy on either side of the spectrum moves S_full twice more
+        # S_full); the spectrum stays in the private layout between the two transforms (no d_mid requested)
         passes = 2 * R + 10 * S_full
         roundtrip = {"ms": rt_ms, "rel_l2_identity_error": rt_err, "fields": 1, "dealias": 0,
                      "alg_bytes_min": 2 * (R + S_full), "gbs_min": 2 * (R + S_full) / (rt_ms * 1e-3) / 1e9,

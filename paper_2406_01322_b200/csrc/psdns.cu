@@ -1102,11 +1102,12 @@ int psdns_transform_roundtrip(psdns_handle *h, int start_space, const void *d_in
         CUDA_TRY(h, launch_ypass(h, true, f, 1, d.kxpf, d.ny, d.ny));
         f.in[0] = B; f.out[0] = C;
         CUDA_TRY(h, launch_zpass(h, true, f, 1, ncols_f, d.nz, d.kxpf, d.ny, d.ny));
-        CUDA_TRY(h, launch_relayout(h, spec_boundary, C, side_boundary(d), side_full(d), d.nz));
+        // the boundary-layout copy of the spectrum is only made when somebody looks at it (d_mid / spectral output)
+        if (spec_boundary) CUDA_TRY(h, launch_relayout(h, spec_boundary, C, side_boundary(d), side_full(d), d.nz));
         return PSDNS_OK;
     };
     auto backward = [&](const cplx *spec_boundary, double *phys) -> int {
-        CUDA_TRY(h, launch_relayout(h, C, spec_boundary, side_full(d), side_boundary(d), d.nz));
+        if (spec_boundary) CUDA_TRY(h, launch_relayout(h, C, spec_boundary, side_full(d), side_boundary(d), d.nz));
         FieldPtrs f{};
         f.in[0] = C; f.out[0] = B;
         CUDA_TRY(h, launch_zpass(h, false, f, 1, ncols_f, d.nz, d.kxpf, d.ny, d.ny));
@@ -1118,7 +1119,8 @@ int psdns_transform_roundtrip(psdns_handle *h, int start_space, const void *d_in
     };
     int rc;
     if (start_space == PSDNS_PHYSICAL) {
-        cplx *mid = d_mid ? (cplx *)d_mid : h->at<cplx>(L.stage[0]);
+        // without d_mid the spectrum stays in the private layout between the two transforms (same values, two copies less)
+        cplx *mid = (cplx *)d_mid;
         if ((rc = forward((const double *)d_in, mid)) != PSDNS_OK) return rc;
         if ((rc = backward(mid, (double *)d_out)) != PSDNS_OK) return rc;
     } else {

@@ -25,6 +25,8 @@ def test_roundtrip_from_physical(nx, ny, nz):
     g = O.Grid(nx, ny, nz)
     f = I.random_physical_field(nx, ny, nz, seed=nx + ny + nz)
     out, mid = s.transform_roundtrip(P.PHYSICAL, to_dev(f), want_mid=True)
+    import torch
+    assert torch.equal(out, s.transform_roundtrip(P.PHYSICAL, to_dev(f)))   # without d_mid: private layout in between, same bits
     out, mid = to_np(out), to_np(mid)
     ref_mid = O.forward_transform(f, g)
     assert O.rel_l2(mid, ref_mid) < TOL          # forward transform, element by element
