@@ -503,6 +503,19 @@ def run_ours(args):
                     "frac": k["frac"], "traffic": traffic.get(dominant), "traffic_unit": "bytes per launch (ncu dram read + write)",
                     "alg_bytes_per_launch": k["alg_bytes_per_step"] / max(k["launches_per_step"], 1), "peak_source": peak_src,
                     "launch_ms": k["ms_per_step"] / max(k["launches_per_step"], 1)}
+        # second view of the dominant kernel when it is the fused x kernel: it is FP64-issue bound as much as HBM bound
+        # (ncu: FP64 pipe 56 %, DRAM 28 %).  Algorithmic flops: 2.5 N_x log2 N_x per real line and transform,
+        # 45 per grid point for the products; peak = 148 SMs x 64 FP64 FMA/clk x 2 x max SM clock.
+        roof_alu = None
+        if dominant == "xfused":
+            lines = c.ny * c.nz
+            flops = lines * ((cnt["nin"] + (7 if c.phase_field else 5)) * 2.5 * c.nx * math.log2(c.nx) + 45.0 * c.nx)
+            sm_clock = float((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6
+            peak_tf = 148 * 64 * 2 * sm_clock / 1e12
+            tf = flops / (kernels["xfused"]["ms_per_step"] * 1e-3) / 1e12
+            roof_alu = {"bound": "alu", "kernel": "xfused", "achieved": tf, "peak": peak_tf, "unit": "TFLOP/s (FP64)",
+                        "frac": tf / peak_tf, "alg_flops_per_launch": flops,
+                        "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x max SM clock (B200 guide unit counts)"}
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             sec, desc, threads, parts = oracle_sampled_step_seconds(c)
@@ -522,6 +535,7 @@ def run_ours(args):
                     "call": "psdns_run_host x steps, then psdns_run_host_wait (copy-back of one call overlaps the next call)"},
             "gpu_launches": launches,
             "roofline": roof,
+            "roofline_alu": roof_alu,
             "step_roofline": {"alg_bytes_per_step_fused_design": step_fused_bytes,
                               "alg_bytes_per_grid_point": step_fused_bytes / M,
                               "achieved_gbs": step_fused_bytes / (ms_max / args.steps * 1e-3) / 1e9,
