@@ -445,7 +445,7 @@ def run_ours(args):
     # consecutive calls on one handle: the device -> host copy of call k (side stream) overlaps the upload and the compute
     # of call k + 1; the timed region ends when the LAST copy-back has landed (run_host_wait), so every step's H2D and D2H
     # are inside it.  g1 is recorded after the host has seen that completion.
-    esteps = max(1, min(args.steps, 5))
+    esteps = max(1, min(args.steps, 10))
     g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     g0.record()
     for _ in range(esteps):

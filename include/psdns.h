@@ -131,14 +131,14 @@ int psdns_set_history(psdns_handle *h, const void *d_blob, size_t bytes);
 int psdns_transform_roundtrip(psdns_handle *h, int start_space, const void *d_in, void *d_out,
                               void *d_mid);
 
-/* Host-buffer form of set_state -> step -> get_state, used for the end-to-end number: copies the four fields host ->
- * device (cudaMemcpyAsync on the stream), set_state, nsteps steps, get_state into output staging buffers, then copies
- * those device -> host on a SIDE stream owned by the handle, so that the copy-back of one call overlaps the upload and
- * the compute of the next call on the same handle (PCIe is full duplex; the copies are 92 % of such a call).
+/* Host-buffer form of set_state -> step -> get_state, used for the end-to-end number.  The four fields are copied host ->
+ * device on a side stream of the handle into one of two input staging sets, then set_state, nsteps steps and get_state
+ * (into output staging buffers) run on the init stream, and the result is copied device -> host on a second side stream.
+ * Consecutive calls on one handle therefore pipeline: the upload of call k + 1 and the copy-back of call k - 1 overlap the
+ * compute of call k (PCIe is full duplex; the copies are 90 % of such a call).
  * h_in_* / h_out_* are HOST pointers (pinned, for the copies to be asynchronous) in the boundary layout of `space` (the
- * phi pair may be NULL iff phase_field == 0).  h_out_* are valid after psdns_run_host_wait(h) has returned - synchronising
- * the init stream alone does NOT cover the side stream.  A later psdns_run_host waits by itself for the previous
- * copy-back before it reuses the staging buffers; h_in_* may be reused as soon as the init stream has passed the upload. */
+ * phi pair may be NULL iff phase_field == 0).  h_out_* are valid, and h_in_* may be modified again, after
+ * psdns_run_host_wait(h) has returned - synchronising the init stream alone does NOT cover the side streams. */
 int psdns_run_host(psdns_handle *h, int space, int nsteps, const void *h_in_u, const void *h_in_v,
                    const void *h_in_w, const void *h_in_phi, void *h_out_u, void *h_out_v,
                    void *h_out_w, void *h_out_phi);

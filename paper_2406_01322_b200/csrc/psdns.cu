@@ -67,6 +67,7 @@ struct Layout {
     size_t zb[MAXF], yb[MAXF], ph[MAXF];
     size_t small;                      // ab[2] doubles + counter
     size_t stage[4];                   // host-staging device buffers (boundary layout): inputs of psdns_run_host
+    size_t stage_b[4];                 // second set of input staging buffers: the upload of call k + 1 overlaps the compute of call k
     size_t stage_out[4];               // outputs of psdns_run_host (copied back on the side stream while the next call runs)
     size_t total, total_unfused;
 };
@@ -91,8 +92,10 @@ struct psdns_handle {
     int nf_in, nf_out;
     bool use_xfused, has_unfused_ws;
     cudaStream_t copy_st;        // side stream of psdns_run_host's device -> host copies
-    cudaEvent_t ev_out_ready, ev_d2h_done;
-    bool d2h_pending;
+    cudaStream_t copy_in_st;     // side stream of its host -> device copies
+    cudaEvent_t ev_out_ready, ev_d2h_done, ev_in_ready, ev_in_free[2];
+    bool d2h_pending, in_used[2];
+    long long host_calls;
     int xf_occ, xfv_occ, n_sm;
     int occ_z[2], occ_y[2];     // resident CTAs per SM of the persistent z / y passes, [fwd]
     int use_zgemm;              // psdns_set_option("zgemm"): GEMM-form Chebyshev on the FP64 tensor cores for N <= 64
@@ -189,6 +192,7 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.small = take(64);
     const size_t stage_bytes = std::max(d.s_p * sizeof(double), d.s_bspec * C);
     for (int i = 0; i < 4; ++i) L.stage[i] = take(stage_bytes);
+    for (int i = 0; i < 4; ++i) L.stage_b[i] = take(stage_bytes);
     for (int i = 0; i < 4; ++i) L.stage_out[i] = take(stage_bytes);
     // the force form of the surface tension runs the three-kernel x path: its physical arrays are product state
     if (force_l) for (int i = 0; i < nf; ++i) L.ph[i] = take(d.s_p * sizeof(double));
@@ -937,7 +941,8 @@ int psdns_init(const psdns_grid *grid, const psdns_params *params, void *d_works
     h->has_state = false; h->graph = nullptr; h->graph_ready = false;
     h->use_graph = true;
     h->use_xfused = true;
-    h->copy_st = nullptr; h->ev_out_ready = nullptr; h->ev_d2h_done = nullptr; h->d2h_pending = false;
+    h->copy_st = nullptr; h->copy_in_st = nullptr; h->ev_out_ready = nullptr; h->ev_d2h_done = nullptr; h->d2h_pending = false;
+    h->ev_in_ready = nullptr; h->ev_in_free[0] = h->ev_in_free[1] = nullptr; h->in_used[0] = h->in_used[1] = false; h->host_calls = 0;
     h->grid_cap = 0; h->pf = 2; h->pf_rhs = 4;
     h->use_ztma = 1; h->encode_tiled = nullptr; h->use_zgemm = 0;
     for (int i = 0; i < 4; ++i) (&h->occ_zt[0][0])[i] = 1;
@@ -1200,15 +1205,26 @@ int psdns_run_host(psdns_handle *h, int space, int nsteps, const void *h_in_u, c
     void *dev[4];
     const int nf = phase ? 4 : 3;
     void *dout[4];
-    for (int i = 0; i < 4; ++i) { dev[i] = h->ws + h->L.stage[i]; dout[i] = h->ws + h->L.stage_out[i]; }
-    if (!h->copy_st) {   // side stream and events of the device -> host leg, created on first use
+    const int b = (int)(h->host_calls++ & 1);      // input staging set of this call
+    for (int i = 0; i < 4; ++i) { dev[i] = h->ws + (b ? h->L.stage_b[i] : h->L.stage[i]); dout[i] = h->ws + h->L.stage_out[i]; }
+    if (!h->copy_st) {   // side streams and events of the two copy legs, created on first use
         CUDA_TRY(h, cudaStreamCreateWithFlags(&h->copy_st, cudaStreamNonBlocking));
+        CUDA_TRY(h, cudaStreamCreateWithFlags(&h->copy_in_st, cudaStreamNonBlocking));
         CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_out_ready, cudaEventDisableTiming));
         CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_d2h_done, cudaEventDisableTiming));
+        CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_in_ready, cudaEventDisableTiming));
+        for (int i = 0; i < 2; ++i) CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_in_free[i], cudaEventDisableTiming));
     }
-    for (int i = 0; i < nf; ++i) CUDA_TRY(h, cudaMemcpyAsync(dev[i], hin[i], bytes, cudaMemcpyHostToDevice, h->st));
+    // upload on its own stream, into the staging set that the call before the previous one has already consumed: it runs
+    // while the previous call still computes on the init stream
+    if (h->in_used[b]) CUDA_TRY(h, cudaStreamWaitEvent(h->copy_in_st, h->ev_in_free[b], 0));
+    for (int i = 0; i < nf; ++i) CUDA_TRY(h, cudaMemcpyAsync(dev[i], hin[i], bytes, cudaMemcpyHostToDevice, h->copy_in_st));
+    CUDA_TRY(h, cudaEventRecord(h->ev_in_ready, h->copy_in_st));
+    CUDA_TRY(h, cudaStreamWaitEvent(h->st, h->ev_in_ready, 0));
     int rc = psdns_set_state(h, space, dev[0], dev[1], dev[2], phase ? dev[3] : nullptr);
     if (rc != PSDNS_OK) return rc;
+    CUDA_TRY(h, cudaEventRecord(h->ev_in_free[b], h->st));
+    h->in_used[b] = true;
     if ((rc = psdns_step(h, nsteps)) != PSDNS_OK) return rc;
     // the output staging buffers are still being read by the previous call's device -> host copies
     if (h->d2h_pending) CUDA_TRY(h, cudaStreamWaitEvent(h->st, h->ev_d2h_done, 0));
@@ -1378,7 +1394,12 @@ double psdns_get_info(const psdns_handle *h, const char *name) {
 int psdns_destroy(psdns_handle *h) {
     if (!h) return PSDNS_EINVAL;
     if (h->graph) cudaGraphExecDestroy(h->graph);
-    if (h->copy_st) { cudaStreamSynchronize(h->copy_st); cudaStreamDestroy(h->copy_st); cudaEventDestroy(h->ev_out_ready); cudaEventDestroy(h->ev_d2h_done); }
+    if (h->copy_st) {
+        cudaStreamSynchronize(h->copy_in_st); cudaStreamSynchronize(h->copy_st);
+        cudaStreamDestroy(h->copy_in_st); cudaStreamDestroy(h->copy_st);
+        cudaEventDestroy(h->ev_out_ready); cudaEventDestroy(h->ev_d2h_done); cudaEventDestroy(h->ev_in_ready);
+        cudaEventDestroy(h->ev_in_free[0]); cudaEventDestroy(h->ev_in_free[1]);
+    }
     for (auto &pr : h->tevents) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
     delete h;
     return PSDNS_OK;
