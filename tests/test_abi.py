@@ -38,6 +38,6 @@ def test_no_oracle_import_in_product():
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
-                assert "psdns_oracle" not in txt and "import oracle" not in txt, f
+                assert "psdns_oracle" not in txt and "isosurface_oracle" not in txt and "import oracle" not in txt, f
     orc = open(os.path.join(ROOT, "oracle", "psdns_oracle.py")).read()
     assert "paper_2406_01322_b200" not in orc.replace("`paper_2406_01322_b200`", "")
