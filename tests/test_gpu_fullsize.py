@@ -122,3 +122,42 @@ def test_fullsize_step_properties():
         m = torch.conj(torch.roll(torch.flip(p, dims=[1]), shifts=1, dims=1))
         assert float((p - m).abs().max()) < 1e-10 * max(float(p.abs().max()), 1e-300)
     s.close()
+
+
+def test_fullsize_cross_checks_between_kernel_variants():
+    """1024x512x513, two steps of the bench workload's grid, three ways: the product path (fused x kernel, TMA-fed z
+    passes), the three-kernel x path through physical-space arrays (psdns_set_option "xfuse" 0) and the register-fed z
+    passes ("ztma" 0).  Different kernels, different radix plans and summation orders, same discretisation: the states
+    must agree to rounding, field by field, in relative L2 AND in max-abs - garbage from any of the full-size
+    instantiations (k_xfusedw<1024>, k_zpass_tma<512>, k_ypass<512>, the > 60 k-column sweeps) cannot pass all three."""
+    import gc
+    import torch
+    import paper_2406_01322_b200 as P
+    gc.collect()
+    torch.cuda.empty_cache()
+    _skip_if_small_gpu(105 * 2**30)
+    c = I.scaling_config("5c")
+    host = I.random_spectral_state(c.nx, c.ny, c.nz, c.seed, cut=True)
+    dev = [torch.from_numpy(a).cuda() for a in host]
+    del host
+    results = []
+    for opts in ({}, {"xfuse": 0}, {"ztma": 0}):
+        s = P.Solver(c.nx, c.ny, c.nz, c.lx, c.ly, re=c.re, dt=c.dt, pe=c.pe, ch=c.ch, we=c.we, gradp_x=c.gradp_x,
+                     unfused_workspace="xfuse" in opts)
+        for k, v in opts.items():
+            s.set_option(k, v)
+        s.set_state(P.SPECTRAL, *dev)
+        s.step(2)
+        results.append(s.get_state(P.SPECTRAL))
+        s.close()
+        del s
+        torch.cuda.empty_cache()
+    ref = results[0]
+    vnorm = float(torch.sqrt(sum(torch.linalg.vector_norm(t) ** 2 for t in ref[:3])))
+    vmax = max(float(torch.view_as_real(t).abs().max()) for t in ref[:3])
+    for other in results[1:]:
+        for f, (a, b) in enumerate(zip(other, ref)):
+            den_l2 = vnorm if f < 3 else float(torch.linalg.vector_norm(b))
+            den_mx = vmax if f < 3 else float(torch.view_as_real(b).abs().max())
+            assert float(torch.linalg.vector_norm(a - b)) < 1e-11 * den_l2, f
+            assert float(torch.view_as_real(a - b).abs().max()) < 1e-11 * den_mx, f
