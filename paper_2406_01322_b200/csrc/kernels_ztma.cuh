@@ -56,6 +56,64 @@ template <int N> inline size_t ztma_smem_bytes(int srows) {
     return ((size_t)ztma_fixed_cplx<N>() + 2 * (size_t)srows * TILE_LINES) * sizeof(cplx) + 32;
 }
 
+// Last FFT pass fused with the post-processing E_k = Z_k + c_k (Z_k - Z_{N-k}) (round 2; the kernel is bound by the
+// shared-memory pipe, and this removes one tile write, one tile read and one CTA-wide barrier per tile).  The last pass
+// has stride 1 and no twiddles: butterfly b reads tile rows b RL .. b RL + RL - 1 and produces the elements k0 + KS q
+// (q < RL) with k0 = k0(b) < KS.  The partner N - k of element k0 + KS q is element (KS - k0) + KS (RL - 1 - q) of
+// butterfly KS - k0.  Every thread runs ONE butterfly; the butterflies k0 and KS - k0 sit in lanes that differ in bit 3,
+// so the partner value is one warp shuffle away; k0 = 0 and k0 = KS / 2 are their own partners (a register permutation).
+// With c extended by c_{N-k} = conj(c_k), every element is E_k = Z_k + c_k (Z_k - Z_{N-k}), stored straight to global
+// memory.  Used when the plan has one last-pass butterfly per thread and RL <= 8.
+template <class ZP> __host__ __device__ constexpr int zplan_npass() { return ZP::R2 > 1 ? (ZP::R3 > 1 ? 3 : 2) : 1; }
+template <class ZP> __host__ __device__ constexpr int zplan_rl() { return zplan_npass<ZP>() == 3 ? ZP::R3 : ZP::R2; }
+template <int N, class ZP, int NT> __host__ __device__ constexpr bool z_fuse_last() {
+    return zplan_npass<ZP>() >= 2 && zplan_rl<ZP>() <= 8 && (N / zplan_rl<ZP>()) == NT / TILE_LINES && (N / zplan_rl<ZP>()) >= 4;
+}
+
+template <int N, class ZP, bool FWD, int NT, class Emit>
+__device__ __forceinline__ void z_last_pass_fused(const cplx *__restrict__ s, const cplx *__restrict__ ctab,
+                                                  const cplx *__restrict__ red, int tid, int nout, double sc, Emit emit) {
+    constexpr int R1 = ZP::R1, R2 = ZP::R2;
+    constexpr int NPASS = zplan_npass<ZP>();
+    constexpr int RL = zplan_rl<ZP>();
+    constexpr int KS = NPASS == 3 ? R1 * R2 : R1;
+    constexpr int NW = NT / 32;
+    static_assert(KS * RL == N && KS == NT / TILE_LINES, "one last-pass butterfly per thread");
+    const int line = tid & (TILE_LINES - 1);
+    const int i = tid >> 3, p = i >> 1, h = i & 1;
+    const int k0 = p == 0 ? (h ? KS / 2 : 0) : (h ? KS - p : p);
+    const int b = NPASS == 3 ? (k0 % R1) * R2 + k0 / R1 : k0;
+    cplx v[RL];
+#pragma unroll
+    for (int m = 0; m < RL; ++m) v[m] = s[(b * RL + m) * TILE_LINES + line];
+    RegFFT<RL, -1>::run(v);
+    cplx H0 = make_double2(0.0, 0.0);
+    if (k0 == 0) {
+#pragma unroll
+        for (int w = 0; w < NW; ++w) H0 = cadd(H0, red[w * 8 + line]);
+    }
+#pragma unroll
+    for (int q = 0; q < RL; ++q) {
+        // partner value Z_{N-k}: lane ^ 8 holds butterfly KS - k0, element RL - 1 - q (all lanes shuffle, also the self-paired)
+        cplx zp;
+        zp.x = __shfl_xor_sync(0xffffffffu, v[RL - 1 - q].x, 8);
+        zp.y = __shfl_xor_sync(0xffffffffu, v[RL - 1 - q].y, 8);
+        if (p == 0) zp = h ? v[RL - 1 - q] : v[(RL - q) & (RL - 1)];     // k0 = KS/2: q <-> RL-1-q;  k0 = 0: q <-> RL-q
+        const int k = k0 + KS * q;
+        const cplx z = v[q];
+        if (k == 0) {
+            const cplx G0 = make_double2(z.x + H0.y, z.y - H0.x);          // Z_0 - i H_0
+            emit(0, cscale(cadd(G0, H0), FWD ? 0.5 * sc : sc));
+            if (N < nout) emit(N, cscale(csub(G0, H0), FWD ? 0.5 * sc : sc));
+        } else if (k < nout) {
+            cplx c = ctab[k <= N / 2 ? k : N - k];
+            if (k > N / 2) c.y = -c.y;                                     // c_{N-k} = conj(c_k)
+            const cplx d = csub(z, zp);
+            emit(k, cscale(make_double2(z.x + (c.x * d.x - c.y * d.y), z.y + (c.x * d.y + c.y * d.x)), sc));
+        }
+    }
+}
+
 template <int N, bool FWD>
 __global__ void __launch_bounds__(ztma_threads<N>()) k_zpass_tma(const __grid_constant__ ZTArgs a,
                                                                        const cplx *__restrict__ twn_g,
@@ -132,8 +190,6 @@ __global__ void __launch_bounds__(ztma_threads<N>()) k_zpass_tma(const __grid_co
             fence_proxy_async();
             issue(tile + NSTG * gridDim.x, b);
         }
-        fft_rest_inplace_nb<N, -1, NT, ZP>(s, tw, tid);
-        __syncthreads();
         const bool der = !FWD && fld == a.dfield;
         double kx = 0.0, ky = 0.0;
         cplx *odx = nullptr, *ody = nullptr;
@@ -151,25 +207,36 @@ __global__ void __launch_bounds__(ztma_threads<N>()) k_zpass_tma(const __grid_co
                 if (ody) ody[(size_t)k * stride] = make_double2(-ky * v.y, ky * v.x);
             }
         };
-        for (int k = r0; k <= N / 2; k += RSTEP) {
-            const int kb = N - k;
-            if (k == 0) {
-                cplx H0 = make_double2(0.0, 0.0);
+        if constexpr (z_fuse_last<N, ZP, NT>()) {
+            // middle pass (three-pass plans) in place, then the last pass fused with the post-processing
+            if constexpr (zplan_npass<ZP>() == 3) {
+                fft_pass<N, N / ZP::R1, ZP::R2, -1, NT>(s, tw, tid);
+                __syncthreads();
+            }
+            z_last_pass_fused<N, ZP, FWD, NT>(s, ctab, red, tid, nout, sc, emit);
+        } else {
+            fft_rest_inplace_nb<N, -1, NT, ZP>(s, tw, tid);
+            __syncthreads();
+            for (int k = r0; k <= N / 2; k += RSTEP) {
+                const int kb = N - k;
+                if (k == 0) {
+                    cplx H0 = make_double2(0.0, 0.0);
 #pragma unroll
-                for (int w = 0; w < NW; ++w) H0 = cadd(H0, red[w * 8 + line]);
-                const cplx z0 = s[line];
-                const cplx G0 = make_double2(z0.x + H0.y, z0.y - H0.x);
-                emit(0, cscale(cadd(G0, H0), FWD ? 0.5 * sc : sc));
-                if (N < nout) emit(N, cscale(csub(G0, H0), FWD ? 0.5 * sc : sc));
-            } else {
-                const cplx za = s[fft_pos_f<N, ZP>(k) * TILE_LINES + line];
-                const cplx zb = s[fft_pos_f<N, ZP>(kb) * TILE_LINES + line];
-                const cplx c = ctab[k];
-                const cplx d = csub(za, zb);
-                const cplx cd = make_double2(c.x * d.x - c.y * d.y, c.x * d.y + c.y * d.x);
-                const cplx ccd = make_double2(c.x * d.x + c.y * d.y, c.x * d.y - c.y * d.x);
-                if (k < nout) emit(k, cscale(cadd(za, cd), sc));
-                if (kb != k && kb < nout) emit(kb, cscale(csub(zb, ccd), sc));
+                    for (int w = 0; w < NW; ++w) H0 = cadd(H0, red[w * 8 + line]);
+                    const cplx z0 = s[line];
+                    const cplx G0 = make_double2(z0.x + H0.y, z0.y - H0.x);
+                    emit(0, cscale(cadd(G0, H0), FWD ? 0.5 * sc : sc));
+                    if (N < nout) emit(N, cscale(csub(G0, H0), FWD ? 0.5 * sc : sc));
+                } else {
+                    const cplx za = s[fft_pos_f<N, ZP>(k) * TILE_LINES + line];
+                    const cplx zb = s[fft_pos_f<N, ZP>(kb) * TILE_LINES + line];
+                    const cplx c = ctab[k];
+                    const cplx d = csub(za, zb);
+                    const cplx cd = make_double2(c.x * d.x - c.y * d.y, c.x * d.y + c.y * d.x);
+                    const cplx ccd = make_double2(c.x * d.x + c.y * d.y, c.x * d.y - c.y * d.x);
+                    if (k < nout) emit(k, cscale(cadd(za, cd), sc));
+                    if (kb != k && kb < nout) emit(kb, cscale(csub(zb, ccd), sc));
+                }
             }
         }
         __syncthreads();
