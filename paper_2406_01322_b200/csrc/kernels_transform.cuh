@@ -279,14 +279,24 @@ __global__ void __launch_bounds__(tile_threads<L>()) k_xpass(const __grid_consta
     if (!FWD) {
         const cplx *__restrict__ inA = reinterpret_cast<const cplx *>(a.f.in[blockIdx.y]) + lineA * kxp;
         const cplx *__restrict__ inB = inA + kxp;
-        for (int i = r0; i <= L / 2; i += RSTEP) {
-            cplx ca = make_double2(0.0, 0.0), cb = ca;
-            if (i < nkx) { ca = inA[i]; cb = inB[i]; }
-            if (i == 0 || i == L / 2) {
-                s[i * TILE_LINES + p] = make_double2(ca.x, cb.x);
-            } else {
-                s[i * TILE_LINES + p] = make_double2(ca.x - cb.y, ca.y + cb.x);
-                s[(L - i) * TILE_LINES + p] = make_double2(ca.x + cb.y, cb.x - ca.y);
+        // two consecutive coefficients per thread: 32 contiguous bytes per line (whole sectors)
+        for (int i0 = 2 * r0; i0 <= L / 2; i0 += 2 * RSTEP) {
+            cplx ca[2], cb[2];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                ca[e] = cb[e] = make_double2(0.0, 0.0);
+                if (i0 + e < nkx) { ca[e] = inA[i0 + e]; cb[e] = inB[i0 + e]; }
+            }
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int i = i0 + e;
+                if (i > L / 2) break;
+                if (i == 0 || i == L / 2) {
+                    s[i * TILE_LINES + p] = make_double2(ca[e].x, cb[e].x);
+                } else {
+                    s[i * TILE_LINES + p] = make_double2(ca[e].x - cb[e].y, ca[e].y + cb[e].x);
+                    s[(L - i) * TILE_LINES + p] = make_double2(ca[e].x + cb[e].y, cb[e].x - ca[e].y);
+                }
             }
         }
         __syncthreads();
@@ -294,32 +304,49 @@ __global__ void __launch_bounds__(tile_threads<L>()) k_xpass(const __grid_consta
         __syncthreads();
         double *__restrict__ outA = reinterpret_cast<double *>(a.f.out[blockIdx.y]) + lineA * L;
         double *__restrict__ outB = outA + L;
-        for (int x = r0; x < L; x += RSTEP) {
-            cplx v = s[fft_pos<L>(x) * TILE_LINES + p];
-            outA[x] = v.x;
-            outB[x] = v.y;
+        // a thread stores FOUR consecutive x of its line pair (32 contiguous bytes per line: whole sectors; the 4 threads of a
+        // warp that share a line pair cover one 128-byte line) - one x per thread left every sector 3/4 unused per request
+        for (int xb = r0 * 4; xb < L; xb += RSTEP * 4) {
+            const cplx v0 = s[fft_pos<L>(xb) * TILE_LINES + p], v1 = s[fft_pos<L>(xb + 1) * TILE_LINES + p];
+            const cplx v2 = s[fft_pos<L>(xb + 2) * TILE_LINES + p], v3 = s[fft_pos<L>(xb + 3) * TILE_LINES + p];
+            *reinterpret_cast<double2 *>(outA + xb) = make_double2(v0.x, v1.x);
+            *reinterpret_cast<double2 *>(outA + xb + 2) = make_double2(v2.x, v3.x);
+            *reinterpret_cast<double2 *>(outB + xb) = make_double2(v0.y, v1.y);
+            *reinterpret_cast<double2 *>(outB + xb + 2) = make_double2(v2.y, v3.y);
         }
     } else {
         const double *__restrict__ inA = reinterpret_cast<const double *>(a.f.in[blockIdx.y]) + lineA * L;
         const double *__restrict__ inB = inA + L;
-        for (int x = r0; x < L; x += RSTEP) s[x * TILE_LINES + p] = make_double2(inA[x], inB[x]);
+        for (int xb = r0 * 4; xb < L; xb += RSTEP * 4) {      // four consecutive x per thread: whole 32-byte sectors per line
+            const double2 a0 = *reinterpret_cast<const double2 *>(inA + xb), a1 = *reinterpret_cast<const double2 *>(inA + xb + 2);
+            const double2 b0 = *reinterpret_cast<const double2 *>(inB + xb), b1 = *reinterpret_cast<const double2 *>(inB + xb + 2);
+            s[xb * TILE_LINES + p] = make_double2(a0.x, b0.x);
+            s[(xb + 1) * TILE_LINES + p] = make_double2(a0.y, b0.y);
+            s[(xb + 2) * TILE_LINES + p] = make_double2(a1.x, b1.x);
+            s[(xb + 3) * TILE_LINES + p] = make_double2(a1.y, b1.y);
+        }
         __syncthreads();
         fft_tile<L, -1, NT>(s, tw, tid);
         __syncthreads();
         cplx *__restrict__ outA = reinterpret_cast<cplx *>(a.f.out[blockIdx.y]) + lineA * kxp;
         cplx *__restrict__ outB = outA + kxp;
         const double sc = 0.5 / L;
-        for (int i = r0; i < kxp; i += RSTEP) {
-            cplx ra = make_double2(0.0, 0.0), rb = ra;
-            if (i < nkx) {
-                cplx z1 = s[fft_pos<L>(i) * TILE_LINES + p];
-                cplx z2 = s[fft_pos<L>((L - i) & (L - 1)) * TILE_LINES + p];
-                // A^ = (z1 + conj z2)/2 ; B^ = (z1 - conj z2)/(2i) = (-i/2)(z1 - conj z2)
-                ra = make_double2((z1.x + z2.x) * sc, (z1.y - z2.y) * sc);
-                rb = make_double2((z1.y + z2.y) * sc, (z2.x - z1.x) * sc);
+        for (int i0 = 2 * r0; i0 < kxp; i0 += 2 * RSTEP) {   // kxp is a multiple of 8: both coefficients of a pair are inside the row
+            cplx ra[2], rb[2];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int i = i0 + e;
+                ra[e] = rb[e] = make_double2(0.0, 0.0);
+                if (i < nkx) {
+                    const cplx z1 = s[fft_pos<L>(i) * TILE_LINES + p];
+                    const cplx z2 = s[fft_pos<L>((L - i) & (L - 1)) * TILE_LINES + p];
+                    // A^ = (z1 + conj z2)/2 ; B^ = (z1 - conj z2)/(2i) = (-i/2)(z1 - conj z2)
+                    ra[e] = make_double2((z1.x + z2.x) * sc, (z1.y - z2.y) * sc);
+                    rb[e] = make_double2((z1.y + z2.y) * sc, (z2.x - z1.x) * sc);
+                }
             }
-            outA[i] = ra;
-            outB[i] = rb;
+            outA[i0] = ra[0]; outA[i0 + 1] = ra[1];
+            outB[i0] = rb[0]; outB[i0 + 1] = rb[1];
         }
     }
 }
