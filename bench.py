@@ -511,11 +511,14 @@ def run_ours(args):
             lines = c.ny * c.nz
             flops = lines * ((cnt["nin"] + (7 if c.phase_field else 5)) * 2.5 * c.nx * math.log2(c.nx) + 45.0 * c.nx)
             sm_clock = float((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6
-            peak_tf = 148 * 64 * 2 * sm_clock / 1e12
+            nominal_tf = 148 * 64 * 2 * sm_clock / 1e12
+            peak_tf = solver.measure_fp64_peak()        # FMA-chain microbenchmark on this GPU
             tf = flops / (kernels["xfused"]["ms_per_step"] * 1e-3) / 1e12
             roof_alu = {"bound": "alu", "kernel": "xfused", "achieved": tf, "peak": peak_tf, "unit": "TFLOP/s (FP64)",
                         "frac": tf / peak_tf, "alg_flops_per_launch": flops,
-                        "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x max SM clock (B200 guide unit counts)"}
+                        "peak_source": "measured: FP64 FMA-chain microbenchmark (psdns_measure_fp64_peak)",
+                        "peak_nominal": nominal_tf,
+                        "peak_nominal_source": "148 SMs x 64 FP64 FMA/clk x 2 x max SM clock (B200 guide unit counts)"}
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             sec, desc, threads, parts = oracle_sampled_step_seconds(c)

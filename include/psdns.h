@@ -191,6 +191,11 @@ typedef struct {
 int psdns_render_isosurface(psdns_handle *h, const psdns_camera *cam, double iso, const void *d_field,
                             void *d_intensity, void *d_depth);
 
+/* FP64 peak of this GPU as an FMA-chain microbenchmark measures it: 8 independent chains of dependent DFMAs
+ * per thread, 8 CTAs of 256 threads per SM, best of three timed launches; *tflops in TFLOP/s (2 flops per FMA).
+ * Synchronises the stream.  Used by bench.py as the denominator of the FP64 view of the fused x kernel's roofline. */
+int psdns_measure_fp64_peak(psdns_handle *h, double *tflops);
+
 /* Tuning and test switches.  None is needed for normal use; the defaults are the product path.  Changing an option
  * drops the captured CUDA graph of the step (it is re-captured by the next psdns_step).
  *   "graph"    1 (default) / 0 : replay one captured CUDA graph per step / launch the kernels directly

@@ -14,7 +14,7 @@ EXPORTS = [
     "psdns_kernel_time_ms", "psdns_destroy", "psdns_last_error",
     "psdns_history_bytes", "psdns_get_history", "psdns_set_history",
     "psdns_set_option", "psdns_get_info", "psdns_workspace_bytes_unfused", "psdns_diagnostics",
-    "psdns_render_isosurface",
+    "psdns_render_isosurface", "psdns_measure_fp64_peak",
 ]
 
 
@@ -88,6 +88,8 @@ def load_library():
     lib.psdns_diagnostics.argtypes = [vp, vp]
     lib.psdns_render_isosurface.restype = ci
     lib.psdns_render_isosurface.argtypes = [vp, C.POINTER(psdns_camera), cd, vp, vp, vp]
+    lib.psdns_measure_fp64_peak.restype = ci
+    lib.psdns_measure_fp64_peak.argtypes = [vp, C.POINTER(cd)]
     lib.psdns_set_option.restype = ci
     lib.psdns_set_option.argtypes = [vp, C.c_char_p, cd]
     lib.psdns_get_info.restype = cd
@@ -241,6 +243,12 @@ class Solver:
         depth = self.torch.empty((height, width), dtype=self.torch.float64, device=self.device)
         self._check(self.lib.psdns_render_isosurface(self.handle, C.byref(cam), float(iso), _ptr(field), _ptr(inten), _ptr(depth)))
         return inten, depth
+
+    def measure_fp64_peak(self):
+        """FP64 FMA-chain microbenchmark, TFLOP/s (synchronises the stream)."""
+        tf = C.c_double()
+        self._check(self.lib.psdns_measure_fp64_peak(self.handle, C.byref(tf)))
+        return tf.value
 
     def set_option(self, name, value):
         self._check(self.lib.psdns_set_option(self.handle, name.encode(), float(value)))

@@ -115,4 +115,24 @@ __global__ void __launch_bounds__(DIAG_NT) k_diag_final(const double *__restrict
     }
 }
 
+// FP64 FMA-chain microbenchmark ("the builder measures [the FP64 peak] with an FMA-chain microbenchmark"):
+// every thread runs 8 independent chains of dependent DFMAs, `iters` x 8 x 16 FMAs per thread; the result is stored so that
+// nothing is optimised away.
+__global__ void __launch_bounds__(256) k_fp64_fma_chain(double *out, int nslots, int iters, double a, double b) {
+    double x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = 1.0 + 1e-9 * (threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) x[i] = fma(x[i], a, b);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    out[(size_t)(blockIdx.x % nslots) * blockDim.x + threadIdx.x] = s;   // blocks may share a slot: the value is never read
+}
+
 }  // namespace psdns

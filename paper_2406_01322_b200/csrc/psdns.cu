@@ -1354,6 +1354,32 @@ int psdns_render_isosurface(psdns_handle *h, const psdns_camera *cam, double iso
     return PSDNS_OK;
 }
 
+int psdns_measure_fp64_peak(psdns_handle *h, double *tflops) {
+    if (!h || !tflops) return PSDNS_EINVAL;
+    // scratch: the first Z array (transform scratch is free between steps)
+    double *out = h->at<double>(h->L.zb[0]);
+    const int blocks = h->n_sm * 8, iters = 4096;
+    const int nslots = (int)std::max<size_t>(1, std::min<size_t>((size_t)blocks, h->d.s_ret * sizeof(cplx) / (256 * sizeof(double))));
+    cudaEvent_t e0, e1;
+    CUDA_TRY(h, cudaEventCreate(&e0)); CUDA_TRY(h, cudaEventCreate(&e1));
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        CUDA_TRY(h, cudaEventRecord(e0, h->st));
+        k_fp64_fma_chain<<<blocks, 256, 0, h->st>>>(out, nslots, iters, 0.999999, 1e-6);
+        CUDA_TRY(h, cudaGetLastError());
+        CUDA_TRY(h, cudaEventRecord(e1, h->st));
+        CUDA_TRY(h, cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CUDA_TRY(h, cudaEventElapsedTime(&ms, e0, e1));
+        const double flops = 2.0 * 8 * 16 * (double)iters * 256.0 * blocks;
+        if (rep > 0) best = std::max(best, flops / (ms * 1e-3) / 1e12);
+        h->launches++;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *tflops = best;
+    return PSDNS_OK;
+}
+
 int psdns_set_option(psdns_handle *h, const char *name, double value) {
     if (!h || !name) return PSDNS_EINVAL;
     const std::string n(name);

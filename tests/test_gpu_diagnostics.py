@@ -74,3 +74,13 @@ def test_diagnostics_single_phase_and_errors():
     assert d[0] == 0.0 and np.isfinite(d).all()
     assert s.lib.psdns_diagnostics(s.handle, None) == -1
     s.close()
+
+
+def test_fp64_peak_microbenchmark_is_plausible():
+    """psdns_measure_fp64_peak (SURVEY 8(d) FMA-chain microbenchmark): between half and 1.2x of the nominal
+    148 SMs x 64 FMA/clk x 2 x 1.965 GHz = 37.2 TFLOP/s on a B200."""
+    import paper_2406_01322_b200 as P
+    s = P.Solver(32, 32, 33, 12.5, 6.3, re=100.0, dt=1e-3, phase_field=0)
+    tf = s.measure_fp64_peak()
+    assert 18.0 < tf < 45.0, tf
+    s.close()
