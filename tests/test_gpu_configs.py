@@ -48,7 +48,7 @@ def config_state(tag):
 
 
 @pytest.mark.parametrize("tag,nsteps", [("2", 100), ("3", 1), ("3", 3), ("4", 1), ("4", 2), ("5a", 1), ("5a", 3), ("5a", 25),
-                                        ("5b", 1)])
+                                        ("5b", 1), ("5b", 3), ("3", 50)])
 def test_config_full_grid_fixture(tag, nsteps):
     import torch
     import paper_2406_01322_b200 as P
