@@ -169,6 +169,24 @@ int psdns_kernel_time_ms(psdns_handle *h, double *ms_total, long long *launches)
  * Uses the transform scratch (not the state).  PSDNS_ESTATE before the first set_state. */
 int psdns_diagnostics(psdns_handle *h, double *d_out);
 
+/* psdns_diagnostics for callers that may not allocate device memory and have none to spare (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): same inputs (the resident state), same 8 outputs in
+ * DEVICE memory d_out, same kernels and launch shapes - the results are bit-identical to psdns_diagnostics - but the
+ * per-block partials of the two reductions live in a file-scope `static __device__` array of
+ * PSDNS_STATIC_SCRATCH_DOUBLES doubles (16 KiB, held by every GPU that loads the library until the process exits)
+ * instead of the workspace's fourth Z array.  The call itself runs no cudaMalloc, cudaFree or allocating library routine.
+ *   limit    ceil(ncols/256) + 8 * (number of SMs) <= PSDNS_STATIC_SCRATCH_DOUBLES, ncols = the retained (kx, ky) columns
+ *            (1024 x 512 needs 459 + 1184 on a B200; 1024 x 1024 does not fit).  Beyond it: PSDNS_EINVAL, nothing launched,
+ *            the text names the need and the limit.
+ *   sharing  every handle and every call on one GPU shares the array.  Each call overwrites the slots it reads before it
+ *            reads them, so the last call's contents never matter and nothing is cleared; but two calls that OVERLAP on
+ *            the GPU (different streams or handles, no ordering between them) race on it - serialise them.
+ *   errors   PSDNS_ESTATE before the first set_state or while psdns_kernel_timing is enabled (timing creates events);
+ *            PSDNS_EINVAL on a null pointer, a device ordinal > 63 or a grid beyond the limit; PSDNS_ECUDA otherwise.
+ * The device that owns the handle's workspace must be current, as for every other call. */
+#define PSDNS_STATIC_SCRATCH_DOUBLES 2048
+int psdns_diagnostics_static(psdns_handle *h, double *d_out);
+
 /* Iso-surface ray-caster (Fig. 5: the drops are rendered as the iso-surface phi = 0).
  * Pure compute into headless DEVICE buffers, no graphics API.  One ray per pixel:
  *   camera : f = unit(target - eye), r = unit(f x up), v = r x f; pixel (px, py), py = 0 the top row:

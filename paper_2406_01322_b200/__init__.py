@@ -4,5 +4,5 @@ Argument marshalling only - every step of the hot path runs in the CUDA kernels 
 `csrc/`.  There is no CPU fallback: importing `paper_2406_01322_b200.binding` raises if
 `libpsdns.so` is missing."""
 from .binding import (  # noqa: F401
-    PHYSICAL, SPECTRAL, PsdnsError, Solver, lib_path, load_library, exported_symbols,
+    PHYSICAL, SPECTRAL, STATIC_SCRATCH_DOUBLES, PsdnsError, Solver, lib_path, load_library, exported_symbols,
 )

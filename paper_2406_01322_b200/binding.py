@@ -14,8 +14,10 @@ EXPORTS = [
     "psdns_kernel_time_ms", "psdns_destroy", "psdns_last_error",
     "psdns_history_bytes", "psdns_get_history", "psdns_set_history",
     "psdns_set_option", "psdns_get_info", "psdns_workspace_bytes_unfused", "psdns_diagnostics",
-    "psdns_render_isosurface", "psdns_measure_fp64_peak",
+    "psdns_render_isosurface", "psdns_measure_fp64_peak", "psdns_diagnostics_static",
 ]
+
+STATIC_SCRATCH_DOUBLES = 2048   # PSDNS_STATIC_SCRATCH_DOUBLES of include/psdns.h
 
 
 class PsdnsError(RuntimeError):
@@ -86,6 +88,8 @@ def load_library():
     lib.psdns_set_history.argtypes = [vp, vp, C.c_size_t]
     lib.psdns_diagnostics.restype = ci
     lib.psdns_diagnostics.argtypes = [vp, vp]
+    lib.psdns_diagnostics_static.restype = ci
+    lib.psdns_diagnostics_static.argtypes = [vp, vp]
     lib.psdns_render_isosurface.restype = ci
     lib.psdns_render_isosurface.argtypes = [vp, C.POINTER(psdns_camera), cd, vp, vp, vp]
     lib.psdns_measure_fp64_peak.restype = ci
@@ -230,6 +234,14 @@ class Solver:
         """psdns_diagnostics into a fresh device tensor of 8 doubles (asynchronous; index with DIAG_NAMES order)."""
         out = self.torch.empty(8, dtype=self.torch.float64, device=self.device)
         self._check(self.lib.psdns_diagnostics(self.handle, _ptr(out)))
+        return out
+
+    def diagnostics_static(self, out):
+        """psdns_diagnostics_static into the caller's device tensor `out` (8 doubles): no allocation on either side of the
+        boundary; the reduction partials live in the library's file-scope device array (include/psdns.h)."""
+        if out.dtype != self.torch.float64 or out.numel() != 8 or not out.is_cuda or not out.is_contiguous():
+            raise PsdnsError("diagnostics_static: out must be a contiguous CUDA tensor of 8 doubles")
+        self._check(self.lib.psdns_diagnostics_static(self.handle, _ptr(out)))
         return out
 
     def render_isosurface(self, eye, target, up=(0.0, 0.0, 1.0), fov_y_deg=40.0, width=64, height=48, step=0.02,

@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1305,6 +1306,75 @@ int psdns_diagnostics(psdns_handle *h, double *d_out) {
         k_diag_final<<<1, DIAG_NT, 0, h->st>>>(part_max, nb_cols, part_sum, nb_en, d_out);
         CUDA_TRY(h, cudaGetLastError());
     }
+    return PSDNS_OK;
+}
+
+// ---- psdns_diagnostics_static: the same diagnostics with the reduction partials in a file-scope device array ----------
+// For callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc) and whose
+// workspace is not theirs to hand out: nothing below calls cudaMalloc, cudaFree or an allocating library routine.
+// Every GPU that loads the library holds the array (PSDNS_STATIC_SCRATCH_DOUBLES x 8 bytes = 16 KiB) until exit.
+// g_static_scratch is a HOST-side stand-in in host code, not a device address: the kernels get the address that
+// cudaGetSymbolAddress returns, looked up once per device with that device current.
+static __device__ __align__(256) double g_static_scratch[PSDNS_STATIC_SCRATCH_DOUBLES];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+double *g_static_scratch_ptr[STATIC_MAX_DEVICES];   // device address of g_static_scratch on each ordinal, nullptr = not looked up
+std::mutex g_static_scratch_mu;
+
+int static_scratch_address(psdns_handle *h, double **out) {
+    int dev = -1;
+    CUDA_TRY(h, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) { h->err = "psdns_diagnostics_static: device ordinal beyond 63"; return PSDNS_EINVAL; }
+    std::lock_guard<std::mutex> lk(g_static_scratch_mu);
+    if (!g_static_scratch_ptr[dev]) {
+        void *p = nullptr;
+        CUDA_TRY(h, cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p) { h->err = "psdns_diagnostics_static: cudaGetSymbolAddress returned a null address"; return PSDNS_ECUDA; }
+        g_static_scratch_ptr[dev] = (double *)p;
+    }
+    *out = g_static_scratch_ptr[dev];
+    return PSDNS_OK;
+}
+}  // namespace
+
+int psdns_diagnostics_static(psdns_handle *h, double *d_out) {
+    if (!h) return PSDNS_EINVAL;
+    if (!d_out) { h->err = "psdns_diagnostics_static: null output pointer"; return PSDNS_EINVAL; }
+    if (!h->has_state) { h->err = "psdns_diagnostics_static: no state set"; return PSDNS_ESTATE; }
+    if (h->timed_class >= 0) {   // psdns_kernel_timing creates a pair of CUDA events per launch
+        h->err = "psdns_diagnostics_static: kernel timing is enabled (it creates events); disable it first";
+        return PSDNS_ESTATE;
+    }
+    const Dims &d = h->d;
+    const Layout &L = h->L;
+    const bool phase = h->p.phase_field != 0;
+    const int nb_cols = (int)((d.ncols + DIAG_NT - 1) / DIAG_NT);
+    const int nb_en = h->n_sm * 8;
+    if ((long long)nb_cols + nb_en > PSDNS_STATIC_SCRATCH_DOUBLES) {
+        h->err = "psdns_diagnostics_static: this grid needs " + std::to_string((long long)nb_cols + nb_en) +
+                 " doubles of static scratch, the limit is " + std::to_string(PSDNS_STATIC_SCRATCH_DOUBLES) +
+                 " (PSDNS_STATIC_SCRATCH_DOUBLES); use psdns_diagnostics";
+        return PSDNS_EINVAL;
+    }
+    double *scratch = nullptr;
+    const int rc = static_scratch_address(h, &scratch);
+    if (rc != PSDNS_OK) return rc;
+    // every slot the final kernel reads is written by this call's two partial kernels first: the last call's
+    // contents never reach the result and nothing has to be cleared
+    double *part_max = scratch, *part_sum = scratch + nb_cols;
+    const cplx *U = h->at<cplx>(L.state[0]), *V = h->at<cplx>(L.state[1]), *W = h->at<cplx>(L.state[2]);
+    k_diag_columns<<<nb_cols, DIAG_NT, 0, h->st>>>(geom(h), U, V, W, phase ? h->at<cplx>(L.state[3]) : nullptr, part_max, d_out);
+    CUDA_TRY(h, cudaGetLastError());
+    FieldPtrs fz{};
+    for (int i = 0; i < 3; ++i) { fz.in[i] = h->at<cplx>(L.state[i]); fz.out[i] = h->at<cplx>(L.zb[i]); }
+    CUDA_TRY(h, launch_zpass(h, false, fz, 3, d.ncols, d.nz, d.kxp, d.nky, d.jpos));
+    k_diag_energy<<<nb_en, DIAG_NT, 0, h->st>>>(h->at<cplx>(L.zb[0]), h->at<cplx>(L.zb[1]), h->at<cplx>(L.zb[2]),
+                                                 h->at<double>(L.ccw), d.nz, (int)d.ncols, d.kxp, part_sum);
+    CUDA_TRY(h, cudaGetLastError());
+    k_diag_final<<<1, DIAG_NT, 0, h->st>>>(part_max, nb_cols, part_sum, nb_en, d_out);
+    CUDA_TRY(h, cudaGetLastError());
+    h->launches += 3;
     return PSDNS_OK;
 }
 
