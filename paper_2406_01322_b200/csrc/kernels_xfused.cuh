@@ -18,6 +18,7 @@
 // i.e. 4 tile exchanges per line instead of 9.  The backward FFT is decimation in frequency, the
 // products are elementwise, the forward FFT is decimation in time: no reordering anywhere.
 #pragma once
+#include <type_traits>
 #include "fft_tile.cuh"
 #include "kernels_transform.cuh"
 
@@ -200,83 +201,124 @@ template <int L> __host__ __device__ constexpr int xfw_lpi() {
     return ((L / 2) / XPlan<L / 2>::R1) >= 32 ? 1 : 32 / ((L / 2) / XPlan<L / 2>::R1);
 }
 
+// compile-time loop: f(std::integral_constant<int, I>) for I = 0 .. N-1 (the body can use `if constexpr` on I)
+template <int I, int N, class F>
+__device__ __forceinline__ void static_for(F &&f) {
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        static_for<I + 1, N>(f);
+    }
+}
+// global store with a compile-time byte offset folded into the instruction
+template <int OFF>
+__device__ __forceinline__ void stg_off(cplx *p, cplx v) {
+    asm volatile("st.global.v2.f64 [%0+%3], {%1, %2};" ::"l"(__cvta_generic_to_global(p)), "d"(v.x), "d"(v.y), "n"(OFF));
+}
+
+// nx = 1024 (S1 = 32: one butterfly per lane).  The retained k_x of the step are functions of L alone (reading S3), so the
+// cut-offs are compile-time constants here: which rows of stage A have a partner, which rows of stage F are stored, every
+// stage address.  Measured against the run-time form of the same kernel (profiles/r2c_experiments.md): 4.76e9 -> 4.0e9
+// warp instructions per launch (no predicated zero loads, no per-row branches, 40 DADD less per line), 8.2-8.4 -> 7.4-7.6 ms.
 template <int L, bool PHASE>
-__global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 512 ? 2 : 3))) k_xfusedw(const __grid_constant__ XFArgs a,
-                                                                             const cplx *__restrict__ twx) {
+__global__ void __launch_bounds__(XFW_THREADS, XF_MINB) k_xfusedw(const __grid_constant__ XFArgs a, const cplx *__restrict__ twx) {
     constexpr int H = L / 2;
     constexpr int R1 = XPlan<H>::R1, R2 = XPlan<H>::R2;
     constexpr int NT = XFW_THREADS;
-    constexpr int S1 = H / R1;              // butterflies per field of pass R1 (<= 32)
+    constexpr int S1 = H / R1;              // butterflies per field of pass R1
     constexpr int LS = 2 * R2;              // sub-length of the inner pass
-    constexpr int NB2 = H / R2;             // butterflies per field of the inner pass (<= 32)
+    constexpr int NB2 = H / R2;             // butterflies per field of the inner pass
     constexpr int LG = ilog2(LS) < 3 ? 3 : ilog2(LS);
     constexpr int NIN = PHASE ? 7 : 3, NOUT = PHASE ? 7 : 5;
     constexpr int NTMA = PHASE ? 6 : 3;
     constexpr int NST = xf_nstage<PHASE>();
-    static_assert(R1 * R2 * 2 == H && S1 <= 32 && NB2 <= 32, "plan");
+    // the step's retained k_x (reading S3) are functions of L alone: compile-time cut-offs (the host checks a.nkx == NKX)
+    constexpr int NKX = L / 3 + 1, KXP = (NKX + 7) & ~7;
+    constexpr int SP = NKX | 1;
+    static_assert(R1 * R2 * 2 == H && S1 == 32 && NB2 == 32, "plan");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
     cplx *stage = s + H * TILE_LINES;
-    const int kxp = a.kxp, nkx = a.nkx;
-    const int spitch = xf_spitch(nkx);
-    unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)NST * spitch);
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)NST * SP);
     unsigned long long *bar_free = bar + 1;         // stage consumed by every input-field warp
     const int tid = threadIdx.x, f = tid >> 5, lane = tid & 31;
-    const bool service = (f == TILE_LINES - 1);     // eighth warp
+    const bool service = (f == TILE_LINES - 1);
     cplx *outf = a.out[f < NOUT ? f : 0];
     const double sc = 0.5 / L;
-    const unsigned row_bytes = (unsigned)(nkx * sizeof(cplx));
+    constexpr unsigned row_bytes = (unsigned)(NKX * sizeof(cplx));
     auto issue = [&](int line) {
         mbar_expect_tx(bar, row_bytes * NTMA);
 #pragma unroll
-        for (int q = 0; q < NTMA; ++q) bulk_g2s(stage + (size_t)q * spitch, a.in[q] + (size_t)line * kxp, row_bytes, bar);
+        for (int q = 0; q < NTMA; ++q) bulk_g2s(stage + (size_t)q * SP, a.in[q] + (size_t)line * KXP, row_bytes, bar);
     };
+    unsigned long long *bar_drv = bar + 2;          // i kx phi^ row of the staged line derived (service warp -> phx warp)
     if (tid == 0) {
         mbar_init(bar, 1);
         mbar_init(bar_free, NIN);
+        mbar_init(bar_drv, 1);
         if ((int)blockIdx.x < a.nlines) issue(blockIdx.x);
     }
     __syncthreads();
+    // row a1: phx^ = i kx phi^, formed in the stage by the service warp as soon as the line's rows have landed - for the
+    // first line here, for every later line while the field warps run stages D-F of the line before
+    auto derive = [&](unsigned par) {
+        mbar_wait(bar, par);
+        for (int k = lane; k < NKX; k += 32) {
+            const cplx p = stage[3 * SP + k];
+            const double kk = a.kxf * (double)k;
+            stage[6 * SP + k] = make_double2(-kk * p.y, kk * p.x);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_drv);
+    };
+    if constexpr (PHASE) {
+        if (service && (int)blockIdx.x < a.nlines) derive(0);
+    }
     const int j = lane;                             // butterfly of passes A, E, F
-    const bool itemA = j < S1;
-    cplx wj = twx[itemA ? j : 0];                   // w_L^j
+    cplx wj = twx[j];                               // w_L^j
     // pointwise-stage twiddle of this thread's row pair: w_LS^(t mod R2) = w_L^((t mod R2) L / LS)
     cplx wc = twx[(tid % R2) * (L / LS)];
     unsigned parity = 0;
     // field -> staged row: u v w phi phx phy phz  <-  0 1 2 3 6 4 5
     const int srow = !PHASE ? (f < NST ? f : 0) : (f < 4 ? f : (f == 4 ? 6 : (f < NIN ? f - 1 : 0)));
-    const cplx *sf = stage + (size_t)srow * spitch;
+    const cplx *sf = stage + (size_t)srow * SP;
     for (int line = blockIdx.x; line < a.nlines; line += gridDim.x) {
-        const size_t base = (size_t)line * kxp;
-        mbar_wait(bar, parity);
+        const size_t base = (size_t)line * KXP;
+        if (f < NIN) mbar_wait(bar, parity);
         if constexpr (PHASE) {
-            if (service) {                          // row a1: phx^ = i kx phi^
-                for (int k = lane; k < nkx; k += 32) {
-                    const cplx p = stage[3 * spitch + k];
-                    const double kk = a.kxf * (double)k;
-                    stage[6 * spitch + k] = make_double2(-kk * p.y, kk * p.x);
-                }
-            }
-            __syncthreads();
+            if (srow == 6) mbar_wait(bar_drv, parity);
         }
         asm volatile("" : "+d"(wj.x), "+d"(wj.y), "+d"(wc.x), "+d"(wc.y));
         if (f < NIN) {
             // ---- A: pre-twiddle from the staged rows + DIF pass R1 (inverse transform, sign +) ----
-            if (itemA) {
-                const int jj = opaque(j);
+            {
+                const int jj = opaque(j) & (S1 - 1);
                 cplx v[R1];
-#pragma unroll
-                for (int m = 0; m < R1; ++m) {
+                static_for<0, R1>([&](auto M) {
+                    constexpr int m = decltype(M)::value;
                     if (m && (m & 3) == 0) asm volatile("" ::: "memory");
+                    // rows k = jj + S1 m of this m: X_k is retained for k < NKX, the partner X_{H-k} for k > H - NKX
+                    constexpr bool a_all = (S1 * m + S1 - 1 < NKX), a_none = (S1 * m >= NKX);
+                    constexpr bool b_all = (S1 * m > H - NKX), b_none = (S1 * m + S1 - 1 <= H - NKX);
                     const int k = jj + S1 * m, kb = H - k;
-                    cplx xa = make_double2(0.0, 0.0), xb = xa;
-                    if (k < nkx) xa = sf[k];
-                    if (kb < nkx) xb = sf[kb];
-                    if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
                     const cplx w = m ? cmul(wj, make_double2(wc_re<2 * R1>(m), wc_im<2 * R1>(m))) : wj;
-                    const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
-                    v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
-                }
+                    if constexpr (b_none) {
+                        static_assert(a_all, "cut-offs");
+                        cplx xa = sf[k];
+                        if (m == 0 && k == 0) xa.y = 0.0;           // reading S20
+                        v[m] = make_double2(fma(w.y, xa.x, fma(-w.x, xa.y, xa.x)), fma(w.y, xa.y, fma(w.x, xa.x, xa.y)));
+                    } else if constexpr (a_none) {
+                        static_assert(b_all, "cut-offs");
+                        const cplx xb = sf[kb];
+                        // S = conj(xb), D = -conj(xb)
+                        v[m] = make_double2(fma(-w.y, xb.x, fma(-w.x, xb.y, xb.x)), fma(w.y, xb.y, fma(-w.x, xb.x, -xb.y)));
+                    } else {
+                        cplx xa = make_double2(0.0, 0.0), xb = xa;
+                        if (a_all || k < NKX) xa = sf[k];
+                        if (b_all || kb < NKX) xb = sf[kb];
+                        const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
+                        v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
+                    }
+                });
                 RegFFT<R1, +1>::run(v);
                 TwPow<R1> tp;
                 tp.init(cmul(wj, wj));
@@ -286,16 +328,14 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 512 
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_free);   // this field's staged row is consumed
             // ---- B: DIF pass R2, no twiddles (they are applied in the pointwise stage) ----
-            if constexpr (R2 > 1) {
-                if (lane < NB2) {
-                    const int b = opaque(lane), row0 = (b >> 1) * LS + (b & 1);
-                    cplx v[R2];
+            {
+                const int b = opaque(lane) & 31, row0 = (b >> 1) * LS + (b & 1);
+                cplx v[R2];
 #pragma unroll
-                    for (int m = 0; m < R2; ++m) v[m] = s[widx<LG>(row0 + 2 * m, f)];
-                    RegFFT<R2, +1>::run(v);
+                for (int m = 0; m < R2; ++m) v[m] = s[widx<LG>(row0 + 2 * m, f)];
+                RegFFT<R2, +1>::run(v);
 #pragma unroll
-                    for (int q = 0; q < R2; ++q) s[widx<LG>(row0 + 2 * q, f)] = v[q];
-                }
+                for (int q = 0; q < R2; ++q) s[widx<LG>(row0 + 2 * q, f)] = v[q];
             }
         } else if (service) {
             if (lane == 0) {                        // all input warps are done with the stage: prefetch the next line
@@ -309,13 +349,15 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 512 
         parity ^= 1;
         __syncthreads();
         // ---- C: last DIF radix 2 (with the inner pass's twiddle), pointwise products, first DIT radix 2 ----
-        for (int t = opaque(tid); t < H / 2; t += NT) {
+        {
+            const int t = opaque(tid) & (NT - 1);
+            static_assert(H / 2 == NT, "one row pair per thread");
             double p00[8], p01[8], p10[8], p11[8];
 #pragma unroll
             for (int q = 0; q < NIN; ++q) {
                 const cplx p = s[widx<LG>(2 * t, q)];
                 cplx m = s[widx<LG>(2 * t + 1, q)];
-                if (R2 > 1) m = cmultw<+1>(m, wc);
+                m = cmultw<+1>(m, wc);
                 p00[q] = p.x + m.x; p01[q] = p.y + m.y;
                 p10[q] = p.x - m.x; p11[q] = p.y - m.y;
             }
@@ -325,31 +367,30 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 512 
                 nl_quad<PHASE>(q, p00, p01, p10, p11, a.cs, o00, o01, o10, o11);
                 s[widx<LG>(2 * t, q)] = make_double2(o00 + o10, o01 + o11);
                 cplx m = make_double2(o00 - o10, o01 - o11);
-                if (R2 > 1) m = cmultw<-1>(m, wc);
+                m = cmultw<-1>(m, wc);
                 s[widx<LG>(2 * t + 1, q)] = m;
             }
         }
         __syncthreads();
+        if constexpr (PHASE) {
+            if (service && line + (int)gridDim.x < a.nlines) derive(parity);     // parity is already the next line's
+        }
         if (f < NOUT) {
             // ---- D: DIT pass R2 (forward transform, sign -), no twiddles ----
-            if constexpr (R2 > 1) {
-                if (lane < NB2) {
-                    const int b = opaque(lane), row0 = (b >> 1) * LS + (b & 1);
-                    cplx v[R2];
+            {
+                const int b = opaque(lane) & 31, row0 = (b >> 1) * LS + (b & 1);
+                cplx v[R2];
 #pragma unroll
-                    for (int m = 0; m < R2; ++m) v[m] = s[widx<LG>(row0 + 2 * m, f)];
-                    RegFFT<R2, -1>::run(v);
+                for (int m = 0; m < R2; ++m) v[m] = s[widx<LG>(row0 + 2 * m, f)];
+                RegFFT<R2, -1>::run(v);
 #pragma unroll
-                    for (int q = 0; q < R2; ++q) s[widx<LG>(row0 + 2 * q, f)] = v[q];
-                }
-                __syncwarp();
+                for (int q = 0; q < R2; ++q) s[widx<LG>(row0 + 2 * q, f)] = v[q];
             }
+            __syncwarp();
             // ---- E: DIT pass R1; the results stay in registers ----
             cplx v[R1];
-#pragma unroll
-            for (int q = 0; q < R1; ++q) v[q] = make_double2(0.0, 0.0);
-            if (itemA) {
-                const int jj = opaque(j);
+            {
+                const int jj = opaque(j) & (S1 - 1);
                 TwPow<R1> tp;
                 tp.init(cmul(wj, wj));
                 v[0] = s[widx<LG>(jj, f)];
@@ -361,27 +402,29 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 512 
             // lane of THIS warp, fetched by shuffle - no shared-memory exchange and no barrier.
             {
                 const int src = (S1 - j) & (S1 - 1);
-                cplx *o = outf + base;
-#pragma unroll
-                for (int q = 0; q < R1; ++q) {
-                    if (S1 * q < kxp) {                        // CTA-uniform: no row of this q is kept otherwise
+                cplx *o = outf + base + j;
+                static_for<0, R1>([&](auto Q) {
+                    constexpr int q = decltype(Q)::value;
+                    if constexpr (S1 * q < KXP) {
+                        constexpr bool all = (S1 * q + S1 - 1 < NKX);
                         const cplx mine = (j == 0) ? v[(R1 - q) & (R1 - 1)] : v[R1 - 1 - q];
                         cplx zp;
                         zp.x = __shfl_sync(0xffffffffu, mine.x, src);
                         zp.y = __shfl_sync(0xffffffffu, mine.y, src);
                         const int k = j + S1 * q;
-                        if (itemA && k < nkx) {
-                            const cplx za = v[q];
-                            if (k == 0) zp = za;               // k = 0 is its own partner
-                            const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
-                            const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
-                            // X_k = (S - i w D) / (2 L)
-                            stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
-                        } else if (itemA && k < kxp) {
-                            stg(o + k, make_double2(0.0, 0.0));
+                        const cplx za = v[q];
+                        if (q == 0 && k == 0) zp = za;
+                        const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
+                        const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
+                        cplx r = make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy)));
+                        if constexpr (all) {
+                            stg_off<q * S1 * (int)sizeof(cplx)>(o, r);
+                        } else {
+                            if (k >= NKX) r = make_double2(0.0, 0.0);
+                            if (k < KXP) stg_off<q * S1 * (int)sizeof(cplx)>(o, r);
                         }
                     }
-                }
+                });
             }
             __syncwarp();     // this warp's F reads are done before its next stage A overwrites the field
         }

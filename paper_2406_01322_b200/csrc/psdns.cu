@@ -431,15 +431,17 @@ cudaError_t setup_xfused_L(psdns_handle *h) {
 }
 
 template <int LL>
-void launch_xfused_L(psdns_handle *h, const XFArgs &a, const cplx *tw, int grid) {
+cudaError_t launch_xfused_L(psdns_handle *h, const XFArgs &a, const cplx *tw, int grid) {
     const size_t sm = xfusedw_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);
     if constexpr (xfw_lpi<LL>() == 1) {
+        if (a.nkx != LL / 3 + 1 || a.kxp != round_up8(a.nkx)) return cudaErrorInvalidValue;   // k_xfusedw's compile-time cut-offs
         if (h->p.phase_field) k_xfusedw<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);
         else k_xfusedw<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);
     } else {
         if (h->p.phase_field) k_xfusedwm<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);
         else k_xfusedwm<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);
     }
+    return cudaSuccess;
 }
 
 // opt-in to > 48 KB dynamic shared memory once, at init (not inside graph capture), and size the persistent grids
@@ -499,7 +501,7 @@ cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
     const cplx *tw = h->at<cplx>(h->L.tw_x);
     const int grid = h->persistent_grid(KC_XFUSED, a.nlines, h->xf_occ);   // persistent: one wave
     LaunchScope ls(h, KC_XFUSED);
-#define XF(LL) launch_xfused_L<LL>(h, a, tw, grid);
+#define XF(LL) { const cudaError_t e = launch_xfused_L<LL>(h, a, tw, grid); if (e != cudaSuccess) return e; }
     DISPATCH_L(h->d.nx, XF)
 #undef XF
     return cudaGetLastError();
