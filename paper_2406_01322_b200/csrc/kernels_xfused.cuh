@@ -449,19 +449,22 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 128 
     constexpr int NTMA = PHASE ? 6 : 3;
     constexpr int NST = xf_nstage<PHASE>();
     constexpr int LPI = xfw_lpi<L>();       // lines per iteration
+    // compile-time cut-offs, as in k_xfusedw (the host checks a.nkx == NKX)
+    constexpr int NKX = L / 3 + 1, KXP = (NKX + 7) & ~7;
+    constexpr int SP = NKX | 1;
     static_assert(R1 * R2 * 2 == H && S1 * LPI == 32, "plan");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
     cplx *stage = s + LPI * H * TILE_LINES;         // [LPI][NST][spitch]
-    const int kxp = a.kxp, nkx = a.nkx;
-    const int spitch = xf_spitch(nkx);
+    constexpr int spitch = SP;
     unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)LPI * NST * spitch);
     unsigned long long *bar_free = bar + 1;         // stage consumed by every input-field warp
+    unsigned long long *bar_drv = bar + 2;          // i kx phi^ rows of the staged lines derived (service warp -> phx warp)
     const int tid = threadIdx.x, f = tid >> 5, lane = tid & 31;
     const bool service = (f == TILE_LINES - 1);     // eighth warp
     cplx *outf = a.out[f < NOUT ? f : 0];
     const double sc = 0.5 / L;
-    const unsigned row_bytes = (unsigned)(nkx * sizeof(cplx));
+    constexpr unsigned row_bytes = (unsigned)(NKX * sizeof(cplx));
     const int ngroups = a.nlines / LPI;             // nlines = nz * ny is a multiple of LPI (ny >= 16, power of two)
     auto issue = [&](int grp) {
         mbar_expect_tx(bar, row_bytes * NTMA * LPI);
@@ -469,14 +472,32 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 128 
         for (int l = 0; l < LPI; ++l)
 #pragma unroll
             for (int q = 0; q < NTMA; ++q)
-                bulk_g2s(stage + (size_t)(l * NST + q) * spitch, a.in[q] + (size_t)(grp * LPI + l) * kxp, row_bytes, bar);
+                bulk_g2s(stage + (size_t)(l * NST + q) * spitch, a.in[q] + (size_t)(grp * LPI + l) * KXP, row_bytes, bar);
     };
     if (tid == 0) {
         mbar_init(bar, 1);
         mbar_init(bar_free, NIN);
+        mbar_init(bar_drv, 1);
         if ((int)blockIdx.x < ngroups) issue(blockIdx.x);
     }
     __syncthreads();
+    // row a1: phx^ = i kx phi^, formed in the stage by the service warp as soon as the rows have landed - for the first
+    // group here, for every later group while the field warps run stages D-F of the group before
+    auto derive = [&](unsigned par) {
+        mbar_wait(bar, par);
+#pragma unroll
+        for (int l = 0; l < LPI; ++l)
+            for (int k = lane; k < NKX; k += 32) {
+                const cplx p = stage[(l * NST + 3) * spitch + k];
+                const double kk = a.kxf * (double)k;
+                stage[(l * NST + 6) * spitch + k] = make_double2(-kk * p.y, kk * p.x);
+            }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_drv);
+    };
+    if constexpr (PHASE) {
+        if (service && (int)blockIdx.x < ngroups) derive(0);
+    }
     const int j = LPI == 1 ? lane : (lane & (S1 - 1)), ln = LPI == 1 ? 0 : lane / S1;   // butterfly of passes A, E, F; its line
     constexpr bool itemA = true;                    // S1 * LPI = 32: every lane owns a butterfly
     const int lrow = ln * H;                        // first tile row of that line
@@ -488,38 +509,43 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 128 
     const int srow = !PHASE ? (f < NST ? f : 0) : (f < 4 ? f : (f == 4 ? 6 : (f < NIN ? f - 1 : 0)));
     const cplx *sf = stage + (size_t)(ln * NST + srow) * spitch;
     for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
-        const size_t base = (size_t)(grp * LPI + ln) * kxp;
-        mbar_wait(bar, parity);
+        const size_t base = (size_t)(grp * LPI + ln) * KXP;
+        if (f < NIN) mbar_wait(bar, parity);
         if constexpr (PHASE) {
-            if (service) {                          // row a1: phx^ = i kx phi^
-#pragma unroll
-                for (int l = 0; l < LPI; ++l)
-                    for (int k = lane; k < nkx; k += 32) {
-                        const cplx p = stage[(l * NST + 3) * spitch + k];
-                        const double kk = a.kxf * (double)k;
-                        stage[(l * NST + 6) * spitch + k] = make_double2(-kk * p.y, kk * p.x);
-                    }
-            }
-            __syncthreads();
+            if (srow == 6) mbar_wait(bar_drv, parity);
         }
         asm volatile("" : "+d"(wj.x), "+d"(wj.y), "+d"(wc.x), "+d"(wc.y));
         if (f < NIN) {
             // ---- A: pre-twiddle from the staged rows + DIF pass R1 (inverse transform, sign +) ----
             if (itemA) {
-                const int jj = opaque(j);
+                const int jj = opaque(j) & (S1 - 1);
                 cplx v[R1];
-#pragma unroll
-                for (int m = 0; m < R1; ++m) {
+                static_for<0, R1>([&](auto M) {
+                    constexpr int m = decltype(M)::value;
                     if (m && (m & 3) == 0) asm volatile("" ::: "memory");
+                    // rows k = jj + S1 m of this m: X_k is retained for k < NKX, the partner X_{H-k} for k > H - NKX
+                    constexpr bool a_all = (S1 * m + S1 - 1 < NKX), a_none = (S1 * m >= NKX);
+                    constexpr bool b_all = (S1 * m > H - NKX), b_none = (S1 * m + S1 - 1 <= H - NKX);
                     const int k = jj + S1 * m, kb = H - k;
-                    cplx xa = make_double2(0.0, 0.0), xb = xa;
-                    if (k < nkx) xa = sf[k];
-                    if (kb < nkx) xb = sf[kb];
-                    if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
                     const cplx w = m ? cmul(wj, make_double2(wc_re<2 * R1>(m), wc_im<2 * R1>(m))) : wj;
-                    const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
-                    v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
-                }
+                    if constexpr (b_none) {
+                        static_assert(a_all, "cut-offs");
+                        cplx xa = sf[k];
+                        if (m == 0 && k == 0) xa.y = 0.0;           // reading S20
+                        v[m] = make_double2(fma(w.y, xa.x, fma(-w.x, xa.y, xa.x)), fma(w.y, xa.y, fma(w.x, xa.x, xa.y)));
+                    } else if constexpr (a_none) {
+                        static_assert(b_all, "cut-offs");
+                        const cplx xb = sf[kb];                     // S = conj(xb), D = -conj(xb)
+                        v[m] = make_double2(fma(-w.y, xb.x, fma(-w.x, xb.y, xb.x)), fma(w.y, xb.y, fma(-w.x, xb.x, -xb.y)));
+                    } else {
+                        cplx xa = make_double2(0.0, 0.0), xb = xa;
+                        if (a_all || k < NKX) xa = sf[k];
+                        if (b_all || kb < NKX) xb = sf[kb];
+                        if (m == 0 && k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
+                        const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
+                        v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
+                    }
+                });
                 RegFFT<R1, +1>::run(v);
                 TwPow<R1> tp;
                 tp.init(cmul(wj, wj));
@@ -578,6 +604,9 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 128 
             }
         }
         __syncthreads();
+        if constexpr (PHASE) {
+            if (service && grp + (int)gridDim.x < ngroups) derive(parity);      // parity is already the next group's
+        }
         if (f < NOUT) {
             // ---- D: DIT pass R2 (forward transform, sign -), no twiddles ----
             if constexpr (R2 > 1) {
@@ -598,10 +627,8 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 128 
             }
             // ---- E: DIT pass R1; the results stay in registers ----
             cplx v[R1];
-#pragma unroll
-            for (int q = 0; q < R1; ++q) v[q] = make_double2(0.0, 0.0);
-            if (itemA) {
-                const int jj = opaque(j);
+            {
+                const int jj = opaque(j) & (S1 - 1);
                 TwPow<R1> tp;
                 tp.init(cmul(wj, wj));
                 v[0] = s[widx<LG>(lrow + jj, f)];
@@ -613,27 +640,30 @@ __global__ void __launch_bounds__(XFW_THREADS, (L >= 1024 ? XF_MINB : (L >= 128 
             // lane of THIS warp, fetched by shuffle - no shared-memory exchange and no barrier.
             {
                 const int src = ln * S1 + ((S1 - j) & (S1 - 1));
-                cplx *o = outf + base;
-#pragma unroll
-                for (int q = 0; q < R1; ++q) {
-                    if (S1 * q < kxp) {                        // CTA-uniform: no row of this q is kept otherwise
+                cplx *o = outf + base + j;
+                static_for<0, R1>([&](auto Q) {
+                    constexpr int q = decltype(Q)::value;
+                    if constexpr (S1 * q < KXP) {              // no row of this q is kept otherwise
+                        constexpr bool all = (S1 * q + S1 - 1 < NKX);
                         const cplx mine = (j == 0) ? v[(R1 - q) & (R1 - 1)] : v[R1 - 1 - q];
                         cplx zp;
                         zp.x = __shfl_sync(0xffffffffu, mine.x, src);
                         zp.y = __shfl_sync(0xffffffffu, mine.y, src);
                         const int k = j + S1 * q;
-                        if (itemA && k < nkx) {
-                            const cplx za = v[q];
-                            if (k == 0) zp = za;               // k = 0 is its own partner
-                            const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
-                            const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
-                            // X_k = (S - i w D) / (2 L)
-                            stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
-                        } else if (itemA && k < kxp) {
-                            stg(o + k, make_double2(0.0, 0.0));
+                        const cplx za = v[q];
+                        if (q == 0 && k == 0) zp = za;         // k = 0 is its own partner
+                        const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
+                        const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
+                        // X_k = (S - i w D) / (2 L)
+                        cplx r = make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy)));
+                        if constexpr (all) {
+                            stg_off<q * S1 * (int)sizeof(cplx)>(o, r);
+                        } else {
+                            if (k >= NKX) r = make_double2(0.0, 0.0);
+                            if (k < KXP) stg_off<q * S1 * (int)sizeof(cplx)>(o, r);
                         }
                     }
-                }
+                });
             }
             __syncwarp();     // this warp's F reads are done before its next stage A overwrites the field
         }

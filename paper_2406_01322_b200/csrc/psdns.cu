@@ -433,8 +433,8 @@ cudaError_t setup_xfused_L(psdns_handle *h) {
 template <int LL>
 cudaError_t launch_xfused_L(psdns_handle *h, const XFArgs &a, const cplx *tw, int grid) {
     const size_t sm = xfusedw_smem<LL>(h->d.nkx, h->p.phase_field ? 7 : 3);
+    if (a.nkx != LL / 3 + 1 || a.kxp != round_up8(a.nkx)) return cudaErrorInvalidValue;   // the kernels' compile-time cut-offs
     if constexpr (xfw_lpi<LL>() == 1) {
-        if (a.nkx != LL / 3 + 1 || a.kxp != round_up8(a.nkx)) return cudaErrorInvalidValue;   // k_xfusedw's compile-time cut-offs
         if (h->p.phase_field) k_xfusedw<LL, true><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);
         else k_xfusedw<LL, false><<<grid, XFW_THREADS, sm, h->st>>>(a, tw);
     } else {
