@@ -79,18 +79,20 @@ __global__ void __launch_bounds__(xv_threads<L>(), (L >= 1024 ? 1 : 2)) k_xfused
     constexpr int R1 = XPlan<H>::R1, R2 = XPlan<H>::R2;
     constexpr int NT = xv_threads<L>();
     constexpr int S1 = H / R1;
+    // compile-time cut-offs, as in k_xfusedw (the host checks a.nkx == NKX)
+    constexpr int NKX = L / 3 + 1, KXP = (NKX + 7) & ~7;
     static_assert(R1 * R2 * 2 == H, "plan");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *s = reinterpret_cast<cplx *>(smem_raw);
     cplx *stage = s + H * XV_SLOTS;
-    const int kxp = a.kxp, nkx = a.nkx;
-    const int spitch = xf_spitch(nkx);
+    constexpr int kxp = KXP, nkx = NKX;
+    constexpr int spitch = NKX | 1;
     unsigned long long *bar = reinterpret_cast<unsigned long long *>(stage + (size_t)XV_NST * spitch);
     const int tid = threadIdx.x, f = tid & (XV_SLOTS - 1), j = tid >> 4;
     const bool item = j < S1;
     cplx *outf = a.out[f < XV_NOUT ? f : 0];
     const double sc = 0.5 / L;
-    const unsigned row_bytes = (unsigned)(nkx * sizeof(cplx));
+    constexpr unsigned row_bytes = (unsigned)(NKX * sizeof(cplx));
     auto issue = [&](int line) {
         mbar_expect_tx(bar, row_bytes * XV_NTMA);
 #pragma unroll
@@ -119,22 +121,37 @@ __global__ void __launch_bounds__(xv_threads<L>(), (L >= 1024 ? 1 : 2)) k_xfused
         asm volatile("" : "+d"(wj.x), "+d"(wj.y));
         // ---- A: pre-twiddle from the staged rows + DIF pass R1 (inverse transform, sign +) ----
         if (item) {
-            const int jj = opaque(tid) >> 4;
+            const int jj = (opaque(tid) >> 4) & (S1 - 1);
+            const bool live = f < XV_NIN;              // slots 12..15 carry zeros through the backward passes
             cplx v[R1];
-#pragma unroll
-            for (int m = 0; m < R1; ++m) {
+            static_for<0, R1>([&](auto M) {
+                constexpr int m = decltype(M)::value;
                 if (m && (m & 3) == 0) asm volatile("" ::: "memory");
+                // rows k = jj + S1 m of this m: X_k is retained for k < NKX, the partner X_{H-k} for k > H - NKX
+                constexpr bool a_all = (S1 * m + S1 - 1 < NKX), a_none = (S1 * m >= NKX);
+                constexpr bool b_all = (S1 * m > H - NKX), b_none = (S1 * m + S1 - 1 <= H - NKX);
                 const int k = jj + S1 * m, kb = H - k;
-                cplx xa = make_double2(0.0, 0.0), xb = xa;
-                if (f < XV_NIN) {
-                    if (k < nkx) xa = sf[k];
-                    if (kb < nkx) xb = sf[kb];
-                }
-                if (k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
                 const cplx w = m ? cmul(wj, make_double2(wc_re<2 * R1>(m), wc_im<2 * R1>(m))) : wj;
-                const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
-                v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
-            }
+                if constexpr (b_none) {
+                    static_assert(a_all, "cut-offs");
+                    cplx xa = make_double2(0.0, 0.0);
+                    if (live) xa = sf[k];
+                    if (m == 0 && k == 0) xa.y = 0.0;           // reading S20
+                    v[m] = make_double2(fma(w.y, xa.x, fma(-w.x, xa.y, xa.x)), fma(w.y, xa.y, fma(w.x, xa.x, xa.y)));
+                } else if constexpr (a_none) {
+                    static_assert(b_all, "cut-offs");
+                    cplx xb = make_double2(0.0, 0.0);
+                    if (live) xb = sf[kb];                      // S = conj(xb), D = -conj(xb)
+                    v[m] = make_double2(fma(-w.y, xb.x, fma(-w.x, xb.y, xb.x)), fma(w.y, xb.y, fma(-w.x, xb.x, -xb.y)));
+                } else {
+                    cplx xa = make_double2(0.0, 0.0), xb = xa;
+                    if (live && (a_all || k < NKX)) xa = sf[k];
+                    if (live && (b_all || kb < NKX)) xb = sf[kb];
+                    if (m == 0 && k == 0) { xa.y = 0.0; xb.y = 0.0; }   // reading S20
+                    const double Sx = xa.x + xb.x, Sy = xa.y - xb.y, Dx = xa.x - xb.x, Dy = xa.y + xb.y;
+                    v[m] = make_double2(fma(w.y, Dx, fma(-w.x, Dy, Sx)), fma(w.y, Dy, fma(w.x, Dx, Sy)));
+                }
+            });
             RegFFT<R1, +1>::run(v);
             TwPow<R1> tp;
             tp.init(cmul(wj, wj));
@@ -184,7 +201,7 @@ __global__ void __launch_bounds__(xv_threads<L>(), (L >= 1024 ? 1 : 2)) k_xfused
         asm volatile("" : "+d"(wj.x), "+d"(wj.y));
         cplx v[R1];
         if (item) {
-            const int jj = opaque(tid) >> 4;
+            const int jj = (opaque(tid) >> 4) & (S1 - 1);
             TwPow<R1> tp;
             tp.init(cmul(wj, wj));
             v[0] = s[xvidx(jj, f)];
@@ -193,38 +210,45 @@ __global__ void __launch_bounds__(xv_threads<L>(), (L >= 1024 ? 1 : 2)) k_xfused
 #pragma unroll
             for (int q = 0; q < R1; ++q) {
                 const int r = jj + S1 * q;
-                if (r > H - nkx) s[xvidx(r, f)] = v[q];
+                if (S1 * q + S1 - 1 > H - NKX && (S1 * q > H - NKX || r > H - NKX)) s[xvidx(r, f)] = v[q];
             }
         }
         __syncthreads();
         // ---- F: post-twiddle of row k against the partner row H - k, truncated store ----
         if (item && f < XV_NOUT) {
-            const int jj = opaque(tid) >> 4;
-            cplx *o = outf + base;
-#pragma unroll
-            for (int q0 = 0; q0 < R1; q0 += 4) {
-                if (S1 * q0 < kxp) {
+            const int jj = (opaque(tid) >> 4) & (S1 - 1);
+            cplx *o = outf + base + jj;
+            static_for<0, R1 / 4>([&](auto Q0) {
+                constexpr int q0 = 4 * decltype(Q0)::value;
+                if constexpr (S1 * q0 < KXP) {
                     cplx zb[4];
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
                         const int k = jj + S1 * (q0 + i);
-                        zb[i] = s[xvidx((H - k) & (H - 1), f)];
+                        zb[i] = make_double2(0.0, 0.0);
+                        if (S1 * (q0 + i) < NKX) zb[i] = s[xvidx((H - k) & (H - 1), f)];
                     }
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int q = q0 + i, k = jj + S1 * q;
-                        if (k < nkx) {
+                    static_for<0, 4>([&](auto I) {
+                        constexpr int i = decltype(I)::value, q = q0 + i;
+                        if constexpr (S1 * q < KXP) {
+                            constexpr bool all = (S1 * q + S1 - 1 < NKX);
+                            const int k = jj + S1 * q;
                             const cplx za = v[q];
-                            const cplx zp = k ? zb[i] : za;
+                            cplx zp = zb[i];
+                            if (q == 0 && k == 0) zp = za;
                             const cplx w = q ? cmul(wj, make_double2(wc_re<2 * R1>(q), wc_im<2 * R1>(q))) : wj;
                             const double Sx = za.x + zp.x, Sy = za.y - zp.y, Dx = za.x - zp.x, Dy = za.y + zp.y;
-                            stg(o + k, make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy))));
-                        } else if (k < kxp) {
-                            stg(o + k, make_double2(0.0, 0.0));
+                            cplx r = make_double2(sc * fma(w.y, Dx, fma(w.x, Dy, Sx)), sc * fma(w.y, Dy, fma(-w.x, Dx, Sy)));
+                            if constexpr (all) {
+                                stg_off<q * S1 * (int)sizeof(cplx)>(o, r);
+                            } else {
+                                if (k >= NKX) r = make_double2(0.0, 0.0);
+                                if (k < KXP) stg_off<q * S1 * (int)sizeof(cplx)>(o, r);
+                            }
                         }
-                    }
+                    });
                 }
-            }
+            });
         }
         __syncthreads();
     }

@@ -510,6 +510,7 @@ cudaError_t launch_xfused(psdns_handle *h, const XFArgs &a) {
 cudaError_t launch_xfusedv(psdns_handle *h, const XFVArgs &a) {
     const cplx *tw = h->at<cplx>(h->L.tw_x);
     const int grid = h->persistent_grid(KC_XFUSED, a.nlines, h->xfv_occ);   // persistent: one wave
+    if (a.nkx != h->d.nx / 3 + 1 || a.kxp != round_up8(a.nkx)) return cudaErrorInvalidValue;   // the kernel's compile-time cut-offs
     LaunchScope ls(h, KC_XFUSED);
 #define XFV(LL) k_xfusedv<LL><<<grid, xv_threads<LL>(), xfusedv_smem<LL>(h->d.nkx), h->st>>>(a, tw);
     DISPATCH_L(h->d.nx, XFV)
