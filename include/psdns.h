@@ -228,6 +228,9 @@ int psdns_measure_fp64_peak(psdns_handle *h, double *tflops);
  *   "zgemm"    0 (default) / 1 : nz <= 65 only: Chebyshev transform as a dense FP64 matrix product on the tensor cores
  *                                (k_zgemm, DMMA) instead of the FFT path - kept for the measurement of SURVEY 8(f)-1
  *   "pf", "pf_rhs" n >= 0      : L2 prefetch distance, in rows, of the solver sweeps (defaults 2 and 4)
+ *   "phi3"     1 (default) / 0 : phase field only: the second Helmholtz solve of the phi problem eliminated upwards inside
+ *                                the up sweep that produces psi and back-substituted by the last (downward) sweep - three
+ *                                sweeps over the phi column, psi never stored - / the five-sweep form; equal to rounding
  * PSDNS_EINVAL on an unknown name or a bad value. */
 int psdns_set_option(psdns_handle *h, const char *name, double value);
 

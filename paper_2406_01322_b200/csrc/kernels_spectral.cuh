@@ -480,6 +480,97 @@ struct ElimDown2R {
     }
 };
 
+// ================================================================================================
+// UPWARD elimination of the same system, used for the SECOND solve of the phi problem ((D^2 - k^2 - lambda) phi = psi)
+// so that it can ride on the up sweep that produces psi (k_subst) and finish in the down sweep that k_finish makes
+// anyway: psi never reaches HBM and two sweeps over the phi column disappear (three sweeps instead of five for this
+// problem).  Rows k = 2, 3, .. ascending, each parity on its own; u_par (par = k & 1) is carried symbolically:
+//   d''_k u_k + c_k u_{k+2} = g''_k + e_k u_par,
+//   first row of a parity (k = 2, 3):  d''_k = d_k, g''_k = g_k, e_k = -a_k,
+//   then  m_k = a_k / d''_{k-2}:       d''_k = d_k - m_k c_{k-2}, g''_k = g_k - m_k g''_{k-2}, e_k = -m_k e_{k-2}.
+// Back substitution (descending): u_k = g^_k + e^_k u_par - c^_k u_{k+2},  g^ = g''/d'', e^ = e/d'', c^ = c/d''.
+// u_par comes from the boundary row BEFORE that sweep through the adjoint of the upper-bidiagonal system:
+//   y_k = (w_k - c_{k-2} y_{k-2}) / d''_k   =>   sum_{k>=2} w_k u_k = sum_k y_k g''_k + u_par sum_k y_k e_k,
+//   u_par = (target - sum y_k g''_k) / (w_par + sum y_k e_k)       (Neumann rows: w_k = k^2, target 0).
+// d''_k and e_k depend on (k, sigma) only; the up sweep recomputes them, the down sweep reads (c^_k, e^_k) from a table
+// (they obey an ascending recurrence, and the backward form d''_{k-2} = a_k c_{k-2} / (d_k - d''_k) cancels).
+// The system is diagonally dominant in both directions (|a_k| + |c_k| < d_k - 1 + 1), so no pivoting either way.
+// ================================================================================================
+struct PivotUp {
+    double dm1, dm2;   // 1/d''_{k-1}, 1/d''_{k-2}
+    double em1, em2;   // e_{k-1}, e_{k-2}
+    __device__ __forceinline__ void init() { dm1 = dm2 = em1 = em2 = 0.0; }
+    // row k (2 <= k <= N): returns 1/d''_k; m = a_k / d''_{k-2} (0 in the first row of a parity), e = e_k, c = c_k,
+    // cm2 = c_{k-2} (c_j = -sigma r_j for j + 4 <= N, else 0)
+    __device__ __forceinline__ double step(int k, int N, double sigma, double &m, double &e, double &c, double &cm2) {
+        const double ak = -sigma * helm_p(k);
+        double d = 1.0 + ((k + 2 <= N) ? sigma * (-helm_q(k)) : 0.0);
+        c = (k + 4 <= N) ? -sigma * helm_r(k) : 0.0;
+        cm2 = (k >= 4 && k + 2 <= N) ? -sigma * helm_r(k - 2) : 0.0;
+        if (k < 4) { m = 0.0; e = -ak; }
+        else {
+            m = ak * dm2;
+            d -= m * cm2;
+            e = -m * em2;
+        }
+        const double di = 1.0 / d;
+        dm2 = dm1; dm1 = di;
+        em2 = em1; em1 = e;
+        return di;
+    }
+};
+
+struct ElimUpNeu {   // Neumann rows (sum k^2 u_k = 0 per parity), complex right-hand side
+    PivotUp pv;
+    cplx gm2, gm1;            // g''_{k-2}, g''_{k-1}
+    double ym2, ym1;          // adjoint weights y_{k-2}, y_{k-1}
+    cplx Je, Jo;              // sum y_k g''_k per parity
+    double Ee, Eo;            // sum y_k e_k per parity
+    __device__ __forceinline__ void init() { pv.init(); gm2 = gm1 = Je = Jo = cz(); ym2 = ym1 = Ee = Eo = 0.0; }
+    // row k: F(k-2), F(k), F(k+2) of the right-hand side (zero-extended above N-2).  Returns g^_k = g''_k / d''_k.
+    __device__ __forceinline__ cplx row(int k, int N, double sigma, cplx fm2, cplx f0, cplx fp2) {
+        double m, e, c, cm2;
+        const double di = pv.step(k, N, sigma, m, e, c, cm2);
+        cplx g = cfma(helm_p(k), fm2, cfma(helm_q(k), f0, cscale(fp2, helm_r(k))));
+        g = cfma(-m, gm2, g);
+        const double y = ((double)k * k - cm2 * ym2) * di;
+        if (k & 1) { Jo = cfma(y, g, Jo); Eo = fma(y, e, Eo); } else { Je = cfma(y, g, Je); Ee = fma(y, e, Ee); }
+        gm2 = gm1; gm1 = g;
+        ym2 = ym1; ym1 = y;
+        return cscale(g, di);
+    }
+    __device__ __forceinline__ void finish(cplx &u0, cplx &u1) const {
+        u0 = cscale(Je, -1.0 / Ee);              // weight of u_0 itself: 0^2
+        u1 = cscale(Jo, -1.0 / (1.0 + Eo));      // weight of u_1 itself: 1^2
+    }
+};
+
+// table of the down sweep: tab[k] = (c^_k, e^_k) = (c_k, e_k) / d''_k, k = 2..N (rows 0, 1 unused)
+struct ElimUpSetupArgs {
+    ColGeom g;
+    double2 *tab;   // [N+1][ncols]
+    double shift;   // sigma = k^2 + shift
+};
+
+__global__ void __launch_bounds__(NT_COL) k_elimup_setup(const __grid_constant__ ElimUpSetupArgs a) {
+    const ColGeom &g = a.g;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    double kx, ky;
+    col_wavenumbers(g, col, kx, ky);
+    const double sigma = kx * kx + ky * ky + a.shift;
+    const size_t st = g.ncols;
+    PivotUp pv;
+    pv.init();
+    a.tab[col] = make_double2(0.0, 0.0);
+    a.tab[st + col] = make_double2(0.0, 0.0);
+    for (int k = 2; k <= g.N; ++k) {
+        double m, e, c, cm2;
+        const double di = pv.step(k, g.N, sigma, m, e, c, cm2);
+        a.tab[k * st + col] = make_double2(c * di, e * di);
+    }
+}
+
 // ---- K_A: row a9 + first elimination ------------------------------------------------------------------
 // CTA = 32 consecutive columns, three warps.  Warps 0 and 1: the omega_z AND theta chains of 16 columns each, one
 // thread per (column, real / imaginary part) - both chains need the same five product rows and the same pivots,
@@ -719,17 +810,19 @@ struct SubstArgs {
 // 4 on small grids (latency-bound), 2 above 60 k columns (DRAM-bound: more resident threads win; measured at
 // 1024x512x513: solve 4.23 ms with 2, 4.36 with 4, 4.51 with 8; at 256x256x257: 0.43 with 4, 0.42 with 8).
 
-template <int G>
-__global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstArgs a) {
+// UP: the psi chain (chain 2 of the first substitution) does not store psi but feeds it, row by row, into the upward
+// elimination of the phi solve (ElimUpNeu) and stores g^_k of that solve instead; k_finish completes it on its way down.
+template <int G, bool UP>
+__device__ __forceinline__ void subst_body(const SubstArgs &a, int by) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= g.ncols) return;
-    const int chain = a.pair01 ? blockIdx.y + 1 : blockIdx.y;
+    const int chain = UP ? 2 : (a.pair01 ? by + 1 : by);   // UP: the psi chain, in a block row of k_elim2up
     double kx, ky;
     col_wavenumbers(g, col, kx, ky);
     const size_t st = g.ncols;
     const int N = g.N;
-    if (a.pair01 && blockIdx.y == 0) {      // omega_z and theta: same recurrence coefficients, two right-hand sides
+    if (!UP && a.pair01 && by == 0) {      // omega_z and theta: same recurrence coefficients, two right-hand sides
         const double sigma = kx * kx + ky * ky + a.shift[0];
         cplx *x0 = a.x[0] + col, *x1 = a.x[1] + col;
         const double *__restrict__ dinv = a.dinv[0] + col;
@@ -771,10 +864,14 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
     const double sigma = kx * kx + ky * ky + a.shift[chain];
     cplx *x = a.x[chain] + col;
     const double *__restrict__ dinv = a.dinv[chain] + col;
-    const bool corr = (chain == 0 && a.coef != nullptr);
+    const bool corr = !UP && (chain == 0 && a.coef != nullptr);
     cplx Ae = cz(), Ao = cz();
     if (corr) { Ae = a.coef[col]; Ao = a.coef[st + col]; }
     cplx um2 = x[0], um1 = x[st];
+    constexpr bool upel = UP;
+    ElimUpNeu eu;
+    cplx w4 = cz(), w3 = cz(), w2 = um2, w1 = um1;      // F(k-4) .. F(k-1) of the phi solve's right-hand side psi
+    if (UP) eu.init();
     if (corr) {
         x[0] = cfma(a.wh[col], Ae, um2);
         x[st] = cfma(a.wh[st + col], Ao, um1);
@@ -811,7 +908,11 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
                 const double ak = -sigma * helm_p(k);
                 const cplx u = cscale(cfma(-ak, um2, q[i].x), q[i].di);
                 um2 = um1; um1 = u;
-                if (corr) {
+                if (UP && upel) {
+                    const cplx fk = (k <= N - 2) ? u : cz();        // the right-hand side is zero-extended above N - 2
+                    if (k >= 4) x[(k - 2) * st] = eu.row(k - 2, N, sigma, w4, w2, fk);
+                    w4 = w3; w3 = w2; w2 = w1; w1 = fk;
+                } else if (corr) {
                     const size_t o = k * st + col;
                     const cplx A = (k & 1) ? Ao : Ae;
                     x[k * st] = cfma(q[i].wh, A, u);
@@ -824,7 +925,17 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
 #pragma unroll
         for (int i = 0; i < G; ++i) q[i] = nx[i];
     }
+    if (UP && upel) {       // rows N - 1 and N: F(k) = F(k + 2) = 0
+        x[(N - 1) * st] = eu.row(N - 1, N, sigma, w4, cz(), cz());
+        x[N * st] = eu.row(N, N, sigma, w3, cz(), cz());
+        cplx u0, u1;
+        eu.finish(u0, u1);
+        x[0] = u0; x[st] = u1;
+    }
 }
+
+template <int G>
+__global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstArgs a) { subst_body<G, false>(a, blockIdx.y); }
 
 // ---- K_C: second elimination of the two-stage problems (RHS = the first stage's solution) ----------------
 // chain 0: (D^2 - k^2) w = theta_p, Dirichlet, plus the influence coefficient A_par = -sum k^2 w_p / sum k^2 w_h
@@ -842,11 +953,10 @@ struct Elim2Args {
 };
 
 template <int G, bool GEN>
-__global__ void __launch_bounds__(NT_COL, 3) k_elim2(const __grid_constant__ Elim2Args a) {
+__device__ __forceinline__ void elim2_body(const Elim2Args &a, int chain) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= g.ncols) return;
-    const int chain = blockIdx.y;
     double kx, ky;
     col_wavenumbers(g, col, kx, ky);
     const double k2 = kx * kx + ky * ky;
@@ -942,6 +1052,17 @@ __global__ void __launch_bounds__(NT_COL, 3) k_elim2(const __grid_constant__ Eli
     }
 }
 
+template <int G, bool GEN>
+__global__ void __launch_bounds__(NT_COL, 3) k_elim2(const __grid_constant__ Elim2Args a) { elim2_body<G, GEN>(a, blockIdx.y); }
+
+// Three-sweep form of the phi problem (ElimUpNeu): block row 0 = the w elimination of k_elim2, block row 1 = the up sweep of
+// the psi chain feeding the upward elimination of the phi solve (psi is not stored).
+template <int G, bool GEN>
+__global__ void __launch_bounds__(NT_COL, 3) k_elim2up(const __grid_constant__ Elim2Args a, const __grid_constant__ SubstArgs b) {
+    if (blockIdx.y == 0) elim2_body<G, GEN>(a, 0);
+    else subst_body<G, true>(b, 0);
+}
+
 // ---- init helper: real copies of the homogeneous solutions and their k^2 sums --------------------------
 __global__ void __launch_bounds__(NT_COL) k_hom_tables(const __grid_constant__ ColGeom g, const cplx *__restrict__ thh_c,
                                                        const cplx *__restrict__ wh_c, double *__restrict__ thh,
@@ -970,8 +1091,9 @@ struct FinishArgs {
     const cplx *om;    // omega_z^{n+1} (column 0: u-bar^{n+1})
     const cplx *th;    // column 0 only: v-bar^{n+1}
     cplx *u, *v, *w;
-    const cplx *phi;   // nullable (single-phase)
+    cplx *phi;         // nullable (single-phase)
     cplx *phz;         // [nkz][ncols]: D phi^, truncated (operator P)
+    const double2 *tab_phi;   // non-null: phi holds g^ of the upward elimination (k_subst<., true>); this sweep substitutes
 };
 
 template <int G>
@@ -988,7 +1110,11 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
     const bool phase = a.phi != nullptr;
     Chain1 cW, cP;
     cW.init(); cP.init();
-    struct Row { cplx w, om, phi; };
+    // phi_k = g^_k + e^_k phi_par - c^_k phi_{k+2} (back substitution of ElimUpNeu), in place
+    const bool upphi = phase && a.tab_phi != nullptr;
+    cplx pu0 = cz(), pu1 = cz(), pp2 = cz(), pp1 = cz();
+    if (upphi) { pu0 = a.phi[col]; pu1 = a.phi[st + col]; }
+    struct Row { cplx w, om, phi; double2 tb; };
     auto load = [&](int n0, Row (&r)[G]) {               // rows n0, n0 - 1, .. (descending)
 #pragma unroll
         for (int i = 0; i < G; ++i) {
@@ -997,7 +1123,8 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
                 const size_t o = n * st + col;
                 r[i].w = a.w[o];
                 r[i].om = a.om[o];
-                if (phase && n < g.nkz) r[i].phi = a.phi[o];
+                if (phase && (upphi || n < g.nkz)) r[i].phi = a.phi[o];
+                if (upphi && n >= 2) r[i].tb = a.tab_phi[o];
                 if (mean) r[i].w = a.th[o];              // column (0,0): v-bar lives in the theta slot
             }
         }
@@ -1014,7 +1141,8 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
             if (np >= 0) {
                 const size_t op = np * st + col;
                 pf_l2(a.w + op); pf_l2(a.om + op);
-                if (phase && np < g.nkz) pf_l2(a.phi + op);
+                if (phase && (upphi || np < g.nkz)) pf_l2(a.phi + op);
+                if (upphi) pf_l2(a.tab_phi + op);
             }
         }
 #pragma unroll
@@ -1023,7 +1151,15 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
             if (n < 0) continue;
             const size_t o = n * st + col;
             const double f = 2.0 * (n + 1), h = (n == 0) ? 0.5 : 1.0;
-            if (phase && n < g.nkz) a.phz[o] = cP.step(q[i].phi, f, h);   // D of the truncated phi^ (P first, then D)
+            cplx ph = q[i].phi;
+            if (upphi) {
+                if (n >= 2) {
+                    ph = cfma(q[i].tb.y, (n & 1) ? pu1 : pu0, cfma(-q[i].tb.x, pp2, ph));
+                    a.phi[o] = ph;
+                }
+                pp2 = pp1; pp1 = ph;
+            }
+            if (phase && n < g.nkz) a.phz[o] = cP.step(ph, f, h);   // D of the truncated phi^ (P first, then D)
             if (mean) {   // mean flow: u-bar from the omega slot, v-bar from the theta slot, w = 0 (reading S12)
                 a.u[o] = q[i].om;
                 a.v[o] = q[i].w;

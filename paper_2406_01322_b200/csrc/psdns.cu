@@ -62,6 +62,7 @@ struct Layout {
     size_t dinv[3];                    // NS (beta^2), PO (k^2), CH (k^2 + lambda)
     size_t thh, wh;                    // real homogeneous solutions [nz][ncols]
     size_t hw, coef;                   // [2][ncols] doubles / cplx
+    size_t tab_phi;                    // (c^_k, e^_k) of the phi solve's upward elimination, [nz][ncols] double2 (phase field)
     size_t xom;
     size_t derived[8];                 // phz [exx eyy exy exz eyz]
     size_t prod[10];                   // txx-tzz txy txz tyy-tzz tyz q c [fx fy fz: force form of the surface tension]
@@ -105,6 +106,7 @@ struct psdns_handle {
     PFN_cuTensorMapEncodeTiled encode_tiled;
     int grid_cap;               // psdns_set_option("grid_cap"): upper bound on the grid of every persistent kernel (0 = none)
     int pf, pf_rhs;             // L2 prefetch distances of the column sweeps, in rows
+    bool phi3 = true;           // phi problem in three sweeps (ElimUpNeu)
     long long last_grid[KC_COUNT], last_items[KC_COUNT];   // grid / work items of the last launch of each persistent class
 
     int persistent_grid(int kc, long long items, int occ) {
@@ -175,6 +177,7 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.wh = take(d.s_ret * sizeof(double));
     L.hw = take(4 * d.ncols * sizeof(double));
     L.coef = take(2 * d.ncols * C);
+    L.tab_phi = p.phase_field ? take(d.s_ret * sizeof(double2)) : 0;
     L.xom = take(d.s_ret * C);
     const bool visc_l = p.phase_field && p.visc_ratio != 1.0;
     for (int i = 0; i < 8; ++i) L.derived[i] = 0;
@@ -712,6 +715,9 @@ cudaError_t enqueue_step(psdns_handle *h) {
     // influence-matrix correction (K_D), velocity recovery (a11)
     const double inv_g = 1.0 / c.gamma;
     const bool la2 = d.ncols > 60000;   // register look-ahead depth of the solver sweeps (kernels_spectral.cuh)
+    // phi problem in three sweeps: its second solve is eliminated upwards inside the first substitution (psi never stored)
+    // and back-substituted by k_finish on its way down (ElimUpNeu); phi3 = 0 keeps the five-sweep form for cross-checks
+    const bool phi3 = phase && h->phi3;
     const bool walls_gen = p.wall_top != 0 || p.wall_bottom != 0;   // free-slip or mixed walls (row f3)
     const double *dNS = h->at<double>(L.dinv[0]), *dPO = h->at<double>(L.dinv[1]), *dCH = h->at<double>(L.dinv[2]);
     {
@@ -747,9 +753,11 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.pair01 = 1;
         a.coef = nullptr; a.wh = nullptr; a.thh = nullptr; a.th = nullptr;
         LaunchScope ls(h, KC_SOLVE);
-        if (la2) k_subst<2><<<dim3(col_grid(d), a.nchains - 1), NT_COL, 0, h->st>>>(a);
-        else k_subst<4><<<dim3(col_grid(d), a.nchains - 1), NT_COL, 0, h->st>>>(a);
+        const dim3 g1(col_grid(d), phi3 ? 1 : a.nchains - 1);
+        if (la2) k_subst<2><<<g1, NT_COL, 0, h->st>>>(a);
+        else k_subst<4><<<g1, NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
+
     }
     {
         Elim2Args a;
@@ -758,7 +766,19 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.wall_top = p.wall_top; a.wall_bot = p.wall_bottom;
         LaunchScope ls(h, KC_SOLVE);
         const dim3 g2(col_grid(d), phase ? 2 : 1);
-        if (walls_gen) { if (la2) k_elim2<2, true><<<g2, NT_COL, 0, h->st>>>(a); else k_elim2<4, true><<<g2, NT_COL, 0, h->st>>>(a); }
+        if (phi3) {   // block row 1: the psi chain's up sweep feeding the upward elimination of the phi solve
+            SubstArgs b;
+            b.g = a.g;
+            b.x[0] = nullptr; b.x[1] = nullptr; b.x[2] = PHI;
+            b.dinv[0] = nullptr; b.dinv[1] = nullptr; b.dinv[2] = dCH;
+            b.shift[0] = 0.0; b.shift[1] = 0.0; b.shift[2] = c.lam_phi;
+            b.nchains = 3; b.pair01 = 1;
+            b.coef = nullptr; b.wh = nullptr; b.thh = nullptr; b.th = nullptr;
+            if (walls_gen) { if (la2) k_elim2up<2, true><<<g2, NT_COL, 0, h->st>>>(a, b); else k_elim2up<4, true><<<g2, NT_COL, 0, h->st>>>(a, b); }
+            else if (la2) k_elim2up<2, false><<<g2, NT_COL, 0, h->st>>>(a, b);
+            else k_elim2up<4, false><<<g2, NT_COL, 0, h->st>>>(a, b);
+        }
+        else if (walls_gen) { if (la2) k_elim2<2, true><<<g2, NT_COL, 0, h->st>>>(a); else k_elim2<4, true><<<g2, NT_COL, 0, h->st>>>(a); }
         else if (la2) k_elim2<2, false><<<g2, NT_COL, 0, h->st>>>(a);
         else k_elim2<4, false><<<g2, NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
@@ -769,7 +789,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.x[0] = W; a.x[1] = PHI; a.x[2] = nullptr;
         a.dinv[0] = dPO; a.dinv[1] = dCH; a.dinv[2] = nullptr;
         a.shift[0] = 0.0; a.shift[1] = c.lam_phi; a.shift[2] = 0.0;
-        a.nchains = phase ? 2 : 1;
+        a.nchains = (phase && !phi3) ? 2 : 1;
         a.pair01 = 0;
         a.coef = h->at<cplx>(L.coef); a.wh = h->at<double>(L.wh); a.thh = h->at<double>(L.thh); a.th = TH;
         LaunchScope ls(h, KC_SOLVE);
@@ -782,6 +802,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
         FinishArgs a;
         a.g = geom(h); a.om = OM; a.th = TH; a.u = U; a.v = V; a.w = W;
         a.phi = phase ? PHI : nullptr; a.phz = PHZ;
+        a.tab_phi = phi3 ? h->at<double2>(L.tab_phi) : nullptr;
         LaunchScope ls(h, KC_SOLVE);
         if (la2) k_finish<2><<<col_grid(d), NT_COL, 0, h->st>>>(a);
         else k_finish<4><<<col_grid(d), NT_COL, 0, h->st>>>(a);
@@ -872,6 +893,13 @@ cudaError_t build_tables(psdns_handle *h) {
         a.g = geom(h); a.dinv = h->at<double>(L.dinv[t]); a.shift = shifts[t];
         LaunchScope ls(h, KC_MISC);
         k_helm_setup<<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        CU(cudaGetLastError());
+    }
+    if (h->p.phase_field) {   // down-sweep table of the phi solve's upward elimination (kernels_spectral.cuh, ElimUpNeu)
+        ElimUpSetupArgs a;
+        a.g = geom(h); a.tab = h->at<double2>(L.tab_phi); a.shift = c.lam_phi;
+        LaunchScope ls(h, KC_MISC);
+        k_elimup_setup<<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
     // homogeneous solutions of the w problem: theta_h = Helmholtz(beta^2) with zero rhs and unit boundary
@@ -1469,6 +1497,7 @@ int psdns_set_option(psdns_handle *h, const char *name, double value) {
     else if (n == "grid_cap" && iv >= 0) h->grid_cap = iv;
     else if (n == "ztma") h->use_ztma = iv != 0;
     else if (n == "zgemm") h->use_zgemm = iv != 0;
+    else if (n == "phi3") h->phi3 = iv != 0;
     else if (n == "pf" && iv >= 0) h->pf = iv;
     else if (n == "pf_rhs" && iv >= 0) h->pf_rhs = iv;
     else { h->err = "psdns_set_option: unknown option or bad value: " + n; return PSDNS_EINVAL; }

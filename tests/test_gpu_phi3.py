@@ -1,0 +1,58 @@
+"""The phi problem in three sweeps (kernels_spectral.cuh, ElimUpNeu: the second Helmholtz solve of the Cahn-Hilliard split
+is eliminated UPWARDS inside the up sweep that produces psi and back-substituted by k_finish on its way down) against the
+five-sweep form of the same solve (`psdns_set_option("phi3", 0)`): both are Gauss eliminations of the same diagonally
+dominant system, so the states agree to rounding - on every variant of the step that carries a phase field.  Parity with
+the oracle is covered by the ordinary step tests, which run the default (three-sweep) path."""
+import numpy as np
+import pytest
+
+import psdns_inputs as I
+from helpers import solver_from_config, to_dev, to_np
+
+pytestmark = pytest.mark.gpu
+
+CASES = [
+    dict(nx=32, ny=32, nz=33),
+    dict(nx=16, ny=16, nz=9),                                   # shortest column: rows 2..8 only
+    dict(nx=64, ny=16, nz=65),
+    dict(nx=128, ny=64, nz=129, over=dict(visc_ratio=0.5)),     # variable viscosity (k_xfusedv)
+    dict(nx=32, ny=64, nz=33, over=dict(wall_top=1, wall_bottom=0)),          # mixed walls
+    dict(nx=32, ny=32, nz=33, over=dict(surface_tension_form=1)),             # force form, three-kernel x path
+    dict(nx=256, ny=128, nz=129),                               # 11 k columns: the look-ahead depth of small grids
+]
+
+
+@pytest.mark.parametrize("case", CASES, ids=lambda c: "%dx%dx%d%s" % (c["nx"], c["ny"], c["nz"], "".join("-" + k for k in c.get("over", {}))))
+def test_three_sweep_phi_equals_five_sweep(case):
+    import paper_2406_01322_b200 as P
+    c = I.small_config(nx=case["nx"], ny=case["ny"], nz=case["nz"])
+    st = I.channel_state(c)
+    outs = []
+    for opt in (0, 1):
+        s = solver_from_config(c, **case.get("over", {}))
+        s.set_option("phi3", opt)
+        s.set_state(P.PHYSICAL, *[to_dev(f) for f in st])
+        s.step(4)
+        outs.append([to_np(t) for t in s.get_state(P.SPECTRAL)])
+        s.close()
+    vel = max(float(np.abs(a).max()) for a in outs[0][:3])
+    for name, a, b, scale in zip("uvwp", outs[0], outs[1], (vel, vel, vel, float(np.abs(outs[0][3]).max()))):
+        assert np.all(np.isfinite(b)), name
+        assert float(np.abs(a - b).max()) <= 1e-12 * scale, (name, float(np.abs(a - b).max()), scale)
+
+
+def test_three_sweep_phi_many_columns():
+    """Above 60 k columns the sweeps use the shallow register look-ahead (G = 2): 512 x 512 x 17."""
+    import paper_2406_01322_b200 as P
+    c = I.small_config(nx=512, ny=512, nz=17, band=2)
+    st = I.channel_state(c)
+    outs = []
+    for opt in (0, 1):
+        s = solver_from_config(c)
+        s.set_option("phi3", opt)
+        s.set_state(P.PHYSICAL, *[to_dev(f) for f in st])
+        s.step(3)
+        outs.append([to_np(t) for t in s.get_state(P.SPECTRAL)])
+        s.close()
+    for a, b in zip(*outs):
+        assert float(np.abs(a - b).max()) <= 1e-12 * max(float(np.abs(a).max()), 1.0)
