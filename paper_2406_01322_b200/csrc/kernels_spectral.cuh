@@ -545,6 +545,43 @@ struct ElimUpNeu {   // Neumann rows (sum k^2 u_k = 0 per parity), complex right
     }
 };
 
+// Dirichlet rows (sum u_k = 0 per parity) plus the k^2-weighted functional of the solution: the w problem
+// (D^2 - k^2) w = theta_p, whose influence-matrix coefficient needs sum k^2 w_p per parity (k_elim2 / ElimDown::second).
+struct ElimUpDir2 {
+    PivotUp pv;
+    cplx gm2, gm1;            // g''_{k-2}, g''_{k-1}
+    double ym2, ym1;          // adjoint of the boundary row (weights 1)
+    double sm2, sm1;          // adjoint of the second functional (weights k^2)
+    cplx Je, Jo, Ke, Ko;      // sum y_k g''_k, sum s_k g''_k per parity
+    double Ee, Eo, Fe, Fo;    // sum y_k e_k, sum s_k e_k per parity
+    __device__ __forceinline__ void init() {
+        pv.init();
+        gm2 = gm1 = Je = Jo = Ke = Ko = cz();
+        ym2 = ym1 = sm2 = sm1 = Ee = Eo = Fe = Fo = 0.0;
+    }
+    __device__ __forceinline__ cplx row(int k, int N, double sigma, cplx fm2, cplx f0, cplx fp2) {
+        double m, e, c, cm2;
+        const double di = pv.step(k, N, sigma, m, e, c, cm2);
+        cplx g = cfma(helm_p(k), fm2, cfma(helm_q(k), f0, cscale(fp2, helm_r(k))));
+        g = cfma(-m, gm2, g);
+        const double y = (1.0 - cm2 * ym2) * di;
+        const double sq = ((double)k * k - cm2 * sm2) * di;
+        if (k & 1) { Jo = cfma(y, g, Jo); Eo = fma(y, e, Eo); Ko = cfma(sq, g, Ko); Fo = fma(sq, e, Fo); }
+        else       { Je = cfma(y, g, Je); Ee = fma(y, e, Ee); Ke = cfma(sq, g, Ke); Fe = fma(sq, e, Fe); }
+        gm2 = gm1; gm1 = g;
+        ym2 = ym1; ym1 = y;
+        sm2 = sm1; sm1 = sq;
+        return cscale(g, di);
+    }
+    // u_0, u_1 of the particular solution and its k^2-weighted parity sums
+    __device__ __forceinline__ void finish(cplx &u0, cplx &u1, cplx &de, cplx &dodd) const {
+        u0 = cscale(Je, -1.0 / (1.0 + Ee));
+        u1 = cscale(Jo, -1.0 / (1.0 + Eo));
+        de = cfma(Fe, u0, Ke);                   // 0^2 u_0 + K_e + u_0 F_e
+        dodd = cadd(u1, cfma(Fo, u1, Ko));       // 1^2 u_1 + K_o + u_1 F_o
+    }
+};
+
 // table of the down sweep: tab[k] = (c^_k, e^_k) = (c_k, e_k) / d''_k, k = 2..N (rows 0, 1 unused)
 struct ElimUpSetupArgs {
     ColGeom g;
@@ -801,6 +838,10 @@ struct SubstArgs {
     const cplx *coef;           // [2][ncols]: A_e, A_o
     const double *wh, *thh;     // real homogeneous solutions [nz][ncols]
     cplx *th;
+    // W3 (three-sweep w problem): the pair's theta_p rows feed the upward elimination of (D^2 - k^2) w = theta_p
+    cplx *w3_out;               // g^ of that elimination (slots 0, 1 = w_p,0, w_p,1)
+    const double *w3_hw;        // [2][ncols]: sum k^2 w_h per parity
+    cplx *w3_coef;              // [2][ncols] out: influence-matrix coefficients A_e, A_o
 };
 
 // The sweeps work in place, so the compiler cannot move the load of row k + 1 above the store of row k (same
@@ -812,7 +853,7 @@ struct SubstArgs {
 
 // UP: the psi chain (chain 2 of the first substitution) does not store psi but feeds it, row by row, into the upward
 // elimination of the phi solve (ElimUpNeu) and stores g^_k of that solve instead; k_finish completes it on its way down.
-template <int G, bool UP>
+template <int G, bool UP, bool W3 = false>
 __device__ __forceinline__ void subst_body(const SubstArgs &a, int by) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
@@ -827,6 +868,11 @@ __device__ __forceinline__ void subst_body(const SubstArgs &a, int by) {
         cplx *x0 = a.x[0] + col, *x1 = a.x[1] + col;
         const double *__restrict__ dinv = a.dinv[0] + col;
         cplx um2 = x0[0], um1 = x0[st], vm2 = x1[0], vm1 = x1[st];
+        ElimUpDir2 ew;
+        cplx w4 = cz(), w3 = cz(), w2 = vm2, w1 = vm1;      // F(k-4) .. F(k-1) of the w solve's right-hand side theta_p
+        const double k2w = kx * kx + ky * ky;
+        cplx *wout = W3 ? a.w3_out + col : nullptr;
+        if (W3) ew.init();
         cplx q0[G], q1[G];
         double dq[G];
         auto load = [&](int k0, cplx (&p0)[G], cplx (&p1)[G], double (&d)[G]) {
@@ -854,10 +900,25 @@ __device__ __forceinline__ void subst_body(const SubstArgs &a, int by) {
                     const cplx v = cscale(cfma(-ak, vm2, q1[i]), dq[i]);
                     um2 = um1; um1 = u; vm2 = vm1; vm1 = v;
                     x0[k * st] = u; x1[k * st] = v;
+                    if (W3) {
+                        const cplx fk = (k <= N - 2) ? v : cz();    // the right-hand side is zero-extended above N - 2
+                        if (k >= 4) wout[(k - 2) * st] = ew.row(k - 2, N, k2w, w4, w2, fk);
+                        w4 = w3; w3 = w2; w2 = w1; w1 = fk;
+                    }
                 }
             }
 #pragma unroll
             for (int i = 0; i < G; ++i) { q0[i] = n0[i]; q1[i] = n1[i]; dq[i] = dn[i]; }
+        }
+        if (W3) {       // rows N - 1 and N, boundary unknowns, influence-matrix coefficients (as k_elim2, no-slip walls)
+            wout[(N - 1) * st] = ew.row(N - 1, N, k2w, w4, cz(), cz());
+            wout[N * st] = ew.row(N, N, k2w, w3, cz(), cz());
+            cplx u0, u1, de, dodd;
+            ew.finish(u0, u1, de, dodd);
+            wout[0] = u0; wout[st] = u1;
+            const bool off = (col == 0);
+            a.w3_coef[col] = off ? cz() : cscale(de, -1.0 / a.w3_hw[col]);
+            a.w3_coef[st + col] = off ? cz() : cscale(dodd, -1.0 / a.w3_hw[st + col]);
         }
         return;
     }
@@ -936,6 +997,15 @@ __device__ __forceinline__ void subst_body(const SubstArgs &a, int by) {
 
 template <int G>
 __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstArgs a) { subst_body<G, false>(a, blockIdx.y); }
+
+// Three-sweep form of both two-stage problems: block row 0 = the (omega_z, theta_p) pair, whose theta_p rows also feed the
+// upward elimination of the w solve (ElimUpDir2); block row 1 (phase field) = the psi chain feeding the upward
+// elimination of the phi solve (ElimUpNeu).  k_finish<., true> back-substitutes both on its way down.
+template <int G>
+__global__ void __launch_bounds__(NT_COL) k_subst3(const __grid_constant__ SubstArgs a) {
+    if (blockIdx.y == 0) subst_body<G, false, true>(a, 0);
+    else subst_body<G, true>(a, 0);
+}
 
 // ---- K_C: second elimination of the two-stage problems (RHS = the first stage's solution) ----------------
 // chain 0: (D^2 - k^2) w = theta_p, Dirichlet, plus the influence coefficient A_par = -sum k^2 w_p / sum k^2 w_h
@@ -1094,9 +1164,15 @@ struct FinishArgs {
     cplx *phi;         // nullable (single-phase)
     cplx *phz;         // [nkz][ncols]: D phi^, truncated (operator P)
     const double2 *tab_phi;   // non-null: phi holds g^ of the upward elimination (k_subst<., true>); this sweep substitutes
+    // W3: w holds g^ of the w solve's upward elimination (k_subst3); this sweep substitutes, adds the influence-matrix
+    // correction w += A_par w_h, theta += A_par theta_h (what the second k_subst does in the five-sweep form)
+    const double2 *tab_w;
+    const double *wh, *thh;
+    const cplx *coef;
+    cplx *th_rw;
 };
 
-template <int G>
+template <int G, bool W3 = false>
 __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ FinishArgs a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
@@ -1114,7 +1190,10 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
     const bool upphi = phase && a.tab_phi != nullptr;
     cplx pu0 = cz(), pu1 = cz(), pp2 = cz(), pp1 = cz();
     if (upphi) { pu0 = a.phi[col]; pu1 = a.phi[st + col]; }
-    struct Row { cplx w, om, phi; double2 tb; };
+    // w_p,k = g^_k + e^_k w_p,par - c^_k w_p,k+2 (back substitution of ElimUpDir2), then w = w_p + A_par w_h
+    cplx wu0 = cz(), wu1 = cz(), wp2 = cz(), wp1 = cz(), Ae = cz(), Ao = cz();
+    if (W3) { wu0 = a.w[col]; wu1 = a.w[st + col]; Ae = a.coef[col]; Ao = a.coef[st + col]; }
+    struct Row { cplx w, om, phi, thv; double2 tb, tw; double whv, thhv; };
     auto load = [&](int n0, Row (&r)[G]) {               // rows n0, n0 - 1, .. (descending)
 #pragma unroll
         for (int i = 0; i < G; ++i) {
@@ -1125,7 +1204,10 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
                 r[i].om = a.om[o];
                 if (phase && (upphi || n < g.nkz)) r[i].phi = a.phi[o];
                 if (upphi && n >= 2) r[i].tb = a.tab_phi[o];
-                if (mean) r[i].w = a.th[o];              // column (0,0): v-bar lives in the theta slot
+                if (W3) {
+                    if (n >= 2) r[i].tw = a.tab_w[o];
+                    r[i].whv = a.wh[o]; r[i].thhv = a.thh[o]; r[i].thv = a.th_rw[o];
+                } else if (mean) r[i].w = a.th[o];       // column (0,0): v-bar lives in the theta slot
             }
         }
     };
@@ -1143,6 +1225,7 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
                 pf_l2(a.w + op); pf_l2(a.om + op);
                 if (phase && (upphi || np < g.nkz)) pf_l2(a.phi + op);
                 if (upphi) pf_l2(a.tab_phi + op);
+                if (W3) { pf_l2(a.tab_w + op); pf_l2(a.wh + op); pf_l2(a.thh + op); pf_l2(a.th_rw + op); }
             }
         }
 #pragma unroll
@@ -1160,12 +1243,21 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
                 pp2 = pp1; pp1 = ph;
             }
             if (phase && n < g.nkz) a.phz[o] = cP.step(ph, f, h);   // D of the truncated phi^ (P first, then D)
+            cplx wv = q[i].w;
+            if (W3) {
+                if (n >= 2) wv = cfma(q[i].tw.y, (n & 1) ? wu1 : wu0, cfma(-q[i].tw.x, wp2, wv));
+                wp2 = wp1; wp1 = wv;
+                const cplx A = (n & 1) ? Ao : Ae;
+                wv = cfma(q[i].whv, A, wv);
+                if (!mean) { a.w[o] = wv; a.th_rw[o] = cfma(q[i].thhv, A, q[i].thv); }
+                else wv = q[i].thv;                       // column (0,0): v-bar lives in the theta slot
+            }
             if (mean) {   // mean flow: u-bar from the omega slot, v-bar from the theta slot, w = 0 (reading S12)
                 a.u[o] = q[i].om;
-                a.v[o] = q[i].w;
+                a.v[o] = wv;
                 a.w[o] = cz();
             } else {
-                const cplx dw = cW.step(q[i].w, f, h);
+                const cplx dw = cW.step(wv, f, h);
                 const cplx om = q[i].om;
                 a.u[o] = cscale(ci(cadd(cscale(dw, kx), cscale(om, ky))), ik2);
                 a.v[o] = cscale(ci(csub(cscale(dw, ky), cscale(om, kx))), ik2);

@@ -63,6 +63,7 @@ struct Layout {
     size_t thh, wh;                    // real homogeneous solutions [nz][ncols]
     size_t hw, coef;                   // [2][ncols] doubles / cplx
     size_t tab_phi;                    // (c^_k, e^_k) of the phi solve's upward elimination, [nz][ncols] double2 (phase field)
+    size_t tab_w;                      // the same for the w solve (sigma = k^2)
     size_t xom;
     size_t derived[8];                 // phz [exx eyy exy exz eyz]
     size_t prod[10];                   // txx-tzz txy txz tyy-tzz tyz q c [fx fy fz: force form of the surface tension]
@@ -107,6 +108,7 @@ struct psdns_handle {
     int grid_cap;               // psdns_set_option("grid_cap"): upper bound on the grid of every persistent kernel (0 = none)
     int pf, pf_rhs;             // L2 prefetch distances of the column sweeps, in rows
     bool phi3 = true;           // phi problem in three sweeps (ElimUpNeu)
+    bool w3 = true;             // w problem in three sweeps (ElimUpDir2; no-slip walls, needs phi3 with a phase field)
     long long last_grid[KC_COUNT], last_items[KC_COUNT];   // grid / work items of the last launch of each persistent class
 
     int persistent_grid(int kc, long long items, int occ) {
@@ -178,6 +180,7 @@ Layout make_layout(const Dims &d, const psdns_params &p) {
     L.hw = take(4 * d.ncols * sizeof(double));
     L.coef = take(2 * d.ncols * C);
     L.tab_phi = p.phase_field ? take(d.s_ret * sizeof(double2)) : 0;
+    L.tab_w = take(d.s_ret * sizeof(double2));
     L.xom = take(d.s_ret * C);
     const bool visc_l = p.phase_field && p.visc_ratio != 1.0;
     for (int i = 0; i < 8; ++i) L.derived[i] = 0;
@@ -715,10 +718,13 @@ cudaError_t enqueue_step(psdns_handle *h) {
     // influence-matrix correction (K_D), velocity recovery (a11)
     const double inv_g = 1.0 / c.gamma;
     const bool la2 = d.ncols > 60000;   // register look-ahead depth of the solver sweeps (kernels_spectral.cuh)
+    const bool walls_gen = p.wall_top != 0 || p.wall_bottom != 0;   // free-slip or mixed walls (row f3)
     // phi problem in three sweeps: its second solve is eliminated upwards inside the first substitution (psi never stored)
     // and back-substituted by k_finish on its way down (ElimUpNeu); phi3 = 0 keeps the five-sweep form for cross-checks
     const bool phi3 = phase && h->phi3;
-    const bool walls_gen = p.wall_top != 0 || p.wall_bottom != 0;   // free-slip or mixed walls (row f3)
+    // w problem likewise (ElimUpDir2; no-slip walls): the solver stage is then three launches - k_rhs_elim (down),
+    // k_subst3 (up), k_finish (down) - instead of five
+    const bool w3 = h->w3 && !walls_gen && (!phase || phi3);
     const double *dNS = h->at<double>(L.dinv[0]), *dPO = h->at<double>(L.dinv[1]), *dCH = h->at<double>(L.dinv[2]);
     {
         RhsElimArgs a;
@@ -752,14 +758,19 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.nchains = phase ? 3 : 2;
         a.pair01 = 1;
         a.coef = nullptr; a.wh = nullptr; a.thh = nullptr; a.th = nullptr;
+        a.w3_out = W; a.w3_hw = h->at<double>(L.hw); a.w3_coef = h->at<cplx>(L.coef);
         LaunchScope ls(h, KC_SOLVE);
         const dim3 g1(col_grid(d), phi3 ? 1 : a.nchains - 1);
-        if (la2) k_subst<2><<<g1, NT_COL, 0, h->st>>>(a);
+        if (w3) {
+            const dim3 g3(col_grid(d), phase ? 2 : 1);
+            if (la2) k_subst3<2><<<g3, NT_COL, 0, h->st>>>(a); else k_subst3<4><<<g3, NT_COL, 0, h->st>>>(a);
+        }
+        else if (la2) k_subst<2><<<g1, NT_COL, 0, h->st>>>(a);
         else k_subst<4><<<g1, NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
 
     }
-    {
+    if (!w3) {
         Elim2Args a;
         a.g = geom(h); a.th = TH; a.w = W; a.phi = PHI; a.dinv_po = dPO; a.dinv_ch = dCH;
         a.hw = h->at<double>(L.hw); a.coef = h->at<cplx>(L.coef); a.lam_phi = c.lam_phi; a.phase = phase;
@@ -774,6 +785,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
             b.shift[0] = 0.0; b.shift[1] = 0.0; b.shift[2] = c.lam_phi;
             b.nchains = 3; b.pair01 = 1;
             b.coef = nullptr; b.wh = nullptr; b.thh = nullptr; b.th = nullptr;
+            b.w3_out = nullptr; b.w3_hw = nullptr; b.w3_coef = nullptr;
             if (walls_gen) { if (la2) k_elim2up<2, true><<<g2, NT_COL, 0, h->st>>>(a, b); else k_elim2up<4, true><<<g2, NT_COL, 0, h->st>>>(a, b); }
             else if (la2) k_elim2up<2, false><<<g2, NT_COL, 0, h->st>>>(a, b);
             else k_elim2up<4, false><<<g2, NT_COL, 0, h->st>>>(a, b);
@@ -783,7 +795,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
         else k_elim2<4, false><<<g2, NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
-    {
+    if (!w3) {
         SubstArgs a;
         a.g = geom(h);
         a.x[0] = W; a.x[1] = PHI; a.x[2] = nullptr;
@@ -792,6 +804,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.nchains = (phase && !phi3) ? 2 : 1;
         a.pair01 = 0;
         a.coef = h->at<cplx>(L.coef); a.wh = h->at<double>(L.wh); a.thh = h->at<double>(L.thh); a.th = TH;
+        a.w3_out = nullptr; a.w3_hw = nullptr; a.w3_coef = nullptr;
         LaunchScope ls(h, KC_SOLVE);
         if (la2) k_subst<2><<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
         else k_subst<4><<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
@@ -803,8 +816,13 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.g = geom(h); a.om = OM; a.th = TH; a.u = U; a.v = V; a.w = W;
         a.phi = phase ? PHI : nullptr; a.phz = PHZ;
         a.tab_phi = phi3 ? h->at<double2>(L.tab_phi) : nullptr;
+        a.tab_w = h->at<double2>(L.tab_w); a.wh = h->at<double>(L.wh); a.thh = h->at<double>(L.thh);
+        a.coef = h->at<cplx>(L.coef); a.th_rw = TH;
         LaunchScope ls(h, KC_SOLVE);
-        if (la2) k_finish<2><<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        // look-ahead 2 at every size: 4 rows of this kernel's eleven operand streams do not fit in registers (measured at
+        // 1024x512x513 / 256x256x257, solve stage: depth 1 3.85-3.91 / 0.29-0.30 ms, depth 2 3.74-3.77 / 0.25 ms)
+        if (w3) k_finish<2, true><<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        else if (la2) k_finish<2><<<col_grid(d), NT_COL, 0, h->st>>>(a);
         else k_finish<4><<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
@@ -895,9 +913,10 @@ cudaError_t build_tables(psdns_handle *h) {
         k_helm_setup<<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
     }
-    if (h->p.phase_field) {   // down-sweep table of the phi solve's upward elimination (kernels_spectral.cuh, ElimUpNeu)
+    for (int t = 0; t < 2; ++t) {   // down-sweep tables of the upward eliminations (kernels_spectral.cuh, ElimUpNeu / ElimUpDir2)
+        if (t == 0 && !h->p.phase_field) continue;
         ElimUpSetupArgs a;
-        a.g = geom(h); a.tab = h->at<double2>(L.tab_phi); a.shift = c.lam_phi;
+        a.g = geom(h); a.tab = h->at<double2>(t == 0 ? L.tab_phi : L.tab_w); a.shift = t == 0 ? c.lam_phi : 0.0;
         LaunchScope ls(h, KC_MISC);
         k_elimup_setup<<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
@@ -1498,6 +1517,8 @@ int psdns_set_option(psdns_handle *h, const char *name, double value) {
     else if (n == "ztma") h->use_ztma = iv != 0;
     else if (n == "zgemm") h->use_zgemm = iv != 0;
     else if (n == "phi3") h->phi3 = iv != 0;
+    else if (n == "w3") h->w3 = iv != 0;
+
     else if (n == "pf" && iv >= 0) h->pf = iv;
     else if (n == "pf_rhs" && iv >= 0) h->pf_rhs = iv;
     else { h->err = "psdns_set_option: unknown option or bad value: " + n; return PSDNS_EINVAL; }

@@ -20,7 +20,10 @@ NX, NY, NZ = I.SCALING_GRIDS["5c"]
 
 
 def _skip_if_small_gpu(nbytes):
+    import gc
     import torch
+    gc.collect()
+    torch.cuda.empty_cache()          # blocks cached by earlier tests are not "in use"
     free, _ = torch.cuda.mem_get_info()
     if free < nbytes:
         pytest.skip(f"needs {nbytes / 2**30:.0f} GiB of free device memory")

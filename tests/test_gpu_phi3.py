@@ -1,7 +1,8 @@
-"""The phi problem in three sweeps (kernels_spectral.cuh, ElimUpNeu: the second Helmholtz solve of the Cahn-Hilliard split
-is eliminated UPWARDS inside the up sweep that produces psi and back-substituted by k_finish on its way down) against the
-five-sweep form of the same solve (`psdns_set_option("phi3", 0)`): both are Gauss eliminations of the same diagonally
-dominant system, so the states agree to rounding - on every variant of the step that carries a phase field.  Parity with
+"""The two-stage problems in three sweeps (kernels_spectral.cuh, ElimUpNeu / ElimUpDir2: the second Helmholtz solve of the
+phi and of the w problem is eliminated UPWARDS inside the up sweep that produces its right-hand side, and back-substituted
+by k_finish on its way down) against the five-sweep form of the same solves (`psdns_set_option("phi3" / "w3", 0)`): both
+are Gauss eliminations of the same diagonally dominant systems, so the states agree to rounding - on every variant of
+the step.  Parity with
 the oracle is covered by the ordinary step tests, which run the default (three-sweep) path."""
 import numpy as np
 import pytest
@@ -19,26 +20,29 @@ CASES = [
     dict(nx=32, ny=64, nz=33, over=dict(wall_top=1, wall_bottom=0)),          # mixed walls
     dict(nx=32, ny=32, nz=33, over=dict(surface_tension_form=1)),             # force form, three-kernel x path
     dict(nx=256, ny=128, nz=129),                               # 11 k columns: the look-ahead depth of small grids
+    dict(nx=64, ny=32, nz=65, cfg=dict(phase_field=0)),         # single-phase: the w problem alone
 ]
 
 
-@pytest.mark.parametrize("case", CASES, ids=lambda c: "%dx%dx%d%s" % (c["nx"], c["ny"], c["nz"], "".join("-" + k for k in c.get("over", {}))))
+@pytest.mark.parametrize("case", CASES, ids=lambda c: "%dx%dx%d%s" % (c["nx"], c["ny"], c["nz"], "".join("-" + k for k in {**c.get("over", {}), **c.get("cfg", {})})))
 def test_three_sweep_phi_equals_five_sweep(case):
     import paper_2406_01322_b200 as P
-    c = I.small_config(nx=case["nx"], ny=case["ny"], nz=case["nz"])
-    st = I.channel_state(c)
+    c = I.small_config(nx=case["nx"], ny=case["ny"], nz=case["nz"], **case.get("cfg", {}))
+    st = [f for f in I.channel_state(c) if f is not None]
     outs = []
-    for opt in (0, 1):
+    for opt in (0, 1, 2):            # five sweeps | phi in three | phi and w in three (the default)
         s = solver_from_config(c, **case.get("over", {}))
-        s.set_option("phi3", opt)
+        s.set_option("phi3", int(opt >= 1))
+        s.set_option("w3", int(opt >= 2))
         s.set_state(P.PHYSICAL, *[to_dev(f) for f in st])
         s.step(4)
         outs.append([to_np(t) for t in s.get_state(P.SPECTRAL)])
         s.close()
     vel = max(float(np.abs(a).max()) for a in outs[0][:3])
-    for name, a, b, scale in zip("uvwp", outs[0], outs[1], (vel, vel, vel, float(np.abs(outs[0][3]).max()))):
-        assert np.all(np.isfinite(b)), name
-        assert float(np.abs(a - b).max()) <= 1e-12 * scale, (name, float(np.abs(a - b).max()), scale)
+    for other in outs[1:]:
+        for name, a, b, scale in zip("uvwp", outs[0], other, (vel, vel, vel, float(np.abs(outs[0][-1]).max()))):
+            assert np.all(np.isfinite(b)), name
+            assert float(np.abs(a - b).max()) <= 1e-12 * scale, (name, float(np.abs(a - b).max()), scale)
 
 
 def test_three_sweep_phi_many_columns():
@@ -50,6 +54,7 @@ def test_three_sweep_phi_many_columns():
     for opt in (0, 1):
         s = solver_from_config(c)
         s.set_option("phi3", opt)
+        s.set_option("w3", opt)
         s.set_state(P.PHYSICAL, *[to_dev(f) for f in st])
         s.step(3)
         outs.append([to_np(t) for t in s.get_state(P.SPECTRAL)])
