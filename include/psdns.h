@@ -231,7 +231,7 @@ int psdns_measure_fp64_peak(psdns_handle *h, double *tflops);
  *   "phi3"     1 (default) / 0 : phase field only: the second Helmholtz solve of the phi problem eliminated upwards inside
  *                                the up sweep that produces psi and back-substituted by the last (downward) sweep - three
  *                                sweeps over the phi column, psi never stored - / the five-sweep form; equal to rounding
- *   "w3"       1 (default) / 0 : no-slip walls: the w problem likewise (its second solve eliminated upwards inside the up
+ *   "w3"       1 (default) / 0 : the w problem likewise (its second solve eliminated upwards inside the up
  *                                sweep of the (omega_z, theta) pair, influence-matrix correction in the last sweep): the
  *                                solver stage is then three launches instead of five; needs "phi3" with a phase field
  * PSDNS_EINVAL on an unknown name or a bad value. */

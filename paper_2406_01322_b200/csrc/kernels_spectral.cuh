@@ -547,27 +547,35 @@ struct ElimUpNeu {   // Neumann rows (sum k^2 u_k = 0 per parity), complex right
 
 // Dirichlet rows (sum u_k = 0 per parity) plus the k^2-weighted functional of the solution: the w problem
 // (D^2 - k^2) w = theta_p, whose influence-matrix coefficient needs sum k^2 w_p per parity (k_elim2 / ElimDown::second).
+template <bool GEN = false>   // GEN: also the k^2 (k^2 - 1) / 3 functional (T_k''(+-1): free-slip walls, row f3)
 struct ElimUpDir2 {
     PivotUp pv;
     cplx gm2, gm1;            // g''_{k-2}, g''_{k-1}
     double ym2, ym1;          // adjoint of the boundary row (weights 1)
     double sm2, sm1;          // adjoint of the second functional (weights k^2)
-    cplx Je, Jo, Ke, Ko;      // sum y_k g''_k, sum s_k g''_k per parity
-    double Ee, Eo, Fe, Fo;    // sum y_k e_k, sum s_k e_k per parity
+    double tm2, tm1;          // GEN: adjoint of the third functional (weights k^2 (k^2 - 1) / 3)
+    cplx Je, Jo, Ke, Ko, Me, Mo;      // sum y_k g''_k, sum s_k g''_k, sum t_k g''_k per parity
+    double Ee, Eo, Fe, Fo, Ge, Go;    // sum y_k e_k, sum s_k e_k, sum t_k e_k per parity
     __device__ __forceinline__ void init() {
         pv.init();
-        gm2 = gm1 = Je = Jo = Ke = Ko = cz();
-        ym2 = ym1 = sm2 = sm1 = Ee = Eo = Fe = Fo = 0.0;
+        gm2 = gm1 = Je = Jo = Ke = Ko = Me = Mo = cz();
+        ym2 = ym1 = sm2 = sm1 = tm2 = tm1 = Ee = Eo = Fe = Fo = Ge = Go = 0.0;
     }
     __device__ __forceinline__ cplx row(int k, int N, double sigma, cplx fm2, cplx f0, cplx fp2) {
         double m, e, c, cm2;
         const double di = pv.step(k, N, sigma, m, e, c, cm2);
         cplx g = cfma(helm_p(k), fm2, cfma(helm_q(k), f0, cscale(fp2, helm_r(k))));
         g = cfma(-m, gm2, g);
+        const double k2 = (double)k * k;
         const double y = (1.0 - cm2 * ym2) * di;
-        const double sq = ((double)k * k - cm2 * sm2) * di;
+        const double sq = (k2 - cm2 * sm2) * di;
         if (k & 1) { Jo = cfma(y, g, Jo); Eo = fma(y, e, Eo); Ko = cfma(sq, g, Ko); Fo = fma(sq, e, Fo); }
         else       { Je = cfma(y, g, Je); Ee = fma(y, e, Ee); Ke = cfma(sq, g, Ke); Fe = fma(sq, e, Fe); }
+        if (GEN) {
+            const double t = (k2 * (k2 - 1.0) * (1.0 / 3.0) - cm2 * tm2) * di;
+            if (k & 1) { Mo = cfma(t, g, Mo); Go = fma(t, e, Go); } else { Me = cfma(t, g, Me); Ge = fma(t, e, Ge); }
+            tm2 = tm1; tm1 = t;
+        }
         gm2 = gm1; gm1 = g;
         ym2 = ym1; ym1 = y;
         sm2 = sm1; sm1 = sq;
@@ -579,6 +587,11 @@ struct ElimUpDir2 {
         u1 = cscale(Jo, -1.0 / (1.0 + Eo));
         de = cfma(Fe, u0, Ke);                   // 0^2 u_0 + K_e + u_0 F_e
         dodd = cadd(u1, cfma(Fo, u1, Ko));       // 1^2 u_1 + K_o + u_1 F_o
+    }
+    // GEN: its k^2 (k^2 - 1) / 3 - weighted parity sums (the weights of k = 0, 1 vanish)
+    __device__ __forceinline__ void third(cplx u0, cplx u1, cplx &me, cplx &mo) const {
+        me = cfma(Ge, u0, Me);
+        mo = cfma(Go, u1, Mo);
     }
 };
 
@@ -840,8 +853,9 @@ struct SubstArgs {
     cplx *th;
     // W3 (three-sweep w problem): the pair's theta_p rows feed the upward elimination of (D^2 - k^2) w = theta_p
     cplx *w3_out;               // g^ of that elimination (slots 0, 1 = w_p,0, w_p,1)
-    const double *w3_hw;        // [2][ncols]: sum k^2 w_h per parity
+    const double *w3_hw;        // [4][ncols]: sum k^2 w_h per parity, then sum k^2 (k^2 - 1)/3 w_h (k_hom_tables)
     cplx *w3_coef;              // [2][ncols] out: influence-matrix coefficients A_e, A_o
+    int wall_top, wall_bot;     // GEN: 0 = no-slip (Dw = 0), 1 = free-slip (D^2 w = 0)
 };
 
 // The sweeps work in place, so the compiler cannot move the load of row k + 1 above the store of row k (same
@@ -853,7 +867,7 @@ struct SubstArgs {
 
 // UP: the psi chain (chain 2 of the first substitution) does not store psi but feeds it, row by row, into the upward
 // elimination of the phi solve (ElimUpNeu) and stores g^_k of that solve instead; k_finish completes it on its way down.
-template <int G, bool UP, bool W3 = false>
+template <int G, bool UP, bool W3 = false, bool GEN = false>
 __device__ __forceinline__ void subst_body(const SubstArgs &a, int by) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
@@ -868,7 +882,7 @@ __device__ __forceinline__ void subst_body(const SubstArgs &a, int by) {
         cplx *x0 = a.x[0] + col, *x1 = a.x[1] + col;
         const double *__restrict__ dinv = a.dinv[0] + col;
         cplx um2 = x0[0], um1 = x0[st], vm2 = x1[0], vm1 = x1[st];
-        ElimUpDir2 ew;
+        ElimUpDir2<GEN> ew;
         cplx w4 = cz(), w3 = cz(), w2 = vm2, w1 = vm1;      // F(k-4) .. F(k-1) of the w solve's right-hand side theta_p
         const double k2w = kx * kx + ky * ky;
         cplx *wout = W3 ? a.w3_out + col : nullptr;
@@ -917,8 +931,27 @@ __device__ __forceinline__ void subst_body(const SubstArgs &a, int by) {
             ew.finish(u0, u1, de, dodd);
             wout[0] = u0; wout[st] = u1;
             const bool off = (col == 0);
-            a.w3_coef[col] = off ? cz() : cscale(de, -1.0 / a.w3_hw[col]);
-            a.w3_coef[st + col] = off ? cz() : cscale(dodd, -1.0 / a.w3_hw[st + col]);
+            if (!GEN) {
+                a.w3_coef[col] = off ? cz() : cscale(de, -1.0 / a.w3_hw[col]);
+                a.w3_coef[st + col] = off ? cz() : cscale(dodd, -1.0 / a.w3_hw[st + col]);
+            } else {     // per wall Dw = 0 (no-slip) or D^2 w = 0 (free-slip): the 2 x 2 closure of k_elim2<., true>
+                cplx me, mo;
+                ew.third(u0, u1, me, mo);
+                const double Keh = a.w3_hw[col], Koh = a.w3_hw[st + col], Meh = a.w3_hw[2 * st + col], Moh = a.w3_hw[3 * st + col];
+                cplx Ae, Ao;
+                if (a.wall_top == 1 && a.wall_bot == 1) { Ae = cscale(me, -1.0 / Meh); Ao = cscale(mo, -1.0 / Moh); }
+                else {
+                    double a11, a12, a21, a22;
+                    cplx b1, b2;
+                    if (a.wall_top == 1) { a11 = Meh; a12 = Moh; b1 = cscale(cadd(me, mo), -1.0); a21 = -Keh; a22 = Koh; b2 = csub(de, dodd); }
+                    else                 { a11 = Keh; a12 = Koh; b1 = cscale(cadd(de, dodd), -1.0); a21 = Meh; a22 = -Moh; b2 = cscale(csub(me, mo), -1.0); }
+                    const double idet = 1.0 / (a11 * a22 - a12 * a21);
+                    Ae = cscale(csub(cscale(b1, a22), cscale(b2, a12)), idet);
+                    Ao = cscale(csub(cscale(b2, a11), cscale(b1, a21)), idet);
+                }
+                a.w3_coef[col] = off ? cz() : Ae;
+                a.w3_coef[st + col] = off ? cz() : Ao;
+            }
         }
         return;
     }
@@ -1001,9 +1034,9 @@ __global__ void __launch_bounds__(NT_COL) k_subst(const __grid_constant__ SubstA
 // Three-sweep form of both two-stage problems: block row 0 = the (omega_z, theta_p) pair, whose theta_p rows also feed the
 // upward elimination of the w solve (ElimUpDir2); block row 1 (phase field) = the psi chain feeding the upward
 // elimination of the phi solve (ElimUpNeu).  k_finish<., true> back-substitutes both on its way down.
-template <int G>
+template <int G, bool GEN = false>
 __global__ void __launch_bounds__(NT_COL) k_subst3(const __grid_constant__ SubstArgs a) {
-    if (blockIdx.y == 0) subst_body<G, false, true>(a, 0);
+    if (blockIdx.y == 0) subst_body<G, false, true, GEN>(a, 0);
     else subst_body<G, true>(a, 0);
 }
 

@@ -108,7 +108,7 @@ struct psdns_handle {
     int grid_cap;               // psdns_set_option("grid_cap"): upper bound on the grid of every persistent kernel (0 = none)
     int pf, pf_rhs;             // L2 prefetch distances of the column sweeps, in rows
     bool phi3 = true;           // phi problem in three sweeps (ElimUpNeu)
-    bool w3 = true;             // w problem in three sweeps (ElimUpDir2; no-slip walls, needs phi3 with a phase field)
+    bool w3 = true;             // w problem in three sweeps (ElimUpDir2; needs phi3 with a phase field)
     long long last_grid[KC_COUNT], last_items[KC_COUNT];   // grid / work items of the last launch of each persistent class
 
     int persistent_grid(int kc, long long items, int occ) {
@@ -722,9 +722,9 @@ cudaError_t enqueue_step(psdns_handle *h) {
     // phi problem in three sweeps: its second solve is eliminated upwards inside the first substitution (psi never stored)
     // and back-substituted by k_finish on its way down (ElimUpNeu); phi3 = 0 keeps the five-sweep form for cross-checks
     const bool phi3 = phase && h->phi3;
-    // w problem likewise (ElimUpDir2; no-slip walls): the solver stage is then three launches - k_rhs_elim (down),
+    // w problem likewise (ElimUpDir2): the solver stage is then three launches - k_rhs_elim (down),
     // k_subst3 (up), k_finish (down) - instead of five
-    const bool w3 = h->w3 && !walls_gen && (!phase || phi3);
+    const bool w3 = h->w3 && (!phase || phi3);
     const double *dNS = h->at<double>(L.dinv[0]), *dPO = h->at<double>(L.dinv[1]), *dCH = h->at<double>(L.dinv[2]);
     {
         RhsElimArgs a;
@@ -759,11 +759,13 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.pair01 = 1;
         a.coef = nullptr; a.wh = nullptr; a.thh = nullptr; a.th = nullptr;
         a.w3_out = W; a.w3_hw = h->at<double>(L.hw); a.w3_coef = h->at<cplx>(L.coef);
+        a.wall_top = p.wall_top; a.wall_bot = p.wall_bottom;
         LaunchScope ls(h, KC_SOLVE);
         const dim3 g1(col_grid(d), phi3 ? 1 : a.nchains - 1);
         if (w3) {
             const dim3 g3(col_grid(d), phase ? 2 : 1);
-            if (la2) k_subst3<2><<<g3, NT_COL, 0, h->st>>>(a); else k_subst3<4><<<g3, NT_COL, 0, h->st>>>(a);
+            if (walls_gen) { if (la2) k_subst3<2, true><<<g3, NT_COL, 0, h->st>>>(a); else k_subst3<4, true><<<g3, NT_COL, 0, h->st>>>(a); }
+            else if (la2) k_subst3<2><<<g3, NT_COL, 0, h->st>>>(a); else k_subst3<4><<<g3, NT_COL, 0, h->st>>>(a);
         }
         else if (la2) k_subst<2><<<g1, NT_COL, 0, h->st>>>(a);
         else k_subst<4><<<g1, NT_COL, 0, h->st>>>(a);
@@ -785,7 +787,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
             b.shift[0] = 0.0; b.shift[1] = 0.0; b.shift[2] = c.lam_phi;
             b.nchains = 3; b.pair01 = 1;
             b.coef = nullptr; b.wh = nullptr; b.thh = nullptr; b.th = nullptr;
-            b.w3_out = nullptr; b.w3_hw = nullptr; b.w3_coef = nullptr;
+            b.w3_out = nullptr; b.w3_hw = nullptr; b.w3_coef = nullptr; b.wall_top = 0; b.wall_bot = 0;
             if (walls_gen) { if (la2) k_elim2up<2, true><<<g2, NT_COL, 0, h->st>>>(a, b); else k_elim2up<4, true><<<g2, NT_COL, 0, h->st>>>(a, b); }
             else if (la2) k_elim2up<2, false><<<g2, NT_COL, 0, h->st>>>(a, b);
             else k_elim2up<4, false><<<g2, NT_COL, 0, h->st>>>(a, b);
@@ -804,7 +806,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.nchains = (phase && !phi3) ? 2 : 1;
         a.pair01 = 0;
         a.coef = h->at<cplx>(L.coef); a.wh = h->at<double>(L.wh); a.thh = h->at<double>(L.thh); a.th = TH;
-        a.w3_out = nullptr; a.w3_hw = nullptr; a.w3_coef = nullptr;
+        a.w3_out = nullptr; a.w3_hw = nullptr; a.w3_coef = nullptr; a.wall_top = 0; a.wall_bot = 0;
         LaunchScope ls(h, KC_SOLVE);
         if (la2) k_subst<2><<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);
         else k_subst<4><<<dim3(col_grid(d), a.nchains), NT_COL, 0, h->st>>>(a);

@@ -17,7 +17,9 @@ CASES = [
     dict(nx=16, ny=16, nz=9),                                   # shortest column: rows 2..8 only
     dict(nx=64, ny=16, nz=65),
     dict(nx=128, ny=64, nz=129, over=dict(visc_ratio=0.5)),     # variable viscosity (k_xfusedv)
-    dict(nx=32, ny=64, nz=33, over=dict(wall_top=1, wall_bottom=0)),          # mixed walls
+    dict(nx=32, ny=64, nz=33, over=dict(wall_top=1, wall_bottom=0)),          # mixed walls: 2 x 2 influence closure
+    dict(nx=64, ny=32, nz=33, over=dict(wall_top=0, wall_bottom=1)),
+    dict(nx=32, ny=32, nz=65, over=dict(wall_top=1, wall_bottom=1)),          # free-slip at both walls
     dict(nx=32, ny=32, nz=33, over=dict(surface_tension_form=1)),             # force form, three-kernel x path
     dict(nx=256, ny=128, nz=129),                               # 11 k columns: the look-ahead depth of small grids
     dict(nx=64, ny=32, nz=65, cfg=dict(phase_field=0)),         # single-phase: the w problem alone
