@@ -234,6 +234,9 @@ int psdns_measure_fp64_peak(psdns_handle *h, double *tflops);
  *   "w3"       1 (default) / 0 : the w problem likewise (its second solve eliminated upwards inside the up
  *                                sweep of the (omega_z, theta) pair, influence-matrix correction in the last sweep): the
  *                                solver stage is then three launches instead of five; needs "phi3" with a phase field
+ *   "lazy"     1 (default) / 0 : with "w3": the influence-matrix correction of the hidden state theta^ is not written back
+ *                                by the last sweep but applied by the next step's right-hand-side kernel where it reads
+ *                                theta^ anyway (psdns_get_history and psdns_set_option materialise it first) / written back
  * PSDNS_EINVAL on an unknown name or a bad value. */
 int psdns_set_option(psdns_handle *h, const char *name, double value);
 

@@ -641,6 +641,8 @@ struct RhsElimArgs {
     double dt, gamma, inv_pe, e_phi, gradp, lam_phi, gam_phi;
     int phase;
     int wall_top, wall_bot;           // 0 = no-slip, 1 = free-slip
+    const double *thh;                // LAZY: real homogeneous solution theta_h [nz][ncols]
+    const cplx *coef;                 // LAZY: [2][ncols] influence-matrix coefficients of the last step (0 after set_state)
 };
 
 constexpr int RHS_COLS = 32;   // columns per CTA of k_rhs_elim (blockDim = 32 * number of chains)
@@ -651,7 +653,10 @@ constexpr int RHS_COLS = 32;   // columns per CTA of k_rhs_elim (blockDim = 32 *
 // GEN: walls that are not both no-slip (row f3).  FORCE: the surface tension enters as a force vector F next to the flux
 // tensor: N_omega += i (kx F_y - ky F_x), N_w += -k^2 F_z - D (i kx F_x + i ky F_y), S-bar += F(0,0).
 // <false, false> is the product path, unchanged.
-template <bool GEN, bool FORCE>
+// LAZY: theta^n in memory is the particular solution theta_p of the last step; its influence-matrix correction
+// A_par theta_h (the coefficients are still in a.coef) is applied here, where theta^n is read anyway, instead of by a
+// read-modify-write of the whole array in k_finish (three-sweep form).
+template <bool GEN, bool FORCE, bool LAZY = false>
 __global__ void __launch_bounds__(96, (FORCE ? 3 : RHS_MINB)) k_rhs_elim(const __grid_constant__ RhsElimArgs a) {
     const ColGeom &g = a.g;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -679,12 +684,18 @@ __global__ void __launch_bounds__(96, (FORCE ? 3 : RHS_MINB)) k_rhs_elim(const _
         double *xo = reinterpret_cast<double *>(a.om + col) + c, *xt = reinterpret_cast<double *>(a.th + col) + c;
         double *ho = reinterpret_cast<double *>(a.h_om + col) + c, *hw = reinterpret_cast<double *>(a.h_w + col) + c;
         const size_t st2 = 2 * st;
-        struct RowIn { double xo, xt, ho, hw, t0, t1, t3; cplx t2, t4; cplx f0, f1; double f2; };
+        struct RowIn { double xo, xt, ho, hw, t0, t1, t3; cplx t2, t4; cplx f0, f1; double f2; double thh; };
         PivotDown pv;
         pv.init();
+        double lazy_e = 0.0, lazy_o = 0.0;
+        if (LAZY) {
+            lazy_e = reinterpret_cast<const double *>(a.coef + col)[c];
+            lazy_o = reinterpret_cast<const double *>(a.coef + st + col)[c];
+        }
         auto load = [&](int n) {
             RowIn r;
             r.xo = xo[n * st2]; r.xt = xt[n * st2];
+            if (LAZY) r.thh = a.thh[n * st + col];
             r.ho = r.hw = r.t0 = r.t1 = r.t3 = 0.0; r.t2 = r.t4 = cz();
             if (n < nkz) {
                 const size_t o = n * st;
@@ -710,11 +721,13 @@ __global__ void __launch_bounds__(96, (FORCE ? 3 : RHS_MINB)) k_rhs_elim(const _
         el.init();
         RowIn nx = load(N);
         for (int n = N; n >= 0; --n) {
-            const RowIn r = nx;
+            RowIn r = nx;
             if (n > 0) nx = load(n - 1);
+            if (LAZY) r.xt = fma(r.thh, (n & 1) ? lazy_o : lazy_e, r.xt);     // theta^n = theta_p + A_par theta_h
             const int np = n - g.pf_rhs;
             if (np >= 0 && c == 0) {
                 pf_l2(a.om + col + np * st); pf_l2(a.th + col + np * st);
+                if (LAZY) pf_l2(a.thh + col + np * st);
                 if (np < nkz) {
                     pf_l2(txz + np * st); pf_l2(txx + np * st); pf_l2(txy + np * st); pf_l2(tyy + np * st); pf_l2(tyz + np * st);
                     pf_l2(a.h_om + col + np * st); pf_l2(a.h_w + col + np * st);
@@ -1205,7 +1218,8 @@ struct FinishArgs {
     cplx *th_rw;
 };
 
-template <int G, bool W3 = false>
+// LZ (with W3): theta^ is left as theta_p; the next step's k_rhs_elim<., ., true> applies A_par theta_h where it reads theta^.
+template <int G, bool W3 = false, bool LZ = false>
 __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ FinishArgs a) {
     const ColGeom &g = a.g;
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
@@ -1239,7 +1253,9 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
                 if (upphi && n >= 2) r[i].tb = a.tab_phi[o];
                 if (W3) {
                     if (n >= 2) r[i].tw = a.tab_w[o];
-                    r[i].whv = a.wh[o]; r[i].thhv = a.thh[o]; r[i].thv = a.th_rw[o];
+                    r[i].whv = a.wh[o];
+                    if (!LZ) { r[i].thhv = a.thh[o]; r[i].thv = a.th_rw[o]; }
+                    else if (mean) r[i].thv = a.th_rw[o];
                 } else if (mean) r[i].w = a.th[o];       // column (0,0): v-bar lives in the theta slot
             }
         }
@@ -1258,7 +1274,7 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
                 pf_l2(a.w + op); pf_l2(a.om + op);
                 if (phase && (upphi || np < g.nkz)) pf_l2(a.phi + op);
                 if (upphi) pf_l2(a.tab_phi + op);
-                if (W3) { pf_l2(a.tab_w + op); pf_l2(a.wh + op); pf_l2(a.thh + op); pf_l2(a.th_rw + op); }
+                if (W3) { pf_l2(a.tab_w + op); pf_l2(a.wh + op); if (!LZ) { pf_l2(a.thh + op); pf_l2(a.th_rw + op); } }
             }
         }
 #pragma unroll
@@ -1282,7 +1298,7 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
                 wp2 = wp1; wp1 = wv;
                 const cplx A = (n & 1) ? Ao : Ae;
                 wv = cfma(q[i].whv, A, wv);
-                if (!mean) { a.w[o] = wv; a.th_rw[o] = cfma(q[i].thhv, A, q[i].thv); }
+                if (!mean) { a.w[o] = wv; if (!LZ) a.th_rw[o] = cfma(q[i].thhv, A, q[i].thv); }
                 else wv = q[i].thv;                       // column (0,0): v-bar lives in the theta slot
             }
             if (mean) {   // mean flow: u-bar from the omega slot, v-bar from the theta slot, w = 0 (reading S12)
@@ -1299,6 +1315,21 @@ __global__ void __launch_bounds__(NT_COL) k_finish(const __grid_constant__ Finis
 #pragma unroll
         for (int i = 0; i < G; ++i) q[i] = nx[i];
     }
+}
+
+// ---- pending influence-matrix correction of theta^ (three-sweep form with LZ): theta += A_par theta_h, then A := 0 --------
+__global__ void __launch_bounds__(NT_COL) k_theta_apply(const __grid_constant__ ColGeom g, cplx *__restrict__ th,
+                                                        const double *__restrict__ thh, cplx *__restrict__ coef) {
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= g.ncols) return;
+    const size_t st = g.ncols;
+    const cplx Ae = coef[col], Ao = coef[st + col];
+    for (int n = 0; n <= g.N; ++n) {
+        const size_t o = n * st + col;
+        th[o] = cfma(thh[o], (n & 1) ? Ao : Ae, th[o]);      // the same fma per component as k_rhs_elim<., ., true>
+    }
+    coef[col] = cz();
+    coef[st + col] = cz();
 }
 
 // ---- per-step bookkeeping ---------------------------------------------------------------------------

@@ -108,6 +108,8 @@ struct psdns_handle {
     int grid_cap;               // psdns_set_option("grid_cap"): upper bound on the grid of every persistent kernel (0 = none)
     int pf, pf_rhs;             // L2 prefetch distances of the column sweeps, in rows
     bool phi3 = true;           // phi problem in three sweeps (ElimUpNeu)
+    bool lazy = true;           // with w3: theta^ stays theta_p, corrected where the next step reads it
+    bool th_pending = false;    // theta^ in memory lacks the influence-matrix correction of the last step (coef holds it)
     bool w3 = true;             // w problem in three sweeps (ElimUpDir2; needs phi3 with a phase field)
     long long last_grid[KC_COUNT], last_items[KC_COUNT];   // grid / work items of the last launch of each persistent class
 
@@ -725,6 +727,7 @@ cudaError_t enqueue_step(psdns_handle *h) {
     // w problem likewise (ElimUpDir2): the solver stage is then three launches - k_rhs_elim (down),
     // k_subst3 (up), k_finish (down) - instead of five
     const bool w3 = h->w3 && (!phase || phi3);
+    const bool lazy = w3 && h->lazy;   // theta^'s influence-matrix correction deferred to the next step's k_rhs_elim
     const double *dNS = h->at<double>(L.dinv[0]), *dPO = h->at<double>(L.dinv[1]), *dCH = h->at<double>(L.dinv[2]);
     {
         RhsElimArgs a;
@@ -741,10 +744,17 @@ cudaError_t enqueue_step(psdns_handle *h) {
         a.e_phi = 1.0 + c.s_coef * p.ch * p.ch;
         a.gradp = p.gradp_x; a.lam_phi = c.lam_phi; a.gam_phi = c.gam_phi; a.phase = phase;
         a.wall_top = p.wall_top; a.wall_bot = p.wall_bottom;
+        a.thh = h->at<double>(L.thh); a.coef = h->at<cplx>(L.coef);
         const int grid = (int)((d.ncols + RHS_COLS - 1) / RHS_COLS);
         LaunchScope ls(h, KC_RHS);
         const int nt = 32 * (phase ? 3 : 2);
-        if (force) { if (walls_gen) k_rhs_elim<true, true><<<grid, nt, 0, h->st>>>(a); else k_rhs_elim<false, true><<<grid, nt, 0, h->st>>>(a); }
+        // lazy: theta^n is still the particular solution of the last step; its influence-matrix correction is applied here
+        if (lazy) {
+            if (force) { if (walls_gen) k_rhs_elim<true, true, true><<<grid, nt, 0, h->st>>>(a); else k_rhs_elim<false, true, true><<<grid, nt, 0, h->st>>>(a); }
+            else if (walls_gen) k_rhs_elim<true, false, true><<<grid, nt, 0, h->st>>>(a);
+            else k_rhs_elim<false, false, true><<<grid, nt, 0, h->st>>>(a);
+        }
+        else if (force) { if (walls_gen) k_rhs_elim<true, true><<<grid, nt, 0, h->st>>>(a); else k_rhs_elim<false, true><<<grid, nt, 0, h->st>>>(a); }
         else if (walls_gen) k_rhs_elim<true, false><<<grid, nt, 0, h->st>>>(a);
         else k_rhs_elim<false, false><<<grid, nt, 0, h->st>>>(a);
         CU(cudaGetLastError());
@@ -823,7 +833,8 @@ cudaError_t enqueue_step(psdns_handle *h) {
         LaunchScope ls(h, KC_SOLVE);
         // look-ahead 2 at every size: 4 rows of this kernel's eleven operand streams do not fit in registers (measured at
         // 1024x512x513 / 256x256x257, solve stage: depth 1 3.85-3.91 / 0.29-0.30 ms, depth 2 3.74-3.77 / 0.25 ms)
-        if (w3) k_finish<2, true><<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        if (w3 && lazy) k_finish<2, true, true><<<col_grid(d), NT_COL, 0, h->st>>>(a);
+        else if (w3) k_finish<2, true><<<col_grid(d), NT_COL, 0, h->st>>>(a);
         else if (la2) k_finish<2><<<col_grid(d), NT_COL, 0, h->st>>>(a);
         else k_finish<4><<<col_grid(d), NT_COL, 0, h->st>>>(a);
         CU(cudaGetLastError());
@@ -959,7 +970,20 @@ int finish_set_state(psdns_handle *h) {
     }
     for (int i = 0; i < 3; ++i) CUDA_TRY(h, cudaMemsetAsync(h->ws + L.hist[i], 0, d.s_low * sizeof(cplx), h->st));
     CUDA_TRY(h, cudaMemsetAsync(h->ws + L.small, 0, 64, h->st));
+    CUDA_TRY(h, cudaMemsetAsync(h->ws + L.coef, 0, 2 * d.ncols * sizeof(cplx), h->st));   // no pending theta correction
+    h->th_pending = false;
     h->has_state = true;
+    return PSDNS_OK;
+}
+
+// theta^ of the three-sweep form is corrected lazily (k_rhs_elim<., ., true>); whoever needs the array itself calls this
+int materialise_theta(psdns_handle *h) {
+    if (!h->th_pending) return PSDNS_OK;
+    LaunchScope ls(h, KC_MISC);
+    k_theta_apply<<<col_grid(h->d), NT_COL, 0, h->st>>>(geom(h), h->at<cplx>(h->L.state[4]), h->at<double>(h->L.thh),
+                                                      h->at<cplx>(h->L.coef));
+    CUDA_TRY(h, cudaGetLastError());
+    h->th_pending = false;
     return PSDNS_OK;
 }
 
@@ -1101,6 +1125,8 @@ int psdns_step(psdns_handle *h, int nsteps) {
     if (nsteps < 0) { h->err = "psdns_step: nsteps < 0"; return PSDNS_EINVAL; }
     if (!h->p.dealias) { h->err = "psdns_step: dealias must be 1 (2/3 rule, reading S3)"; return PSDNS_EINVAL; }
     if (!h->has_state) { h->err = "psdns_step: no state set"; return PSDNS_ESTATE; }
+    // the three-sweep solver with the lazy correction leaves theta^ as theta_p + (its coefficients): see materialise_theta
+    if (nsteps > 0 && h->lazy && h->w3 && (!h->p.phase_field || h->phi3)) h->th_pending = true;
     const bool direct = !h->use_graph || h->timed_class >= 0;
     if (direct) {
         for (int i = 0; i < nsteps; ++i) CUDA_TRY(h, enqueue_step(h));
@@ -1218,6 +1244,7 @@ int psdns_get_history(psdns_handle *h, void *d_blob, size_t bytes) {
     if (!h) return PSDNS_EINVAL;
     if (!d_blob || bytes != psdns_history_bytes(h)) { h->err = "psdns_get_history: null blob or size mismatch"; return PSDNS_EINVAL; }
     if (!h->has_state) { h->err = "psdns_get_history: no state set"; return PSDNS_ESTATE; }
+    { const int rc = materialise_theta(h); if (rc != PSDNS_OK) return rc; }
     HistPiece pc[8];
     const int n = hist_pieces(h, pc);
     size_t o = 0;
@@ -1239,6 +1266,8 @@ int psdns_set_history(psdns_handle *h, const void *d_blob, size_t bytes) {
         CUDA_TRY(h, cudaMemcpyAsync(h->ws + pc[i].off, (const char *)d_blob + o, pc[i].bytes, cudaMemcpyDeviceToDevice, h->st));
         o += align_up(pc[i].bytes);
     }
+    CUDA_TRY(h, cudaMemsetAsync(h->ws + h->L.coef, 0, 2 * h->d.ncols * sizeof(cplx), h->st));   // the blob's theta^ is complete
+    h->th_pending = false;
     return PSDNS_OK;
 }
 
@@ -1506,6 +1535,11 @@ int psdns_set_option(psdns_handle *h, const char *name, double value) {
     if (!h || !name) return PSDNS_EINVAL;
     const std::string n(name);
     const int iv = (int)value;
+    if (h->has_state) {   // the options choose who corrects theta^: complete it now, and leave no stale coefficients behind
+        const int rc = materialise_theta(h);
+        if (rc != PSDNS_OK) return rc;
+        CUDA_TRY(h, cudaMemsetAsync(h->ws + h->L.coef, 0, 2 * h->d.ncols * sizeof(cplx), h->st));
+    }
     if (n == "graph") h->use_graph = iv != 0;
     else if (n == "xfuse" && iv && ((h->p.phase_field && h->p.surface_tension_form == 1) || h->p.convection_form == 1)) {
         h->err = "psdns_set_option: the alternative non-linear forms have no fused x kernel";
@@ -1520,6 +1554,7 @@ int psdns_set_option(psdns_handle *h, const char *name, double value) {
     else if (n == "zgemm") h->use_zgemm = iv != 0;
     else if (n == "phi3") h->phi3 = iv != 0;
     else if (n == "w3") h->w3 = iv != 0;
+    else if (n == "lazy") h->lazy = iv != 0;
 
     else if (n == "pf" && iv >= 0) h->pf = iv;
     else if (n == "pf_rhs" && iv >= 0) h->pf_rhs = iv;

@@ -32,10 +32,11 @@ def test_three_sweep_phi_equals_five_sweep(case):
     c = I.small_config(nx=case["nx"], ny=case["ny"], nz=case["nz"], **case.get("cfg", {}))
     st = [f for f in I.channel_state(c) if f is not None]
     outs = []
-    for opt in (0, 1, 2):            # five sweeps | phi in three | phi and w in three (the default)
+    for opt in (0, 1, 2, 3):         # five sweeps | phi in three | phi and w in three | + lazy theta correction (the default)
         s = solver_from_config(c, **case.get("over", {}))
         s.set_option("phi3", int(opt >= 1))
         s.set_option("w3", int(opt >= 2))
+        s.set_option("lazy", int(opt >= 3))
         s.set_state(P.PHYSICAL, *[to_dev(f) for f in st])
         s.step(4)
         outs.append([to_np(t) for t in s.get_state(P.SPECTRAL)])
@@ -63,3 +64,48 @@ def test_three_sweep_phi_many_columns():
         s.close()
     for a, b in zip(*outs):
         assert float(np.abs(a - b).max()) <= 1e-12 * max(float(np.abs(a).max()), 1.0)
+
+
+def test_lazy_theta_correction_survives_restart_and_option_changes():
+    """The three-sweep form leaves theta^ = theta_p + (coefficients of A_par theta_h) between steps.  psdns_get_history must
+    hand out the completed theta^ (bit-exact restart), and changing an option in the middle of a run must not lose or
+    double the pending correction."""
+    import torch
+    import paper_2406_01322_b200 as P
+    c = I.small_config(nx=64, ny=32, nz=33)
+    st = I.channel_state(c)
+
+    def fresh():
+        s = solver_from_config(c)
+        s.set_state(P.PHYSICAL, *[to_dev(f) for f in st])
+        return s
+
+    a = fresh()
+    a.step(6)
+    ref = [to_np(t) for t in a.get_state(P.SPECTRAL)]
+    a.close()
+    # restart in the middle through the history blob
+    b = fresh()
+    b.step(3)
+    blob = b.get_history()
+    mid = [t.clone() for t in b.get_state(P.SPECTRAL)]
+    b.step(3)
+    cont = [to_np(t) for t in b.get_state(P.SPECTRAL)]
+    b.close()
+    r = solver_from_config(c)
+    r.set_state(P.SPECTRAL, *mid)
+    r.set_history(blob)
+    r.step(3)
+    rest = [to_np(t) for t in r.get_state(P.SPECTRAL)]
+    r.close()
+    for x, y, z in zip(ref, cont, rest):
+        assert np.array_equal(x, y)            # taking the blob does not disturb the run
+        assert np.array_equal(y, z)            # and the restart is bit-exact
+    # switch the lazy correction off and on again in mid-run: rounding-level agreement with the plain run
+    d = fresh()
+    d.step(2); d.set_option("lazy", 0); d.step(2); d.set_option("w3", 0); d.step(1); d.set_option("w3", 1); d.set_option("lazy", 1); d.step(1)
+    mixed = [to_np(t) for t in d.get_state(P.SPECTRAL)]
+    d.close()
+    vel = max(float(np.abs(x).max()) for x in ref[:3])
+    for x, y, scale in zip(ref, mixed, (vel, vel, vel, float(np.abs(ref[3]).max()))):
+        assert float(np.abs(x - y).max()) <= 1e-12 * scale
