@@ -31,7 +31,7 @@ import numpy as np  # noqa: E402
 import psdns_inputs as I  # noqa: E402
 
 METRIC = "grid-point-steps/s"
-TRAFFIC_CSV = "r2d_traffic_5c.csv"   # ncu dram bytes per launch and kernel class, written from the --set full capture
+TRAFFIC_CSV = "r2e_traffic_5c.csv"   # ncu dram bytes per launch and kernel class, written from the --set full capture
 
 
 # ------------------------------------------------------------------------------------------------
