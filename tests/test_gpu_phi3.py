@@ -109,3 +109,19 @@ def test_lazy_theta_correction_survives_restart_and_option_changes():
     vel = max(float(np.abs(x).max()) for x in ref[:3])
     for x, y, scale in zip(ref, mixed, (vel, vel, vel, float(np.abs(ref[3]).max()))):
         assert float(np.abs(x - y).max()) <= 1e-12 * scale
+
+
+def test_launches_per_step():
+    """One step of the default (three-sweep) path is nine launches in the captured graph: k_begin_step, z / y backward,
+    fused x, y / z forward, k_rhs_elim, k_subst3, k_finish; the five-sweep form has two more."""
+    import paper_2406_01322_b200 as P
+    c = I.small_config(nx=32, ny=32, nz=33)
+    st = I.channel_state(c)
+    for opts, want in (({}, 9), ({"w3": 0}, 11), ({"w3": 0, "phi3": 0}, 11)):
+        s = solver_from_config(c)
+        for k, v in opts.items():
+            s.set_option(k, v)
+        s.set_state(P.PHYSICAL, *[to_dev(f) for f in st])
+        s.step(2)
+        assert int(s.get_info("launches_per_step")) == want, (opts, s.get_info("launches_per_step"))
+        s.close()
