@@ -119,6 +119,9 @@ int psdns_get_state(psdns_handle *h, int space, void *d_u, void *d_v, void *d_w,
  * later, on a handle of the same grid and params: psdns_set_state(PSDNS_SPECTRAL, state) then
  * psdns_set_history(blob) - the following steps are bit-identical to the uninterrupted run.
  * d_blob: DEVICE memory of psdns_history_bytes(h) bytes (256-byte aligned), owned by the caller.
+ * Between steps theta^ is held as the particular solution plus the coefficients of its influence-matrix correction
+ * (option "lazy"); psdns_get_history first completes the array on the stream (one small kernel), which does not change
+ * what the following steps compute.  Asynchronous on the stream.
  * PSDNS_ESTATE before the first set_state; PSDNS_EINVAL on a null pointer or a size mismatch. */
 size_t psdns_history_bytes(const psdns_handle *h);
 int psdns_get_history(psdns_handle *h, void *d_blob, size_t bytes);
