@@ -1,13 +1,16 @@
 // Spectral-space kernels: one thread per retained (kx, ky) column, sweeping the Chebyshev index
 // n sequentially; consecutive threads own consecutive columns so every access is coalesced.
-//   k_relayout   boundary <-> private spectral layouts
-//   k_lap        theta = (D^2 - k^2) w                         (hidden state, reading S13)
-//   k_prep       row a1: grad(phi) spectra [+ strain spectra]
-//   k_rhs        row a9: S = div T, N_omega (Eq. 14), N_w (Eq. 15), S_phi (Eq. 17), AB2, CN/IE
-//                right-hand sides, all derivative recurrences fused in ONE downward sweep
-//   k_helm_setup / k_helm   row a10: quasi-tridiagonal Chebyshev-tau Helmholtz solve
-//   k_infl       row a10: influence-matrix closure of the w problem (Dw(+-1) = 0)
-//   k_finish     row a11: u^, v^ from continuity (Eq. 6) and the vorticity definition (Eq. 16)
+//   k_relayout      boundary <-> private spectral layouts
+//   k_hidden_state  theta = (D^2 - k^2) w, omega_z = i kx v - i ky u            (hidden state, reading S13)
+//   k_prep          row a1: grad(phi) spectra [+ strain spectra]
+//   k_helm_setup / k_helm / k_elimup_setup / k_hom_tables   init: pivot tables, homogeneous solutions
+//   The solver stage of a step is three sweeps over the columns (rows a9-a11):
+//   k_rhs_elim      DOWN: S = div T, N_omega (Eq. 14), N_w (Eq. 15), S_phi (Eq. 17), AB2, CN/IE right-hand sides, all
+//                   derivative recurrences, streamed into the Gauss elimination of the omega_z, theta, psi problems
+//   k_subst3        UP:   their substitution; theta_p and psi feed the UPWARD elimination of the w and phi solves
+//   k_finish        DOWN: back substitution of w and phi, influence-matrix correction (Dw(+-1) = 0), u^, v^ from
+//                   continuity (Eq. 6) and the vorticity definition (Eq. 16), D phi^
+//   k_subst / k_elim2 / k_elim2up   the five-sweep forms of the same solves (options "w3", "phi3": cross-checks)
 #pragma once
 #include "fft_tile.cuh"
 
